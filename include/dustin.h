@@ -1,0 +1,151 @@
+/* dustin.h -- C ABI of the B200-native sparse verification attention of "Dustin" (arxiv/paper_2606_24957).
+ *
+ * One decoder layer's sparse verification is four device stages:
+ *   a1 dustin_score_heads        head-subset scoring against the full KV cache
+ *   a2 dustin_fuse_scores        Eq. 5 accumulation of the target signal           PAPER.md:157-164 (Eq. 5)
+ *   a3 dustin_topk_select        tiered top-k with protected sink + window         PAPER.md:166-169 (Eq. 6), :443
+ *   a4 dustin_sparse_verify_attn (gamma+1)-query attention over the selected KV    PAPER.md:153, App. G :568
+ *   a5 the same call with idx == NULL is the full-cache verification baseline
+ *   a6 dustin_verify_layer_fused a1..a4 enqueued on one stream, no host sync
+ *
+ * Conventions (all entry points):
+ *  - Every pointer marked "device" is a CUDA device pointer owned by the caller; the library never allocates,
+ *    frees, synchronises, or dereferences device memory on the host.  Structs and scalars are host values.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Work is only enqueued.
+ *  - Return value: DUSTIN_OK (0) or a negative dustin_status.  Only host-visible arguments are validated.
+ *    No exception crosses the ABI.  After DUSTIN_ERR_CUDA, dustin_last_cuda_error() gives the cudaError_t.
+ *  - bf16 tensors are raw 16-bit patterns; the last (head_dim) dimension is contiguous; 16-byte aligned rows.
+ *  - Outputs are fully overwritten; `hist_inout` is the only in/out state.  Identical inputs give
+ *    bit-identical outputs (no order-dependent floating-point atomics anywhere).
+ *  - Limits: head_dim in {64,128}; n_q_heads <= 64 (the head subset is a 64-bit mask); n_new (T) <= 16;
+ *    T * (n_q_heads / n_kv_heads) <= 96 query rows per KV head; at most 8 subset heads per KV group;
+ *    max_ctx <= 2^20.  Outside them the call returns DUSTIN_ERR_UNSUPPORTED.
+ */
+#ifndef DUSTIN_H_
+#define DUSTIN_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DUSTIN_VERSION 100 /* 0.1.0 */
+
+typedef enum dustin_status {
+    DUSTIN_OK = 0,
+    DUSTIN_ERR_INVALID_ARG = -1,   /* null pointer, negative size, Hq % Hkv != 0, S + W > k, empty head mask ...  */
+    DUSTIN_ERR_UNSUPPORTED = -2,   /* a documented limit above is exceeded                                         */
+    DUSTIN_ERR_WORKSPACE = -3,     /* ws == NULL or ws_bytes < dustin_workspace_bytes(...)                          */
+    DUSTIN_ERR_CUDA = -4           /* a launch failed; see dustin_last_cuda_error()                                 */
+} dustin_status;
+
+/* Problem shape of one layer call.  T = n_new = gamma + 1 verify positions (reading A13). */
+typedef struct dustin_shape {
+    int32_t batch;       /* B                                                                                   */
+    int32_t n_q_heads;   /* Hq                                                                                  */
+    int32_t n_kv_heads;  /* Hkv; KV group of query head h is g = h / (Hq / Hkv)  (reading A2)                    */
+    int32_t head_dim;    /* d                                                                                   */
+    int32_t n_new;       /* T = gamma + 1                                                                       */
+    int32_t max_ctx;     /* N: row length of every [.., N] score tensor; N_b <= N                               */
+    float   sm_scale;    /* softmax scale; 0 => 1/sqrt(d)  (reading A5)                                         */
+} dustin_shape_t;
+
+/* bf16 GQA KV cache, contiguous or paged.  Strides are in ELEMENTS.
+ * Contiguous (page_table == NULL): row (b, n, g) starts at  b*stride_seq + n*stride_token + g*stride_head.
+ * Paged: row (b, n, g) starts at  page_table[b*max_pages + n/page_size]*stride_seq + (n%page_size)*stride_token
+ *        + g*stride_head  (stride_seq is then the page stride).  k and v share the layout. */
+typedef struct dustin_kv {
+    const void*    k;            /* device, bf16                                                                */
+    const void*    v;            /* device, bf16 (may be NULL for dustin_score_heads)                            */
+    int64_t        stride_seq;
+    int64_t        stride_token;
+    int64_t        stride_head;
+    const int32_t* page_table;   /* device int32 [batch, max_pages] or NULL                                      */
+    int32_t        page_size;
+    int32_t        max_pages;
+    const int32_t* seq_lens;     /* device int32 [batch] (N_b, clamped to [0, max_ctx]) or NULL => all max_ctx   */
+} dustin_kv_t;
+
+/* Selection rule of Eq. 6.  S and W are counted inside k. */
+typedef struct dustin_select {
+    int32_t        budget;    /* k, used when budgets == NULL                                                     */
+    const int32_t* budgets;   /* device int32 [batch] per-sequence k_b, or NULL; every k_b must be <= k_max and
+                                 >= n_sink + n_recent (a violating row gets cnt = 0 and an all -1 list)          */
+    int32_t        n_sink;    /* S: tokens [0, S) always kept                                                     */
+    int32_t        n_recent;  /* W: tokens [N_b - W, N_b) always kept                                             */
+    int32_t        m_num;     /* draft quota m = floor((k - S - W) * m_num / m_den)  (reading A9)                 */
+    int32_t        m_den;     /*   0 <= m_num <= m_den, m_den > 0                                                 */
+    int32_t        n_lists;   /* G: 1 (one list per sequence) or n_kv_heads (per KV head)           */
+} dustin_select_t;
+
+int         dustin_version(void);
+const char* dustin_status_string(int status);
+int         dustin_last_cuda_error(void);            /* cudaError_t of the last failed launch on this thread     */
+
+/* Scratch (bytes of device memory, 256-byte aligned by the caller) that is enough for every entry point on this
+ * shape: the scoring stage with the head subset `head_mask` (0 => sized for all n_q_heads heads) plus the
+ * attention stage over at most `k_max` selected rows per list (k_max <= 0 => max_ctx rows, the dense case).
+ * One buffer of this size serves dustin_verify_layer_fused.  Returns 0 on invalid arguments. */
+size_t dustin_workspace_bytes(const dustin_shape_t* shape, uint64_t head_mask, int32_t k_max);
+
+/* Tuning aid (process-wide, not thread-safe, affects performance only): cache rows per attention CTA;
+ * 0 restores the built-in heuristic.  Query dustin_workspace_bytes again after changing it. */
+void dustin_tune_attn_split_tokens(int32_t split_tokens);
+
+/* a1 -- head-subset scoring (PAPER.md:159 "target attention tensor of the last generated token", :218, :391).
+ * For every head h with bit h of head_mask set:  p_h[n] = softmax_n( sm_scale * q[b,h,:] . K[b,n,g(h),:] ) over
+ * the N_b cached tokens (reading A4).  n_lists == 1:  scores_now[b,0,n] = sum_h p_h[n];  n_lists == Hkv:
+ * scores_now[b,g,n] = sum over the subset heads of KV group g, and a group with no subset head receives the sum
+ * over all subset heads (reading A2).  Entries n >= N_b are written as 0.
+ *   q: device bf16, row (b,h) at q + b*q_stride_batch + h*q_stride_head (elements): any verify position of the
+ *      [B,T,Hq,d] query tensor can be scored (reading A3: position 0).
+ *   scores_now: device fp32 [B, n_lists, max_ctx], written. */
+int dustin_score_heads(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q, int64_t q_stride_batch,
+                       int64_t q_stride_head, uint64_t head_mask, int32_t n_lists, float* scores_now, void* ws,
+                       size_t ws_bytes, void* stream);
+
+/* a2 -- Eq. 5 accumulation (reading A6):  hist[b,l,n] <- alpha*hist[b,l,n] + scores_now[b,l,n]
+ * for n < N_b (entries n >= N_b untouched).  Both device fp32 [batch, n_lists, max_ctx]. */
+int dustin_fuse_scores(int32_t batch, int32_t n_lists, int32_t max_ctx, const int32_t* seq_lens,
+                       const float* scores_now, float* hist_inout, float alpha, void* stream);
+
+/* a3 -- tiered top-k, Eq. 6.  Per (b, list), N = N_b, k = k_b:
+ *   k >= N: idx = 0..N-1, cnt = N.  Otherwise I_prot = [0,S') U [N-W',N) with S' = min(S,N), W' = min(W,N-S');
+ *   I_draft = the m' = min(m, k-|I_prot|) best candidates of [S',N-W') by s_draft; I_target = the
+ *   k-|I_prot|-m' best remaining candidates by s_target; ties -> lower index; scores compare as max(s, 0)
+ *   (NaN undefined).  idx_out[b,l,:cnt] = I_verify in ascending order, tail = -1;  cnt_out[b,l] = |I_verify|.
+ *   s_draft: device fp32; row (b,l) at s_draft + b*(draft_list_stride ? n_lists*max_ctx : max_ctx)
+ *            + l*draft_list_stride  (draft_list_stride = 0: one [B,N] vector broadcast over the lists; = max_ctx:
+ *            a [B,G,N] tensor).
+ *   s_target: device fp32 [B, G, max_ctx].   idx_out: device int32 [B, G, k_max].   cnt_out: device int32 [B, G]. */
+int dustin_topk_select(int32_t batch, int32_t max_ctx, const int32_t* seq_lens, const dustin_select_t* select,
+                       const float* s_draft, int64_t draft_list_stride, const float* s_target, int32_t* idx_out,
+                       int32_t* cnt_out, int32_t k_max, void* stream);
+
+/* a4 / a5 -- verification attention (App. G :568; reading A13).  For every (b, h, t):
+ * one softmax over the cnt[b,l] cache rows idx[b,l,:] (l = 0 if n_lists == 1 else g(h)) and the new rows u <= t
+ * (causal among the T new tokens, self included), scale sm_scale;  out = sum p * V.
+ * idx == NULL: all N_b cached rows (full-cache verification attention, the dense baseline).
+ *   q: device bf16 [B,T,Hq,d];  k_new, v_new: device bf16 [B,T,Hkv,d];  idx: device int32 [B,n_lists,k_max]
+ *   (entries in [0,N_b), any order);  cnt: device int32 [B,n_lists];  out: device bf16 [B,T,Hq,d];
+ *   lse_out: device fp32 [B,Hq,T] natural-log normaliser, or NULL. */
+int dustin_sparse_verify_attn(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q, const void* k_new,
+                              const void* v_new, const int32_t* idx, const int32_t* cnt, int32_t n_lists,
+                              int32_t k_max, void* out, float* lse_out, void* ws, size_t ws_bytes, void* stream);
+
+/* a6 -- one layer, one call: a1 (query = verify position 0 of q) -> a2 (into hist_inout) -> a3 -> a4, enqueued
+ * back to back on `stream` with no host synchronisation.  scores_now_out may be NULL (the per-call scores are
+ * then never written to memory).  Other arguments as in the stage calls. */
+int dustin_verify_layer_fused(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q, const void* k_new,
+                              const void* v_new, uint64_t head_mask, const float* s_draft,
+                              int64_t draft_list_stride, float* hist_inout, float alpha,
+                              const dustin_select_t* select, int32_t k_max, float* scores_now_out, void* out,
+                              float* lse_out, int32_t* idx_out, int32_t* cnt_out, void* ws, size_t ws_bytes,
+                              void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DUSTIN_H_ */

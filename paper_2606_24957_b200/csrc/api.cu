@@ -1,0 +1,379 @@
+// api.cu -- the C ABI of include/dustin.h: host-side validation, workspace carving and stage launches.
+// No device memory is allocated, freed, read or synchronised here; every call only enqueues on `stream`.
+#include "kernels.cuh"
+
+#include <cmath>
+#include <cstring>
+
+namespace dustin {
+namespace {
+
+thread_local int g_last_cuda_error = 0;
+
+inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+int fail_cuda(cudaError_t e) {
+    g_last_cuda_error = (int)e;
+    return DUSTIN_ERR_CUDA;
+}
+
+// ---- shape / cache validation ---------------------------------------------------------------------------------
+int check_shape(const dustin_shape_t* s) {
+    if (!s) return DUSTIN_ERR_INVALID_ARG;
+    if (s->batch <= 0 || s->n_q_heads <= 0 || s->n_kv_heads <= 0 || s->head_dim <= 0 || s->n_new <= 0 ||
+        s->max_ctx < 0 || !(s->sm_scale >= 0.f) || !std::isfinite(s->sm_scale))
+        return DUSTIN_ERR_INVALID_ARG;
+    if (s->n_q_heads % s->n_kv_heads != 0) return DUSTIN_ERR_INVALID_ARG;
+    if (s->head_dim != 64 && s->head_dim != 128) return DUSTIN_ERR_UNSUPPORTED;
+    if (s->n_q_heads > 64 || s->n_new > 16 || s->max_ctx > (1 << 20) || s->batch > 65535 || s->n_kv_heads > 65535)
+        return DUSTIN_ERR_UNSUPPORTED;
+    if (s->n_new * (s->n_q_heads / s->n_kv_heads) > 96) return DUSTIN_ERR_UNSUPPORTED;
+    return DUSTIN_OK;
+}
+
+int check_kv(const dustin_shape_t* s, const dustin_kv_t* kv, bool need_v, KvView* out) {
+    if (!kv || !kv->k || (need_v && !kv->v)) return DUSTIN_ERR_INVALID_ARG;
+    if (kv->stride_seq < 0 || kv->stride_token <= 0 || kv->stride_head < 0) return DUSTIN_ERR_INVALID_ARG;
+    // 16-byte row alignment (dustin.h): 8 bf16 elements
+    if ((kv->stride_seq | kv->stride_token | kv->stride_head) & 7) return DUSTIN_ERR_INVALID_ARG;
+    if (((uintptr_t)kv->k & 15) || ((uintptr_t)kv->v & 15)) return DUSTIN_ERR_INVALID_ARG;
+    if (kv->page_table) {
+        if (kv->page_size <= 0 || kv->max_pages <= 0) return DUSTIN_ERR_INVALID_ARG;
+        if ((long long)kv->page_size * kv->max_pages < s->max_ctx) return DUSTIN_ERR_INVALID_ARG;
+    }
+    out->k = static_cast<const __nv_bfloat16*>(kv->k);
+    out->v = static_cast<const __nv_bfloat16*>(kv->v);
+    out->stride_seq = kv->stride_seq;
+    out->stride_token = kv->stride_token;
+    out->stride_head = kv->stride_head;
+    out->page_table = kv->page_table;
+    out->page_size = kv->page_table ? kv->page_size : 1;
+    out->max_pages = kv->page_table ? kv->max_pages : 0;
+    out->seq_lens = kv->seq_lens;
+    return DUSTIN_OK;
+}
+
+float scale_log2_of(const dustin_shape_t* s) {
+    const float sc = s->sm_scale == 0.f ? (float)(1.0 / std::sqrt((double)s->head_dim)) : s->sm_scale;
+    return sc * kLog2e;
+}
+
+// ---- scoring plan ---------------------------------------------------------------------------------------------
+// Tokens per scoring CTA: as large as possible while the grid still holds >= 8 CTAs per SM (148 SMs).
+void score_plan(int batch, int n_groups, int max_ctx, int* chunk_tokens, int* n_chunks) {
+    int chunk = 2048;
+    auto ctas = [&](int c) { return (long long)batch * n_groups * ((max_ctx + c - 1) / c); };
+    while (chunk > 256 && ctas(chunk) < 148 * 8) chunk >>= 1;
+    *chunk_tokens = chunk;
+    *n_chunks = max_ctx > 0 ? (max_ctx + chunk - 1) / chunk : 1;
+}
+
+struct ScoreWs {
+    size_t logits, part, stats, total;
+};
+ScoreWs score_ws(int batch, int nsel, int max_ctx) {
+    // n_chunks upper bound: the smallest chunk (256 tokens)
+    const size_t stride = ((size_t)max_ctx + 3) & ~(size_t)3;
+    const size_t n_chunks = ((size_t)max_ctx + 255) / 256 + 1;
+    ScoreWs w;
+    w.logits = 0;
+    w.part = align256(w.logits + (size_t)batch * nsel * stride * sizeof(float));
+    w.stats = align256(w.part + (size_t)batch * nsel * n_chunks * sizeof(float2));
+    w.total = align256(w.stats + (size_t)batch * nsel * sizeof(float2));
+    return w;
+}
+
+// Fills the head-subset tables of ScoreParams.  Ordinals follow ascending head index.
+int build_subset(const dustin_shape_t* s, uint64_t head_mask, int n_lists, ScoreParams* p) {
+    const int Hq = s->n_q_heads, Hkv = s->n_kv_heads, r = Hq / Hkv;
+    if (Hq < 64 && (head_mask >> Hq) != 0) return DUSTIN_ERR_INVALID_ARG;
+    if (head_mask == 0) return DUSTIN_ERR_INVALID_ARG;
+    if (n_lists != 1 && n_lists != Hkv) return DUSTIN_ERR_INVALID_ARG;
+    if (Hkv > 64) return DUSTIN_ERR_UNSUPPORTED;
+    int nsel = 0, n_groups = 0;
+    int first_of_group[64], cnt_of_group[64];
+    for (int g = 0; g < Hkv; ++g) {
+        first_of_group[g] = nsel;
+        cnt_of_group[g] = 0;
+        for (int j = 0; j < r; ++j) {
+            const int h = g * r + j;
+            if ((head_mask >> h) & 1ull) {
+                p->sel_head[nsel++] = (unsigned char)h;
+                cnt_of_group[g]++;
+            }
+        }
+        if (cnt_of_group[g] > 8) return DUSTIN_ERR_UNSUPPORTED;
+        if (cnt_of_group[g] > 0) {
+            p->group_id[n_groups] = (unsigned char)g;
+            p->group_first[n_groups] = (unsigned char)first_of_group[g];
+            p->group_cnt[n_groups] = (unsigned char)cnt_of_group[g];
+            ++n_groups;
+        }
+    }
+    p->nsel = nsel;
+    p->n_groups = n_groups;
+    for (int l = 0; l < n_lists; ++l) {
+        if (n_lists == 1 || cnt_of_group[l] == 0) {   // one global list, or an empty group (reading A2)
+            p->list_first[l] = 0;
+            p->list_cnt[l] = (unsigned char)nsel;
+        } else {
+            p->list_first[l] = (unsigned char)first_of_group[l];
+            p->list_cnt[l] = (unsigned char)cnt_of_group[l];
+        }
+    }
+    return DUSTIN_OK;
+}
+
+int popcount64(uint64_t x) {
+    int c = 0;
+    for (; x; x &= x - 1) ++c;
+    return c;
+}
+
+// ---- attention plan -------------------------------------------------------------------------------------------
+struct AttnWs {
+    size_t part_o, part_lse, total;
+    int split_tokens, n_splits;
+};
+AttnWs attn_ws(const dustin_shape_t* s, int max_tokens) {
+    AttnWs w;
+    attn_plan(s->batch, s->n_kv_heads, max_tokens, &w.split_tokens, &w.n_splits);
+    const size_t rows = (size_t)s->n_new * (s->n_q_heads / s->n_kv_heads);
+    const size_t units = (size_t)s->batch * s->n_kv_heads * w.n_splits * rows;
+    w.part_o = 0;
+    w.part_lse = align256(units * s->head_dim * sizeof(float));
+    w.total = align256(w.part_lse + units * sizeof(float));
+    if (w.n_splits == 1) w.part_lse = w.total = 0;
+    return w;
+}
+
+int run_score(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q, int64_t q_stride_batch,
+              int64_t q_stride_head, uint64_t head_mask, int32_t n_lists, float* scores_now, float* hist,
+              float alpha, void* ws, size_t ws_bytes, cudaStream_t stream) {
+    int rc = check_shape(shape);
+    if (rc) return rc;
+    ScoreParams p;
+    std::memset(&p, 0, sizeof p);
+    rc = check_kv(shape, kv, false, &p.kv);
+    if (rc) return rc;
+    if (!q || ((uintptr_t)q & 15) || ((q_stride_batch | q_stride_head) & 7) || q_stride_batch < 0 ||
+        q_stride_head < 0)
+        return DUSTIN_ERR_INVALID_ARG;
+    if (!scores_now && !hist) return DUSTIN_ERR_INVALID_ARG;
+    rc = build_subset(shape, head_mask, n_lists, &p);
+    if (rc) return rc;
+    const ScoreWs w = score_ws(shape->batch, p.nsel, shape->max_ctx);
+    if (!ws || ws_bytes < w.total || ((uintptr_t)ws & 255)) return DUSTIN_ERR_WORKSPACE;
+    p.q = static_cast<const __nv_bfloat16*>(q);
+    p.q_stride_batch = q_stride_batch;
+    p.q_stride_head = q_stride_head;
+    p.batch = shape->batch;
+    p.head_dim = shape->head_dim;
+    p.max_ctx = shape->max_ctx;
+    p.n_lists = n_lists;
+    p.scale_log2 = scale_log2_of(shape);
+    score_plan(p.batch, p.n_groups, p.max_ctx, &p.chunk_tokens, &p.n_chunks);
+    p.logit_stride = ((long long)p.max_ctx + 3) & ~3ll;
+    char* base = static_cast<char*>(ws);
+    p.logits = reinterpret_cast<float*>(base + w.logits);
+    p.part = reinterpret_cast<float2*>(base + w.part);
+    p.stats = reinterpret_cast<float2*>(base + w.stats);
+    if (p.max_ctx == 0) return DUSTIN_OK;
+    const cudaError_t e = launch_score(p, scores_now, hist, alpha, stream);
+    return e == cudaSuccess ? DUSTIN_OK : fail_cuda(e);
+}
+
+int check_select(const dustin_select_t* sel, int32_t k_max) {
+    if (!sel) return DUSTIN_ERR_INVALID_ARG;
+    if (sel->n_sink < 0 || sel->n_recent < 0 || sel->m_num < 0 || sel->m_den <= 0 || sel->m_num > sel->m_den ||
+        sel->n_lists <= 0 || k_max <= 0)
+        return DUSTIN_ERR_INVALID_ARG;
+    if (!sel->budgets) {
+        if (sel->budget < 0 || sel->budget > k_max) return DUSTIN_ERR_INVALID_ARG;
+        if (sel->n_sink + sel->n_recent > sel->budget) return DUSTIN_ERR_INVALID_ARG;   // reading A12
+    }
+    return DUSTIN_OK;
+}
+
+int run_select(int32_t batch, int32_t max_ctx, const int32_t* seq_lens, const dustin_select_t* sel,
+               const float* s_draft, int64_t draft_list_stride, const float* s_target, int32_t* idx_out,
+               int32_t* cnt_out, int32_t k_max, cudaStream_t stream) {
+    int rc = check_select(sel, k_max);
+    if (rc) return rc;
+    if (batch <= 0 || max_ctx < 0 || !s_draft || !s_target || !idx_out || !cnt_out) return DUSTIN_ERR_INVALID_ARG;
+    if (draft_list_stride != 0 && draft_list_stride != max_ctx) return DUSTIN_ERR_INVALID_ARG;
+    if (max_ctx > (1 << 20) || batch > 65535) return DUSTIN_ERR_UNSUPPORTED;
+    SelectParams p;
+    p.batch = batch;
+    p.max_ctx = max_ctx;
+    p.n_lists = sel->n_lists;
+    p.k_max = k_max;
+    p.seq_lens = seq_lens;
+    p.budget = sel->budget;
+    p.budgets = sel->budgets;
+    p.n_sink = sel->n_sink;
+    p.n_recent = sel->n_recent;
+    p.m_num = sel->m_num;
+    p.m_den = sel->m_den;
+    p.s_draft = s_draft;
+    p.draft_list_stride = draft_list_stride;
+    p.draft_batch_stride = draft_list_stride == 0 ? (long long)max_ctx : (long long)sel->n_lists * max_ctx;
+    p.s_target = s_target;
+    p.idx_out = idx_out;
+    p.cnt_out = cnt_out;
+    const cudaError_t e = launch_select(p, stream);
+    return e == cudaSuccess ? DUSTIN_OK : fail_cuda(e);
+}
+
+int run_attn(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q, const void* k_new,
+             const void* v_new, const int32_t* idx, const int32_t* cnt, int32_t n_lists, int32_t k_max, void* out,
+             float* lse_out, void* ws, size_t ws_bytes, cudaStream_t stream) {
+    int rc = check_shape(shape);
+    if (rc) return rc;
+    AttnParams p;
+    std::memset(&p, 0, sizeof p);
+    rc = check_kv(shape, kv, true, &p.kv);
+    if (rc) return rc;
+    if (!q || !k_new || !v_new || !out) return DUSTIN_ERR_INVALID_ARG;
+    if (((uintptr_t)q | (uintptr_t)k_new | (uintptr_t)v_new | (uintptr_t)out) & 15) return DUSTIN_ERR_INVALID_ARG;
+    if (idx) {
+        if (!cnt || k_max <= 0 || (n_lists != 1 && n_lists != shape->n_kv_heads)) return DUSTIN_ERR_INVALID_ARG;
+    } else {
+        n_lists = 1;
+        k_max = 0;
+    }
+    const int max_tokens = idx ? (k_max < shape->max_ctx ? k_max : shape->max_ctx) : shape->max_ctx;
+    const AttnWs w = attn_ws(shape, max_tokens > 0 ? max_tokens : 1);
+    if (w.total > 0 && (!ws || ws_bytes < w.total || ((uintptr_t)ws & 255))) return DUSTIN_ERR_WORKSPACE;
+    p.q = static_cast<const __nv_bfloat16*>(q);
+    p.k_new = static_cast<const __nv_bfloat16*>(k_new);
+    p.v_new = static_cast<const __nv_bfloat16*>(v_new);
+    p.idx = idx;
+    p.cnt = cnt;
+    p.batch = shape->batch;
+    p.n_q_heads = shape->n_q_heads;
+    p.n_kv_heads = shape->n_kv_heads;
+    p.group = shape->n_q_heads / shape->n_kv_heads;
+    p.head_dim = shape->head_dim;
+    p.n_new = shape->n_new;
+    p.max_ctx = shape->max_ctx;
+    p.n_lists = n_lists;
+    p.k_max = k_max;
+    p.scale_log2 = scale_log2_of(shape);
+    p.rows = p.n_new * p.group;
+    p.split_tokens = w.split_tokens;
+    p.n_splits = w.n_splits;
+    char* base = static_cast<char*>(ws);
+    p.part_o = w.total ? reinterpret_cast<float*>(base + w.part_o) : nullptr;
+    p.part_lse = w.total ? reinterpret_cast<float*>(base + w.part_lse) : nullptr;
+    p.out = static_cast<__nv_bfloat16*>(out);
+    p.lse_out = lse_out;
+    const cudaError_t e = launch_attn(p, stream);
+    return e == cudaSuccess ? DUSTIN_OK : fail_cuda(e);
+}
+
+}  // namespace
+}  // namespace dustin
+
+using namespace dustin;
+
+extern "C" {
+
+int dustin_version(void) { return DUSTIN_VERSION; }
+
+const char* dustin_status_string(int status) {
+    switch (status) {
+        case DUSTIN_OK: return "ok";
+        case DUSTIN_ERR_INVALID_ARG: return "invalid argument";
+        case DUSTIN_ERR_UNSUPPORTED: return "unsupported shape (see the limits in dustin.h)";
+        case DUSTIN_ERR_WORKSPACE: return "workspace missing, misaligned or too small";
+        case DUSTIN_ERR_CUDA: return "CUDA launch error (see dustin_last_cuda_error)";
+        default: return "unknown status";
+    }
+}
+
+int dustin_last_cuda_error(void) { return g_last_cuda_error; }
+
+void dustin_tune_attn_split_tokens(int32_t split_tokens) { attn_set_split_override(split_tokens); }
+
+size_t dustin_workspace_bytes(const dustin_shape_t* shape, uint64_t head_mask, int32_t k_max) {
+    if (check_shape(shape) != DUSTIN_OK) return 0;
+    const int nsel = head_mask ? popcount64(head_mask) : shape->n_q_heads;
+    const ScoreWs sw = score_ws(shape->batch, nsel, shape->max_ctx);
+    int max_tokens = (k_max > 0 && k_max < shape->max_ctx) ? k_max : shape->max_ctx;
+    if (max_tokens < 1) max_tokens = 1;
+    const AttnWs aw = attn_ws(shape, max_tokens);
+    return sw.total + aw.total + 256;
+}
+
+int dustin_score_heads(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q, int64_t q_stride_batch,
+                       int64_t q_stride_head, uint64_t head_mask, int32_t n_lists, float* scores_now, void* ws,
+                       size_t ws_bytes, void* stream) {
+    if (!scores_now) return DUSTIN_ERR_INVALID_ARG;
+    return run_score(shape, kv, q, q_stride_batch, q_stride_head, head_mask, n_lists, scores_now, nullptr, 0.f, ws,
+                     ws_bytes, static_cast<cudaStream_t>(stream));
+}
+
+int dustin_fuse_scores(int32_t batch, int32_t n_lists, int32_t max_ctx, const int32_t* seq_lens,
+                       const float* scores_now, float* hist_inout, float alpha, void* stream) {
+    if (batch <= 0 || n_lists <= 0 || max_ctx < 0 || !scores_now || !hist_inout || !std::isfinite(alpha))
+        return DUSTIN_ERR_INVALID_ARG;
+    if (batch > 65535 || n_lists > 65535) return DUSTIN_ERR_UNSUPPORTED;
+    if (max_ctx == 0) return DUSTIN_OK;
+    const cudaError_t e = launch_fuse(batch, n_lists, max_ctx, seq_lens, scores_now, hist_inout, alpha,
+                                     static_cast<cudaStream_t>(stream));
+    return e == cudaSuccess ? DUSTIN_OK : fail_cuda(e);
+}
+
+int dustin_topk_select(int32_t batch, int32_t max_ctx, const int32_t* seq_lens, const dustin_select_t* select,
+                       const float* s_draft, int64_t draft_list_stride, const float* s_target, int32_t* idx_out,
+                       int32_t* cnt_out, int32_t k_max, void* stream) {
+    return run_select(batch, max_ctx, seq_lens, select, s_draft, draft_list_stride, s_target, idx_out, cnt_out,
+                      k_max, static_cast<cudaStream_t>(stream));
+}
+
+int dustin_sparse_verify_attn(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q, const void* k_new,
+                              const void* v_new, const int32_t* idx, const int32_t* cnt, int32_t n_lists,
+                              int32_t k_max, void* out, float* lse_out, void* ws, size_t ws_bytes, void* stream) {
+    return run_attn(shape, kv, q, k_new, v_new, idx, cnt, n_lists, k_max, out, lse_out, ws, ws_bytes,
+                    static_cast<cudaStream_t>(stream));
+}
+
+int dustin_verify_layer_fused(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q, const void* k_new,
+                              const void* v_new, uint64_t head_mask, const float* s_draft,
+                              int64_t draft_list_stride, float* hist_inout, float alpha,
+                              const dustin_select_t* select, int32_t k_max, float* scores_now_out, void* out,
+                              float* lse_out, int32_t* idx_out, int32_t* cnt_out, void* ws, size_t ws_bytes,
+                              void* stream) {
+    // Validate everything before the first launch so that an argument error enqueues nothing.
+    int rc = check_shape(shape);
+    if (rc) return rc;
+    rc = check_select(select, k_max);
+    if (rc) return rc;
+    if (!hist_inout || !s_draft || !idx_out || !cnt_out || !out || !q || !k_new || !v_new || !kv || !kv->v ||
+        !std::isfinite(alpha))
+        return DUSTIN_ERR_INVALID_ARG;
+    if (select->n_lists != 1 && select->n_lists != shape->n_kv_heads) return DUSTIN_ERR_INVALID_ARG;
+    if (draft_list_stride != 0 && draft_list_stride != shape->max_ctx) return DUSTIN_ERR_INVALID_ARG;
+    const int nsel = popcount64(head_mask);
+    if (nsel == 0) return DUSTIN_ERR_INVALID_ARG;
+    const ScoreWs sw = score_ws(shape->batch, nsel, shape->max_ctx);
+    const int max_tokens = k_max < shape->max_ctx ? k_max : shape->max_ctx;
+    const AttnWs aw = attn_ws(shape, max_tokens > 0 ? max_tokens : 1);
+    if (!ws || ((uintptr_t)ws & 255) || ws_bytes < sw.total + aw.total) return DUSTIN_ERR_WORKSPACE;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    char* base = static_cast<char*>(ws);
+    // a1 + a2: scores of verify position 0 (reading A3), accumulated straight into hist (Eq. 5)
+    rc = run_score(shape, kv, q, (int64_t)shape->n_new * shape->n_q_heads * shape->head_dim, shape->head_dim,
+                   head_mask, select->n_lists, scores_now_out, hist_inout, alpha, base, sw.total, st);
+    if (rc) return rc;
+    // a3
+    rc = run_select(shape->batch, shape->max_ctx, kv->seq_lens, select, s_draft, draft_list_stride, hist_inout,
+                    idx_out, cnt_out, k_max, st);
+    if (rc) return rc;
+    // a4
+    return run_attn(shape, kv, q, k_new, v_new, idx_out, cnt_out, select->n_lists, k_max, out, lse_out,
+                    base + sw.total, ws_bytes - sw.total, st);
+}
+
+}  // extern "C"

@@ -1,0 +1,96 @@
+// common.cuh -- device helpers shared by the sm_100a kernels of the Dustin sparse-verification path.
+// (CUDA path only; the CPU oracle under oracle/ shares nothing with this tree.)
+#pragma once
+
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/dustin.h"
+
+namespace dustin {
+
+constexpr float kLog2e = 1.4426950408889634f;
+constexpr float kLn2 = 0.6931471805599453f;
+
+// Device view of dustin_kv_t (strides in elements).
+struct KvView {
+    const __nv_bfloat16* k;
+    const __nv_bfloat16* v;
+    long long stride_seq, stride_token, stride_head;
+    const int* page_table;
+    int page_size, max_pages;
+    const int* seq_lens;
+};
+
+__device__ __forceinline__ int seq_len_of(const int* seq_lens, int b, int max_ctx) {
+    if (seq_lens == nullptr) return max_ctx;
+    int n = seq_lens[b];
+    return n < 0 ? 0 : (n > max_ctx ? max_ctx : n);
+}
+
+// Element offset of cache row (b, n, g).
+__device__ __forceinline__ long long kv_row_offset(const KvView& kv, int b, int n, int g) {
+    if (kv.page_table == nullptr)
+        return (long long)b * kv.stride_seq + (long long)n * kv.stride_token + (long long)g * kv.stride_head;
+    const int pg = n / kv.page_size;
+    const int page = __ldg(kv.page_table + (long long)b * kv.max_pages + pg);
+    return (long long)page * kv.stride_seq + (long long)(n - pg * kv.page_size) * kv.stride_token +
+           (long long)g * kv.stride_head;
+}
+
+// ---- memory -------------------------------------------------------------------------------------------------
+// 16-byte streaming load that does not pollute L1 (the K stream is read exactly once).
+__device__ __forceinline__ uint4 ldg_stream16(const void* p) {
+    uint4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+                 : "l"(p));
+    return r;
+}
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+// cp.async 16 B global -> shared, bypassing L1; src_bytes = 0 zero-fills the destination.
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, int src_bytes) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() {
+    asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
+}
+
+// ---- tensor-core fragments (warp-level mma.sync; see DESIGN.md §5 for why not tcgen05 on this path) ----------
+__device__ __forceinline__ void ldmatrix_x4(uint32_t& r0, uint32_t& r1, uint32_t& r2, uint32_t& r3, uint32_t addr) {
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3)
+                 : "r"(addr));
+}
+__device__ __forceinline__ void ldmatrix_x4_trans(uint32_t& r0, uint32_t& r1, uint32_t& r2, uint32_t& r3,
+                                                  uint32_t addr) {
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3)
+                 : "r"(addr));
+}
+// D(16x8,f32) += A(16x16,bf16,row) * B(16x8,bf16,col)
+__device__ __forceinline__ void mma_bf16_16816(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3,
+                                               uint32_t b0, uint32_t b1) {
+    asm volatile(
+        "mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+        : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+        : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
+    __nv_bfloat162 t = __floats2bfloat162_rn(lo, hi);
+    return *reinterpret_cast<uint32_t*>(&t);
+}
+
+__device__ __forceinline__ float fast_exp2(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+}  // namespace dustin

@@ -1,0 +1,72 @@
+// kernels.cuh -- parameter blocks and launchers of the four stages (internal; the public surface is dustin.h).
+#pragma once
+
+#include "common.cuh"
+
+namespace dustin {
+
+// ---- a1 / a2 ------------------------------------------------------------------------------------------------
+struct ScoreParams {
+    KvView kv;
+    const __nv_bfloat16* q;
+    long long q_stride_batch, q_stride_head;
+    int batch, head_dim, max_ctx, n_lists;
+    float scale_log2;        // sm_scale * log2(e): logits live in the log2 domain
+    int nsel;                // |subset|; ordinals follow ascending head index, so a KV group's heads are contiguous
+    int n_groups;            // KV groups holding >= 1 subset head (the only K rows that are read)
+    int chunk_tokens, n_chunks;
+    unsigned char sel_head[64];     // ordinal -> query head
+    unsigned char group_id[64];     // scored group slot -> KV head
+    unsigned char group_first[64];  // scored group slot -> first ordinal
+    unsigned char group_cnt[64];    // scored group slot -> number of subset heads (<= 8)
+    unsigned char list_first[64];   // list -> first ordinal feeding it
+    unsigned char list_cnt[64];     // list -> number of ordinals feeding it (empty group => all, reading A2)
+    long long logit_stride;         // max_ctx rounded up to a multiple of 4
+    float* logits;                  // ws: [B, nsel, logit_stride] log2-domain logits
+    float2* part;                   // ws: [B, nsel, n_chunks] (max, sum) in the log2 domain
+    float2* stats;                  // ws: [B, nsel] (M, 1/Z)
+};
+
+cudaError_t launch_score(const ScoreParams& p, float* scores_now, float* hist, float alpha, cudaStream_t stream);
+cudaError_t launch_fuse(int batch, int n_lists, int max_ctx, const int* seq_lens, const float* now, float* hist,
+                        float alpha, cudaStream_t stream);
+
+// ---- a3 -----------------------------------------------------------------------------------------------------
+struct SelectParams {
+    int batch, max_ctx, n_lists, k_max;
+    const int* seq_lens;
+    int budget;
+    const int* budgets;
+    int n_sink, n_recent, m_num, m_den;
+    const float* s_draft;
+    long long draft_batch_stride, draft_list_stride;
+    const float* s_target;
+    int* idx_out;
+    int* cnt_out;
+};
+cudaError_t launch_select(const SelectParams& p, cudaStream_t stream);
+size_t select_smem_bytes(int max_ctx);
+
+// ---- a4 / a5 ------------------------------------------------------------------------------------------------
+struct AttnParams {
+    KvView kv;
+    const __nv_bfloat16* q;       // [B,T,Hq,d]
+    const __nv_bfloat16* k_new;   // [B,T,Hkv,d]
+    const __nv_bfloat16* v_new;
+    const int* idx;               // [B,G,k_max] or nullptr (dense)
+    const int* cnt;               // [B,G]
+    int batch, n_q_heads, n_kv_heads, group, head_dim, n_new, max_ctx, n_lists, k_max;
+    float scale_log2;
+    int rows;                     // T * group query rows per KV head
+    int split_tokens, n_splits;   // cache tokens per CTA; CTAs per (b, KV head)
+    float* part_o;                // ws: [B,Hkv,n_splits,rows,d] normalised partial outputs
+    float* part_lse;              // ws: [B,Hkv,n_splits,rows]   log2-domain normalisers
+    __nv_bfloat16* out;           // [B,T,Hq,d]
+    float* lse_out;               // [B,Hq,T] or nullptr
+};
+cudaError_t launch_attn(const AttnParams& p, cudaStream_t stream);
+// Host-side split heuristic shared by workspace sizing and launch.
+void attn_plan(int batch, int n_kv_heads, int max_tokens, int* split_tokens, int* n_splits);
+void attn_set_split_override(int split_tokens);
+
+}  // namespace dustin

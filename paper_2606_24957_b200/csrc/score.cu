@@ -1,0 +1,276 @@
+// score.cu -- stage a1 (head-subset scoring) and stage a2 (Eq. 5 accumulation,
+// PAPER.md:161-164) for sm_100a.
+//
+// a1 is one streaming read of the K rows of every KV group that holds a subset head (HBM-bound: DESIGN.md §4).
+//   score_logits_kernel   K rows go global -> registers with 16-byte loads and straight into mma.sync fragments
+//                         (tokens on M, the <= 8 subset heads of the KV group on N, head_dim on K; the head_dim
+//                         axis is permuted identically for both operands so each thread's 16 B feed two k-steps).
+//                         Writes log2-domain logits [B, nsel, N] (L2-resident scratch) and per-CTA softmax
+//                         partials (max, sum).
+//   score_stats_kernel    folds the partials into (M, 1/Z) per (sequence, head), in a fixed order.
+//   score_normalize_kernel p = exp2(l - M) / Z summed over the heads of each list; optionally fused with the
+//                         Eq. 5 accumulation into hist (the fused entry point never writes scores_now).
+#include "kernels.cuh"
+
+namespace dustin {
+
+namespace {
+
+constexpr int kScoreWarps = 8;
+constexpr int kScoreThreads = kScoreWarps * 32;
+constexpr int kTileTokens = 16;  // one m16n8k16 M tile
+
+template <int D>
+struct KFrag {
+    uint4 lo[D / 32];  // row g      : 8 bf16 at dims j*32 + c*8
+    uint4 hi[D / 32];  // row g + 8
+};
+
+template <int D>
+__device__ __forceinline__ void load_tile(KFrag<D>& f, const ScoreParams& p, int b, int grp, int n0, int N, int lane) {
+    const int g = lane >> 2, c = lane & 3;
+    const int n_lo = n0 + g, n_hi = n0 + g + 8;
+#pragma unroll
+    for (int j = 0; j < D / 32; ++j) {
+        f.lo[j] = make_uint4(0, 0, 0, 0);
+        f.hi[j] = make_uint4(0, 0, 0, 0);
+    }
+    if (n_lo < N) {
+        const __nv_bfloat16* row = p.kv.k + kv_row_offset(p.kv, b, n_lo, grp) + c * 8;
+#pragma unroll
+        for (int j = 0; j < D / 32; ++j) f.lo[j] = ldg_stream16(row + j * 32);
+    }
+    if (n_hi < N) {
+        const __nv_bfloat16* row = p.kv.k + kv_row_offset(p.kv, b, n_hi, grp) + c * 8;
+#pragma unroll
+        for (int j = 0; j < D / 32; ++j) f.hi[j] = ldg_stream16(row + j * 32);
+    }
+}
+
+template <int D>
+__global__ void __launch_bounds__(kScoreThreads) score_logits_kernel(const ScoreParams p) {
+    const int chunk = blockIdx.x, gi = blockIdx.y, b = blockIdx.z;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int g = lane >> 2, c = lane & 3;
+    const int grp = p.group_id[gi], first = p.group_first[gi], nh = p.group_cnt[gi];
+    const int N = seq_len_of(p.kv.seq_lens, b, p.max_ctx);
+
+    // B fragments: head slot n = g of this KV group (zero beyond the subset), dims j*32 + c*8 .. +8.
+    uint4 qf[D / 32];
+#pragma unroll
+    for (int j = 0; j < D / 32; ++j) qf[j] = make_uint4(0, 0, 0, 0);
+    if (g < nh) {
+        const int h = p.sel_head[first + g];
+        const __nv_bfloat16* qrow = p.q + (long long)b * p.q_stride_batch + (long long)h * p.q_stride_head + c * 8;
+#pragma unroll
+        for (int j = 0; j < D / 32; ++j) qf[j] = *reinterpret_cast<const uint4*>(qrow + j * 32);
+    }
+
+    // this thread's logits: heads 2c, 2c+1 of tokens (g, g+8) of each tile
+    float m0 = -INFINITY, m1 = -INFINITY, s0 = 0.f, s1 = 0.f;
+    const int chunk_lo = chunk * p.chunk_tokens;
+    const int chunk_hi = min(chunk_lo + p.chunk_tokens, N);
+    const bool h0 = 2 * c < nh, h1 = 2 * c + 1 < nh;
+    float* l0 = p.logits + ((long long)b * p.nsel + first + 2 * c) * p.logit_stride;
+    float* l1 = l0 + p.logit_stride;
+
+    KFrag<D> cur, nxt;
+    int n0 = chunk_lo + warp * kTileTokens;
+    if (n0 < chunk_hi) load_tile<D>(cur, p, b, grp, n0, N, lane);
+    for (; n0 < chunk_hi; n0 += kScoreWarps * kTileTokens) {
+        const int n1 = n0 + kScoreWarps * kTileTokens;
+        if (n1 < chunk_hi) load_tile<D>(nxt, p, b, grp, n1, N, lane);
+        float acc[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+        for (int j = 0; j < D / 32; ++j) {
+            mma_bf16_16816(acc, cur.lo[j].x, cur.hi[j].x, cur.lo[j].y, cur.hi[j].y, qf[j].x, qf[j].y);
+            mma_bf16_16816(acc, cur.lo[j].z, cur.hi[j].z, cur.lo[j].w, cur.hi[j].w, qf[j].z, qf[j].w);
+        }
+        const int n_lo = n0 + g, n_hi = n0 + g + 8;
+        const bool v_lo = n_lo < N, v_hi = n_hi < N;
+        const float a0 = v_lo ? acc[0] * p.scale_log2 : -INFINITY;   // (token g    , head 2c  )
+        const float a1 = v_lo ? acc[1] * p.scale_log2 : -INFINITY;   // (token g    , head 2c+1)
+        const float a2 = v_hi ? acc[2] * p.scale_log2 : -INFINITY;   // (token g + 8, head 2c  )
+        const float a3 = v_hi ? acc[3] * p.scale_log2 : -INFINITY;   // (token g + 8, head 2c+1)
+        if (h0) {
+            if (v_lo) l0[n_lo] = a0;
+            if (v_hi) l0[n_hi] = a2;
+            const float mn = fmaxf(m0, fmaxf(a0, a2));
+            if (mn > -INFINITY) {
+                s0 = s0 * exp2f(m0 - mn) + exp2f(a0 - mn) + exp2f(a2 - mn);
+                m0 = mn;
+            }
+        }
+        if (h1) {
+            if (v_lo) l1[n_lo] = a1;
+            if (v_hi) l1[n_hi] = a3;
+            const float mn = fmaxf(m1, fmaxf(a1, a3));
+            if (mn > -INFINITY) {
+                s1 = s1 * exp2f(m1 - mn) + exp2f(a1 - mn) + exp2f(a3 - mn);
+                m1 = mn;
+            }
+        }
+        if (n1 < chunk_hi) cur = nxt;
+    }
+
+    // (max, sum) over the 8 lanes that share c, then over the warps (fixed order => deterministic).
+#pragma unroll
+    for (int off = 4; off < 32; off <<= 1) {
+        const float om0 = __shfl_xor_sync(0xffffffffu, m0, off), os0 = __shfl_xor_sync(0xffffffffu, s0, off);
+        const float om1 = __shfl_xor_sync(0xffffffffu, m1, off), os1 = __shfl_xor_sync(0xffffffffu, s1, off);
+        const float n0m = fmaxf(m0, om0), n1m = fmaxf(m1, om1);
+        s0 = (n0m > -INFINITY) ? s0 * exp2f(m0 - n0m) + os0 * exp2f(om0 - n0m) : 0.f;
+        s1 = (n1m > -INFINITY) ? s1 * exp2f(m1 - n1m) + os1 * exp2f(om1 - n1m) : 0.f;
+        m0 = n0m;
+        m1 = n1m;
+    }
+    __shared__ float2 wpart[kScoreWarps][8];
+    if (g == 0) {
+        wpart[warp][2 * c] = make_float2(m0, s0);
+        wpart[warp][2 * c + 1] = make_float2(m1, s1);
+    }
+    __syncthreads();
+    if (threadIdx.x < nh) {
+        float m = -INFINITY, s = 0.f;
+        for (int w = 0; w < kScoreWarps; ++w) {
+            const float2 o = wpart[w][threadIdx.x];
+            const float mn = fmaxf(m, o.x);
+            s = (mn > -INFINITY) ? s * exp2f(m - mn) + o.y * exp2f(o.x - mn) : 0.f;
+            m = mn;
+        }
+        p.part[((long long)b * p.nsel + first + threadIdx.x) * p.n_chunks + chunk] = make_float2(m, s);
+    }
+
+}
+
+// (M, 1/Z) of every subset head from the per-CTA partials: one CTA per sequence, one warp per head at a time.
+__global__ void __launch_bounds__(256) score_stats_kernel(const ScoreParams p) {
+    const int b = blockIdx.x, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int j = warp; j < p.nsel; j += 8) {
+        const float2* src = p.part + ((long long)b * p.nsel + j) * p.n_chunks;
+        float m = -INFINITY, s = 0.f;
+        for (int i = lane; i < p.n_chunks; i += 32) {
+            const float2 o = __ldcg(src + i);
+            const float mn = fmaxf(m, o.x);
+            s = (mn > -INFINITY) ? s * exp2f(m - mn) + o.y * exp2f(o.x - mn) : 0.f;
+            m = mn;
+        }
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) {
+            const float om = __shfl_xor_sync(0xffffffffu, m, off), os = __shfl_xor_sync(0xffffffffu, s, off);
+            const float mn = fmaxf(m, om);
+            s = (mn > -INFINITY) ? s * exp2f(m - mn) + os * exp2f(om - mn) : 0.f;
+            m = mn;
+        }
+        if (lane == 0) p.stats[(long long)b * p.nsel + j] = make_float2(m, s > 0.f ? 1.f / s : 0.f);
+    }
+}
+
+// p = exp2(l - M) / Z, summed over the heads that feed list l; optional Eq. 5 accumulation into hist.
+// VEC = 4: every row of scores_now / hist is 16-byte aligned (max_ctx % 4 == 0); VEC = 1: any max_ctx.
+template <int VEC>
+__global__ void __launch_bounds__(256) score_normalize_kernel(const ScoreParams p, float* __restrict__ scores_now,
+                                                              float* __restrict__ hist, float alpha) {
+    const int l = blockIdx.y, b = blockIdx.z;
+    const int N = seq_len_of(p.kv.seq_lens, b, p.max_ctx);
+    const int first = p.list_first[l], nh = p.list_cnt[l];
+    __shared__ float2 st[64];
+    if (threadIdx.x < nh) st[threadIdx.x] = p.stats[(long long)b * p.nsel + first + threadIdx.x];
+    __syncthreads();
+    const long long row = ((long long)b * p.n_lists + l) * p.max_ctx;
+    const float* lg = p.logits + ((long long)b * p.nsel + first) * p.logit_stride;
+    for (int n = (blockIdx.x * 256 + threadIdx.x) * VEC; n < p.max_ctx; n += gridDim.x * 256 * VEC) {
+        float a[VEC];
+#pragma unroll
+        for (int i = 0; i < VEC; ++i) a[i] = 0.f;
+        if (n < N) {
+            for (int j = 0; j < nh; ++j) {
+                const float M = st[j].x, iz = st[j].y;
+                float x[VEC];
+                if (VEC == 4) {
+                    const float4 t = __ldcg(reinterpret_cast<const float4*>(lg + (long long)j * p.logit_stride + n));
+                    x[0] = t.x, x[VEC > 1 ? 1 : 0] = t.y, x[VEC > 2 ? 2 : 0] = t.z, x[VEC > 3 ? 3 : 0] = t.w;
+                } else {
+                    x[0] = __ldcg(lg + (long long)j * p.logit_stride + n);
+                }
+#pragma unroll
+                for (int i = 0; i < VEC; ++i) a[i] += exp2f(x[i] - M) * iz;
+            }
+#pragma unroll
+            for (int i = 1; i < VEC; ++i)
+                if (n + i >= N) a[i] = 0.f;
+        }
+        if (VEC == 4) {
+            if (scores_now)
+                *reinterpret_cast<float4*>(scores_now + row + n) = make_float4(a[0], a[VEC > 1 ? 1 : 0], a[VEC > 2 ? 2 : 0], a[VEC > 3 ? 3 : 0]);
+            if (hist && n < N) {
+                float4 h = *reinterpret_cast<const float4*>(hist + row + n);
+                h.x = fmaf(alpha, h.x, a[0]);
+                if (n + 1 < N) h.y = fmaf(alpha, h.y, a[VEC > 1 ? 1 : 0]);
+                if (n + 2 < N) h.z = fmaf(alpha, h.z, a[VEC > 2 ? 2 : 0]);
+                if (n + 3 < N) h.w = fmaf(alpha, h.w, a[VEC > 3 ? 3 : 0]);
+                *reinterpret_cast<float4*>(hist + row + n) = h;
+            }
+        } else {
+            if (scores_now) scores_now[row + n] = a[0];
+            if (hist && n < N) hist[row + n] = fmaf(alpha, hist[row + n], a[0]);
+        }
+    }
+}
+
+template <int VEC>
+__global__ void __launch_bounds__(256) fuse_kernel(int max_ctx, const int* __restrict__ seq_lens,
+                                                   const float* __restrict__ now, float* __restrict__ hist,
+                                                   float alpha, int n_lists) {
+    const int b = blockIdx.z, l = blockIdx.y;
+    const int N = seq_len_of(seq_lens, b, max_ctx);
+    const long long row = ((long long)b * n_lists + l) * max_ctx;
+    for (int n = (blockIdx.x * 256 + threadIdx.x) * VEC; n < N; n += gridDim.x * 256 * VEC) {
+        if (VEC == 4 && n + 3 < N) {
+            const float4 a = *reinterpret_cast<const float4*>(now + row + n);
+            float4 h = *reinterpret_cast<const float4*>(hist + row + n);
+            h.x = fmaf(alpha, h.x, a.x);
+            h.y = fmaf(alpha, h.y, a.y);
+            h.z = fmaf(alpha, h.z, a.z);
+            h.w = fmaf(alpha, h.w, a.w);
+            *reinterpret_cast<float4*>(hist + row + n) = h;
+        } else {
+            for (int i = n; i < min(n + VEC, N); ++i) hist[row + i] = fmaf(alpha, hist[row + i], now[row + i]);
+        }
+    }
+}
+
+}  // namespace
+
+cudaError_t launch_score(const ScoreParams& p, float* scores_now, float* hist, float alpha, cudaStream_t stream) {
+    dim3 grid(p.n_chunks, p.n_groups, p.batch);
+    if (p.head_dim == 128)
+        score_logits_kernel<128><<<grid, kScoreThreads, 0, stream>>>(p);
+    else
+        score_logits_kernel<64><<<grid, kScoreThreads, 0, stream>>>(p);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    score_stats_kernel<<<p.batch, 256, 0, stream>>>(p);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    const int nblk = max(1, min((p.max_ctx + 1023) / 1024, 64));
+    const bool vec = (p.max_ctx & 3) == 0 && (((uintptr_t)scores_now | (uintptr_t)hist) & 15) == 0;
+    if (vec)
+        score_normalize_kernel<4><<<dim3(nblk, p.n_lists, p.batch), 256, 0, stream>>>(p, scores_now, hist, alpha);
+    else
+        score_normalize_kernel<1><<<dim3(nblk, p.n_lists, p.batch), 256, 0, stream>>>(p, scores_now, hist, alpha);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_fuse(int batch, int n_lists, int max_ctx, const int* seq_lens, const float* now, float* hist,
+                        float alpha, cudaStream_t stream) {
+    const int nblk = max(1, min((max_ctx + 1023) / 1024, 64));
+    const bool vec = (max_ctx & 3) == 0 && (((uintptr_t)now | (uintptr_t)hist) & 15) == 0;
+    if (vec)
+        fuse_kernel<4><<<dim3(nblk, n_lists, batch), 256, 0, stream>>>(max_ctx, seq_lens, now, hist, alpha, n_lists);
+    else
+        fuse_kernel<1><<<dim3(nblk, n_lists, batch), 256, 0, stream>>>(max_ctx, seq_lens, now, hist, alpha, n_lists);
+    return cudaGetLastError();
+}
+
+}  // namespace dustin

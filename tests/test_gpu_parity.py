@@ -1,0 +1,166 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same seeded
+inputs.  Sizes are small enough for the oracle to finish in seconds yet span several tiles, several CTAs per row
+and ragged tails.  Acceptance rules: tests/harness.py."""
+import pytest
+import torch
+
+from paper_2606_24957_b200 import api, synth
+from tests import harness as H
+
+pytestmark = pytest.mark.gpu
+
+
+def small_cases():
+    llama = synth.config_llama8b()
+    qwen = synth.config_qwen72b()
+    tiny = synth.config_tiny()
+    return {
+        "tiny": tiny,                                                                         # BASELINE configs[0]
+        "llama_spread": synth.shrink(llama, batch=2, ctx=4999, budget=700, n_sink=16, n_recent=100),
+        "llama_packed": synth.shrink(llama, batch=2, ctx=3000, budget=512, n_sink=8, n_recent=64,
+                                     heads=synth.packed_heads(4), n_lists=1),
+        "qwen_spread": synth.shrink(qwen, batch=2, ctx=4100, budget=600, n_sink=64, n_recent=256),
+        "qwen_packed": synth.shrink(qwen, batch=1, ctx=2500, budget=300, n_sink=4, n_recent=16,
+                                    heads=synth.packed_heads(8), n_lists=1),
+        "qwen_packed_perkv": synth.shrink(qwen, batch=1, ctx=2049, budget=333, n_sink=4, n_recent=16,
+                                          heads=(0, 1, 2, 17, 63), n_lists=8),                # empty groups (A2)
+        "qwen_gamma8": synth.shrink(qwen, batch=1, ctx=1500, budget=256, n_sink=8, n_recent=32, gamma=8),
+        "qwen_gamma2_d64": synth.shrink(qwen, batch=2, ctx=1100, budget=200, n_sink=8, n_recent=32, gamma=2,
+                                        head_dim=64),
+        "paged_ragged": synth.shrink(synth.config_paged(), batch=3, ctx=4000, ragged_min=900, n_sink=4, n_recent=16),
+        "target_only": synth.shrink(tiny, m_num=0, m_den=1),                                  # Dustin-T
+        "draft_only": synth.shrink(tiny, m_num=1, m_den=1),                                   # Dustin-D
+    }
+
+
+CASES = small_cases()
+
+
+def _both(cfg, layer=0):
+    cpu = synth.make_layer(cfg, layer, "cpu")
+    return cpu, cpu.to("cuda")
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_staged_path_matches_oracle(name):
+    cfg = CASES[name]
+    cpu, dev = _both(cfg)
+    got = H.run_gpu_staged(dev)
+    a_ref, h_ref = H.oracle_scores(cpu)
+    # a1, a2: fp32 scores within 1e-5 relative of the fp64 oracle
+    H.check_scores(got.scores_now, a_ref, "scores_now")
+    H.check_scores(got.hist, h_ref, "hist")
+    # a3 (i): fed the GPU's own fp32 scores the oracle must return the GPU's lists bit for bit
+    idx_same, cnt_same = H.oracle_select(cpu, got.hist.cpu())
+    assert torch.equal(got.cnt.cpu(), cnt_same)
+    assert torch.equal(got.idx.cpu(), idx_same)
+    # a3 (ii): against the oracle's own scores only near-tie swaps are allowed
+    idx_ref, cnt_ref = H.oracle_select(cpu, h_ref)
+    H.check_index_lists_valid(cpu, got.idx, got.cnt)
+    H.check_near_tie_only(cpu, got.idx, got.cnt, idx_ref, cnt_ref, h_ref)
+    # a4: attention on the GPU's lists
+    o_ref, lse_ref = H.oracle_attn(cpu, got.idx.cpu(), got.cnt.cpu())
+    H.check_attn(got.out, o_ref)
+    assert torch.allclose(got.lse.cpu().double(), lse_ref, atol=2e-3, rtol=0)
+
+
+@pytest.mark.parametrize("name", ["tiny", "llama_spread", "qwen_packed", "paged_ragged"])
+def test_fused_equals_staged_bitwise_and_is_deterministic(name):
+    cfg = CASES[name]
+    dev = synth.make_layer(cfg, 0, "cuda")
+    staged = H.run_gpu_staged(dev)
+    fused = H.run_gpu_fused(dev)
+    again = H.run_gpu_fused(dev, want_scores=False)
+    for r in (fused, again):
+        assert torch.equal(r.idx, staged.idx) and torch.equal(r.cnt, staged.cnt)
+        assert torch.equal(r.hist, staged.hist)
+        assert torch.equal(r.out.view(torch.int16), staged.out.view(torch.int16))
+        assert torch.equal(r.lse, staged.lse)
+    assert torch.equal(fused.scores_now, staged.scores_now)
+
+
+@pytest.mark.parametrize("name", ["tiny", "llama_spread", "qwen_gamma8", "paged_ragged", "qwen_gamma2_d64"])
+def test_dense_baseline_matches_oracle(name):
+    cfg = CASES[name]
+    cpu, dev = _both(cfg)
+    sh = H.shape_of(cfg)
+    ws = api.alloc_workspace(sh, cfg.head_mask, 0)
+    out = torch.full_like(dev.q, float("nan"))
+    lse = torch.full((cfg.batch, cfg.n_q_heads, cfg.n_new), float("nan"), device="cuda")
+    api.sparse_verify_attn(sh, H.gpu_kv(dev), dev.q, dev.k_new, dev.v_new, None, None, out, ws, lse)
+    torch.cuda.synchronize()
+    o_ref, lse_ref = H.oracle_attn(cpu, None, None)
+    H.check_attn(out, o_ref, "dense attention")
+    assert torch.allclose(lse.cpu().double(), lse_ref, atol=2e-3, rtol=0)
+
+
+def test_budget_equal_context_reproduces_dense():
+    """k = N: the sparse call with the full index list must equal the dense call (PAPER.md:92 ARR = 1)."""
+    cfg = synth.shrink(CASES["llama_spread"], ctx=1111, budget=1111, n_sink=4, n_recent=8)
+    dev = synth.make_layer(cfg, 0, "cuda")
+    got = H.run_gpu_staged(dev)
+    assert (got.cnt == 1111).all()
+    assert torch.equal(got.idx[0, 0].cpu(), torch.arange(1111, dtype=torch.int32))
+    sh = H.shape_of(cfg)
+    ws = api.alloc_workspace(sh, cfg.head_mask, 0)
+    dense = torch.empty_like(dev.q)
+    api.sparse_verify_attn(sh, H.gpu_kv(dev), dev.q, dev.k_new, dev.v_new, None, None, dense, ws)
+    torch.cuda.synchronize()
+    assert (got.out.float() - dense.float()).abs().max().item() <= 2e-2
+
+
+@pytest.mark.parametrize("split", [64, 128, 1024])
+def test_split_size_does_not_change_results_beyond_rounding(split):
+    cfg = CASES["qwen_spread"]
+    cpu, dev = _both(cfg)
+    base = H.run_gpu_staged(dev)
+    api.tune_attn_split_tokens(split)
+    try:
+        other = H.run_gpu_staged(dev)
+    finally:
+        api.tune_attn_split_tokens(0)
+    assert torch.equal(base.idx, other.idx)
+    o_ref, _ = H.oracle_attn(cpu, base.idx.cpu(), base.cnt.cpu())
+    H.check_attn(other.out, o_ref)
+
+
+def test_hnd_layout_and_alpha_and_scale_and_query_position():
+    cfg = CASES["llama_packed"]
+    cpu, dev = _both(cfg)
+    sh = H.shape_of(cfg, sm_scale=0.11)
+    k_hnd = dev.k.permute(0, 2, 1, 3).contiguous()
+    v_hnd = dev.v.permute(0, 2, 1, 3).contiguous()
+    kv = api.KV.contiguous_hnd(k_hnd, v_hnd)
+    ws = api.alloc_workspace(sh, cfg.head_mask, dev.k_max)
+    scores = torch.empty((cfg.batch, cfg.n_lists, cfg.ctx), device="cuda")
+    api.score_heads(sh, kv, dev.q[:, 2], cfg.head_mask, cfg.n_lists, scores, ws)      # verify position 2 (A3)
+    hist = dev.hist.clone()
+    api.fuse_scores(scores, hist, 0.25)
+    torch.cuda.synchronize()
+    from oracle import ref
+    a_ref = ref.score_heads(H.cpu_kv(cpu), cpu.q[:, 2], cfg.head_mask, cfg.n_lists, cfg.n_kv_heads, cfg.ctx, 0.11)
+    h_ref = ref.fuse_scores(a_ref, cpu.hist, 0.25)
+    H.check_scores(scores, a_ref)
+    H.check_scores(hist, h_ref)
+    idx, cnt = H.oracle_select(cpu, h_ref)
+    out = torch.empty_like(dev.q)
+    api.sparse_verify_attn(sh, kv, dev.q, dev.k_new, dev.v_new, idx.cuda(), cnt.cuda(), out, ws)
+    torch.cuda.synchronize()
+    o_ref, _ = H.oracle_attn(cpu, idx, cnt, sm_scale=0.11)
+    H.check_attn(out, o_ref)
+
+
+def test_unordered_index_list_gives_same_attention():
+    cfg = CASES["qwen_packed"]
+    cpu, dev = _both(cfg)
+    got = H.run_gpu_staged(dev)
+    perm = torch.randperm(int(got.cnt[0, 0]), generator=torch.Generator().manual_seed(3)).cuda()
+    idx2 = got.idx.clone()
+    idx2[0, 0, :perm.numel()] = got.idx[0, 0, :perm.numel()][perm]
+    sh = H.shape_of(cfg)
+    ws = api.alloc_workspace(sh, cfg.head_mask, dev.k_max)
+    out = torch.empty_like(dev.q)
+    api.sparse_verify_attn(sh, H.gpu_kv(dev), dev.q, dev.k_new, dev.v_new, idx2, got.cnt, out, ws)
+    torch.cuda.synchronize()
+    o_ref, _ = H.oracle_attn(cpu, got.idx.cpu(), got.cnt.cpu())
+    H.check_attn(out, o_ref)
