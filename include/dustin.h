@@ -94,6 +94,17 @@ size_t dustin_workspace_bytes(const dustin_shape_t* shape, uint64_t head_mask, i
  * 0 restores the built-in heuristic.  Query dustin_workspace_bytes again after changing it. */
 void dustin_tune_attn_split_tokens(int32_t split_tokens);
 
+/* Measurement aids (bench.py).  dustin_launch_count: kernels launched by this library in this process so far.
+ * dustin_profile_enable(1) starts bracketing every kernel launch with a CUDA event pair on the launching stream
+ * (and drops earlier records); dustin_profile_enable(0) stops.  dustin_profile_collect is the one call that
+ * synchronises: it waits for the recorded events and writes, per kernel id in [0, DUSTIN_N_KERNELS), the summed
+ * device time in ms and the number of launches (host arrays), then clears the records.  Process-wide. */
+#define DUSTIN_N_KERNELS 7
+uint64_t    dustin_launch_count(void);
+void        dustin_profile_enable(int32_t on);
+int         dustin_profile_collect(double* ms_out, int64_t* launches_out);
+const char* dustin_kernel_name(int32_t kernel_id);   /* NULL outside [0, DUSTIN_N_KERNELS) */
+
 /* a1 -- head-subset scoring (PAPER.md:159 "target attention tensor of the last generated token", :218, :391).
  * For every head h with bit h of head_mask set:  p_h[n] = softmax_n( sm_scale * q[b,h,:] . K[b,n,g(h),:] ) over
  * the N_b cached tokens (reading A4).  n_lists == 1:  scores_now[b,0,n] = sum_h p_h[n];  n_lists == Hkv:

@@ -67,6 +67,14 @@ def lib():
         L.dustin_last_cuda_error.argtypes = []
         L.dustin_tune_attn_split_tokens.restype = None
         L.dustin_tune_attn_split_tokens.argtypes = [i32]
+        L.dustin_launch_count.restype = ctypes.c_uint64
+        L.dustin_launch_count.argtypes = []
+        L.dustin_profile_enable.restype = None
+        L.dustin_profile_enable.argtypes = [i32]
+        L.dustin_profile_collect.restype = ctypes.c_int
+        L.dustin_profile_collect.argtypes = [ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int64)]
+        L.dustin_kernel_name.restype = ctypes.c_char_p
+        L.dustin_kernel_name.argtypes = [i32]
         L.dustin_workspace_bytes.restype = sz
         L.dustin_workspace_bytes.argtypes = [sp, u64, i32]
         L.dustin_score_heads.restype = ctypes.c_int
@@ -84,7 +92,10 @@ def lib():
     return _lib
 
 
+N_KERNELS = 7
+
 EXPORTS = ("dustin_version", "dustin_status_string", "dustin_last_cuda_error", "dustin_tune_attn_split_tokens",
+           "dustin_launch_count", "dustin_profile_enable", "dustin_profile_collect", "dustin_kernel_name",
            "dustin_workspace_bytes", "dustin_score_heads", "dustin_fuse_scores", "dustin_topk_select",
            "dustin_sparse_verify_attn", "dustin_verify_layer_fused")
 
@@ -173,6 +184,22 @@ def version() -> int:
 
 def tune_attn_split_tokens(split_tokens: int) -> None:
     lib().dustin_tune_attn_split_tokens(int(split_tokens))
+
+
+def launch_count() -> int:
+    return int(lib().dustin_launch_count())
+
+
+def profile_enable(on: bool) -> None:
+    lib().dustin_profile_enable(1 if on else 0)
+
+
+def profile_collect() -> dict:
+    """{kernel name: (total ms, launches)} of everything launched since profile_enable(True); synchronises."""
+    ms = (ctypes.c_double * N_KERNELS)()
+    n = (ctypes.c_int64 * N_KERNELS)()
+    _check("dustin_profile_collect", lib().dustin_profile_collect(ms, n))
+    return {lib().dustin_kernel_name(i).decode(): (float(ms[i]), int(n[i])) for i in range(N_KERNELS)}
 
 
 def workspace_bytes(shape: Shape, head_mask: int = 0, k_max: int = 0) -> int:

@@ -296,6 +296,20 @@ int dustin_last_cuda_error(void) { return g_last_cuda_error; }
 
 void dustin_tune_attn_split_tokens(int32_t split_tokens) { attn_set_split_override(split_tokens); }
 
+uint64_t dustin_launch_count(void) { return prof_launch_count(); }
+
+void dustin_profile_enable(int32_t on) { prof_enable(on != 0); }
+
+int dustin_profile_collect(double* ms_out, int64_t* launches_out) {
+    if (!ms_out || !launches_out) return DUSTIN_ERR_INVALID_ARG;
+    long long n[kKernCount];
+    const cudaError_t e = prof_collect(ms_out, n);
+    for (int i = 0; i < kKernCount; ++i) launches_out[i] = n[i];
+    return e == cudaSuccess ? DUSTIN_OK : fail_cuda(e);
+}
+
+const char* dustin_kernel_name(int32_t kernel_id) { return prof_kernel_name(kernel_id); }
+
 size_t dustin_workspace_bytes(const dustin_shape_t* shape, uint64_t head_mask, int32_t k_max) {
     if (check_shape(shape) != DUSTIN_OK) return 0;
     const int nsel = head_mask ? popcount64(head_mask) : shape->n_q_heads;

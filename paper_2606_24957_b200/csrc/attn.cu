@@ -335,6 +335,7 @@ cudaError_t launch_cfg(const AttnParams& p, cudaStream_t stream) {
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
+    ProfScope prof(kKernAttn, stream);
     attn_kernel<D, MT, KS><<<dim3(p.n_splits, p.n_kv_heads, p.batch), C::kThreads, smem, stream>>>(p);
     return cudaGetLastError();
 }
@@ -354,6 +355,7 @@ cudaError_t launch_d(const AttnParams& p, cudaStream_t stream) {
     }
     if (e != cudaSuccess || p.n_splits == 1) return e;
     const int warps = p.batch * p.n_kv_heads * p.rows;
+    ProfScope prof(kKernAttnCombine, stream);
     attn_combine_kernel<D><<<(warps + 3) / 4, 128, 0, stream>>>(p);
     return cudaGetLastError();
 }

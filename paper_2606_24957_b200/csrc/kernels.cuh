@@ -69,4 +69,26 @@ cudaError_t launch_attn(const AttnParams& p, cudaStream_t stream);
 void attn_plan(int batch, int n_kv_heads, int max_tokens, int* split_tokens, int* n_splits);
 void attn_set_split_override(int split_tokens);
 
+// ---- launch bookkeeping (profile.cu) ----------------------------------------------------------------------------
+enum KernelId {
+    kKernScoreLogits = 0, kKernScoreStats, kKernScoreNormalize, kKernFuse, kKernSelect, kKernAttn, kKernAttnCombine,
+    kKernCount
+};
+// Put one on the stack around a kernel launch: counts it and, when profiling is on, brackets it with CUDA events.
+class ProfScope {
+public:
+    ProfScope(int kid, cudaStream_t stream);
+    ~ProfScope();
+    ProfScope(const ProfScope&) = delete;
+    ProfScope& operator=(const ProfScope&) = delete;
+private:
+    int kid_;
+    cudaStream_t stream_;
+    long long slot_;
+};
+unsigned long long prof_launch_count();
+void prof_enable(bool on);
+cudaError_t prof_collect(double* ms_out, long long* launches_out);
+const char* prof_kernel_name(int kid);
+
 }  // namespace dustin

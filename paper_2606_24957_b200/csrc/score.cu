@@ -244,15 +244,22 @@ __global__ void __launch_bounds__(256) fuse_kernel(int max_ctx, const int* __res
 
 cudaError_t launch_score(const ScoreParams& p, float* scores_now, float* hist, float alpha, cudaStream_t stream) {
     dim3 grid(p.n_chunks, p.n_groups, p.batch);
-    if (p.head_dim == 128)
-        score_logits_kernel<128><<<grid, kScoreThreads, 0, stream>>>(p);
-    else
-        score_logits_kernel<64><<<grid, kScoreThreads, 0, stream>>>(p);
+    {
+        ProfScope prof(kKernScoreLogits, stream);
+        if (p.head_dim == 128)
+            score_logits_kernel<128><<<grid, kScoreThreads, 0, stream>>>(p);
+        else
+            score_logits_kernel<64><<<grid, kScoreThreads, 0, stream>>>(p);
+    }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    score_stats_kernel<<<p.batch, 256, 0, stream>>>(p);
+    {
+        ProfScope prof(kKernScoreStats, stream);
+        score_stats_kernel<<<p.batch, 256, 0, stream>>>(p);
+    }
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
+    ProfScope prof(kKernScoreNormalize, stream);
     const int nblk = max(1, min((p.max_ctx + 1023) / 1024, 64));
     const bool vec = (p.max_ctx & 3) == 0 && (((uintptr_t)scores_now | (uintptr_t)hist) & 15) == 0;
     if (vec)
@@ -266,6 +273,7 @@ cudaError_t launch_fuse(int batch, int n_lists, int max_ctx, const int* seq_lens
                         float alpha, cudaStream_t stream) {
     const int nblk = max(1, min((max_ctx + 1023) / 1024, 64));
     const bool vec = (max_ctx & 3) == 0 && (((uintptr_t)now | (uintptr_t)hist) & 15) == 0;
+    ProfScope prof(kKernFuse, stream);
     if (vec)
         fuse_kernel<4><<<dim3(nblk, n_lists, batch), 256, 0, stream>>>(max_ctx, seq_lens, now, hist, alpha, n_lists);
     else

@@ -213,6 +213,7 @@ cudaError_t launch_select(const SelectParams& p, cudaStream_t stream) {
         cudaError_t e = cudaFuncSetAttribute(select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
+    ProfScope prof(kKernSelect, stream);
     select_kernel<<<dim3(p.n_lists, p.batch), kSelThreads, smem, stream>>>(p);
     return cudaGetLastError();
 }
