@@ -43,6 +43,7 @@ struct SelectParams {
     const float* s_target;
     int* idx_out;
     int* cnt_out;
+    int mask_words, replicas, list_cap;   // shared-memory plan, filled by launch_select
 };
 cudaError_t launch_select(const SelectParams& p, cudaStream_t stream);
 size_t select_smem_bytes(int max_ctx);

@@ -19,8 +19,9 @@ __device__ __forceinline__ uint32_t key_of(float s) { return s > 0.f ? __float_a
 
 struct SelShared {
     uint32_t hist[kBins];
-    uint32_t warp_tot[kSelWarps];
+    uint32_t warp_tot[kSelWarps + 1];
     uint32_t res_bin, res_rank, res_cnt;
+    uint32_t list_n;
 };
 
 // Exclusive prefix of v over the block in thread order; *total (optional) receives the block sum.
@@ -35,15 +36,20 @@ __device__ __forceinline__ uint32_t block_excl_scan(uint32_t v, SelShared& sh, u
     __syncthreads();   // protects warp_tot against the previous use
     if (lane == 31) sh.warp_tot[warp] = inc;
     __syncthreads();
-    uint32_t base = 0, tot = 0;
+    if (warp == 0) {   // scan of the 32 warp totals: warp_tot[w] <- exclusive prefix, warp_tot[32] <- block sum
+        const uint32_t t = sh.warp_tot[lane];
+        uint32_t ti = t;
 #pragma unroll
-    for (int w = 0; w < kSelWarps; ++w) {
-        const uint32_t t = sh.warp_tot[w];
-        if (w < warp) base += t;
-        tot += t;
+        for (int off = 1; off < 32; off <<= 1) {
+            const uint32_t o = __shfl_up_sync(0xffffffffu, ti, off);
+            if (lane >= off) ti += o;
+        }
+        sh.warp_tot[lane] = ti - t;
+        if (lane == 31) sh.warp_tot[32] = ti;
     }
-    if (total) *total = tot;
-    return base + inc - v;
+    __syncthreads();
+    if (total) *total = sh.warp_tot[32];
+    return sh.warp_tot[warp] + inc - v;
 }
 
 // Key of descending rank `rank` (1-based) among the candidates n in [lo, hi) whose bit in `mem` is clear.
@@ -129,11 +135,198 @@ __device__ void admit_tier(const float* __restrict__ s, int lo, int hi, uint32_t
     __syncthreads();
 }
 
+__device__ __noinline__ void full_scan_tier(const float* __restrict__ s, int lo, int hi, uint32_t* mem, int n_words,
+                                            int rank, SelShared& sh) {
+    int need_eq, eq_total;
+    const uint32_t T = radix_select(s, lo, hi, mem, rank, sh, need_eq, eq_total);
+    admit_tier(s, lo, hi, mem, n_words, T, need_eq, eq_total, sh);
+}
+
+// ---- fast path --------------------------------------------------------------------------------------------------
+// One full scan builds the histogram of the top 11 key bits (R lane-interleaved replicas keep same-address shared
+// atomics apart); a second full scan admits everything above the threshold bin and compacts the threshold bin
+// itself into a short (key, index) list in shared memory; the remaining 21 key bits -- and, when equal keys
+// straddle the threshold, the index order among them -- are resolved on that list alone.  A threshold bin that
+// does not fit the list (massive ties) takes the full-scan path above instead.
+struct SelLayout {
+    uint32_t* mem;        // membership bitmask
+    uint32_t* hist;       // kBins * R counters
+    uint32_t* list_key;   // cap
+    uint32_t* list_idx;   // cap
+    int R, cap;
+};
+
+// f(idx, key) for every candidate n in [lo, hi) whose membership bit is clear.  VEC: 16-byte loads (row aligned).
+template <bool VEC, typename F>
+__device__ __forceinline__ void for_each_candidate(const float* __restrict__ s, int lo, int hi, const uint32_t* mem,
+                                                   F f) {
+    if (VEC) {
+        const float4* s4 = reinterpret_cast<const float4*>(s);
+        const int v_end = (hi + 3) >> 2;
+        for (int v = (lo >> 2) + threadIdx.x; v < v_end; v += 4 * kSelThreads) {
+            float4 x[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int vv = v + u * kSelThreads;
+                x[u] = vv < v_end ? __ldcg(s4 + vv) : make_float4(0.f, 0.f, 0.f, 0.f);
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int n = (v + u * kSelThreads) << 2;
+                if (n >= hi) break;
+                const uint32_t nib = mem[n >> 5] >> (n & 31);
+                const float xs[4] = {x[u].x, x[u].y, x[u].z, x[u].w};
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const int idx = n + e;
+                    if (idx >= lo && idx < hi && !((nib >> e) & 1u)) f(idx, key_of(xs[e]));
+                }
+            }
+        }
+    } else {
+        for (int n = lo + threadIdx.x; n < hi; n += kSelThreads)
+            if (!((mem[n >> 5] >> (n & 31)) & 1u)) f(n, key_of(__ldcg(s + n)));
+    }
+}
+
+// hist layout: [bin][R] (the R replicas of a bin are contiguous); kBins * R words, 16-byte aligned.
+__device__ __forceinline__ void clear_hist(uint32_t* hist, int R) {
+    uint4* h4 = reinterpret_cast<uint4*>(hist);
+    for (int i = threadIdx.x; i < kBins * R / 4; i += kSelThreads) h4[i] = make_uint4(0, 0, 0, 0);
+}
+
+__device__ __forceinline__ uint32_t bin_count(const uint32_t* hist, int R, int bin) {
+    if (R == 1) return hist[bin];
+    const uint4* h4 = reinterpret_cast<const uint4*>(hist + (size_t)bin * R);
+    uint32_t c = 0;
+    for (int r = 0; r < R / 4; ++r) {
+        const uint4 x = h4[r];
+        c += x.x + x.y + x.z + x.w;
+    }
+    return c;
+}
+
+// Bin holding rank `rank` (1-based, bins in ascending bin order); leaves (bin, rank inside the bin, bin count)
+// in sh.res_*.  Thread t owns bins t and t + 1024.  R in {1, 4, 8}.  Ends with a barrier.
+__device__ __forceinline__ void find_bin(const uint32_t* hist, int R, uint32_t rank, SelShared& sh) {
+    const uint32_t c0 = bin_count(hist, R, threadIdx.x), c1 = bin_count(hist, R, threadIdx.x + kSelThreads);
+    uint32_t tot0;
+    const uint32_t e0 = block_excl_scan(c0, sh, &tot0);          // prefix over bins [0, 1024)
+    if (rank <= tot0) {
+        if (e0 < rank && rank <= e0 + c0) {
+            sh.res_bin = threadIdx.x;
+            sh.res_rank = rank - e0;
+            sh.res_cnt = c0;
+        }
+    } else {
+        const uint32_t e1 = tot0 + block_excl_scan(c1, sh, nullptr);   // block-uniform branch
+        if (e1 < rank && rank <= e1 + c1) {
+            sh.res_bin = threadIdx.x + kSelThreads;
+            sh.res_rank = rank - e1;
+            sh.res_cnt = c1;
+        }
+    }
+    __syncthreads();
+}
+
+__device__ __forceinline__ void set_member(uint32_t* mem, int idx) { atomicOr(&mem[idx >> 5], 1u << (idx & 31)); }
+
+// One tier of Eq. 6: admits into `mem` the `rank` best candidates of [lo, hi) by s (ties -> lower index).
+template <bool VEC>
+__device__ void select_tier(const float* __restrict__ s, int lo, int hi, int rank, const SelLayout& L, int n_words,
+                            SelShared& sh) {
+    const int R = L.R, rep = threadIdx.x & (R - 1);
+    uint32_t* hist = L.hist;
+    clear_hist(hist, R);
+    if (threadIdx.x == 0) sh.list_n = 0;
+    __syncthreads();
+    for_each_candidate<VEC>(s, lo, hi, L.mem, [&](int, uint32_t key) {
+        atomicAdd(&hist[(size_t)(kBins - 1 - (key >> 21)) * R + rep], 1u);   // bin 0 = largest keys
+    });
+    __syncthreads();
+    find_bin(hist, R, (uint32_t)rank, sh);
+    const uint32_t bin1 = sh.res_bin, rank1 = sh.res_rank, cnt1 = sh.res_cnt;
+    __syncthreads();
+    if (cnt1 > (uint32_t)L.cap) {   // threshold bin too large for the list: full-scan path
+        full_scan_tier(s, lo, hi, L.mem, n_words, rank, sh);
+        return;
+    }
+    // scan 2: admit above the threshold bin, compact the threshold bin (warp-aggregated append, any order)
+    const int lane = threadIdx.x & 31;
+    for_each_candidate<VEC>(s, lo, hi, L.mem, [&](int idx, uint32_t key) {
+        const uint32_t rb = kBins - 1 - (key >> 21);
+        if (rb < bin1) {
+            set_member(L.mem, idx);
+        } else if (rb == bin1) {
+            const uint32_t peers = __activemask();   // lanes appending together (any subset is correct)
+            const int leader = __ffs(peers) - 1;
+            uint32_t base = 0;
+            if (lane == leader) base = atomicAdd(&sh.list_n, (uint32_t)__popc(peers));
+            base = __shfl_sync(peers, base, leader);
+            const uint32_t pos = base + __popc(peers & ((1u << lane) - 1u));
+            L.list_key[pos] = key;
+            L.list_idx[pos] = (uint32_t)idx;
+        }
+    });
+    __syncthreads();
+    const int n_list = (int)sh.list_n;   // == cnt1
+    // digit 2: key bits 20..10 of the listed keys (short list: one histogram replica is enough from here on)
+    clear_hist(hist, 1);
+    __syncthreads();
+    for (int j = threadIdx.x; j < n_list; j += kSelThreads)
+        atomicAdd(&hist[kBins - 1 - ((L.list_key[j] >> 10) & 0x7ffu)], 1u);
+    __syncthreads();
+    find_bin(hist, 1, rank1, sh);
+    const uint32_t d2 = kBins - 1 - sh.res_bin, rank2 = sh.res_rank;
+    __syncthreads();
+    // digit 3: key bits 9..0 among the keys matching digit 2
+    clear_hist(hist, 1);
+    __syncthreads();
+    for (int j = threadIdx.x; j < n_list; j += kSelThreads) {
+        const uint32_t key = L.list_key[j];
+        if (((key >> 10) & 0x7ffu) == d2) atomicAdd(&hist[1023 - (key & 0x3ffu)], 1u);
+    }
+    __syncthreads();
+    find_bin(hist, 1, rank2, sh);
+    const uint32_t d3 = 1023 - sh.res_bin, need_eq = sh.res_rank, eq_total = sh.res_cnt;
+    __syncthreads();
+    const uint32_t T = ((uint32_t)(kBins - 1 - bin1) << 21) | (d2 << 10) | d3;
+    if (need_eq == eq_total) {   // every key equal to T is admitted: no order needed
+        for (int j = threadIdx.x; j < n_list; j += kSelThreads)
+            if (L.list_key[j] >= T) set_member(L.mem, (int)L.list_idx[j]);
+        __syncthreads();
+        return;
+    }
+    // Equal keys straddle the threshold: admit the need_eq lowest indices among them (indices < 2^20).
+    clear_hist(hist, 1);
+    __syncthreads();
+    for (int j = threadIdx.x; j < n_list; j += kSelThreads) {
+        const uint32_t key = L.list_key[j];
+        if (key > T) set_member(L.mem, (int)L.list_idx[j]);
+        if (key == T) atomicAdd(&hist[L.list_idx[j] >> 10], 1u);
+    }
+    __syncthreads();
+    find_bin(hist, 1, need_eq, sh);
+    const uint32_t i_hi = sh.res_bin, rank_lo = sh.res_rank;
+    __syncthreads();
+    clear_hist(hist, 1);
+    __syncthreads();
+    for (int j = threadIdx.x; j < n_list; j += kSelThreads)
+        if (L.list_key[j] == T && (L.list_idx[j] >> 10) == i_hi) atomicAdd(&hist[L.list_idx[j] & 0x3ffu], 1u);
+    __syncthreads();
+    find_bin(hist, 1, rank_lo, sh);
+    const uint32_t i_star = (i_hi << 10) | sh.res_bin;
+    __syncthreads();
+    for (int j = threadIdx.x; j < n_list; j += kSelThreads)
+        if (L.list_key[j] == T && L.list_idx[j] <= i_star) set_member(L.mem, (int)L.list_idx[j]);
+    __syncthreads();
+}
+
+template <bool VEC>
 __global__ void __launch_bounds__(kSelThreads) select_kernel(const SelectParams p) {
-    extern __shared__ uint32_t mem[];   // membership bitmask, ceil(max_ctx / 32) words
+    extern __shared__ __align__(16) uint32_t smem_dyn[];
     __shared__ SelShared sh;
     const int l = blockIdx.x, b = blockIdx.y;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int N = seq_len_of(p.seq_lens, b, p.max_ctx);
     const int k = p.budgets ? p.budgets[b] : p.budget;
     int* out = p.idx_out + ((long long)b * p.n_lists + l) * p.k_max;
@@ -156,6 +349,14 @@ __global__ void __launch_bounds__(kSelThreads) select_kernel(const SelectParams 
     const int n_words = (N + 31) >> 5;
     const float* sd = p.s_draft + (long long)b * p.draft_batch_stride + (long long)l * p.draft_list_stride;
     const float* st = p.s_target + ((long long)b * p.n_lists + l) * p.max_ctx;
+    SelLayout L;
+    L.mem = smem_dyn;
+    L.hist = smem_dyn + p.mask_words;
+    L.list_key = L.hist + (size_t)kBins * p.replicas;
+    L.list_idx = L.list_key + p.list_cap;
+    L.R = p.replicas;
+    L.cap = p.list_cap;
+    uint32_t* mem = L.mem;
 
     // I_prot = I_sink U I_window
     for (int w = threadIdx.x; w < n_words; w += kSelThreads) {
@@ -171,14 +372,11 @@ __global__ void __launch_bounds__(kSelThreads) select_kernel(const SelectParams 
     }
     __syncthreads();
 
-    int need_eq, eq_total;
-    if (m > 0) {        // I_draft = TopK(S_Draft \ I_prot, m)
-        const uint32_t T = radix_select(sd, lo, hi, mem, m, sh, need_eq, eq_total);
-        admit_tier(sd, lo, hi, mem, n_words, T, need_eq, eq_total, sh);
-    }
-    if (c - m > 0) {    // I_target = TopK(S_Target \ (I_prot U I_draft), k - m - |I_prot|)
-        const uint32_t T = radix_select(st, lo, hi, mem, c - m, sh, need_eq, eq_total);
-        admit_tier(st, lo, hi, mem, n_words, T, need_eq, eq_total, sh);
+    // tier 0: I_draft = TopK(S_Draft \ I_prot, m);  tier 1: I_target = TopK(S_Target \ (I_prot U I_draft), k-m-|I_prot|)
+#pragma unroll 1
+    for (int tier = 0; tier < 2; ++tier) {
+        const int want = tier == 0 ? m : c - m;
+        if (want > 0) select_tier<VEC>(tier == 0 ? sd : st, lo, hi, want, L, n_words, sh);
     }
 
     // I_verify in ascending order: prefix sum over the popcounts of the bitmask words.
@@ -199,22 +397,50 @@ __global__ void __launch_bounds__(kSelThreads) select_kernel(const SelectParams 
     }
     for (int i = (int)total + threadIdx.x; i < p.k_max; i += kSelThreads) out[i] = -1;
     if (threadIdx.x == 0) *cnt_out = (int)total;
-    (void)lane;
-    (void)warp;
 }
 
 }  // namespace
 
-size_t select_smem_bytes(int max_ctx) { return (size_t)((max_ctx + 31) / 32) * 4; }
+// Shared-memory plan: bitmask (max_ctx / 8 bytes) + kBins * R histogram counters + a 2 * cap word candidate list,
+// shrunk for very long rows so that everything fits the 227 KB of one SM.
+void select_plan(int max_ctx, int* mask_words, int* replicas, int* list_cap) {
+    *mask_words = ((max_ctx + 31) / 32 + 3) & ~3;
+    const size_t mask_bytes = (size_t)*mask_words * 4;
+    int R = 8, cap = 8192;
+    if (mask_bytes > 64 * 1024) R = 4, cap = 4096;   // rows beyond 512k tokens
+    *replicas = R;
+    *list_cap = cap;
+}
 
-cudaError_t launch_select(const SelectParams& p, cudaStream_t stream) {
+size_t select_smem_bytes(int max_ctx) {
+    int mw, R, cap;
+    select_plan(max_ctx, &mw, &R, &cap);
+    return ((size_t)mw + (size_t)kBins * R + 2 * (size_t)cap) * 4;
+}
+
+cudaError_t launch_select(const SelectParams& p_in, cudaStream_t stream) {
+    SelectParams p = p_in;
+    select_plan(p.max_ctx, &p.mask_words, &p.replicas, &p.list_cap);
     const size_t smem = select_smem_bytes(p.max_ctx);
-    if (smem > 48 * 1024) {
-        cudaError_t e = cudaFuncSetAttribute(select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    const bool vec = (p.max_ctx & 3) == 0 && (((uintptr_t)p.s_draft | (uintptr_t)p.s_target) & 15) == 0 &&
+                     (p.draft_batch_stride & 3) == 0 && (p.draft_list_stride & 3) == 0;
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaFuncAttributes fa;
+        cudaError_t e = cudaFuncGetAttributes(&fa, select_kernel<true>);
         if (e != cudaSuccess) return e;
+        const int max_smem = 227 * 1024 - (int)fa.sharedSizeBytes;   // opt-in limit counts static shared memory too
+        e = cudaFuncSetAttribute(select_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(select_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
     }
     ProfScope prof(kKernSelect, stream);
-    select_kernel<<<dim3(p.n_lists, p.batch), kSelThreads, smem, stream>>>(p);
+    if (vec)
+        select_kernel<true><<<dim3(p.n_lists, p.batch), kSelThreads, smem, stream>>>(p);
+    else
+        select_kernel<false><<<dim3(p.n_lists, p.batch), kSelThreads, smem, stream>>>(p);
     return cudaGetLastError();
 }
 
