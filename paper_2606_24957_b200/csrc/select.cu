@@ -21,7 +21,7 @@ struct SelShared {
     uint32_t hist[kBins];
     uint32_t warp_tot[kSelWarps + 1];
     uint32_t res_bin, res_rank, res_cnt;
-    uint32_t list_n;
+    uint32_t list_n, res_total;
 };
 
 // Exclusive prefix of v over the block in thread order; *total (optional) receives the block sum.
@@ -36,20 +36,15 @@ __device__ __forceinline__ uint32_t block_excl_scan(uint32_t v, SelShared& sh, u
     __syncthreads();   // protects warp_tot against the previous use
     if (lane == 31) sh.warp_tot[warp] = inc;
     __syncthreads();
-    if (warp == 0) {   // scan of the 32 warp totals: warp_tot[w] <- exclusive prefix, warp_tot[32] <- block sum
-        const uint32_t t = sh.warp_tot[lane];
-        uint32_t ti = t;
+    const uint32_t t = sh.warp_tot[lane];   // every warp scans the 32 warp totals redundantly
+    uint32_t ti = t;
 #pragma unroll
-        for (int off = 1; off < 32; off <<= 1) {
-            const uint32_t o = __shfl_up_sync(0xffffffffu, ti, off);
-            if (lane >= off) ti += o;
-        }
-        sh.warp_tot[lane] = ti - t;
-        if (lane == 31) sh.warp_tot[32] = ti;
+    for (int off = 1; off < 32; off <<= 1) {
+        const uint32_t o = __shfl_up_sync(0xffffffffu, ti, off);
+        if (lane >= off) ti += o;
     }
-    __syncthreads();
-    if (total) *total = sh.warp_tot[32];
-    return sh.warp_tot[warp] + inc - v;
+    if (total) *total = __shfl_sync(0xffffffffu, ti, 31);
+    return __shfl_sync(0xffffffffu, ti - t, warp) + inc - v;
 }
 
 // Key of descending rank `rank` (1-based) among the candidates n in [lo, hi) whose bit in `mem` is clear.
@@ -156,10 +151,16 @@ struct SelLayout {
     int R, cap;
 };
 
-// f(idx, key) for every candidate n in [lo, hi) whose membership bit is clear.  VEC: 16-byte loads (row aligned).
-template <bool VEC, typename F>
-__device__ __forceinline__ void for_each_candidate(const float* __restrict__ s, int lo, int hi, const uint32_t* mem,
-                                                   F f) {
+// Key of a score: the uint32 image of max(s, 0) (order-preserving for s >= 0; negatives and -0 tie at 0).
+__device__ __forceinline__ uint32_t key_max0(float s) { return __float_as_uint(fmaxf(s, 0.f)); }
+
+// Scan 1: histogram of the top 11 key bits over the candidates.  A candidate is an index of [lo, hi) whose bit in
+// `mem` is clear; every non-candidate index that a 16-byte load can touch (sink, window, tail of the last word)
+// has its bit set, so the bitmask alone decides.  hist_rep = hist + replica; bin 0 holds the largest keys.
+template <bool VEC>
+__device__ __forceinline__ void scan_hist(const float* __restrict__ s, int lo, int hi, const uint32_t* mem,
+                                          uint32_t* hist_rep, int R) {
+    uint32_t* top = hist_rep + (size_t)(kBins - 1) * R;
     if (VEC) {
         const float4* s4 = reinterpret_cast<const float4*>(s);
         const int v_end = (hi + 3) >> 2;
@@ -173,19 +174,106 @@ __device__ __forceinline__ void for_each_candidate(const float* __restrict__ s, 
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
                 const int n = (v + u * kSelThreads) << 2;
-                if (n >= hi) break;
-                const uint32_t nib = mem[n >> 5] >> (n & 31);
-                const float xs[4] = {x[u].x, x[u].y, x[u].z, x[u].w};
-#pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                    const int idx = n + e;
-                    if (idx >= lo && idx < hi && !((nib >> e) & 1u)) f(idx, key_of(xs[e]));
-                }
+                const uint32_t nib = n < hi ? mem[n >> 5] >> (n & 31) : 0xfu;
+                if (!(nib & 1u)) atomicAdd(top - (key_max0(x[u].x) >> 21) * R, 1u);
+                if (!(nib & 2u)) atomicAdd(top - (key_max0(x[u].y) >> 21) * R, 1u);
+                if (!(nib & 4u)) atomicAdd(top - (key_max0(x[u].z) >> 21) * R, 1u);
+                if (!(nib & 8u)) atomicAdd(top - (key_max0(x[u].w) >> 21) * R, 1u);
             }
         }
     } else {
         for (int n = lo + threadIdx.x; n < hi; n += kSelThreads)
-            if (!((mem[n >> 5] >> (n & 31)) & 1u)) f(n, key_of(__ldcg(s + n)));
+            if (!((mem[n >> 5] >> (n & 31)) & 1u)) atomicAdd(top - (key_max0(__ldcg(s + n)) >> 21) * R, 1u);
+    }
+}
+
+// Scan 2: candidates whose top key bits exceed t1 are admitted (their bits set in mem); those equal to t1 are
+// appended, in any order, to the (key, index) list.
+struct ListAppender {
+    uint32_t* key;
+    uint32_t* idx;
+    uint32_t* count;
+    uint32_t cap;   // entries beyond cap are counted but not stored (the caller then takes another path)
+    // One lane, any time (divergent callers): lanes that arrive together share one counter update.
+    __device__ __forceinline__ void operator()(uint32_t k, int i) const {
+        const uint32_t peers = __activemask();   // lanes appending together (any subset is correct)
+        const int lane = threadIdx.x & 31, leader = __ffs(peers) - 1;
+        uint32_t base = 0;
+        if (lane == leader) base = atomicAdd(count, (uint32_t)__popc(peers));
+        base = __shfl_sync(peers, base, leader);
+        const uint32_t pos = base + __popc(peers & ((1u << lane) - 1u));
+        if (pos < cap) {
+            key[pos] = k;
+            idx[pos] = (uint32_t)i;
+        }
+    }
+    // Whole warp, converged: lane holds 4 consecutive elements n..n+3, bit e of `hit` says element e is appended.
+    // One shared-memory counter update per warp call (only when some lane has a hit).
+    __device__ __forceinline__ void warp4(uint32_t hit, uint32_t k0, uint32_t k1, uint32_t k2, uint32_t k3,
+                                          int n) const {
+        const int lane = threadIdx.x & 31;
+        const uint32_t mine = __popc(hit & 0xfu);
+        if (!__any_sync(0xffffffffu, mine != 0)) return;
+        uint32_t inc = mine;   // inclusive prefix of the per-lane counts
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            const uint32_t o = __shfl_up_sync(0xffffffffu, inc, off);
+            if (lane >= off) inc += o;
+        }
+        uint32_t base = 0;
+        if (lane == 31) base = atomicAdd(count, inc);
+        base = __shfl_sync(0xffffffffu, base, 31);
+        uint32_t pos = base + inc - mine;
+        if (hit & 1u) { if (pos < cap) { key[pos] = k0; idx[pos] = (uint32_t)n; } ++pos; }
+        if (hit & 2u) { if (pos < cap) { key[pos] = k1; idx[pos] = (uint32_t)(n + 1); } ++pos; }
+        if (hit & 4u) { if (pos < cap) { key[pos] = k2; idx[pos] = (uint32_t)(n + 2); } ++pos; }
+        if (hit & 8u) { if (pos < cap) { key[pos] = k3; idx[pos] = (uint32_t)(n + 3); } ++pos; }
+    }
+};
+
+template <bool VEC>
+__device__ __forceinline__ void scan_admit(const float* __restrict__ s, int lo, int hi, uint32_t* mem, uint32_t t1,
+                                           const ListAppender& app) {
+    if (VEC) {
+        const float4* s4 = reinterpret_cast<const float4*>(s);
+        const int v_end = (hi + 3) >> 2;
+        // warp-uniform trip count: the list append below needs the whole warp converged
+        for (int vb = (lo >> 2) + (threadIdx.x & ~31); vb < v_end; vb += 4 * kSelThreads) {
+            const int v = vb + (threadIdx.x & 31);
+            float4 x[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int vv = v + u * kSelThreads;
+                x[u] = vv < v_end ? __ldcg(s4 + vv) : make_float4(0.f, 0.f, 0.f, 0.f);
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int n = (v + u * kSelThreads) << 2;
+                const uint32_t nib = n < hi ? mem[n >> 5] >> (n & 31) : 0xfu;
+                const uint32_t k0 = key_max0(x[u].x), k1 = key_max0(x[u].y), k2 = key_max0(x[u].z),
+                               k3 = key_max0(x[u].w);
+                uint32_t add = 0;
+                add |= ((k0 >> 21) > t1) ? 1u : 0u;
+                add |= ((k1 >> 21) > t1) ? 2u : 0u;
+                add |= ((k2 >> 21) > t1) ? 4u : 0u;
+                add |= ((k3 >> 21) > t1) ? 8u : 0u;
+                add &= ~nib;
+                if (add) atomicOr(&mem[n >> 5], add << (n & 31));
+                uint32_t eq = 0;
+                eq |= ((k0 >> 21) == t1) ? 1u : 0u;
+                eq |= ((k1 >> 21) == t1) ? 2u : 0u;
+                eq |= ((k2 >> 21) == t1) ? 4u : 0u;
+                eq |= ((k3 >> 21) == t1) ? 8u : 0u;
+                app.warp4(eq & ~nib, k0, k1, k2, k3, n);
+            }
+        }
+    } else {
+        for (int n = lo + threadIdx.x; n < hi; n += kSelThreads) {
+            if ((mem[n >> 5] >> (n & 31)) & 1u) continue;
+            const uint32_t k = key_max0(__ldcg(s + n));
+            if ((k >> 21) > t1) atomicOr(&mem[n >> 5], 1u << (n & 31));
+            if ((k >> 21) == t1) app(k, n);
+        }
     }
 }
 
@@ -195,102 +283,103 @@ __device__ __forceinline__ void clear_hist(uint32_t* hist, int R) {
     for (int i = threadIdx.x; i < kBins * R / 4; i += kSelThreads) h4[i] = make_uint4(0, 0, 0, 0);
 }
 
-__device__ __forceinline__ uint32_t bin_count(const uint32_t* hist, int R, int bin) {
-    if (R == 1) return hist[bin];
-    const uint4* h4 = reinterpret_cast<const uint4*>(hist + (size_t)bin * R);
-    uint32_t c = 0;
-    for (int r = 0; r < R / 4; ++r) {
-        const uint4 x = h4[r];
-        c += x.x + x.y + x.z + x.w;
-    }
-    return c;
-}
-
 // Bin holding rank `rank` (1-based, bins in ascending bin order); leaves (bin, rank inside the bin, bin count)
-// in sh.res_*.  Thread t owns bins t and t + 1024.  R in {1, 4, 8}.  Ends with a barrier.
+// in sh.res_*.  Thread t owns bins 2t and 2t + 1 (2R contiguous words).  R in {1, 4, 8}.  Ends with a barrier.
 __device__ __forceinline__ void find_bin(const uint32_t* hist, int R, uint32_t rank, SelShared& sh) {
-    const uint32_t c0 = bin_count(hist, R, threadIdx.x), c1 = bin_count(hist, R, threadIdx.x + kSelThreads);
-    uint32_t tot0;
-    const uint32_t e0 = block_excl_scan(c0, sh, &tot0);          // prefix over bins [0, 1024)
-    if (rank <= tot0) {
-        if (e0 < rank && rank <= e0 + c0) {
-            sh.res_bin = threadIdx.x;
-            sh.res_rank = rank - e0;
-            sh.res_cnt = c0;
-        }
+    uint32_t c0 = 0, c1 = 0;
+    if (R == 1) {
+        const uint2 x = reinterpret_cast<const uint2*>(hist)[threadIdx.x];
+        c0 = x.x;
+        c1 = x.y;
     } else {
-        const uint32_t e1 = tot0 + block_excl_scan(c1, sh, nullptr);   // block-uniform branch
-        if (e1 < rank && rank <= e1 + c1) {
-            sh.res_bin = threadIdx.x + kSelThreads;
-            sh.res_rank = rank - e1;
-            sh.res_cnt = c1;
+        const uint4* h4 = reinterpret_cast<const uint4*>(hist + (size_t)(2 * threadIdx.x) * R);
+        const int q = R / 4;
+        for (int r = 0; r < q; ++r) {
+            const uint4 a = h4[r], b = h4[q + r];
+            c0 += a.x + a.y + a.z + a.w;
+            c1 += b.x + b.y + b.z + b.w;
         }
+    }
+    uint32_t total;
+    const uint32_t excl = block_excl_scan(c0 + c1, sh, &total);
+    if (threadIdx.x == 0) sh.res_total = total;
+    if (excl < rank && rank <= excl + c0) {
+        sh.res_bin = 2 * threadIdx.x;
+        sh.res_rank = rank - excl;
+        sh.res_cnt = c0;
+    } else if (excl + c0 < rank && rank <= excl + c0 + c1) {
+        sh.res_bin = 2 * threadIdx.x + 1;
+        sh.res_rank = rank - excl - c0;
+        sh.res_cnt = c1;
     }
     __syncthreads();
 }
 
 __device__ __forceinline__ void set_member(uint32_t* mem, int idx) { atomicOr(&mem[idx >> 5], 1u << (idx & 31)); }
 
-// One tier of Eq. 6: admits into `mem` the `rank` best candidates of [lo, hi) by s (ties -> lower index).
+// Scan of the sampled path: every candidate whose top 11 key bits are >= tau_top is appended to the list.
 template <bool VEC>
-__device__ void select_tier(const float* __restrict__ s, int lo, int hi, int rank, const SelLayout& L, int n_words,
-                            SelShared& sh) {
-    const int R = L.R, rep = threadIdx.x & (R - 1);
-    uint32_t* hist = L.hist;
-    clear_hist(hist, R);
-    if (threadIdx.x == 0) sh.list_n = 0;
-    __syncthreads();
-    for_each_candidate<VEC>(s, lo, hi, L.mem, [&](int, uint32_t key) {
-        atomicAdd(&hist[(size_t)(kBins - 1 - (key >> 21)) * R + rep], 1u);   // bin 0 = largest keys
-    });
-    __syncthreads();
-    find_bin(hist, R, (uint32_t)rank, sh);
-    const uint32_t bin1 = sh.res_bin, rank1 = sh.res_rank, cnt1 = sh.res_cnt;
-    __syncthreads();
-    if (cnt1 > (uint32_t)L.cap) {   // threshold bin too large for the list: full-scan path
-        full_scan_tier(s, lo, hi, L.mem, n_words, rank, sh);
-        return;
-    }
-    // scan 2: admit above the threshold bin, compact the threshold bin (warp-aggregated append, any order)
-    const int lane = threadIdx.x & 31;
-    for_each_candidate<VEC>(s, lo, hi, L.mem, [&](int idx, uint32_t key) {
-        const uint32_t rb = kBins - 1 - (key >> 21);
-        if (rb < bin1) {
-            set_member(L.mem, idx);
-        } else if (rb == bin1) {
-            const uint32_t peers = __activemask();   // lanes appending together (any subset is correct)
-            const int leader = __ffs(peers) - 1;
-            uint32_t base = 0;
-            if (lane == leader) base = atomicAdd(&sh.list_n, (uint32_t)__popc(peers));
-            base = __shfl_sync(peers, base, leader);
-            const uint32_t pos = base + __popc(peers & ((1u << lane) - 1u));
-            L.list_key[pos] = key;
-            L.list_idx[pos] = (uint32_t)idx;
+__device__ __forceinline__ void scan_collect(const float* __restrict__ s, int lo, int hi, const uint32_t* mem,
+                                             uint32_t tau_top, const ListAppender& app) {
+    if (VEC) {
+        const float4* s4 = reinterpret_cast<const float4*>(s);
+        const int v_end = (hi + 3) >> 2;
+        // warp-uniform trip count: the list append below needs the whole warp converged
+        for (int vb = (lo >> 2) + (threadIdx.x & ~31); vb < v_end; vb += 4 * kSelThreads) {
+            const int v = vb + (threadIdx.x & 31);
+            float4 x[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int vv = v + u * kSelThreads;
+                x[u] = vv < v_end ? __ldcg(s4 + vv) : make_float4(0.f, 0.f, 0.f, 0.f);
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int n = (v + u * kSelThreads) << 2;
+                const uint32_t k0 = key_max0(x[u].x), k1 = key_max0(x[u].y), k2 = key_max0(x[u].z),
+                               k3 = key_max0(x[u].w);
+                uint32_t hit = 0;
+                hit |= ((k0 >> 21) >= tau_top) ? 1u : 0u;
+                hit |= ((k1 >> 21) >= tau_top) ? 2u : 0u;
+                hit |= ((k2 >> 21) >= tau_top) ? 4u : 0u;
+                hit |= ((k3 >> 21) >= tau_top) ? 8u : 0u;
+                if (hit) hit &= n < hi ? ~(mem[n >> 5] >> (n & 31)) : 0u;
+                app.warp4(hit, k0, k1, k2, k3, n);
+            }
         }
-    });
-    __syncthreads();
-    const int n_list = (int)sh.list_n;   // == cnt1
-    // digit 2: key bits 20..10 of the listed keys (short list: one histogram replica is enough from here on)
-    clear_hist(hist, 1);
-    __syncthreads();
-    for (int j = threadIdx.x; j < n_list; j += kSelThreads)
-        atomicAdd(&hist[kBins - 1 - ((L.list_key[j] >> 10) & 0x7ffu)], 1u);
-    __syncthreads();
-    find_bin(hist, 1, rank1, sh);
-    const uint32_t d2 = kBins - 1 - sh.res_bin, rank2 = sh.res_rank;
-    __syncthreads();
-    // digit 3: key bits 9..0 among the keys matching digit 2
-    clear_hist(hist, 1);
-    __syncthreads();
-    for (int j = threadIdx.x; j < n_list; j += kSelThreads) {
-        const uint32_t key = L.list_key[j];
-        if (((key >> 10) & 0x7ffu) == d2) atomicAdd(&hist[1023 - (key & 0x3ffu)], 1u);
+    } else {
+        for (int n = lo + threadIdx.x; n < hi; n += kSelThreads) {
+            const uint32_t k = key_max0(__ldcg(s + n));
+            if ((k >> 21) >= tau_top && !((mem[n >> 5] >> (n & 31)) & 1u)) app(k, n);
+        }
     }
-    __syncthreads();
-    find_bin(hist, 1, rank2, sh);
-    const uint32_t d3 = 1023 - sh.res_bin, need_eq = sh.res_rank, eq_total = sh.res_cnt;
-    __syncthreads();
-    const uint32_t T = ((uint32_t)(kBins - 1 - bin1) << 21) | (d2 << 10) | d3;
+}
+
+// Exact selection on the candidate list: admits the `rank` best of the n_list entries (key descending, ties toward
+// the lower index).  first_pass = 0: all 32 key bits are resolved here; 1: the entries share their top 11 bits.
+__device__ void list_select(const SelLayout& L, int n_list, uint32_t rank, int first_pass, uint32_t prefix,
+                            SelShared& sh) {
+    uint32_t* hist = L.hist;
+    uint32_t eq_total = 0;
+#pragma unroll 1
+    for (int pass = first_pass; pass < 3; ++pass) {
+        const int shift = pass == 0 ? 21 : (pass == 1 ? 10 : 0);
+        const uint32_t nb = pass == 2 ? 1024u : 2048u;
+        const int hs = pass == 1 ? 21 : 10;   // bits above the digit (pass 0 has none)
+        clear_hist(hist, 1);
+        __syncthreads();
+        for (int j = threadIdx.x; j < n_list; j += kSelThreads) {
+            const uint32_t key = L.list_key[j];
+            if (pass == 0 || (key >> hs) == (prefix >> hs)) atomicAdd(&hist[nb - 1 - ((key >> shift) & (nb - 1))], 1u);
+        }
+        __syncthreads();
+        find_bin(hist, 1, rank, sh);
+        prefix |= (nb - 1 - sh.res_bin) << shift;
+        rank = sh.res_rank;
+        eq_total = sh.res_cnt;
+        __syncthreads();
+    }
+    const uint32_t T = prefix, need_eq = rank;
     if (need_eq == eq_total) {   // every key equal to T is admitted: no order needed
         for (int j = threadIdx.x; j < n_list; j += kSelThreads)
             if (L.list_key[j] >= T) set_member(L.mem, (int)L.list_idx[j]);
@@ -320,6 +409,66 @@ __device__ void select_tier(const float* __restrict__ s, int lo, int hi, int ran
     for (int j = threadIdx.x; j < n_list; j += kSelThreads)
         if (L.list_key[j] == T && L.list_idx[j] <= i_star) set_member(L.mem, (int)L.list_idx[j]);
     __syncthreads();
+}
+
+// One tier of Eq. 6: admits into `mem` the `rank` best candidates of [lo, hi) by s (ties -> lower index).
+//  (1) sampled path: 1024 strided samples give a conservative threshold on the top 11 key bits; one scan compacts
+//      every candidate at or above it into the list; if the list holds >= rank entries (and fits) the exact answer
+//      is selected from the list alone.  The sample only decides which path runs, never the result.
+//  (2) histogram path: full histogram of the top 11 bits, second scan admits / compacts the threshold bin.
+//  (3) full-scan path for a threshold bin larger than the list (massive ties).
+template <bool VEC>
+__device__ void select_tier(const float* __restrict__ s, int lo, int hi, int rank, const SelLayout& L, int n_words,
+                            SelShared& sh) {
+    const int R = L.R, rep = threadIdx.x & (R - 1);
+    uint32_t* hist = L.hist;
+    const ListAppender app{L.list_key, L.list_idx, &sh.list_n, (uint32_t)L.cap};
+    const int n_cand = hi - lo;
+    // ---- (1) sampled threshold ----
+    {
+        clear_hist(hist, 1);
+        if (threadIdx.x == 0) sh.list_n = 0;
+        __syncthreads();
+        const int stride = max(1, n_cand / kSelThreads);
+        const int n_slots = min(kSelThreads, (n_cand + stride - 1) / stride);
+        const int pos = lo + threadIdx.x * stride;
+        if (threadIdx.x < n_slots && !((L.mem[pos >> 5] >> (pos & 31)) & 1u))
+            atomicAdd(&hist[kBins - 1 - (key_max0(__ldcg(s + pos)) >> 21)], 1u);
+        __syncthreads();
+        // sample rank that the true rank-th key exceeds with overwhelming probability (mean * 1.25 + 3.5 sigma + 4)
+        const float mean = (float)n_slots * (float)rank / (float)n_cand;
+        const uint32_t j = (uint32_t)(mean * 1.25f + 3.5f * sqrtf(mean) + 4.f);
+        uint32_t tau_top = 0;
+        find_bin(hist, 1, j, sh);
+        if (j <= sh.res_total) tau_top = (uint32_t)(kBins - 1) - sh.res_bin;
+        __syncthreads();
+        scan_collect<VEC>(s, lo, hi, L.mem, tau_top, app);
+        __syncthreads();
+        const uint32_t n_list = sh.list_n;
+        if (n_list >= (uint32_t)rank && n_list <= (uint32_t)L.cap) {
+            list_select(L, (int)n_list, (uint32_t)rank, 0, 0u, sh);
+            return;
+        }
+        __syncthreads();
+    }
+    // ---- (2) histogram of the top 11 key bits ----
+    clear_hist(hist, R);
+    if (threadIdx.x == 0) sh.list_n = 0;
+    __syncthreads();
+    scan_hist<VEC>(s, lo, hi, L.mem, hist + rep, R);
+    __syncthreads();
+    find_bin(hist, R, (uint32_t)rank, sh);
+    const uint32_t bin1 = sh.res_bin, rank1 = sh.res_rank, cnt1 = sh.res_cnt;
+    __syncthreads();
+    if (cnt1 > (uint32_t)L.cap) {   // ---- (3) threshold bin too large for the list ----
+        full_scan_tier(s, lo, hi, L.mem, n_words, rank, sh);
+        return;
+    }
+    // scan 2: admit above the threshold bin, compact the threshold bin (warp-aggregated append, any order)
+    const uint32_t t1 = (uint32_t)(kBins - 1) - bin1;
+    scan_admit<VEC>(s, lo, hi, L.mem, t1, app);
+    __syncthreads();
+    list_select(L, (int)sh.list_n, rank1, 1, t1 << 21, sh);
 }
 
 template <bool VEC>
@@ -357,16 +506,14 @@ __global__ void __launch_bounds__(kSelThreads) select_kernel(const SelectParams 
     L.R = p.replicas;
     L.cap = p.list_cap;
     uint32_t* mem = L.mem;
-
     // I_prot = I_sink U I_window
     for (int w = threadIdx.x; w < n_words; w += kSelThreads) {
         uint32_t bits = 0;
         const int n0 = w * 32;
         if (n0 < S) bits |= (S - n0 >= 32) ? 0xffffffffu : ((1u << (S - n0)) - 1u);
-        if (n0 + 32 > hi) {
-            const int from = max(hi - n0, 0), to = min(N - n0, 32);   // bits [from, to)
-            const uint32_t upto = to >= 32 ? 0xffffffffu : ((1u << to) - 1u);
-            bits |= upto & ~((1u << from) - 1u);
+        if (n0 + 32 > hi) {   // window [hi, N) and, for now, the tail [N, 32 * n_words) of the last word
+            const int from = max(hi - n0, 0);
+            bits |= ~((1u << from) - 1u);
         }
         mem[w] = bits;
     }
@@ -378,7 +525,8 @@ __global__ void __launch_bounds__(kSelThreads) select_kernel(const SelectParams 
         const int want = tier == 0 ? m : c - m;
         if (want > 0) select_tier<VEC>(tier == 0 ? sd : st, lo, hi, want, L, n_words, sh);
     }
-
+    if (threadIdx.x == 0 && (N & 31)) mem[n_words - 1] &= (1u << (N & 31)) - 1u;   // drop the tail bits >= N
+    __syncthreads();
     // I_verify in ascending order: prefix sum over the popcounts of the bitmask words.
     const int wpt = (n_words + kSelThreads - 1) / kSelThreads;   // consecutive words per thread
     const int w_lo = threadIdx.x * wpt, w_hi = min(w_lo + wpt, n_words);
