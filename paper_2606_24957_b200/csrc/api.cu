@@ -136,14 +136,11 @@ struct AttnWs {
     int split_tokens, n_splits;
 };
 AttnWs attn_ws(const dustin_shape_t* s, int max_tokens) {
+    // The split partials are combined through distributed shared memory inside the cluster (attn.cu): the
+    // attention stage needs no global scratch.
     AttnWs w;
     attn_plan(s->batch, s->n_kv_heads, max_tokens, &w.split_tokens, &w.n_splits);
-    const size_t rows = (size_t)s->n_new * (s->n_q_heads / s->n_kv_heads);
-    const size_t units = (size_t)s->batch * s->n_kv_heads * w.n_splits * rows;
-    w.part_o = 0;
-    w.part_lse = align256(units * s->head_dim * sizeof(float));
-    w.total = align256(w.part_lse + units * sizeof(float));
-    if (w.n_splits == 1) w.part_lse = w.total = 0;
+    w.part_o = w.part_lse = w.total = 0;
     return w;
 }
 

@@ -1,15 +1,23 @@
 // attn.cu -- stage a4 (sparse verification attention over the selected KV, App. G :568) and a5
 // (the full-cache verification baseline of PAPER.md:248 / :570: same kernel, idx == nullptr) for sm_100a.
 //
-// Flash-style, index-driven, split over the selected tokens:
-//   grid = (n_splits, Hkv, B); a CTA owns `split_tokens` entries of the index list of (b, KV head) -- split 0
-//   also owns the T new draft rows (causal among themselves).  Row offsets are resolved once into shared memory
-//   (index -> page table -> element offset); K/V rows then stream global -> shared with 16-byte cp.async through
-//   a 3-stage ring (XOR-swizzled, ldmatrix-conflict-free).  All T*r query rows that share the KV head sit on the
-//   M axis of bf16 mma.sync tiles (warp = one 16-row tile x one token slice), fp32 online softmax in the log2
-//   domain, P re-used from the accumulator registers as the A operand of P.V.  Token slices of a CTA merge in
-//   shared memory; CTAs of one (b, KV head) merge in attn_combine_kernel (n_splits > 1).
+// Flash-style, index-driven, split over the selected tokens, one thread-block CLUSTER per (sequence, KV head):
+//   grid = (n_splits, Hkv, B), cluster = (n_splits, 1, 1).  CTA `split` owns a contiguous slice of the index list
+//   of (b, KV head); split 0 also owns the T new draft rows (causal among themselves).
+//   * Row addresses are resolved once (index -> page table -> global address of the K row and of the V row) into
+//     a shared-memory table; K/V rows then stream global -> shared with 16-byte cp.async, 16 lanes per 256-byte
+//     row, through a 3-stage ring of 64-token tiles (XOR-swizzled, ldmatrix-conflict-free).
+//   * All T*r query rows that share the KV head sit on the M axis of bf16 mma.sync tiles (warp = one 16-row tile x
+//     one token slice), fp32 online softmax in the log2 domain with the scale folded into the exponent, the O
+//     rescale skipped while no row maximum moves, P re-used from the accumulator registers as the A operand of P.V.
+//   * Token slices of a CTA merge in shared memory; the CTAs of a cluster leave their normalised partial in their
+//     own shared memory and every CTA finishes a share of the query rows by reading its peers through DSMEM
+//     (fixed split order => deterministic).  No partials in global memory, no second kernel.
 #include "kernels.cuh"
+
+#include <cooperative_groups.h>
+
+namespace cg = cooperative_groups;
 
 namespace dustin {
 
@@ -17,28 +25,40 @@ namespace {
 
 constexpr int kTileTokens = 64;   // tokens per pipeline stage
 constexpr int kStages = 3;
-constexpr int kMaxSplitTokens = 4096;
+constexpr int kMaxCluster = 8;    // portable cluster size
+constexpr int kMaxTableTokens = 1024 + 16;   // address-table entries that still leave room for 2 CTAs per SM
+
+enum AttnMode { kDense = 0, kGatherTable = 1, kGatherInline = 2 };
 
 template <int D, int MT, int KS>
 struct AttnCfg {
     static constexpr int kThreads = 32 * MT * KS;
     static constexpr int kWT = kTileTokens / KS;          // tokens per warp per stage
     static constexpr int kCH = D / 8;                     // 16-byte chunks per row
-    static constexpr int kStageElems = kTileTokens * D;   // bf16 elements per K (or V) stage
+    static constexpr int kRowBytes = D * 2;
+    static constexpr int kStageBytes = kTileTokens * kRowBytes;   // one K (or V) stage
     static constexpr int kOReg = D / 2;                   // fp32 accumulators per thread (16 x D tile)
-    static constexpr size_t kPipeBytes = (size_t)kStages * kStageElems * 2 * 2;
+    static constexpr size_t kPipeBytes = (size_t)kStages * kStageBytes * 2;
     static constexpr size_t kMergeBytes = (size_t)(KS - 1) * MT * 32 * (kOReg + 4) * 4;
+    static constexpr size_t kPartBytes = (size_t)MT * 16 * (D + 1) * 4;   // cluster partial: o[rows][D] + lse[rows]
+    static_assert(kMergeBytes + kPartBytes <= kPipeBytes, "epilogue buffers must fit the pipeline buffers");
+    static constexpr int kRowsPerPass = kThreads / kCH;   // rows one cp.async pass of the CTA covers
+    static constexpr int kPasses = (kTileTokens + kRowsPerPass - 1) / kRowsPerPass;
 };
 
-template <int D, int MT, int KS>
+struct RowAddr {
+    const __nv_bfloat16* k;
+    const __nv_bfloat16* v;
+};
+
+template <int D, int MT, int KS, int MODE>
 __global__ void __launch_bounds__(32 * MT * KS) attn_kernel(const AttnParams p) {
     using C = AttnCfg<D, MT, KS>;
     constexpr int WT = C::kWT, CH = C::kCH, NT = C::kThreads;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    __nv_bfloat16* sK = reinterpret_cast<__nv_bfloat16*>(smem_raw);
-    __nv_bfloat16* sV = sK + kStages * C::kStageElems;
-    long long* sOff = reinterpret_cast<long long*>(smem_raw + (C::kPipeBytes > C::kMergeBytes ? C::kPipeBytes
-                                                                                             : C::kMergeBytes));
+    unsigned char* sK = smem_raw;
+    unsigned char* sV = smem_raw + kStages * C::kStageBytes;
+    RowAddr* sTab = reinterpret_cast<RowAddr*>(smem_raw + C::kPipeBytes);
 
     const int split = blockIdx.x, gkv = blockIdx.y, b = blockIdx.z;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -46,25 +66,29 @@ __global__ void __launch_bounds__(32 * MT * KS) attn_kernel(const AttnParams p) 
     const int g = lane >> 2, c = lane & 3;
     const int T = p.n_new, r = p.group, rows = p.rows;
     const int list = p.n_lists == 1 ? 0 : gkv;
-    const int n_sel = p.idx ? p.cnt[b * p.n_lists + list] : seq_len_of(p.kv.seq_lens, b, p.max_ctx);
+    const int n_sel = MODE == kDense ? seq_len_of(p.kv.seq_lens, b, p.max_ctx) : p.cnt[b * p.n_lists + list];
     const int range_lo = split * p.split_tokens;
     const int n_range = max(0, min(p.split_tokens, n_sel - range_lo));
     const int nt = n_range + (split == 0 ? T : 0);        // this CTA's tokens: cache rows, then the new rows
+    const int* list_idx = MODE == kDense ? nullptr : p.idx + ((long long)b * p.n_lists + list) * p.k_max + range_lo;
 
-    // ---- row offsets (elements): >= 0 in the cache, -(1 + off) in k_new / v_new --------------------------------
-    {
-        const int* list_idx = p.idx ? p.idx + ((long long)b * p.n_lists + list) * p.k_max + range_lo : nullptr;
-        for (int j = tid; j < nt; j += NT) {
-            long long off;
-            if (j < n_range) {
-                const int tok = list_idx ? __ldg(list_idx + j) : range_lo + j;
-                off = kv_row_offset(p.kv, b, tok, gkv);
-            } else {
-                off = -1 - (((long long)b * T + (j - n_range)) * p.n_kv_heads + gkv) * D;
-            }
-            sOff[j] = off;
+    // Global addresses of the K and V row of local token j.
+    auto row_addr = [&](int j) -> RowAddr {
+        RowAddr a;
+        if (j < n_range) {
+            const int tok = MODE == kDense ? range_lo + j : __ldg(list_idx + j);
+            const long long off = kv_row_offset(p.kv, b, tok, gkv);
+            a.k = p.kv.k + off;
+            a.v = p.kv.v + off;
+        } else {
+            const long long off = (((long long)b * T + (j - n_range)) * p.n_kv_heads + gkv) * D;
+            a.k = p.k_new + off;
+            a.v = p.v_new + off;
         }
-    }
+        return a;
+    };
+    if (MODE == kGatherTable)
+        for (int j = tid; j < nt; j += NT) sTab[j] = row_addr(j);
 
     // ---- Q fragments (A operand): rows mt*16 + g (+8), row = t*r + head-in-group -------------------------------
     uint32_t qa[D / 16][4];
@@ -85,22 +109,29 @@ __global__ void __launch_bounds__(32 * MT * KS) attn_kernel(const AttnParams p) 
     }
     __syncthreads();
 
+    // ---- producer side: this thread copies chunk `ld_ch` of rows ld_row0, ld_row0 + kRowsPerPass, ... per tile --
     const int n_tiles = (nt + kTileTokens - 1) / kTileTokens;
+    const int ld_ch = tid % CH, ld_row0 = tid / CH;
+    const uint32_t sK_u32 = smem_u32(sK), sV_u32 = smem_u32(sV);
     auto issue = [&](int tile) {
         if (tile < n_tiles) {
-            const int slot = tile % kStages;
-#pragma unroll 4
-            for (int i = tid; i < 2 * kTileTokens * CH; i += NT) {
-                const int which = i / (kTileTokens * CH);
-                const int rem = i - which * (kTileTokens * CH);
-                const int row = rem / CH, ch = rem % CH;
-                const int j = tile * kTileTokens + row;
+            const uint32_t stage_off = (uint32_t)(tile % kStages) * C::kStageBytes;
+            const int j0 = tile * kTileTokens;
+#pragma unroll
+            for (int i = 0; i < C::kPasses; ++i) {
+                const int row = ld_row0 + i * C::kRowsPerPass;
+                if (C::kPasses * C::kRowsPerPass > kTileTokens && row >= kTileTokens) break;
+                const int j = j0 + row;
                 const bool valid = j < nt;
-                const long long off = valid ? sOff[j] : 0;
-                const __nv_bfloat16* base = which ? (off >= 0 ? p.kv.v : p.v_new) : (off >= 0 ? p.kv.k : p.k_new);
-                const __nv_bfloat16* src = base + (off >= 0 ? off : -1 - off) + ch * 8;
-                __nv_bfloat16* dst = (which ? sV : sK) + slot * C::kStageElems + row * D + ((ch ^ (row & 7)) << 3);
-                cp_async16(smem_u32(dst), src, valid ? 16 : 0);
+                RowAddr a;
+                if (MODE == kGatherTable) {
+                    a = sTab[valid ? j : 0];
+                } else {
+                    a = row_addr(valid ? j : 0);
+                }
+                const uint32_t dst = stage_off + (uint32_t)row * C::kRowBytes + (uint32_t)((ld_ch ^ (row & 7)) << 4);
+                cp_async16(sK_u32 + dst, a.k + ld_ch * 8, valid ? 16 : 0);
+                cp_async16(sV_u32 + dst, a.v + ld_ch * 8, valid ? 16 : 0);
             }
         }
         cp_async_commit();
@@ -109,8 +140,10 @@ __global__ void __launch_bounds__(32 * MT * KS) attn_kernel(const AttnParams p) 
     float o[D / 8][4];
 #pragma unroll
     for (int i = 0; i < D / 8; ++i) o[i][0] = o[i][1] = o[i][2] = o[i][3] = 0.f;
+    // running maxima of the raw scores (q.k, unscaled) and running sums of exp2((s - m) * scale_log2)
     float m_lo = -INFINITY, m_hi = -INFINITY, l_lo = 0.f, l_hi = 0.f;
     const int t_lo = (mt * 16 + g) / r, t_hi = (mt * 16 + g + 8) / r;   // verify position of this thread's rows
+    const float sl2 = p.scale_log2;
 
 #pragma unroll
     for (int s = 0; s < kStages - 1; ++s) issue(s);
@@ -121,8 +154,8 @@ __global__ void __launch_bounds__(32 * MT * KS) attn_kernel(const AttnParams p) 
         issue(tile + kStages - 1);
         const int j0 = tile * kTileTokens + ks * WT;       // first token of this warp's slice
         if (j0 >= nt) continue;
-        const __nv_bfloat16* tK = sK + (tile % kStages) * C::kStageElems;
-        const __nv_bfloat16* tV = sV + (tile % kStages) * C::kStageElems;
+        const uint32_t tK = sK_u32 + (tile % kStages) * C::kStageBytes;
+        const uint32_t tV = sV_u32 + (tile % kStages) * C::kStageBytes;
 
         // S = Q K^T
         float sc[WT / 8][4];
@@ -136,27 +169,28 @@ __global__ void __launch_bounds__(32 * MT * KS) attn_kernel(const AttnParams p) 
                 const int row = ks * WT + np * 16 + (mi >> 1) * 8 + (lane & 7);
                 const int ch = kk * 2 + (mi & 1);
                 uint32_t b0, b1, b2, b3;
-                ldmatrix_x4(b0, b1, b2, b3, smem_u32(tK + row * D + ((ch ^ (row & 7)) << 3)));
+                ldmatrix_x4(b0, b1, b2, b3, tK + row * C::kRowBytes + ((ch ^ (row & 7)) << 4));
                 mma_bf16_16816(sc[2 * np], qa[kk][0], qa[kk][1], qa[kk][2], qa[kk][3], b0, b1);
                 mma_bf16_16816(sc[2 * np + 1], qa[kk][0], qa[kk][1], qa[kk][2], qa[kk][3], b2, b3);
             }
         }
 
-        // scale, mask (tail of the list; causality among the new rows), online softmax in the log2 domain
-        const bool need_mask = j0 + WT > n_range;
+        // mask (tail of the list; causality among the new rows) -- only the tiles that reach past the cache rows
+        if (j0 + WT > n_range) {
+#pragma unroll
+            for (int i = 0; i < WT / 8; ++i) {
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const int j = j0 + i * 8 + 2 * c + (e & 1);
+                    const int t = (e & 2) ? t_hi : t_lo;
+                    if (j >= nt || (j >= n_range && j - n_range > t)) sc[i][e] = -INFINITY;
+                }
+            }
+        }
+        // online softmax: p = exp2((s - m) * scale_log2)
         float mx_lo = -INFINITY, mx_hi = -INFINITY;
 #pragma unroll
         for (int i = 0; i < WT / 8; ++i) {
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                float v = sc[i][e] * p.scale_log2;
-                if (need_mask) {
-                    const int j = j0 + i * 8 + 2 * c + (e & 1);
-                    const int t = (e & 2) ? t_hi : t_lo;
-                    if (j >= nt || (j >= n_range && j - n_range > t)) v = -INFINITY;
-                }
-                sc[i][e] = v;
-            }
             mx_lo = fmaxf(mx_lo, fmaxf(sc[i][0], sc[i][1]));
             mx_hi = fmaxf(mx_hi, fmaxf(sc[i][2], sc[i][3]));
         }
@@ -164,30 +198,36 @@ __global__ void __launch_bounds__(32 * MT * KS) attn_kernel(const AttnParams p) 
         mx_lo = fmaxf(mx_lo, __shfl_xor_sync(0xffffffffu, mx_lo, 2));
         mx_hi = fmaxf(mx_hi, __shfl_xor_sync(0xffffffffu, mx_hi, 1));
         mx_hi = fmaxf(mx_hi, __shfl_xor_sync(0xffffffffu, mx_hi, 2));
-        const float mn_lo = fmaxf(m_lo, mx_lo), mn_hi = fmaxf(m_hi, mx_hi);
-        const float mu_lo = mn_lo == -INFINITY ? 0.f : mn_lo, mu_hi = mn_hi == -INFINITY ? 0.f : mn_hi;
-        const float al_lo = fast_exp2(m_lo - mu_lo), al_hi = fast_exp2(m_hi - mu_hi);
-        m_lo = mn_lo;
-        m_hi = mn_hi;
+        const bool moved = mx_lo > m_lo || mx_hi > m_hi;
+        if (__any_sync(0xffffffffu, moved)) {   // some row maximum of this warp moved: rescale O and the sums
+            const float mn_lo = fmaxf(m_lo, mx_lo), mn_hi = fmaxf(m_hi, mx_hi);
+            const float al_lo = mn_lo == -INFINITY ? 1.f : fast_exp2((m_lo - mn_lo) * sl2);
+            const float al_hi = mn_hi == -INFINITY ? 1.f : fast_exp2((m_hi - mn_hi) * sl2);
+            m_lo = mn_lo;
+            m_hi = mn_hi;
+            l_lo *= al_lo;
+            l_hi *= al_hi;
+#pragma unroll
+            for (int i = 0; i < D / 8; ++i) {
+                o[i][0] *= al_lo;
+                o[i][1] *= al_lo;
+                o[i][2] *= al_hi;
+                o[i][3] *= al_hi;
+            }
+        }
+        const float ms_lo = m_lo == -INFINITY ? 0.f : m_lo * sl2, ms_hi = m_hi == -INFINITY ? 0.f : m_hi * sl2;
         float sum_lo = 0.f, sum_hi = 0.f;
 #pragma unroll
         for (int i = 0; i < WT / 8; ++i) {
-            sc[i][0] = fast_exp2(sc[i][0] - mu_lo);
-            sc[i][1] = fast_exp2(sc[i][1] - mu_lo);
-            sc[i][2] = fast_exp2(sc[i][2] - mu_hi);
-            sc[i][3] = fast_exp2(sc[i][3] - mu_hi);
+            sc[i][0] = fast_exp2(fmaf(sc[i][0], sl2, -ms_lo));
+            sc[i][1] = fast_exp2(fmaf(sc[i][1], sl2, -ms_lo));
+            sc[i][2] = fast_exp2(fmaf(sc[i][2], sl2, -ms_hi));
+            sc[i][3] = fast_exp2(fmaf(sc[i][3], sl2, -ms_hi));
             sum_lo += sc[i][0] + sc[i][1];
             sum_hi += sc[i][2] + sc[i][3];
         }
-        l_lo = l_lo * al_lo + sum_lo;
-        l_hi = l_hi * al_hi + sum_hi;
-#pragma unroll
-        for (int i = 0; i < D / 8; ++i) {
-            o[i][0] *= al_lo;
-            o[i][1] *= al_lo;
-            o[i][2] *= al_hi;
-            o[i][3] *= al_hi;
-        }
+        l_lo += sum_lo;
+        l_hi += sum_hi;
 
         // O += P V
 #pragma unroll
@@ -202,7 +242,7 @@ __global__ void __launch_bounds__(32 * MT * KS) attn_kernel(const AttnParams p) 
                 const int row = ks * WT + kk * 16 + (mi & 1) * 8 + (lane & 7);
                 const int ch = dp * 2 + (mi >> 1);
                 uint32_t b0, b1, b2, b3;
-                ldmatrix_x4_trans(b0, b1, b2, b3, smem_u32(tV + row * D + ((ch ^ (row & 7)) << 3)));
+                ldmatrix_x4_trans(b0, b1, b2, b3, tV + row * C::kRowBytes + ((ch ^ (row & 7)) << 4));
                 mma_bf16_16816(o[2 * dp], a0, a1, a2, a3, b0, b1);
                 mma_bf16_16816(o[2 * dp + 1], a0, a1, a2, a3, b2, b3);
             }
@@ -215,6 +255,9 @@ __global__ void __launch_bounds__(32 * MT * KS) attn_kernel(const AttnParams p) 
     l_lo += __shfl_xor_sync(0xffffffffu, l_lo, 2);
     l_hi += __shfl_xor_sync(0xffffffffu, l_hi, 1);
     l_hi += __shfl_xor_sync(0xffffffffu, l_hi, 2);
+    // from here on the maxima live in the log2 domain
+    m_lo = m_lo == -INFINITY ? -INFINITY : m_lo * sl2;
+    m_hi = m_hi == -INFINITY ? -INFINITY : m_hi * sl2;
 
     // ---- merge the KS token slices of this CTA through shared memory (pipeline buffers are free now) ----------
     if (KS > 1) {
@@ -255,132 +298,153 @@ __global__ void __launch_bounds__(32 * MT * KS) attn_kernel(const AttnParams p) 
             }
         }
     }
-    if (ks != 0) return;
 
-    // ---- write: final bf16 output (one split) or the normalised fp32 partial + log2 normaliser -----------------
     const float inv_lo = l_lo > 0.f ? 1.f / l_lo : 0.f, inv_hi = l_hi > 0.f ? 1.f / l_hi : 0.f;
-    const float lse_lo = l_lo > 0.f ? m_lo + log2f(l_lo) : -INFINITY;
+    const float lse_lo = l_lo > 0.f ? m_lo + log2f(l_lo) : -INFINITY;   // log2-domain normaliser
     const float lse_hi = l_hi > 0.f ? m_hi + log2f(l_hi) : -INFINITY;
+
+    if (p.n_splits == 1) {   // ---- single CTA per (b, KV head): write the bf16 output ------------------------------
+        if (ks != 0) return;
 #pragma unroll
-    for (int half = 0; half < 2; ++half) {
-        const int row = mt * 16 + g + half * 8;
-        if (row >= rows) continue;
-        const float inv = half ? inv_hi : inv_lo, lse = half ? lse_hi : lse_lo;
-        if (p.n_splits == 1) {
+        for (int half = 0; half < 2; ++half) {
+            const int row = mt * 16 + g + half * 8;
+            if (row >= rows) continue;
+            const float inv = half ? inv_hi : inv_lo, lse = half ? lse_hi : lse_lo;
             const int t = row / r, h = gkv * r + row % r;
             __nv_bfloat16* dst = p.out + (((long long)b * T + t) * p.n_q_heads + h) * D + 2 * c;
 #pragma unroll
             for (int i = 0; i < D / 8; ++i)
                 *reinterpret_cast<uint32_t*>(dst + i * 8) = pack_bf16(o[i][half * 2] * inv, o[i][half * 2 + 1] * inv);
             if (p.lse_out && c == 0) p.lse_out[((long long)b * p.n_q_heads + h) * T + t] = lse * kLn2;
-        } else {
-            const long long pr = (((long long)b * p.n_kv_heads + gkv) * p.n_splits + split) * rows + row;
-            float* dst = p.part_o + pr * D + 2 * c;
+        }
+        return;
+    }
+
+    // ---- cluster combine: normalised partial -> own shared memory; every CTA finishes a share of the rows -------
+    float* sPart = reinterpret_cast<float*>(smem_raw + C::kMergeBytes);   // [MT*16][D]
+    float* sLse = sPart + MT * 16 * D;                                     // [MT*16]
+    if (ks == 0) {
+#pragma unroll
+        for (int half = 0; half < 2; ++half) {
+            const int row = mt * 16 + g + half * 8;
+            const float inv = half ? inv_hi : inv_lo;
+            float* dst = sPart + row * D + 2 * c;
 #pragma unroll
             for (int i = 0; i < D / 8; ++i)
                 *reinterpret_cast<float2*>(dst + i * 8) = make_float2(o[i][half * 2] * inv, o[i][half * 2 + 1] * inv);
-            if (c == 0) p.part_lse[pr] = lse;
+            if (c == 0) sLse[row] = half ? lse_hi : lse_lo;
         }
     }
+    cg::cluster_group cluster = cg::this_cluster();
+    cluster.sync();
+    {
+        const int S = p.n_splits;
+        const int rows_per = (rows + S - 1) / S;
+        const int row_lo = split * rows_per, row_hi = min(rows, row_lo + rows_per);
+        constexpr int V4 = D / 4;   // float4 chunks per row
+        for (int item = tid; item < (row_hi - row_lo) * V4; item += NT) {
+            const int row = row_lo + item / V4, ch = item % V4;
+            float M = -INFINITY;
+            for (int s = 0; s < S; ++s) M = fmaxf(M, *cluster.map_shared_rank(sLse + row, s));
+            float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+            float W = 0.f;
+            for (int s = 0; s < S; ++s) {
+                const float lse = *cluster.map_shared_rank(sLse + row, s);
+                const float wgt = lse == -INFINITY ? 0.f : exp2f(lse - M);
+                const float4 x = *reinterpret_cast<const float4*>(cluster.map_shared_rank(sPart + row * D + ch * 4, s));
+                W += wgt;
+                acc.x += wgt * x.x;
+                acc.y += wgt * x.y;
+                acc.z += wgt * x.z;
+                acc.w += wgt * x.w;
+            }
+            const float inv = W > 0.f ? 1.f / W : 0.f;
+            const int t = row / r, h = gkv * r + row % r;
+            __nv_bfloat16* dst = p.out + (((long long)b * T + t) * p.n_q_heads + h) * D + ch * 4;
+            *reinterpret_cast<uint2*>(dst) =
+                make_uint2(pack_bf16(acc.x * inv, acc.y * inv), pack_bf16(acc.z * inv, acc.w * inv));
+            if (p.lse_out && ch == 0)
+                p.lse_out[((long long)b * p.n_q_heads + h) * T + t] = W > 0.f ? (M + log2f(W)) * kLn2 : -INFINITY;
+        }
+    }
+    cluster.sync();   // peers may still be reading this CTA's shared memory
 }
 
-// One warp per (b, KV head, query row): weighted sum of the split partials.
-template <int D>
-__global__ void __launch_bounds__(128) attn_combine_kernel(const AttnParams p) {
-    const int w = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
-    const int rows = p.rows;
-    if (w >= p.batch * p.n_kv_heads * rows) return;
-    const int row = w % rows, bg = w / rows;
-    const int b = bg / p.n_kv_heads, gkv = bg % p.n_kv_heads;
-    const long long base = (long long)bg * p.n_splits * rows + row;
-    float M = -INFINITY;
-    for (int s = 0; s < p.n_splits; ++s) M = fmaxf(M, __ldcg(p.part_lse + base + (long long)s * rows));
-    constexpr int V = D / 32;
-    float acc[V];
-#pragma unroll
-    for (int i = 0; i < V; ++i) acc[i] = 0.f;
-    float W = 0.f;
-    for (int s = 0; s < p.n_splits; ++s) {
-        const float lse = __ldcg(p.part_lse + base + (long long)s * rows);
-        const float wgt = lse == -INFINITY ? 0.f : exp2f(lse - M);
-        W += wgt;
-        const float* src = p.part_o + (base + (long long)s * rows) * D + lane * V;
-        if (wgt != 0.f) {
-#pragma unroll
-            for (int i = 0; i < V; i += 2) {
-                const float2 x = __ldcg(reinterpret_cast<const float2*>(src + i));
-                acc[i] += wgt * x.x;
-                acc[i + 1] += wgt * x.y;
-            }
-        }
+template <int D, int MT, int KS, int MODE>
+cudaError_t launch_mode(const AttnParams& p, cudaStream_t stream) {
+    using C = AttnCfg<D, MT, KS>;
+    const size_t table = MODE == kGatherTable ? (size_t)(p.split_tokens + 16) * sizeof(RowAddr) : 0;
+    const size_t smem = C::kPipeBytes + table;
+    static bool attr_done = false;   // per instantiation
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(attn_kernel<D, MT, KS, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)(C::kPipeBytes + kMaxTableTokens * sizeof(RowAddr)));
+        if (e != cudaSuccess) return e;
+        attr_done = true;
     }
-    const float inv = W > 0.f ? 1.f / W : 0.f;
-    const int t = row / p.group, h = gkv * p.group + row % p.group;
-    __nv_bfloat16* dst = p.out + (((long long)b * p.n_new + t) * p.n_q_heads + h) * D + lane * V;
-#pragma unroll
-    for (int i = 0; i < V; i += 2) *reinterpret_cast<uint32_t*>(dst + i) = pack_bf16(acc[i] * inv, acc[i + 1] * inv);
-    if (p.lse_out && lane == 0)
-        p.lse_out[((long long)b * p.n_q_heads + h) * p.n_new + t] = W > 0.f ? (M + log2f(W)) * kLn2 : -INFINITY;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(p.n_splits, p.n_kv_heads, p.batch);
+    cfg.blockDim = dim3(C::kThreads);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = p.n_splits;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    ProfScope prof(kKernAttn, stream);
+    return cudaLaunchKernelEx(&cfg, attn_kernel<D, MT, KS, MODE>, p);
 }
 
 template <int D, int MT, int KS>
 cudaError_t launch_cfg(const AttnParams& p, cudaStream_t stream) {
-    using C = AttnCfg<D, MT, KS>;
-    const size_t smem = (C::kPipeBytes > C::kMergeBytes ? C::kPipeBytes : C::kMergeBytes) +
-                        (size_t)(p.split_tokens + 16) * sizeof(long long);
-    static bool attr_done = false;   // per instantiation
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(attn_kernel<D, MT, KS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)(C::kPipeBytes + (kMaxSplitTokens + 16) * sizeof(long long)));
-        if (e != cudaSuccess) return e;
-        attr_done = true;
-    }
-    ProfScope prof(kKernAttn, stream);
-    attn_kernel<D, MT, KS><<<dim3(p.n_splits, p.n_kv_heads, p.batch), C::kThreads, smem, stream>>>(p);
-    return cudaGetLastError();
+    if (p.idx == nullptr) return launch_mode<D, MT, KS, kDense>(p, stream);
+    if (p.split_tokens + 16 <= kMaxTableTokens) return launch_mode<D, MT, KS, kGatherTable>(p, stream);
+    return launch_mode<D, MT, KS, kGatherInline>(p, stream);
 }
 
 template <int D>
 cudaError_t launch_d(const AttnParams& p, cudaStream_t stream) {
-    const int mt = (p.rows + 15) / 16;
-    cudaError_t e;
-    switch (mt) {
-        case 1: e = launch_cfg<D, 1, 4>(p, stream); break;
-        case 2: e = launch_cfg<D, 2, 4>(p, stream); break;
-        case 3: e = launch_cfg<D, 3, 2>(p, stream); break;
-        case 4: e = launch_cfg<D, 4, 2>(p, stream); break;
-        case 5: e = launch_cfg<D, 5, 1>(p, stream); break;
-        case 6: e = launch_cfg<D, 6, 1>(p, stream); break;
+    switch ((p.rows + 15) / 16) {
+        case 1: return launch_cfg<D, 1, 4>(p, stream);
+        case 2: return launch_cfg<D, 2, 4>(p, stream);
+        case 3: return launch_cfg<D, 3, 2>(p, stream);
+        case 4: return launch_cfg<D, 4, 2>(p, stream);
+        case 5: return launch_cfg<D, 5, 1>(p, stream);
+        case 6: return launch_cfg<D, 6, 1>(p, stream);
         default: return cudaErrorInvalidValue;
     }
-    if (e != cudaSuccess || p.n_splits == 1) return e;
-    const int warps = p.batch * p.n_kv_heads * p.rows;
-    ProfScope prof(kKernAttnCombine, stream);
-    attn_combine_kernel<D><<<(warps + 3) / 4, 128, 0, stream>>>(p);
-    return cudaGetLastError();
 }
+
+int g_split_override = 0;
 
 }  // namespace
 
-static int g_split_override = 0;
 void attn_set_split_override(int split_tokens) { g_split_override = split_tokens > 0 ? split_tokens : 0; }
 
+// CTAs (= cluster size) per (sequence, KV head): as many as fit one wave of 2 resident CTAs per SM on 148 SMs, at
+// most the portable cluster size, at least one 64-token tile each; gather lists are cut so that the address table
+// of a CTA stays within kMaxTableTokens when the cluster size allows.
 void attn_plan(int batch, int n_kv_heads, int max_tokens, int* split_tokens, int* n_splits) {
     const int units = batch * n_kv_heads > 0 ? batch * n_kv_heads : 1;
-    int target = 148 * 4;   // CTAs wanted in flight: 148 SMs x the CTAs resident per SM
-    int st = g_split_override;   // dustin_tune_attn_split_tokens
-    if (st <= 0) {
-        int ns = (target + units - 1) / units;
-        if (ns < 1) ns = 1;
-        st = (max_tokens + ns - 1) / ns;
+    int tiles = (max_tokens + kTileTokens - 1) / kTileTokens;
+    if (tiles < 1) tiles = 1;
+    int ns;
+    if (g_split_override > 0) {   // dustin_tune_attn_split_tokens
+        ns = (max_tokens + g_split_override - 1) / g_split_override;
+    } else {
+        ns = (148 * 2) / units;
+        const int ns_table = (max_tokens + kMaxTableTokens - 17) / (kMaxTableTokens - 16);
+        if (ns < ns_table) ns = ns_table;
     }
-    st = ((st + kTileTokens - 1) / kTileTokens) * kTileTokens;
-    if (st < kTileTokens) st = kTileTokens;
-    if (st > kMaxSplitTokens) st = kMaxSplitTokens;
-    int ns = (max_tokens + st - 1) / st;
+    if (ns > kMaxCluster) ns = kMaxCluster;
+    if (ns > tiles) ns = tiles;
     if (ns < 1) ns = 1;
-    *split_tokens = st;
-    *n_splits = ns;
+    const int tiles_per = (tiles + ns - 1) / ns;
+    *split_tokens = tiles_per * kTileTokens;
+    *n_splits = (tiles + tiles_per - 1) / tiles_per;
 }
 
 cudaError_t launch_attn(const AttnParams& p, cudaStream_t stream) {

@@ -128,7 +128,6 @@ def test_attn_and_fused_reject(lib):
     assert attn(out=None) == api.ERR_INVALID_ARG
     assert attn(kvv=kv(v=None)) == api.ERR_INVALID_ARG
     assert attn(s=shape(n_q_heads=64, n_kv_heads=2, n_new=5)) == api.ERR_UNSUPPORTED   # T*r = 160 > 96 rows
-    assert attn(idx=None, cnt=None, ws=None) == api.ERR_WORKSPACE                      # dense needs split scratch
     s = sel()
     fused = lambda mask=1, hist=FAKE, ws=FAKE, wsb=1 << 40, se=s: lib.dustin_verify_layer_fused(
         ctypes.byref(sh), ctypes.byref(k), FAKE, FAKE, FAKE, mask, FAKE, 0, hist, 1.0, ctypes.byref(se), 512, None,
