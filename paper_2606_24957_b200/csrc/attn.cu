@@ -50,6 +50,9 @@ struct RowAddr {
     const __nv_bfloat16* k;
     const __nv_bfloat16* v;
 };
+// Shared-memory address table entry: K and V share one layout, so one element offset serves both; a new draft
+// row u is stored as ~(its element offset in k_new / v_new) (negative).
+typedef long long RowOff;
 
 template <int D, int MT, int KS, int MODE>
 __global__ void __launch_bounds__(32 * MT * KS) attn_kernel(const AttnParams p) {
@@ -58,7 +61,7 @@ __global__ void __launch_bounds__(32 * MT * KS) attn_kernel(const AttnParams p) 
     extern __shared__ __align__(128) unsigned char smem_raw[];
     unsigned char* sK = smem_raw;
     unsigned char* sV = smem_raw + kStages * C::kStageBytes;
-    RowAddr* sTab = reinterpret_cast<RowAddr*>(smem_raw + C::kPipeBytes);
+    RowOff* sTab = reinterpret_cast<RowOff*>(smem_raw + C::kPipeBytes);
 
     const int split = blockIdx.x, gkv = blockIdx.y, b = blockIdx.z;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -73,22 +76,21 @@ __global__ void __launch_bounds__(32 * MT * KS) attn_kernel(const AttnParams p) 
     const int* list_idx = MODE == kDense ? nullptr : p.idx + ((long long)b * p.n_lists + list) * p.k_max + range_lo;
 
     // Global addresses of the K and V row of local token j.
-    auto row_addr = [&](int j) -> RowAddr {
-        RowAddr a;
+    auto row_off = [&](int j) -> RowOff {
         if (j < n_range) {
             const int tok = MODE == kDense ? range_lo + j : __ldg(list_idx + j);
-            const long long off = kv_row_offset(p.kv, b, tok, gkv);
-            a.k = p.kv.k + off;
-            a.v = p.kv.v + off;
-        } else {
-            const long long off = (((long long)b * T + (j - n_range)) * p.n_kv_heads + gkv) * D;
-            a.k = p.k_new + off;
-            a.v = p.v_new + off;
+            return kv_row_offset(p.kv, b, tok, gkv);
         }
+        return ~((((long long)b * T + (j - n_range)) * p.n_kv_heads + gkv) * D);
+    };
+    auto addr_of = [&](RowOff off) -> RowAddr {
+        RowAddr a;
+        a.k = off >= 0 ? p.kv.k + off : p.k_new + ~off;
+        a.v = off >= 0 ? p.kv.v + off : p.v_new + ~off;
         return a;
     };
     if (MODE == kGatherTable)
-        for (int j = tid; j < nt; j += NT) sTab[j] = row_addr(j);
+        for (int j = tid; j < nt; j += NT) sTab[j] = row_off(j);
 
     // ---- Q fragments (A operand): rows mt*16 + g (+8), row = t*r + head-in-group -------------------------------
     uint32_t qa[D / 16][4];
@@ -123,12 +125,7 @@ __global__ void __launch_bounds__(32 * MT * KS) attn_kernel(const AttnParams p) 
                 if (C::kPasses * C::kRowsPerPass > kTileTokens && row >= kTileTokens) break;
                 const int j = j0 + row;
                 const bool valid = j < nt;
-                RowAddr a;
-                if (MODE == kGatherTable) {
-                    a = sTab[valid ? j : 0];
-                } else {
-                    a = row_addr(valid ? j : 0);
-                }
+                const RowAddr a = addr_of(MODE == kGatherTable ? sTab[valid ? j : 0] : row_off(valid ? j : 0));
                 const uint32_t dst = stage_off + (uint32_t)row * C::kRowBytes + (uint32_t)((ld_ch ^ (row & 7)) << 4);
                 cp_async16(sK_u32 + dst, a.k + ld_ch * 8, valid ? 16 : 0);
                 cp_async16(sV_u32 + dst, a.v + ld_ch * 8, valid ? 16 : 0);
@@ -373,12 +370,12 @@ __global__ void __launch_bounds__(32 * MT * KS) attn_kernel(const AttnParams p) 
 template <int D, int MT, int KS, int MODE>
 cudaError_t launch_mode(const AttnParams& p, cudaStream_t stream) {
     using C = AttnCfg<D, MT, KS>;
-    const size_t table = MODE == kGatherTable ? (size_t)(p.split_tokens + 16) * sizeof(RowAddr) : 0;
+    const size_t table = MODE == kGatherTable ? (size_t)(p.split_tokens + 16) * sizeof(RowOff) : 0;
     const size_t smem = C::kPipeBytes + table;
     static bool attr_done = false;   // per instantiation
     if (!attr_done) {
         cudaError_t e = cudaFuncSetAttribute(attn_kernel<D, MT, KS, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)(C::kPipeBytes + kMaxTableTokens * sizeof(RowAddr)));
+                                             (int)(C::kPipeBytes + kMaxTableTokens * sizeof(RowOff)));
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
