@@ -94,6 +94,12 @@ size_t dustin_workspace_bytes(const dustin_shape_t* shape, uint64_t head_mask, i
  * 0 restores the built-in heuristic.  Query dustin_workspace_bytes again after changing it. */
 void dustin_tune_attn_split_tokens(int32_t split_tokens);
 
+/* Tuning / testing aid (process-wide, not thread-safe): which attention kernel serves a4/a5.  0 = automatic (the
+ * tcgen05 kernel for head_dim 128 and batch * n_kv_heads <= 2048, else the mma.sync cluster kernel), 1 = always the
+ * mma.sync cluster kernel, 2 = same as 0.  Results of the two agree within the a4 tolerance, not bitwise.  Query
+ * dustin_workspace_bytes again after changing it. */
+void dustin_tune_attn_impl(int32_t impl);
+
 /* Measurement aids (bench.py).  dustin_launch_count: kernels launched by this library in this process so far.
  * dustin_profile_enable(1) starts bracketing every kernel launch with a CUDA event pair on the launching stream
  * (and drops earlier records); dustin_profile_enable(0) stops.  dustin_profile_collect is the one call that

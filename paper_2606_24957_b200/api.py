@@ -67,6 +67,8 @@ def lib():
         L.dustin_last_cuda_error.argtypes = []
         L.dustin_tune_attn_split_tokens.restype = None
         L.dustin_tune_attn_split_tokens.argtypes = [i32]
+        L.dustin_tune_attn_impl.restype = None
+        L.dustin_tune_attn_impl.argtypes = [i32]
         L.dustin_launch_count.restype = ctypes.c_uint64
         L.dustin_launch_count.argtypes = []
         L.dustin_profile_enable.restype = None
@@ -95,6 +97,7 @@ def lib():
 N_KERNELS = 7
 
 EXPORTS = ("dustin_version", "dustin_status_string", "dustin_last_cuda_error", "dustin_tune_attn_split_tokens",
+           "dustin_tune_attn_impl",
            "dustin_launch_count", "dustin_profile_enable", "dustin_profile_collect", "dustin_kernel_name",
            "dustin_workspace_bytes", "dustin_score_heads", "dustin_fuse_scores", "dustin_topk_select",
            "dustin_sparse_verify_attn", "dustin_verify_layer_fused")
@@ -184,6 +187,11 @@ def version() -> int:
 
 def tune_attn_split_tokens(split_tokens: int) -> None:
     lib().dustin_tune_attn_split_tokens(int(split_tokens))
+
+
+def tune_attn_impl(impl: int) -> None:
+    """0 = automatic, 1 = mma.sync cluster kernel, 2 = tcgen05 kernel where usable (dustin_tune_attn_impl)."""
+    lib().dustin_tune_attn_impl(int(impl))
 
 
 def launch_count() -> int:

@@ -132,15 +132,18 @@ int popcount64(uint64_t x) {
 
 // ---- attention plan -------------------------------------------------------------------------------------------
 struct AttnWs {
-    size_t part_o, part_lse, total;
+    size_t total;
     int split_tokens, n_splits;
+    bool tc;
 };
 AttnWs attn_ws(const dustin_shape_t* s, int max_tokens) {
-    // The split partials are combined through distributed shared memory inside the cluster (attn.cu): the
-    // attention stage needs no global scratch.
+    // tcgen05 kernel (attn_tc.cu): arrival counters + stream-K partials.  mma.sync cluster kernel (attn.cu): the
+    // split partials are combined through distributed shared memory, no global scratch.
     AttnWs w;
     attn_plan(s->batch, s->n_kv_heads, max_tokens, &w.split_tokens, &w.n_splits);
-    w.part_o = w.part_lse = w.total = 0;
+    const int rows = s->n_new * (s->n_q_heads / s->n_kv_heads);
+    w.tc = attn_get_impl() != 1 && attn_tc_usable(s->batch, s->n_kv_heads, s->head_dim, rows, max_tokens, s->n_new);
+    w.total = w.tc ? attn_tc_ws_bytes(s->batch, s->n_kv_heads, rows) : 0;
     return w;
 }
 
@@ -260,9 +263,7 @@ int run_attn(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q, 
     p.rows = p.n_new * p.group;
     p.split_tokens = w.split_tokens;
     p.n_splits = w.n_splits;
-    char* base = static_cast<char*>(ws);
-    p.part_o = w.total ? reinterpret_cast<float*>(base + w.part_o) : nullptr;
-    p.part_lse = w.total ? reinterpret_cast<float*>(base + w.part_lse) : nullptr;
+    p.tc_ws = w.tc ? ws : nullptr;
     p.out = static_cast<__nv_bfloat16*>(out);
     p.lse_out = lse_out;
     const cudaError_t e = launch_attn(p, stream);
@@ -292,6 +293,8 @@ const char* dustin_status_string(int status) {
 int dustin_last_cuda_error(void) { return g_last_cuda_error; }
 
 void dustin_tune_attn_split_tokens(int32_t split_tokens) { attn_set_split_override(split_tokens); }
+
+void dustin_tune_attn_impl(int32_t impl) { attn_set_impl(impl); }
 
 uint64_t dustin_launch_count(void) { return prof_launch_count(); }
 

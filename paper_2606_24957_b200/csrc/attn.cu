@@ -416,8 +416,12 @@ cudaError_t launch_d(const AttnParams& p, cudaStream_t stream) {
 }
 
 int g_split_override = 0;
+int g_impl = 0;
 
 }  // namespace
+
+void attn_set_impl(int impl) { g_impl = impl >= 0 && impl <= 2 ? impl : 0; }
+int attn_get_impl() { return g_impl; }
 
 void attn_set_split_override(int split_tokens) { g_split_override = split_tokens > 0 ? split_tokens : 0; }
 
@@ -445,6 +449,7 @@ void attn_plan(int batch, int n_kv_heads, int max_tokens, int* split_tokens, int
 }
 
 cudaError_t launch_attn(const AttnParams& p, cudaStream_t stream) {
+    if (p.tc_ws != nullptr) return launch_attn_tc(p, p.tc_ws, stream);
     return p.head_dim == 128 ? launch_d<128>(p, stream) : launch_d<64>(p, stream);
 }
 

@@ -1,0 +1,739 @@
+// attn_tc.cu -- stage a4 / a5 on the 5th-generation tensor cores (tcgen05 + TMEM) for head_dim 128.
+// Sparse verification attention over the selected KV (App. G :568) and, with idx == nullptr, the
+// full-cache verification baseline.  DESIGN.md section 5.1.
+//
+// Decomposition ("stream-K" over tokens).  A unit is one (sequence b, KV head g): its token list is the cnt[b,l]
+// selected cache rows followed by the T new draft rows.  The token lists of all units are laid end to end and cut
+// into gridDim.x equal ranges, one persistent CTA per SM; a CTA therefore works on a few SEGMENTS (pieces of
+// units).  A unit that lies inside one CTA is written straight to `out`; otherwise each piece leaves a normalised
+// partial (o, lse) in the workspace and the LAST piece to finish (a per-unit arrival counter) merges them in
+// segment order, so the result does not depend on which CTA happens to be last.
+//
+// Roles inside a CTA (288 threads):
+//   warps 0-3  softmax warpgroup: thread = one token of the 128-token tile = one TMEM lane
+//   warp  4    MMA issuer (one thread) and TMEM allocation
+//   warps 5-8  producers: resolve index -> (page table ->) row address, stream K and V tiles with 16-byte cp.async
+//              into the 128-byte-swizzled UMMA layout [64-dim half][token][128 B]; a ring of 32 KB slots in the
+//              order K0 V0 K1 V1 ...; completion via cp.async.mbarrier.arrive.noinc on the slot's mbarrier.
+// Per tile j:  S^T_j[token,row] = K_j . Q^T   (A = K tile, K-major;  B = Q, K-major;  M = 128, N = NQ, 8 k-steps)
+//              P^T_j = exp2(S^T_j * scale - m_ref[row])  written as bf16 into an MN-major (row-contiguous) buffer
+//              O^T[dim,row] += V_j^T . P^T_j           (A = V tile, MN-major;  B = P^T, MN-major;  M = 128)
+// m_ref is a per-row reference exponent (log2 domain) that is moved only when a score exceeds it by more than 16 (decided
+// CTA-uniformly with one bar.red per tile); O^T and the running sums are then rescaled.
+#include "kernels.cuh"
+
+#include <climits>
+
+namespace dustin {
+
+namespace {
+
+constexpr int kTcThreads = 288;
+constexpr int kTile = 128;            // tokens per tile (UMMA M)
+constexpr int kD = 128;               // head_dim served by this kernel
+constexpr int kSlotBytes = kTile * kD * 2;   // 32 KB: one K or V tile
+constexpr int kMaxUnits = 2048;       // prefix array in shared memory
+constexpr float kRefSlack = 16.f;     // log2 units a score may exceed m_ref before the reference is moved
+constexpr float kRefInit = -1.0e30f;
+constexpr long long kInvalidRow = LLONG_MIN;
+
+// ---- PTX wrappers ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    while (!mbar_try_wait(bar, parity)) {
+    }
+}
+// The mbarrier receives one arrival when all cp.async issued so far by this thread have landed.
+__device__ __forceinline__ void cp_async_mbar_arrive_noinc(uint32_t bar) {
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+// generic-proxy writes (st.shared, cp.async) -> async-proxy reads (tcgen05.mma operands)
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+
+__device__ __forceinline__ void tmem_alloc(uint32_t smem_dst, uint32_t ncols) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(ncols)
+                 : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
+}
+// D[tmem] (+)= A[smem desc] * B[smem desc]; bf16 inputs, fp32 accumulate; issued by ONE thread.
+__device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
+                                          uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d),
+        "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+// The mbarrier receives one arrival when every tcgen05.mma issued so far by this thread has completed.
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+// This thread's TMEM lane, 16 consecutive 32-bit columns.
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
+          "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+        : "r"(taddr)
+        : "memory");
+}
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&v)[16]) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" ::"r"(
+            taddr),
+        "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]), "r"(v[9]),
+        "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15])
+        : "memory");
+}
+__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+
+// Named barrier over the 128 softmax threads (id 1); the .red.or form returns the OR of `pred` over them.
+__device__ __forceinline__ void wg_sync() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
+__device__ __forceinline__ bool wg_any(bool pred) {
+    uint32_t r;
+    asm volatile(
+        "{\n\t.reg .pred p, q;\n\t"
+        "setp.ne.b32 q, %1, 0;\n\t"
+        "bar.red.or.pred p, 1, 128, q;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(r)
+        : "r"((uint32_t)pred)
+        : "memory");
+    return r != 0;
+}
+
+// UMMA shared-memory matrix descriptor (sm_100 format: version 1 in bits [46,48); offsets in 16-byte units).
+__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes, uint32_t layout) {
+    return (uint64_t)((saddr & 0x3FFFFu) >> 4) | ((uint64_t)(lbo_bytes >> 4) << 16) | ((uint64_t)(sbo_bytes >> 4) << 32) |
+           (1ull << 46) | ((uint64_t)layout << 61);
+}
+constexpr uint32_t kLayoutNone = 0, kLayoutSw128 = 2;
+// Instruction descriptor, kind::f16: fp32 accumulate (bit 4), bf16 A (bit 7) and B (bit 10), majors in bits 15/16
+// (0 = K-major, 1 = MN-major), N >> 3 in bits [17,23), M >> 4 in bits [24,29).
+__host__ __device__ constexpr uint32_t umma_idesc(int m, int n, int a_mn_major, int b_mn_major) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)a_mn_major << 15) | ((uint32_t)b_mn_major << 16) |
+           ((uint32_t)(n >> 3) << 17) | ((uint32_t)(m >> 4) << 24);
+}
+
+// Order-preserving map float <-> int32 (for redux.sync.max.s32); its own inverse.
+__device__ __forceinline__ int flip_f32(int b) { return b ^ ((b >> 31) & 0x7fffffff); }
+__device__ __forceinline__ float warp_max_f32(float x) {
+    const int k = __reduce_max_sync(0xffffffffu, flip_f32(__float_as_int(x)));
+    return __int_as_float(flip_f32(k));
+}
+
+// ---- shared-memory plan --------------------------------------------------------------------------------------------
+template <int NQ>
+struct TcCfg {
+    static constexpr int kSlotsN = NQ <= 32 ? 6 : (NQ <= 64 ? 5 : 4);
+    static constexpr int kQBytes = NQ * kD * 2;          // one Q buffer, [64-dim half][row][128 B] swizzled
+    static constexpr int kPBytes = NQ * kTile * 2;       // P^T, [8-row block][token][16 B]
+    static constexpr int kOffSlots = 0;
+    static constexpr int kOffQ = kOffSlots + kSlotsN * kSlotBytes;
+    static constexpr int kOffP = kOffQ + 2 * kQBytes;
+    static constexpr int kOffPrefix = kOffP + kPBytes;                    // int [kMaxUnits + 1]
+    static constexpr int kOffRef = kOffPrefix + (kMaxUnits + 4) * 4;      // float m_ref[NQ]
+    static constexpr int kOffFac = kOffRef + NQ * 4;                      // float fac[NQ]
+    static constexpr int kOffWarp = kOffFac + NQ * 4;                     // float [4][NQ]: per-warp maxima / sums
+    static constexpr int kOffRowOff = kOffWarp + 4 * NQ * 4;              // int row -> element offset inside out[b]
+    static constexpr int kOffScan = kOffRowOff + NQ * 4;                  // int [8] warp totals of the prefix scan
+    static constexpr int kOffBar = (kOffScan + 8 * 4 + 8 + 7) & ~7;       // uint64 barriers
+    static constexpr int kNumBar = 2 * kSlotsN + 10;
+    static constexpr int kOffTmem = kOffBar + kNumBar * 8;                // uint32 TMEM base, uint32 combine flag
+    static constexpr int kSmemBytes = kOffTmem + 16;
+    static_assert(kSmemBytes + 1024 <= 232448, "shared-memory plan exceeds 227 KB");
+    static_assert(kOffQ % 1024 == 0 && kQBytes % 1024 == 0 && kOffP % 1024 == 0, "UMMA operands need 1 KB alignment");
+};
+
+// ---- segments ---------------------------------------------------------------------------------------------------
+// Piece of one unit's token list that falls into this CTA's range of the concatenated token space.
+struct Seg {
+    int u, b, g, list;
+    int cnt;              // cache rows of the unit (its token list is cnt cache rows, then T new rows)
+    int pos_lo, pos_hi;   // this piece: token positions [pos_lo, pos_hi) of the unit
+    int n_tiles;
+    int whole;            // the piece is the entire unit: the result goes straight to `out`
+    int slot;             // partial slot of this CTA (0: the piece continues a unit begun earlier, 1: otherwise)
+    int cta_first, cta_last;   // CTAs that hold pieces of the unit
+};
+
+struct TileCursor {
+    const int* prefix;
+    int n_units, n_kv, n_lists, n_new, lo, hi, chunk;
+    int next_u;
+    Seg s;
+    int ti;        // tile index inside the segment
+    int seg_no;    // running segment number of this CTA
+    bool valid;
+
+    __device__ __forceinline__ bool load_seg() {
+        if (next_u >= n_units) return false;
+        const int ps = prefix[next_u];
+        if (ps >= hi) return false;
+        const int pe = prefix[next_u + 1];
+        s.u = next_u;
+        s.b = next_u / n_kv;
+        s.g = next_u - s.b * n_kv;
+        s.list = n_lists == 1 ? 0 : s.g;
+        s.cnt = pe - ps - n_new;
+        s.pos_lo = max(lo, ps) - ps;
+        s.pos_hi = min(hi, pe) - ps;
+        s.n_tiles = (s.pos_hi - s.pos_lo + kTile - 1) / kTile;
+        s.whole = (s.pos_lo == 0 && s.pos_hi == pe - ps) ? 1 : 0;
+        s.slot = ps <= lo ? 0 : 1;
+        s.cta_first = ps / chunk;
+        s.cta_last = (pe - 1) / chunk;
+        ++next_u;
+        return true;
+    }
+    __device__ __forceinline__ void init(const int* prefix_, int n_units_, int n_kv_, int n_lists_, int n_new_, int lo_,
+                                         int hi_, int chunk_, int u0) {
+        prefix = prefix_; n_units = n_units_; n_kv = n_kv_; n_lists = n_lists_; n_new = n_new_;
+        lo = lo_; hi = hi_; chunk = chunk_; next_u = u0;
+        ti = 0; seg_no = 0;
+        valid = load_seg();
+    }
+    __device__ __forceinline__ bool last_tile() const { return ti == s.n_tiles - 1; }
+    __device__ __forceinline__ void advance() {
+        if (++ti >= s.n_tiles) {
+            ti = 0;
+            ++seg_no;
+            valid = load_seg();
+        }
+    }
+};
+
+// ---- kernel -----------------------------------------------------------------------------------------------------
+struct TcWs {
+    int* counters;      // [B * Hkv] arrivals per unit, zeroed before the launch
+    float* part_o;      // [grid, 2, rows, 128] normalised partial outputs
+    float* part_lse;    // [grid, 2, rows] log2-domain normalisers
+};
+
+template <int NQ, bool GATHER>
+__global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams p, const TcWs ws) {
+    using C = TcCfg<NQ>;
+    constexpr int NS = C::kSlotsN;
+    extern __shared__ unsigned char smem_dyn[];
+    // 1 KB alignment for the 128-byte-swizzled operands
+    unsigned char* smem = reinterpret_cast<unsigned char*>(((uintptr_t)smem_dyn + 1023) & ~(uintptr_t)1023);
+    const uint32_t sbase = smem_u32(smem);
+    int* s_prefix = reinterpret_cast<int*>(smem + C::kOffPrefix);
+    float* s_ref = reinterpret_cast<float*>(smem + C::kOffRef);
+    float* s_fac = reinterpret_cast<float*>(smem + C::kOffFac);
+    float* s_warp = reinterpret_cast<float*>(smem + C::kOffWarp);
+    int* s_rowoff = reinterpret_cast<int*>(smem + C::kOffRowOff);
+    int* s_scan = reinterpret_cast<int*>(smem + C::kOffScan);
+    uint32_t* s_tmem = reinterpret_cast<uint32_t*>(smem + C::kOffTmem);
+    const uint32_t bar0 = sbase + C::kOffBar;
+    auto bar = [&](int i) -> uint32_t { return bar0 + 8u * (uint32_t)i; };
+    // barrier indices
+    constexpr int kSlotFull = 0, kSlotEmpty = NS, kQFull = 2 * NS, kQEmpty = 2 * NS + 2, kSFull = 2 * NS + 4,
+                  kSEmpty = 2 * NS + 6, kPFull = 2 * NS + 8, kPvDone = 2 * NS + 9;
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int T = p.n_new, r = p.group, rows = p.rows, Hkv = p.n_kv_heads, Hq = p.n_q_heads;
+    const int n_units = p.batch * Hkv;
+
+    // ---- token-list lengths of all units -> exclusive prefix sums (threads 0..255) --------------------------------
+    auto unit_len = [&](int u) -> int {
+        const int b = u / Hkv;
+        int c;
+        if (GATHER) {
+            const int list = p.n_lists == 1 ? 0 : u - b * Hkv;
+            c = __ldg(p.cnt + b * p.n_lists + list);
+            c = c < 0 ? 0 : (c > p.k_max ? p.k_max : c);
+        } else {
+            c = seq_len_of(p.kv.seq_lens, b, p.max_ctx);
+        }
+        return c + T;
+    };
+    {
+        const int per = (n_units + 255) / 256;
+        const int u_lo = min(tid * per, n_units), u_hi = tid < 256 ? min(u_lo + per, n_units) : u_lo;
+        int sum = 0;
+        for (int u = u_lo; u < u_hi; ++u) sum += unit_len(u);
+        int inc = sum;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int v = __shfl_up_sync(0xffffffffu, inc, d);
+            if (lane >= d) inc += v;
+        }
+        if (lane == 31 && warp < 8) s_scan[warp] = inc;
+        __syncthreads();
+        int base = 0;
+        for (int w = 0; w < warp && w < 8; ++w) base += s_scan[w];
+        int run = base + inc - sum;
+        for (int u = u_lo; u < u_hi; ++u) {
+            s_prefix[u] = run;
+            run += unit_len(u);
+        }
+        if (tid == 255) s_prefix[n_units] = run;
+        if (tid < NQ) {
+            s_ref[tid] = kRefInit;
+            s_rowoff[tid] = ((tid / r) * Hq + tid % r) * kD;
+        }
+        __syncthreads();
+    }
+    const int total = s_prefix[n_units];
+    const int chunk = (((total + (int)gridDim.x - 1) / (int)gridDim.x) + 31) & ~31;
+    const int lo = (int)blockIdx.x * chunk, hi = min(lo + chunk, total);
+    if (lo >= hi) return;   // the whole CTA leaves before any barrier / TMEM state exists
+    int u0;
+    {
+        int a = 0, bnd = n_units;   // largest u with prefix[u] <= lo
+        while (bnd - a > 1) {
+            const int m = (a + bnd) >> 1;
+            if (s_prefix[m] <= lo) a = m; else bnd = m;
+        }
+        u0 = a;
+    }
+
+    if (tid == 0) {
+        for (int i = 0; i < NS; ++i) {
+            mbar_init(bar(kSlotFull + i), 128);
+            mbar_init(bar(kSlotEmpty + i), 1);
+        }
+        for (int i = 0; i < 2; ++i) {
+            mbar_init(bar(kQFull + i), 128);
+            mbar_init(bar(kQEmpty + i), 1);
+            mbar_init(bar(kSFull + i), 1);
+            mbar_init(bar(kSEmpty + i), 128);
+        }
+        mbar_init(bar(kPFull), 128);
+        mbar_init(bar(kPvDone), 1);
+        fence_mbar_init();
+    }
+    if (warp == 4) tmem_alloc(smem_u32(s_tmem), 512);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = *s_tmem;
+    constexpr uint32_t kColS = 0, kColO = 256;   // S buffers at columns 0 and 128, O^T at 256
+
+    TileCursor cur;
+    cur.init(s_prefix, n_units, Hkv, p.n_lists, T, lo, hi, chunk, u0);
+
+    if (warp >= 5) {
+        // ================= producers ===========================================================================
+        const int pw = warp - 5, ptid = tid - 160;
+        TileCursor pf = cur;   // runs two tiles ahead of `cur`
+        struct Tok { int tok, b, g; };
+        // token code of row 32*pw + lane of the cursor's tile: >= 0 cache row, -1 none, <= -2 new row (-2 - u)
+        auto load_tok = [&](const TileCursor& c) -> Tok {
+            Tok t;
+            t.tok = -1; t.b = 0; t.g = 0;
+            if (!c.valid) return t;
+            const Seg& s = c.s;
+            t.b = s.b; t.g = s.g;
+            const int pos = s.pos_lo + c.ti * kTile + 32 * pw + lane;
+            if (pos < s.pos_hi) {
+                if (pos < s.cnt)
+                    t.tok = GATHER ? __ldg(p.idx + ((long long)s.b * p.n_lists + s.list) * p.k_max + pos) : pos;
+                else
+                    t.tok = -2 - (pos - s.cnt);
+            }
+            return t;
+        };
+        auto resolve = [&](const Tok& t) -> long long {
+            if (t.tok >= 0) return kv_row_offset(p.kv, t.b, t.tok, t.g);
+            if (t.tok == -1) return kInvalidRow;
+            return ~((((long long)t.b * T + (-2 - t.tok)) * Hkv + t.g) * kD);
+        };
+        auto issue_tile = [&](int item, long long off, const __nv_bfloat16* base_cache, const __nv_bfloat16* base_new) {
+            const int slot = item % NS;
+            mbar_wait(bar(kSlotEmpty + slot), (((uint32_t)(item / NS)) & 1u) ^ 1u);
+            const uint32_t dst0 = sbase + C::kOffSlots + (uint32_t)slot * kSlotBytes;
+            const int c = lane & 15;
+            const uint32_t dst_c = dst0 + (uint32_t)(c >> 3) * (kTile * 128);
+#pragma unroll
+            for (int i = 0; i < 16; ++i) {
+                const int rr = 2 * i + (lane >> 4);
+                const long long o = __shfl_sync(0xffffffffu, off, rr);
+                const int row = 32 * pw + rr;
+                const bool ok = o != kInvalidRow;
+                const __nv_bfloat16* src = !ok ? base_cache : (o >= 0 ? base_cache + o : base_new + ~o);
+                cp_async16(dst_c + (uint32_t)row * 128 + (uint32_t)(((c & 7) ^ (row & 7)) << 4), src + c * 8, ok ? 16 : 0);
+            }
+            cp_async_mbar_arrive_noinc(bar(kSlotFull + slot));
+        };
+
+        Tok t1 = load_tok(pf);
+        pf.advance();
+        long long off0 = resolve(t1);
+        t1 = load_tok(pf);
+        if (pf.valid) pf.advance();
+        int gj = 0;
+        while (cur.valid) {
+            Tok t2 = load_tok(pf);                 // tile gj + 2: index load in flight
+            if (pf.valid) pf.advance();
+            const long long off1 = resolve(t1);    // tile gj + 1: page-table lookup in flight
+            if (cur.ti == 0) {                     // new segment: its T*r query rows (zero-padded to NQ)
+                const int k = cur.seg_no, qb = k & 1;
+                mbar_wait(bar(kQEmpty + qb), (((uint32_t)(k >> 1)) & 1u) ^ 1u);
+                const uint32_t qdst = sbase + C::kOffQ + (uint32_t)qb * C::kQBytes;
+                const __nv_bfloat16* qsrc = p.q + ((long long)cur.s.b * T * Hq + (long long)cur.s.g * r) * kD;
+                for (int x = ptid; x < NQ * 16; x += 128) {
+                    const int rr = x >> 4, c = x & 15;
+                    const bool ok = rr < rows;
+                    const __nv_bfloat16* src = ok ? qsrc + s_rowoff[rr] + c * 8 : p.q;
+                    cp_async16(qdst + (uint32_t)(c >> 3) * (NQ * 128) + (uint32_t)rr * 128 +
+                                   (uint32_t)(((c & 7) ^ (rr & 7)) << 4), src, ok ? 16 : 0);
+                }
+                cp_async_mbar_arrive_noinc(bar(kQFull + qb));
+            }
+            issue_tile(2 * gj, off0, p.kv.k, p.k_new);
+            issue_tile(2 * gj + 1, off0, p.kv.v, p.v_new);
+            off0 = off1;
+            t1 = t2;
+            cur.advance();
+            ++gj;
+        }
+    } else if (warp == 4) {
+        // ================= MMA issuer (one thread) ==============================================================
+        if (lane == 0) {
+            constexpr uint32_t idesc_s = umma_idesc(kTile, NQ, 0, 0);    // S^T = K . Q^T : both K-major
+            constexpr uint32_t idesc_pv = umma_idesc(kTile, NQ, 1, 1);   // O^T = V^T . P^T : both MN-major
+            const uint32_t slots = sbase + C::kOffSlots, pbuf = sbase + C::kOffP;
+            auto issue_pv = [&](int j, bool first_of_seg) {
+                mbar_wait(bar(kPFull), (uint32_t)j & 1u);
+                const int item = 2 * j + 1, slot = item % NS;
+                mbar_wait(bar(kSlotFull + slot), ((uint32_t)(item / NS)) & 1u);
+                fence_proxy_async();
+                tc_fence_after();
+                const uint32_t vb = slots + (uint32_t)slot * kSlotBytes;
+#pragma unroll
+                for (int ks = 0; ks < kTile / 16; ++ks) {
+                    // A = V tile as [dim (M), token (K)], dim contiguous: 64-dim halves 16 KB apart (LBO), 8-token
+                    // groups 1 KB apart (SBO);  B = P^T as [row (N), token (K)], row contiguous, no swizzle:
+                    // 8-row blocks 2 KB apart (SBO), 8-token groups 128 B apart (LBO).
+                    const uint64_t ad = umma_desc(vb + (uint32_t)ks * 2048, kTile * 128, 1024, kLayoutSw128);
+                    const uint64_t bd = umma_desc(pbuf + (uint32_t)ks * 256, 128, 2048, kLayoutNone);
+                    umma_bf16(tmem + kColO, ad, bd, idesc_pv, (first_of_seg && ks == 0) ? 0u : 1u);
+                }
+                umma_commit(bar(kSlotEmpty + slot));
+                umma_commit(bar(kPvDone));
+            };
+            int gj = 0;
+            bool have_prev = false, prev_first = false;
+            while (cur.valid) {
+                const int k = cur.seg_no, qb = k & 1;
+                if (cur.ti == 0) mbar_wait(bar(kQFull + qb), ((uint32_t)(k >> 1)) & 1u);
+                const int item = 2 * gj, slot = item % NS, sb = gj & 1;
+                mbar_wait(bar(kSlotFull + slot), ((uint32_t)(item / NS)) & 1u);
+                mbar_wait(bar(kSEmpty + sb), (((uint32_t)(gj >> 1)) & 1u) ^ 1u);
+                fence_proxy_async();
+                tc_fence_after();
+                const uint32_t kb = slots + (uint32_t)slot * kSlotBytes;
+                const uint32_t qbuf = sbase + C::kOffQ + (uint32_t)qb * C::kQBytes;
+#pragma unroll
+                for (int ks = 0; ks < kD / 16; ++ks) {
+                    // both operands K-major, 128-byte swizzle: rows 128 B apart, 8-row groups 1 KB apart (SBO); the
+                    // k-step moves 32 B inside the swizzled row, the second 64-dim half sits one [rows][128 B] on
+                    const uint64_t ad = umma_desc(kb + (uint32_t)(ks >> 2) * (kTile * 128) + (uint32_t)(ks & 3) * 32, 16,
+                                                  1024, kLayoutSw128);
+                    const uint64_t bd = umma_desc(qbuf + (uint32_t)(ks >> 2) * (NQ * 128) + (uint32_t)(ks & 3) * 32, 16,
+                                                  1024, kLayoutSw128);
+                    umma_bf16(tmem + kColS + (uint32_t)sb * 128, ad, bd, idesc_s, ks > 0 ? 1u : 0u);
+                }
+                umma_commit(bar(kSlotEmpty + slot));
+                umma_commit(bar(kSFull + sb));
+                if (cur.last_tile()) umma_commit(bar(kQEmpty + qb));
+                if (have_prev) issue_pv(gj - 1, prev_first);
+                have_prev = true;
+                prev_first = cur.ti == 0;
+                cur.advance();
+                ++gj;
+            }
+            if (have_prev) issue_pv(gj - 1, prev_first);
+        }
+        __syncwarp();
+    } else {
+        // ================= softmax warpgroup: thread = token of the tile = TMEM lane ==============================
+        const int t = tid;
+        const uint32_t lane_base = tmem + ((uint32_t)(warp * 32) << 16);
+        const float sl2 = p.scale_log2;
+        const float4* ref4 = reinterpret_cast<const float4*>(s_ref);
+        const float4* fac4 = reinterpret_cast<const float4*>(s_fac);
+        float lpart[NQ];   // this token lane's share of the running row sums
+#pragma unroll
+        for (int i = 0; i < NQ; ++i) lpart[i] = 0.f;
+        int gj = 0;
+        while (cur.valid) {
+            const Seg& s = cur.s;
+            const int sb = gj & 1;
+            mbar_wait(bar(kSFull + sb), ((uint32_t)(gj >> 1)) & 1u);
+            tc_fence_after();
+            uint32_t xs[NQ];
+#pragma unroll
+            for (int c = 0; c < NQ / 16; ++c)
+                tmem_ld16(lane_base + kColS + (uint32_t)sb * 128 + (uint32_t)c * 16,
+                          reinterpret_cast<uint32_t(&)[16]>(xs[c * 16]));
+            tmem_wait_ld();
+            tc_fence_before();
+            mbar_arrive(bar(kSEmpty + sb));
+
+            // scale into the log2 domain; mask the tail of the piece and, for a new row u, the query rows of
+            // verify positions < u (row i belongs to position i / r, so those are the rows i < u * r)
+            const int pos = s.pos_lo + cur.ti * kTile + t;
+            const int thr = pos >= s.pos_hi ? INT_MAX : (pos > s.cnt ? (pos - s.cnt) * r : 0);
+            float x[NQ];
+            bool over = false;
+#pragma unroll
+            for (int i4 = 0; i4 < NQ / 4; ++i4) {
+                const float4 m = ref4[i4];
+                const float mm[4] = {m.x, m.y, m.z, m.w};
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const int i = i4 * 4 + e;
+                    const float v = i < thr ? -INFINITY : __uint_as_float(xs[i]) * sl2;
+                    x[i] = v;
+                    over |= v - mm[e] > kRefSlack;
+                }
+            }
+            if (wg_any(over)) {
+                // Move the reference exponents to the running row maxima (rare after the first tile).
+#pragma unroll
+                for (int i = 0; i < NQ; ++i) {
+                    const float wm = warp_max_f32(x[i]);
+                    if (lane == 0) s_warp[warp * NQ + i] = wm;
+                }
+                wg_sync();
+                if (t < NQ) {
+                    const float m_old = s_ref[t];
+                    const float m_new = fmaxf(fmaxf(m_old, fmaxf(s_warp[t], s_warp[NQ + t])),
+                                              fmaxf(s_warp[2 * NQ + t], s_warp[3 * NQ + t]));
+                    s_fac[t] = exp2f(m_old - m_new);
+                    s_ref[t] = m_new;
+                }
+                wg_sync();
+#pragma unroll
+                for (int i4 = 0; i4 < NQ / 4; ++i4) {
+                    const float4 f = fac4[i4];
+                    lpart[i4 * 4 + 0] *= f.x;
+                    lpart[i4 * 4 + 1] *= f.y;
+                    lpart[i4 * 4 + 2] *= f.z;
+                    lpart[i4 * 4 + 3] *= f.w;
+                }
+                if (cur.ti > 0) {   // O^T already holds earlier tiles of this piece: rescale it column by column
+                    mbar_wait(bar(kPvDone), (uint32_t)(gj - 1) & 1u);
+                    tc_fence_after();
+#pragma unroll
+                    for (int c = 0; c < NQ / 16; ++c) {
+                        uint32_t o[16];
+                        tmem_ld16(lane_base + kColO + (uint32_t)c * 16, o);
+                        tmem_wait_ld();
+#pragma unroll
+                        for (int e = 0; e < 16; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * s_fac[c * 16 + e]);
+                        tmem_st16(lane_base + kColO + (uint32_t)c * 16, o);
+                    }
+                    tmem_wait_st();
+                    tc_fence_before();
+                }
+            }
+
+            // P^T: this token's NQ weights, bf16, row-contiguous -> 16-byte stores at [8-row block][token]
+            if (gj > 0) mbar_wait(bar(kPvDone), (uint32_t)(gj - 1) & 1u);   // the previous P.V has read the buffer
+            unsigned char* prow = smem + C::kOffP + t * 16;
+#pragma unroll
+            for (int jb = 0; jb < NQ / 8; ++jb) {
+                const float4 m0 = ref4[jb * 2], m1 = ref4[jb * 2 + 1];
+                const float mm[8] = {m0.x, m0.y, m0.z, m0.w, m1.x, m1.y, m1.z, m1.w};
+                float pr[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    pr[e] = fast_exp2(x[jb * 8 + e] - mm[e]);
+                    lpart[jb * 8 + e] += pr[e];
+                }
+                *reinterpret_cast<uint4*>(prow + jb * 2048) = make_uint4(pack_bf16(pr[0], pr[1]), pack_bf16(pr[2], pr[3]),
+                                                                         pack_bf16(pr[4], pr[5]), pack_bf16(pr[6], pr[7]));
+            }
+            fence_proxy_async();
+            mbar_arrive(bar(kPFull));
+
+            if (cur.last_tile()) {
+                // ---- the piece is complete: normalise and write it (out or partial) ---------------------------------
+#pragma unroll
+                for (int i = 0; i < NQ; ++i) {
+                    float v = lpart[i];
+#pragma unroll
+                    for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+                    if (lane == 0) s_warp[warp * NQ + i] = v;
+                    lpart[i] = 0.f;
+                }
+                mbar_wait(bar(kPvDone), (uint32_t)gj & 1u);   // every P.V of the piece has completed
+                tc_fence_after();
+                wg_sync();
+                uint32_t o[NQ];
+#pragma unroll
+                for (int c = 0; c < NQ / 16; ++c)
+                    tmem_ld16(lane_base + kColO + (uint32_t)c * 16, reinterpret_cast<uint32_t(&)[16]>(o[c * 16]));
+                tmem_wait_ld();
+                tc_fence_before();
+                const long long slot_id = (long long)blockIdx.x * 2 + s.slot;
+                __nv_bfloat16* outb = p.out + ((long long)s.b * T * Hq + (long long)s.g * r) * kD + t;   // t = dim
+                float* po = ws.part_o + slot_id * rows * kD + t;
+#pragma unroll
+                for (int i = 0; i < NQ; ++i) {
+                    if (i < rows) {
+                        const float l = (s_warp[i] + s_warp[NQ + i]) + (s_warp[2 * NQ + i] + s_warp[3 * NQ + i]);
+                        const float v = __uint_as_float(o[i]) * (l > 0.f ? 1.f / l : 0.f);
+                        if (s.whole) outb[s_rowoff[i]] = __float2bfloat16_rn(v);
+                        else po[i * kD] = v;
+                    }
+                }
+                if (t < rows) {
+                    const float l = (s_warp[t] + s_warp[NQ + t]) + (s_warp[2 * NQ + t] + s_warp[3 * NQ + t]);
+                    const float lse2 = l > 0.f ? s_ref[t] + log2f(l) : -INFINITY;
+                    if (!s.whole) ws.part_lse[slot_id * rows + t] = lse2;
+                    else if (p.lse_out)
+                        p.lse_out[((long long)s.b * Hq + s.g * r + t % r) * T + t / r] = lse2 * kLn2;
+                }
+                if (!s.whole) {
+                    // last piece of the unit to arrive merges all of them, in CTA order
+                    __threadfence();
+                    wg_sync();
+                    if (t == 0) s_tmem[1] = atomicAdd(ws.counters + s.u, 1) == s.cta_last - s.cta_first ? 1u : 0u;
+                    wg_sync();
+                    if (s_tmem[1]) {
+                        __threadfence();
+                        const int ps = s_prefix[s.u];
+                        for (int i = 0; i < rows; ++i) {
+                            float M = -INFINITY;
+                            for (int c = s.cta_first; c <= s.cta_last; ++c) {
+                                const long long sid = (long long)c * 2 + (ps <= c * chunk ? 0 : 1);
+                                M = fmaxf(M, __ldcg(ws.part_lse + sid * rows + i));
+                            }
+                            float W = 0.f, acc = 0.f;
+                            for (int c = s.cta_first; c <= s.cta_last; ++c) {
+                                const long long sid = (long long)c * 2 + (ps <= c * chunk ? 0 : 1);
+                                const float lse = __ldcg(ws.part_lse + sid * rows + i);
+                                const float w = lse == -INFINITY ? 0.f : exp2f(lse - M);
+                                acc += w * __ldcg(ws.part_o + (sid * rows + i) * kD + t);
+                                W += w;
+                            }
+                            outb[s_rowoff[i]] = __float2bfloat16_rn(W > 0.f ? acc / W : 0.f);
+                            if (p.lse_out && t == 0)
+                                p.lse_out[((long long)s.b * Hq + s.g * r + i % r) * T + i / r] =
+                                    W > 0.f ? (M + log2f(W)) * kLn2 : -INFINITY;
+                        }
+                    }
+                }
+                wg_sync();
+                if (t < NQ) s_ref[t] = kRefInit;
+                wg_sync();
+            }
+            cur.advance();
+            ++gj;
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 4) {
+        tc_fence_after();
+        tmem_dealloc(tmem, 512);
+    }
+}
+
+constexpr int kMaxGrid = 256;   // workspace is sized for this many CTAs
+
+int sm_count() {
+    static int n = 0;
+    if (n == 0) {
+        int dev = 0, v = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess &&
+            cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0)
+            n = v;
+        else
+            n = 148;
+    }
+    return n;
+}
+
+inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+template <int NQ, bool GATHER>
+cudaError_t launch_tc(const AttnParams& p, const TcWs& ws, int grid, cudaStream_t stream) {
+    using C = TcCfg<NQ>;
+    constexpr int smem = C::kSmemBytes + 1024;
+    static bool attr_done = false;   // per instantiation
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(attn_tc_kernel<NQ, GATHER>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    ProfScope prof(kKernAttn, stream);
+    attn_tc_kernel<NQ, GATHER><<<grid, kTcThreads, smem, stream>>>(p, ws);
+    return cudaGetLastError();
+}
+
+template <int NQ>
+cudaError_t launch_tc_nq(const AttnParams& p, const TcWs& ws, int grid, cudaStream_t stream) {
+    return p.idx ? launch_tc<NQ, true>(p, ws, grid, stream) : launch_tc<NQ, false>(p, ws, grid, stream);
+}
+
+}  // namespace
+
+bool attn_tc_usable(int batch, int n_kv_heads, int head_dim, int rows, int max_tokens, int n_new) {
+    if (head_dim != kD || rows > 96 || rows < 1) return false;
+    const long long units = (long long)batch * n_kv_heads;
+    if (units > kMaxUnits) return false;
+    return units * ((long long)max_tokens + n_new) < (1ll << 31) - (1 << 20);
+}
+
+size_t attn_tc_ws_bytes(int batch, int n_kv_heads, int rows) {
+    return align256((size_t)batch * n_kv_heads * sizeof(int)) + align256((size_t)kMaxGrid * 2 * rows * kD * sizeof(float)) +
+           align256((size_t)kMaxGrid * 2 * rows * sizeof(float));
+}
+
+cudaError_t launch_attn_tc(const AttnParams& p, void* ws_base, cudaStream_t stream) {
+    const size_t units = (size_t)p.batch * p.n_kv_heads;
+    char* base = static_cast<char*>(ws_base);
+    TcWs ws;
+    ws.counters = reinterpret_cast<int*>(base);
+    ws.part_o = reinterpret_cast<float*>(base + align256(units * sizeof(int)));
+    ws.part_lse = reinterpret_cast<float*>(base + align256(units * sizeof(int)) +
+                                           align256((size_t)kMaxGrid * 2 * p.rows * kD * sizeof(float)));
+    cudaError_t e = cudaMemsetAsync(ws.counters, 0, units * sizeof(int), stream);
+    if (e != cudaSuccess) return e;
+    const int max_tokens = (p.idx ? (p.k_max < p.max_ctx ? p.k_max : p.max_ctx) : p.max_ctx) + p.n_new;
+    long long tiles = ((long long)units * max_tokens + kTile - 1) / kTile;
+    int grid = sm_count() < kMaxGrid ? sm_count() : kMaxGrid;
+    if (tiles < grid) grid = tiles < 1 ? 1 : (int)tiles;
+    switch ((p.rows + 15) / 16) {
+        case 1: return launch_tc_nq<16>(p, ws, grid, stream);
+        case 2: return launch_tc_nq<32>(p, ws, grid, stream);
+        case 3: return launch_tc_nq<48>(p, ws, grid, stream);
+        case 4: return launch_tc_nq<64>(p, ws, grid, stream);
+        case 5: return launch_tc_nq<80>(p, ws, grid, stream);
+        case 6: return launch_tc_nq<96>(p, ws, grid, stream);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+}  // namespace dustin

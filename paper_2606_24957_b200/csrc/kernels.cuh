@@ -60,8 +60,7 @@ struct AttnParams {
     float scale_log2;
     int rows;                     // T * group query rows per KV head
     int split_tokens, n_splits;   // cache tokens per CTA; CTAs per (b, KV head)
-    float* part_o;                // ws: [B,Hkv,n_splits,rows,d] normalised partial outputs
-    float* part_lse;              // ws: [B,Hkv,n_splits,rows]   log2-domain normalisers
+    void* tc_ws;                  // ws of the tcgen05 kernel (attn_tc_ws_bytes), or nullptr => mma.sync cluster kernel
     __nv_bfloat16* out;           // [B,T,Hq,d]
     float* lse_out;               // [B,Hq,T] or nullptr
 };
@@ -69,6 +68,12 @@ cudaError_t launch_attn(const AttnParams& p, cudaStream_t stream);
 // Host-side split heuristic shared by workspace sizing and launch.
 void attn_plan(int batch, int n_kv_heads, int max_tokens, int* split_tokens, int* n_splits);
 void attn_set_split_override(int split_tokens);
+// tcgen05 kernel (attn_tc.cu): head_dim 128, stream-K over tokens, partials + arrival counters in the workspace.
+bool attn_tc_usable(int batch, int n_kv_heads, int head_dim, int rows, int max_tokens, int n_new);
+size_t attn_tc_ws_bytes(int batch, int n_kv_heads, int rows);
+cudaError_t launch_attn_tc(const AttnParams& p, void* ws_base, cudaStream_t stream);
+void attn_set_impl(int impl);   // 0 auto, 1 mma.sync cluster kernel, 2 tcgen05 kernel where usable
+int attn_get_impl();
 
 // ---- launch bookkeeping (profile.cu) ----------------------------------------------------------------------------
 enum KernelId {
