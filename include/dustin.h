@@ -95,7 +95,7 @@ size_t dustin_workspace_bytes(const dustin_shape_t* shape, uint64_t head_mask, i
 void dustin_tune_attn_split_tokens(int32_t split_tokens);
 
 /* Tuning / testing aid (process-wide, not thread-safe): which attention kernel serves a4/a5.  0 = automatic (the
- * tcgen05 kernel for head_dim 128 and batch * n_kv_heads <= 2048, else the mma.sync cluster kernel), 1 = always the
+ * tcgen05 kernel for head_dim 128 and batch * n_kv_heads <= 1024, else the mma.sync cluster kernel), 1 = always the
  * mma.sync cluster kernel, 2 = same as 0.  Results of the two agree within the a4 tolerance, not bitwise.  Query
  * dustin_workspace_bytes again after changing it. */
 void dustin_tune_attn_impl(int32_t impl);

@@ -23,6 +23,7 @@
 #include "kernels.cuh"
 
 #include <climits>
+#include <cstdlib>
 
 namespace dustin {
 
@@ -32,10 +33,11 @@ constexpr int kTcThreads = 288;
 constexpr int kTile = 128;            // tokens per tile (UMMA M)
 constexpr int kD = 128;               // head_dim served by this kernel
 constexpr int kSlotBytes = kTile * kD * 2;   // 32 KB: one K or V tile
-constexpr int kMaxUnits = 2048;       // prefix array in shared memory
+constexpr int kMaxUnits = 1024;       // prefix array in shared memory
 constexpr float kRefSlack = 16.f;     // log2 units a score may exceed m_ref before the reference is moved
 constexpr float kRefInit = -1.0e30f;
 constexpr long long kInvalidRow = LLONG_MIN;
+constexpr int kMergeFast = 4;          // pieces of one unit merged with all loads in flight (more: sequential path)
 
 // ---- PTX wrappers ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
@@ -159,7 +161,9 @@ struct TcCfg {
     static constexpr int kOffRef = kOffPrefix + (kMaxUnits + 4) * 4;      // float m_ref[NQ]
     static constexpr int kOffFac = kOffRef + NQ * 4;                      // float fac[NQ]
     static constexpr int kOffWarp = kOffFac + NQ * 4;                     // float [4][NQ]: per-warp maxima / sums
-    static constexpr int kOffRowOff = kOffWarp + 4 * NQ * 4;              // int row -> element offset inside out[b]
+    static constexpr int kOffWgt = kOffWarp + 4 * NQ * 4;                 // float [kMergeFast][NQ]: merge weights
+    static constexpr int kOffRowTab = (kOffWgt + kMergeFast * NQ * 4 + 15) & ~15;   // {K row, V row} addresses, 4 x 32
+    static constexpr int kOffRowOff = kOffRowTab + 128 * 16;              // int row -> element offset inside out[b]
     static constexpr int kOffScan = kOffRowOff + NQ * 4;                  // int [8] warp totals of the prefix scan
     static constexpr int kOffBar = (kOffScan + 8 * 4 + 8 + 7) & ~7;       // uint64 barriers
     static constexpr int kNumBar = 2 * kSlotsN + 10;
@@ -230,6 +234,7 @@ struct TileCursor {
 // ---- kernel -----------------------------------------------------------------------------------------------------
 struct TcWs {
     int* counters;      // [B * Hkv] arrivals per unit, zeroed before the launch
+    const void* zero_row;   // 256 zero bytes (zeroed with the counters): source of the rows past the end of a piece
     float* part_o;      // [grid, 2, rows, 128] normalised partial outputs
     float* part_lse;    // [grid, 2, rows] log2-domain normalisers
 };
@@ -246,6 +251,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
     float* s_ref = reinterpret_cast<float*>(smem + C::kOffRef);
     float* s_fac = reinterpret_cast<float*>(smem + C::kOffFac);
     float* s_warp = reinterpret_cast<float*>(smem + C::kOffWarp);
+    float* s_wgt = reinterpret_cast<float*>(smem + C::kOffWgt);
     int* s_rowoff = reinterpret_cast<int*>(smem + C::kOffRowOff);
     int* s_scan = reinterpret_cast<int*>(smem + C::kOffScan);
     uint32_t* s_tmem = reinterpret_cast<uint32_t*>(smem + C::kOffTmem);
@@ -359,56 +365,85 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
             }
             return t;
         };
-        auto resolve = [&](const Tok& t) -> long long {
-            if (t.tok >= 0) return kv_row_offset(p.kv, t.b, t.tok, t.g);
-            if (t.tok == -1) return kInvalidRow;
-            return ~((((long long)t.b * T + (-2 - t.tok)) * Hkv + t.g) * kD);
+        // Absolute addresses of the K row and of the V row of a token code; rows past the end of the piece read
+        // the zeroed row of the workspace, so the copy loop needs no predicate.
+        struct RowPtr { unsigned long long k, v; };
+        const unsigned long long zero_row = (unsigned long long)ws.zero_row;
+        auto resolve = [&](const Tok& t) -> RowPtr {
+            RowPtr a;
+            if (t.tok >= 0) {
+                const long long o = kv_row_offset(p.kv, t.b, t.tok, t.g);
+                a.k = (unsigned long long)(p.kv.k + o);
+                a.v = (unsigned long long)(p.kv.v + o);
+            } else if (t.tok == -1) {
+                a.k = a.v = zero_row;
+            } else {
+                const long long o = (((long long)t.b * T + (-2 - t.tok)) * Hkv + t.g) * kD;
+                a.k = (unsigned long long)(p.k_new + o);
+                a.v = (unsigned long long)(p.v_new + o);
+            }
+            return a;
         };
-        auto issue_tile = [&](int item, long long off, const __nv_bfloat16* base_cache, const __nv_bfloat16* base_new) {
-            const int slot = item % NS;
-            mbar_wait(bar(kSlotEmpty + slot), (((uint32_t)(item / NS)) & 1u) ^ 1u);
-            const uint32_t dst0 = sbase + C::kOffSlots + (uint32_t)slot * kSlotBytes;
-            const int c = lane & 15;
-            const uint32_t dst_c = dst0 + (uint32_t)(c >> 3) * (kTile * 128);
+        // lane = 16-byte chunk c of rows 2i + h (h = lane / 16), i = 0..15, of this warp's 32 rows of the tile.
+        // Destination inside a slot: [64-dim half c/8][row][128 B], chunk XOR (row & 7); rows 2i + h and
+        // 2(i + 4) + h share the swizzle term and lie 1 KB apart.
+        const int c = lane & 15, h = lane >> 4;
+        uint32_t dsw[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int row = 32 * pw + 2 * q + h;
+            dsw[q] = (uint32_t)(c >> 3) * (kTile * 128) + (uint32_t)row * 128 + (uint32_t)(((c & 7) ^ (row & 7)) << 4);
+        }
+        ulonglong2* tab = reinterpret_cast<ulonglong2*>(smem + C::kOffRowTab) + 32 * pw;   // this warp's 32 entries
+        const ulonglong2* tab_rd = tab + h;
+        const unsigned long long coff = (unsigned long long)c * 16;
+        // K and V tiles of tile gj: items 2gj and 2gj+1 of the slot ring
+        auto issue_tile = [&](int gj, const RowPtr& mine) {
+            const int ik = 2 * gj, iv = 2 * gj + 1, sk = ik % NS, sv = iv % NS;
+            __syncwarp();
+            tab[lane] = make_ulonglong2(mine.k, mine.v);
+            __syncwarp();
+            mbar_wait(bar(kSlotEmpty + sk), (((uint32_t)(ik / NS)) & 1u) ^ 1u);
+            mbar_wait(bar(kSlotEmpty + sv), (((uint32_t)(iv / NS)) & 1u) ^ 1u);
+            const uint32_t dk = sbase + C::kOffSlots + (uint32_t)sk * kSlotBytes;
+            const uint32_t dv = sbase + C::kOffSlots + (uint32_t)sv * kSlotBytes;
 #pragma unroll
             for (int i = 0; i < 16; ++i) {
-                const int rr = 2 * i + (lane >> 4);
-                const long long o = __shfl_sync(0xffffffffu, off, rr);
-                const int row = 32 * pw + rr;
-                const bool ok = o != kInvalidRow;
-                const __nv_bfloat16* src = !ok ? base_cache : (o >= 0 ? base_cache + o : base_new + ~o);
-                cp_async16(dst_c + (uint32_t)row * 128 + (uint32_t)(((c & 7) ^ (row & 7)) << 4), src + c * 8, ok ? 16 : 0);
+                const ulonglong2 a = tab_rd[2 * i];
+                const uint32_t d = dsw[i & 3] + (uint32_t)(i >> 2) * 1024;
+                cp_async16(dk + d, reinterpret_cast<const void*>(a.x + coff), 16);
+                cp_async16(dv + d, reinterpret_cast<const void*>(a.y + coff), 16);
             }
-            cp_async_mbar_arrive_noinc(bar(kSlotFull + slot));
+            cp_async_mbar_arrive_noinc(bar(kSlotFull + sk));
+            cp_async_mbar_arrive_noinc(bar(kSlotFull + sv));
         };
 
         Tok t1 = load_tok(pf);
         pf.advance();
-        long long off0 = resolve(t1);
+        RowPtr a0 = resolve(t1);
         t1 = load_tok(pf);
         if (pf.valid) pf.advance();
         int gj = 0;
         while (cur.valid) {
             Tok t2 = load_tok(pf);                 // tile gj + 2: index load in flight
             if (pf.valid) pf.advance();
-            const long long off1 = resolve(t1);    // tile gj + 1: page-table lookup in flight
+            const RowPtr a1 = resolve(t1);         // tile gj + 1: page-table lookup in flight
             if (cur.ti == 0) {                     // new segment: its T*r query rows (zero-padded to NQ)
                 const int k = cur.seg_no, qb = k & 1;
                 mbar_wait(bar(kQEmpty + qb), (((uint32_t)(k >> 1)) & 1u) ^ 1u);
                 const uint32_t qdst = sbase + C::kOffQ + (uint32_t)qb * C::kQBytes;
                 const __nv_bfloat16* qsrc = p.q + ((long long)cur.s.b * T * Hq + (long long)cur.s.g * r) * kD;
                 for (int x = ptid; x < NQ * 16; x += 128) {
-                    const int rr = x >> 4, c = x & 15;
+                    const int rr = x >> 4, cc = x & 15;
                     const bool ok = rr < rows;
-                    const __nv_bfloat16* src = ok ? qsrc + s_rowoff[rr] + c * 8 : p.q;
-                    cp_async16(qdst + (uint32_t)(c >> 3) * (NQ * 128) + (uint32_t)rr * 128 +
-                                   (uint32_t)(((c & 7) ^ (rr & 7)) << 4), src, ok ? 16 : 0);
+                    const __nv_bfloat16* src = ok ? qsrc + s_rowoff[rr] + cc * 8 : p.q;
+                    cp_async16(qdst + (uint32_t)(cc >> 3) * (NQ * 128) + (uint32_t)rr * 128 +
+                                   (uint32_t)(((cc & 7) ^ (rr & 7)) << 4), src, ok ? 16 : 0);
                 }
                 cp_async_mbar_arrive_noinc(bar(kQFull + qb));
             }
-            issue_tile(2 * gj, off0, p.kv.k, p.k_new);
-            issue_tile(2 * gj + 1, off0, p.kv.v, p.v_new);
-            off0 = off1;
+            issue_tile(gj, a0);
+            a0 = a1;
             t1 = t2;
             cur.advance();
             ++gj;
@@ -433,7 +468,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
                     // 8-row blocks 2 KB apart (SBO), 8-token groups 128 B apart (LBO).
                     const uint64_t ad = umma_desc(vb + (uint32_t)ks * 2048, kTile * 128, 1024, kLayoutSw128);
                     const uint64_t bd = umma_desc(pbuf + (uint32_t)ks * 256, 128, 2048, kLayoutNone);
-                    umma_bf16(tmem + kColO, ad, bd, idesc_pv, (first_of_seg && ks == 0) ? 0u : 1u);
+                    if (!(p.dbg & 1)) umma_bf16(tmem + kColO, ad, bd, idesc_pv, (first_of_seg && ks == 0) ? 0u : 1u);
                 }
                 umma_commit(bar(kSlotEmpty + slot));
                 umma_commit(bar(kPvDone));
@@ -458,7 +493,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
                                                   1024, kLayoutSw128);
                     const uint64_t bd = umma_desc(qbuf + (uint32_t)(ks >> 2) * (NQ * 128) + (uint32_t)(ks & 3) * 32, 16,
                                                   1024, kLayoutSw128);
-                    umma_bf16(tmem + kColS + (uint32_t)sb * 128, ad, bd, idesc_s, ks > 0 ? 1u : 0u);
+                    if (!(p.dbg & 2)) umma_bf16(tmem + kColS + (uint32_t)sb * 128, ad, bd, idesc_s, ks > 0 ? 1u : 0u);
                 }
                 umma_commit(bar(kSlotEmpty + slot));
                 umma_commit(bar(kSFull + sb));
@@ -622,24 +657,64 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
                     if (s_tmem[1]) {
                         __threadfence();
                         const int ps = s_prefix[s.u];
-                        for (int i = 0; i < rows; ++i) {
-                            float M = -INFINITY;
-                            for (int c = s.cta_first; c <= s.cta_last; ++c) {
-                                const long long sid = (long long)c * 2 + (ps <= c * chunk ? 0 : 1);
-                                M = fmaxf(M, __ldcg(ws.part_lse + sid * rows + i));
+                        const int nseg = s.cta_last - s.cta_first + 1;
+                        auto slot_of = [&](int c) -> long long { return (long long)c * 2 + (ps <= c * chunk ? 0 : 1); };
+                        if (nseg <= kMergeFast) {
+                            // weights of the pieces, row t by thread t: all normalisers are loaded at once
+                            if (t < rows) {
+                                float l[kMergeFast];
+#pragma unroll
+                                for (int j = 0; j < kMergeFast; ++j)
+                                    l[j] = j < nseg ? __ldcg(ws.part_lse + slot_of(s.cta_first + j) * rows + t) : -INFINITY;
+                                float M = l[0];
+#pragma unroll
+                                for (int j = 1; j < kMergeFast; ++j) M = fmaxf(M, l[j]);
+                                float w[kMergeFast], W = 0.f;
+#pragma unroll
+                                for (int j = 0; j < kMergeFast; ++j) {
+                                    w[j] = l[j] == -INFINITY ? 0.f : exp2f(l[j] - M);
+                                    W += w[j];
+                                }
+                                const float inv = W > 0.f ? 1.f / W : 0.f;
+#pragma unroll
+                                for (int j = 0; j < kMergeFast; ++j) s_wgt[j * NQ + t] = w[j] * inv;
+                                if (p.lse_out)
+                                    p.lse_out[((long long)s.b * Hq + s.g * r + t % r) * T + t / r] =
+                                        W > 0.f ? (M + log2f(W)) * kLn2 : -INFINITY;
                             }
-                            float W = 0.f, acc = 0.f;
-                            for (int c = s.cta_first; c <= s.cta_last; ++c) {
-                                const long long sid = (long long)c * 2 + (ps <= c * chunk ? 0 : 1);
-                                const float lse = __ldcg(ws.part_lse + sid * rows + i);
-                                const float w = lse == -INFINITY ? 0.f : exp2f(lse - M);
-                                acc += w * __ldcg(ws.part_o + (sid * rows + i) * kD + t);
-                                W += w;
+                            wg_sync();
+                            float acc[NQ];
+#pragma unroll
+                            for (int i = 0; i < NQ; ++i) acc[i] = 0.f;
+                            for (int j = 0; j < nseg; ++j) {   // pieces in CTA order; the NQ loads of one piece are independent
+                                const float* src = ws.part_o + slot_of(s.cta_first + j) * rows * kD + t;
+                                float v[NQ];
+#pragma unroll
+                                for (int i = 0; i < NQ; ++i) v[i] = i < rows ? __ldcg(src + i * kD) : 0.f;
+#pragma unroll
+                                for (int i = 0; i < NQ; ++i) acc[i] = fmaf(s_wgt[j * NQ + i], v[i], acc[i]);
                             }
-                            outb[s_rowoff[i]] = __float2bfloat16_rn(W > 0.f ? acc / W : 0.f);
-                            if (p.lse_out && t == 0)
-                                p.lse_out[((long long)s.b * Hq + s.g * r + i % r) * T + i / r] =
-                                    W > 0.f ? (M + log2f(W)) * kLn2 : -INFINITY;
+#pragma unroll
+                            for (int i = 0; i < NQ; ++i)
+                                if (i < rows) outb[s_rowoff[i]] = __float2bfloat16_rn(acc[i]);
+                        } else {
+                            // a unit cut into many pieces (one very long sequence): plain sequential merge
+                            for (int i = 0; i < rows; ++i) {
+                                float M = -INFINITY;
+                                for (int c = s.cta_first; c <= s.cta_last; ++c)
+                                    M = fmaxf(M, __ldcg(ws.part_lse + slot_of(c) * rows + i));
+                                float W = 0.f, acc = 0.f;
+                                for (int c = s.cta_first; c <= s.cta_last; ++c) {
+                                    const float lse = __ldcg(ws.part_lse + slot_of(c) * rows + i);
+                                    const float w = lse == -INFINITY ? 0.f : exp2f(lse - M);
+                                    acc += w * __ldcg(ws.part_o + (slot_of(c) * rows + i) * kD + t);
+                                    W += w;
+                                }
+                                outb[s_rowoff[i]] = __float2bfloat16_rn(W > 0.f ? acc / W : 0.f);
+                                if (p.lse_out && t == 0)
+                                    p.lse_out[((long long)s.b * Hq + s.g * r + i % r) * T + i / r] =
+                                        W > 0.f ? (M + log2f(W)) * kLn2 : -INFINITY;
+                            }
                         }
                     }
                 }
@@ -707,19 +782,22 @@ bool attn_tc_usable(int batch, int n_kv_heads, int head_dim, int rows, int max_t
 }
 
 size_t attn_tc_ws_bytes(int batch, int n_kv_heads, int rows) {
-    return align256((size_t)batch * n_kv_heads * sizeof(int)) + align256((size_t)kMaxGrid * 2 * rows * kD * sizeof(float)) +
+    return align256((size_t)batch * n_kv_heads * sizeof(int)) + 256 + align256((size_t)kMaxGrid * 2 * rows * kD * sizeof(float)) +
            align256((size_t)kMaxGrid * 2 * rows * sizeof(float));
 }
 
-cudaError_t launch_attn_tc(const AttnParams& p, void* ws_base, cudaStream_t stream) {
+cudaError_t launch_attn_tc(const AttnParams& p_in, void* ws_base, cudaStream_t stream) {
+    AttnParams p = p_in;
+    { const char* e = getenv("DUSTIN_DBG"); p.dbg = e ? atoi(e) : 0; }
     const size_t units = (size_t)p.batch * p.n_kv_heads;
     char* base = static_cast<char*>(ws_base);
     TcWs ws;
     ws.counters = reinterpret_cast<int*>(base);
-    ws.part_o = reinterpret_cast<float*>(base + align256(units * sizeof(int)));
-    ws.part_lse = reinterpret_cast<float*>(base + align256(units * sizeof(int)) +
-                                           align256((size_t)kMaxGrid * 2 * p.rows * kD * sizeof(float)));
-    cudaError_t e = cudaMemsetAsync(ws.counters, 0, units * sizeof(int), stream);
+    const size_t head = align256(units * sizeof(int)) + 256;   // counters, then the zero row
+    ws.zero_row = base + head - 256;
+    ws.part_o = reinterpret_cast<float*>(base + head);
+    ws.part_lse = reinterpret_cast<float*>(base + head + align256((size_t)kMaxGrid * 2 * p.rows * kD * sizeof(float)));
+    cudaError_t e = cudaMemsetAsync(base, 0, head, stream);
     if (e != cudaSuccess) return e;
     const int max_tokens = (p.idx ? (p.k_max < p.max_ctx ? p.k_max : p.max_ctx) : p.max_ctx) + p.n_new;
     long long tiles = ((long long)units * max_tokens + kTile - 1) / kTile;

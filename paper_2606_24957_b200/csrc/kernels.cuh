@@ -60,6 +60,7 @@ struct AttnParams {
     float scale_log2;
     int rows;                     // T * group query rows per KV head
     int split_tokens, n_splits;   // cache tokens per CTA; CTAs per (b, KV head)
+    int dbg;
     void* tc_ws;                  // ws of the tcgen05 kernel (attn_tc_ws_bytes), or nullptr => mma.sync cluster kernel
     __nv_bfloat16* out;           // [B,T,Hq,d]
     float* lse_out;               // [B,Hq,T] or nullptr

@@ -10,6 +10,15 @@ from tests import harness as H
 pytestmark = pytest.mark.gpu
 
 
+@pytest.fixture(autouse=True, params=["tcgen05", "mma_sync"])
+def attn_impl(request):
+    """Every test runs once per attention kernel: the tcgen05 kernel (automatic choice for head_dim 128) and the
+    mma.sync cluster kernel (forced; also what head_dim 64 always uses)."""
+    api.tune_attn_impl(1 if request.param == "mma_sync" else 0)
+    yield request.param
+    api.tune_attn_impl(0)
+
+
 def small_cases():
     llama = synth.config_llama8b()
     qwen = synth.config_qwen72b()
@@ -110,7 +119,9 @@ def test_budget_equal_context_reproduces_dense():
 
 
 @pytest.mark.parametrize("split", [64, 128, 1024])
-def test_split_size_does_not_change_results_beyond_rounding(split):
+def test_split_size_does_not_change_results_beyond_rounding(split, attn_impl):
+    if attn_impl != "mma_sync":
+        pytest.skip("the split override only steers the mma.sync cluster kernel")
     cfg = CASES["qwen_spread"]
     cpu, dev = _both(cfg)
     base = H.run_gpu_staged(dev)
