@@ -9,10 +9,10 @@
 // partial (o, lse) in the workspace and the LAST piece to finish (a per-unit arrival counter) merges them in
 // segment order, so the result does not depend on which CTA happens to be last.
 //
-// Roles inside a CTA (288 threads):
+// Roles inside a CTA (384 threads; setmaxnreg moves registers from the other warpgroups to the softmax one):
 //   warps 0-3  softmax warpgroup: thread = one token of the 128-token tile = one TMEM lane
-//   warp  4    MMA issuer (one thread) and TMEM allocation
-//   warps 5-8  producers: resolve index -> (page table ->) row address, stream K and V tiles with 16-byte cp.async
+//   warp  8    MMA issuer (one thread) and TMEM allocation (warps 9-11 only donate their registers)
+//   warps 4-7  producers: resolve index -> (page table ->) row address, stream K and V tiles with 16-byte cp.async
 //              into the 128-byte-swizzled UMMA layout [64-dim half][token][128 B]; a ring of 32 KB slots in the
 //              order K0 V0 K1 V1 ...; completion via cp.async.mbarrier.arrive.noinc on the slot's mbarrier.
 // Per tile j:  S^T_j[token,row] = K_j . Q^T   (A = K tile, K-major;  B = Q, K-major;  M = 128, N = NQ, 8 k-steps)
@@ -29,7 +29,7 @@ namespace dustin {
 
 namespace {
 
-constexpr int kTcThreads = 288;
+constexpr int kTcThreads = 384;        // three warpgroups: softmax | producers | MMA issuer (+ 3 idle warps)
 constexpr int kTile = 128;            // tokens per tile (UMMA M)
 constexpr int kD = 128;               // head_dim served by this kernel
 constexpr int kSlotBytes = kTile * kD * 2;   // 32 KB: one K or V tile
@@ -141,11 +141,52 @@ __host__ __device__ constexpr uint32_t umma_idesc(int m, int n, int a_mn_major, 
            ((uint32_t)(n >> 3) << 17) | ((uint32_t)(m >> 4) << 24);
 }
 
+__device__ __forceinline__ void st_release(int* p, int v) {
+    asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ void wait_flag(const int* p) {
+    int v;
+    do {
+        asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    } while (v == 0);
+}
+
 // Order-preserving map float <-> int32 (for redux.sync.max.s32); its own inverse.
 __device__ __forceinline__ int flip_f32(int b) { return b ^ ((b >> 31) & 0x7fffffff); }
 __device__ __forceinline__ float warp_max_f32(float x) {
     const int k = __reduce_max_sync(0xffffffffu, flip_f32(__float_as_int(x)));
     return __int_as_float(flip_f32(k));
+}
+
+// Transposing warp reduction of N per-lane values: after it, lane L holds the warp-wide result of kFinal<N> rows,
+// row_base(L) + i.  At lane bit B the lanes of a pair split the remaining rows between them (one shuffle per two
+// rows); once the count is odd the remaining steps are plain butterflies.  N = 48 takes 48 shuffles instead of 240.
+template <int N, int B>
+struct TrFinal { static constexpr int value = B == 5 ? N : (N % 2 == 0 ? TrFinal<N / 2, B + 1>::value : TrFinal<N, B + 1>::value); };
+template <int N>
+struct TrFinal<N, 5> { static constexpr int value = N; };
+template <bool MAX>
+__device__ __forceinline__ float tr_op(float a, float b) { return MAX ? fmaxf(a, b) : a + b; }
+template <bool MAX, int N, int B, int NV>
+__device__ __forceinline__ void tr_reduce(float (&v)[NV], int lane, int& row_base) {
+    if constexpr (B < 5) {
+        if constexpr (N % 2 == 0) {
+            constexpr int H = N / 2;
+            const bool up = (lane >> B) & 1;
+#pragma unroll
+            for (int i = 0; i < H; ++i) {
+                const float keep = up ? v[i + H] : v[i];
+                const float send = up ? v[i] : v[i + H];
+                v[i] = tr_op<MAX>(keep, __shfl_xor_sync(0xffffffffu, send, 1 << B));
+            }
+            if (up) row_base += H;
+            tr_reduce<MAX, H, B + 1>(v, lane, row_base);
+        } else {
+#pragma unroll
+            for (int i = 0; i < N; ++i) v[i] = tr_op<MAX>(v[i], __shfl_xor_sync(0xffffffffu, v[i], 1 << B));
+            tr_reduce<MAX, N, B + 1>(v, lane, row_base);
+        }
+    }
 }
 
 // ---- shared-memory plan --------------------------------------------------------------------------------------------
@@ -169,7 +210,7 @@ struct TcCfg {
     static constexpr int kNumBar = 2 * kSlotsN + 10;
     static constexpr int kOffTmem = kOffBar + kNumBar * 8;                // uint32 TMEM base, uint32 combine flag
     static constexpr int kSmemBytes = kOffTmem + 16;
-    static_assert(kSmemBytes + 1024 <= 232448, "shared-memory plan exceeds 227 KB");
+    static_assert(kSmemBytes <= 232448, "shared-memory plan exceeds 227 KB");
     static_assert(kOffQ % 1024 == 0 && kQBytes % 1024 == 0 && kOffP % 1024 == 0, "UMMA operands need 1 KB alignment");
 };
 
@@ -233,20 +274,27 @@ struct TileCursor {
 
 // ---- kernel -----------------------------------------------------------------------------------------------------
 struct TcWs {
-    int* counters;      // [B * Hkv] arrivals per unit, zeroed before the launch
+    int* flags;         // [grid, 2] "partial is in the workspace" flags, zeroed before the launch
+    unsigned long long* dbg_ts;   // optional timeline (DUSTIN_DBG & 8): [grid][64] globaltimer samples
     const void* zero_row;   // 256 zero bytes (zeroed with the counters): source of the rows past the end of a piece
     float* part_o;      // [grid, 2, rows, 128] normalised partial outputs
     float* part_lse;    // [grid, 2, rows] log2-domain normalisers
 };
 
+__device__ __forceinline__ unsigned long long gtimer() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+    return t;
+}
+#define TS(slot) do { if (ws.dbg_ts) ws.dbg_ts[(size_t)blockIdx.x * 64 + (slot)] = gtimer(); } while (0)
+
 template <int NQ, bool GATHER>
 __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams p, const TcWs ws) {
     using C = TcCfg<NQ>;
     constexpr int NS = C::kSlotsN;
-    extern __shared__ unsigned char smem_dyn[];
-    // 1 KB alignment for the 128-byte-swizzled operands
-    unsigned char* smem = reinterpret_cast<unsigned char*>(((uintptr_t)smem_dyn + 1023) & ~(uintptr_t)1023);
+    extern __shared__ __align__(1024) unsigned char smem[];   // 128-byte-swizzled operands need 1 KB alignment
     const uint32_t sbase = smem_u32(smem);
+    if (sbase & 1023u) __trap();
     int* s_prefix = reinterpret_cast<int*>(smem + C::kOffPrefix);
     float* s_ref = reinterpret_cast<float*>(smem + C::kOffRef);
     float* s_fac = reinterpret_cast<float*>(smem + C::kOffFac);
@@ -264,6 +312,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int T = p.n_new, r = p.group, rows = p.rows, Hkv = p.n_kv_heads, Hq = p.n_q_heads;
     const int n_units = p.batch * Hkv;
+    if (tid == 0) TS(0);
 
     // ---- token-list lengths of all units -> exclusive prefix sums (threads 0..255) --------------------------------
     auto unit_len = [&](int u) -> int {
@@ -278,11 +327,28 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
         }
         return c + T;
     };
+    // barriers and TMEM first: neither depends on the list lengths, whose loads are in flight meanwhile
+    const int per = (n_units + 255) / 256;
+    const int u_lo = min(tid * per, n_units), u_hi = tid < 256 ? min(u_lo + per, n_units) : u_lo;
+    int sum = 0;
+    for (int u = u_lo; u < u_hi; ++u) sum += unit_len(u);
+    if (tid == 0) {
+        for (int i = 0; i < NS; ++i) {
+            mbar_init(bar(kSlotFull + i), 128);
+            mbar_init(bar(kSlotEmpty + i), 1);
+        }
+        for (int i = 0; i < 2; ++i) {
+            mbar_init(bar(kQFull + i), 128);
+            mbar_init(bar(kQEmpty + i), 1);
+            mbar_init(bar(kSFull + i), 1);
+            mbar_init(bar(kSEmpty + i), 128);
+        }
+        mbar_init(bar(kPFull), 128);
+        mbar_init(bar(kPvDone), 1);
+        fence_mbar_init();
+    }
+    if (warp == 8) tmem_alloc(smem_u32(s_tmem), 512);
     {
-        const int per = (n_units + 255) / 256;
-        const int u_lo = min(tid * per, n_units), u_hi = tid < 256 ? min(u_lo + per, n_units) : u_lo;
-        int sum = 0;
-        for (int u = u_lo; u < u_hi; ++u) sum += unit_len(u);
         int inc = sum;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
@@ -303,14 +369,19 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
             s_ref[tid] = kRefInit;
             s_rowoff[tid] = ((tid / r) * Hq + tid % r) * kD;
         }
+        tc_fence_before();
         __syncthreads();
+        tc_fence_after();
     }
+    if (tid == 0) TS(1);
+    const uint32_t tmem = *s_tmem;
+    constexpr uint32_t kColS = 0, kColO = 256;   // S buffers at columns 0 and 128, O^T at 256
     const int total = s_prefix[n_units];
     const int chunk = (((total + (int)gridDim.x - 1) / (int)gridDim.x) + 31) & ~31;
     const int lo = (int)blockIdx.x * chunk, hi = min(lo + chunk, total);
-    if (lo >= hi) return;   // the whole CTA leaves before any barrier / TMEM state exists
-    int u0;
-    {
+    const bool active = lo < hi;   // a CTA past the end of the token space only takes part in the teardown
+    int u0 = 0;
+    if (active) {
         int a = 0, bnd = n_units;   // largest u with prefix[u] <= lo
         while (bnd - a > 1) {
             const int m = (a + bnd) >> 1;
@@ -318,35 +389,16 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
         }
         u0 = a;
     }
-
-    if (tid == 0) {
-        for (int i = 0; i < NS; ++i) {
-            mbar_init(bar(kSlotFull + i), 128);
-            mbar_init(bar(kSlotEmpty + i), 1);
-        }
-        for (int i = 0; i < 2; ++i) {
-            mbar_init(bar(kQFull + i), 128);
-            mbar_init(bar(kQEmpty + i), 1);
-            mbar_init(bar(kSFull + i), 1);
-            mbar_init(bar(kSEmpty + i), 128);
-        }
-        mbar_init(bar(kPFull), 128);
-        mbar_init(bar(kPvDone), 1);
-        fence_mbar_init();
-    }
-    if (warp == 4) tmem_alloc(smem_u32(s_tmem), 512);
-    tc_fence_before();
-    __syncthreads();
-    tc_fence_after();
-    const uint32_t tmem = *s_tmem;
-    constexpr uint32_t kColS = 0, kColO = 256;   // S buffers at columns 0 and 128, O^T at 256
+    if (tid == 0) TS(2);
 
     TileCursor cur;
     cur.init(s_prefix, n_units, Hkv, p.n_lists, T, lo, hi, chunk, u0);
+    if (!active) cur.valid = false;
 
-    if (warp >= 5) {
+    if (warp >= 4 && warp < 8) {
         // ================= producers ===========================================================================
-        const int pw = warp - 5, ptid = tid - 160;
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 96;");
+        const int pw = warp - 4, ptid = tid - 128;
         TileCursor pf = cur;   // runs two tiles ahead of `cur`
         struct Tok { int tok, b, g; };
         // token code of row 32*pw + lane of the cursor's tile: >= 0 cache row, -1 none, <= -2 new row (-2 - u)
@@ -418,11 +470,11 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
             cp_async_mbar_arrive_noinc(bar(kSlotFull + sv));
         };
 
-        Tok t1 = load_tok(pf);
-        pf.advance();
-        RowPtr a0 = resolve(t1);
-        t1 = load_tok(pf);
+        const Tok t0 = load_tok(pf);           // tiles 0 and 1: both index loads in flight before the first use
         if (pf.valid) pf.advance();
+        Tok t1 = load_tok(pf);
+        if (pf.valid) pf.advance();
+        RowPtr a0 = resolve(t0);
         int gj = 0;
         while (cur.valid) {
             Tok t2 = load_tok(pf);                 // tile gj + 2: index load in flight
@@ -443,14 +495,16 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
                 cp_async_mbar_arrive_noinc(bar(kQFull + qb));
             }
             issue_tile(gj, a0);
+            if (ptid == 0 && gj < 4) TS(4 + gj);
             a0 = a1;
             t1 = t2;
             cur.advance();
             ++gj;
         }
-    } else if (warp == 4) {
-        // ================= MMA issuer (one thread) ==============================================================
-        if (lane == 0) {
+    } else if (warp >= 8) {
+        // ================= MMA issuer (one thread of warp 8) =====================================================
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
+        if (warp == 8 && lane == 0) {
             constexpr uint32_t idesc_s = umma_idesc(kTile, NQ, 0, 0);    // S^T = K . Q^T : both K-major
             constexpr uint32_t idesc_pv = umma_idesc(kTile, NQ, 1, 1);   // O^T = V^T . P^T : both MN-major
             const uint32_t slots = sbase + C::kOffSlots, pbuf = sbase + C::kOffP;
@@ -497,6 +551,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
                 }
                 umma_commit(bar(kSlotEmpty + slot));
                 umma_commit(bar(kSFull + sb));
+                if (gj < 4) TS(8 + gj);
                 if (cur.last_tile()) umma_commit(bar(kQEmpty + qb));
                 if (have_prev) issue_pv(gj - 1, prev_first);
                 have_prev = true;
@@ -509,6 +564,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
         __syncwarp();
     } else {
         // ================= softmax warpgroup: thread = token of the tile = TMEM lane ==============================
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 240;");
         const int t = tid;
         const uint32_t lane_base = tmem + ((uint32_t)(warp * 32) << 16);
         const float sl2 = p.scale_log2;
@@ -523,6 +579,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
             const int sb = gj & 1;
             mbar_wait(bar(kSFull + sb), ((uint32_t)(gj >> 1)) & 1u);
             tc_fence_after();
+            if (t == 0 && gj < 20) TS(12 + gj);
             uint32_t xs[NQ];
 #pragma unroll
             for (int c = 0; c < NQ / 16; ++c)
@@ -552,10 +609,14 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
             }
             if (wg_any(over)) {
                 // Move the reference exponents to the running row maxima (rare after the first tile).
+                {
+                    float red[NQ];
 #pragma unroll
-                for (int i = 0; i < NQ; ++i) {
-                    const float wm = warp_max_f32(x[i]);
-                    if (lane == 0) s_warp[warp * NQ + i] = wm;
+                    for (int i = 0; i < NQ; ++i) red[i] = x[i];
+                    int rb = 0;
+                    tr_reduce<true, NQ, 0>(red, lane, rb);
+#pragma unroll
+                    for (int i = 0; i < TrFinal<NQ, 0>::value; ++i) s_warp[warp * NQ + rb + i] = red[i];
                 }
                 wg_sync();
                 if (t < NQ) {
@@ -611,113 +672,117 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
             mbar_arrive(bar(kPFull));
 
             if (cur.last_tile()) {
-                // ---- the piece is complete: normalise and write it (out or partial) ---------------------------------
+                if (t == 0) TS(32 + 4 * (cur.seg_no & 3));
+                // ---- the piece is complete ----------------------------------------------------------------------
+                // whole unit: normalise, write `out`.  Piece that does not start its unit: leave a normalised partial
+                // (o, lse) in the workspace and raise its flag.  Piece that starts a unit cut into several (the head;
+                // it runs last in its CTA while the others run first in theirs): pull the other pieces -- normally
+                // long finished -- and merge them with this CTA's accumulator, own piece first, then in CTA order.
+                const bool merge = s.pos_lo == 0 && !s.whole;
+                const int nseg = s.cta_last - s.cta_first + 1;
+                const long long slot_id = (long long)blockIdx.x * 2 + s.slot;
+                float v1[NQ];
+                float lse1 = -INFINITY;
+                if (merge) {   // second piece = slot 0 of the next CTA: loads in flight during the reductions below
+                    const long long sid1 = (long long)(s.cta_first + 1) * 2;
+                    wait_flag(ws.flags + sid1);
+                    const float* src1 = ws.part_o + sid1 * rows * kD + t;
 #pragma unroll
-                for (int i = 0; i < NQ; ++i) {
-                    float v = lpart[i];
+                    for (int i = 0; i < NQ; ++i) v1[i] = i < rows ? __ldcg(src1 + i * kD) : 0.f;
+                    if (t < rows) lse1 = __ldcg(ws.part_lse + sid1 * rows + t);
+                }
+                {
+                    int rb = 0;
+                    tr_reduce<false, NQ, 0>(lpart, lane, rb);
 #pragma unroll
-                    for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
-                    if (lane == 0) s_warp[warp * NQ + i] = v;
-                    lpart[i] = 0.f;
+                    for (int i = 0; i < TrFinal<NQ, 0>::value; ++i) s_warp[warp * NQ + rb + i] = lpart[i];
+#pragma unroll
+                    for (int i = 0; i < NQ; ++i) lpart[i] = 0.f;
+                }
+                wg_sync();
+                float M_row = 0.f, W_row = 0.f;   // thread t < rows: merged maximum and weight sum of row t
+                if (t < NQ) {
+                    const float l = (s_warp[t] + s_warp[NQ + t]) + (s_warp[2 * NQ + t] + s_warp[3 * NQ + t]);
+                    const float lse_own = l > 0.f ? s_ref[t] + log2f(l) : -INFINITY;
+                    float scale = l > 0.f ? 1.f / l : 0.f, lse_fin = lse_own;
+                    if (merge && t < rows) {
+                        float M = fmaxf(lse_own, lse1);
+                        for (int j = 2; j < nseg; ++j) {
+                            const long long sid = (long long)(s.cta_first + j) * 2;
+                            wait_flag(ws.flags + sid);
+                            M = fmaxf(M, __ldcg(ws.part_lse + sid * rows + t));
+                        }
+                        const float e0 = lse_own == -INFINITY ? 0.f : exp2f(lse_own - M);
+                        const float e1 = lse1 == -INFINITY ? 0.f : exp2f(lse1 - M);
+                        float W = e0 + e1;
+                        for (int j = 2; j < nseg; ++j) {
+                            const float lj = __ldcg(ws.part_lse + ((long long)(s.cta_first + j) * 2) * rows + t);
+                            W += lj == -INFINITY ? 0.f : exp2f(lj - M);
+                        }
+                        const float invW = W > 0.f ? 1.f / W : 0.f;
+                        scale *= e0 * invW;
+                        s_wgt[t] = e1 * invW;
+                        lse_fin = W > 0.f ? M + log2f(W) : -INFINITY;
+                        M_row = M;
+                        W_row = invW;
+                    }
+                    s_fac[t] = scale;
+                    if (t < rows) {
+                        if (s.pos_lo != 0) ws.part_lse[slot_id * rows + t] = lse_own;
+                        else if (p.lse_out)
+                            p.lse_out[((long long)s.b * Hq + s.g * r + t % r) * T + t / r] = lse_fin * kLn2;
+                    }
                 }
                 mbar_wait(bar(kPvDone), (uint32_t)gj & 1u);   // every P.V of the piece has completed
                 tc_fence_after();
-                wg_sync();
                 uint32_t o[NQ];
 #pragma unroll
                 for (int c = 0; c < NQ / 16; ++c)
                     tmem_ld16(lane_base + kColO + (uint32_t)c * 16, reinterpret_cast<uint32_t(&)[16]>(o[c * 16]));
                 tmem_wait_ld();
                 tc_fence_before();
-                const long long slot_id = (long long)blockIdx.x * 2 + s.slot;
+                wg_sync();
+                if (t == 0) TS(33 + 4 * (cur.seg_no & 3));
                 __nv_bfloat16* outb = p.out + ((long long)s.b * T * Hq + (long long)s.g * r) * kD + t;   // t = dim
-                float* po = ws.part_o + slot_id * rows * kD + t;
+                if (s.pos_lo != 0) {
+                    float* po = ws.part_o + slot_id * rows * kD + t;
 #pragma unroll
-                for (int i = 0; i < NQ; ++i) {
-                    if (i < rows) {
-                        const float l = (s_warp[i] + s_warp[NQ + i]) + (s_warp[2 * NQ + i] + s_warp[3 * NQ + i]);
-                        const float v = __uint_as_float(o[i]) * (l > 0.f ? 1.f / l : 0.f);
-                        if (s.whole) outb[s_rowoff[i]] = __float2bfloat16_rn(v);
-                        else po[i * kD] = v;
-                    }
-                }
-                if (t < rows) {
-                    const float l = (s_warp[t] + s_warp[NQ + t]) + (s_warp[2 * NQ + t] + s_warp[3 * NQ + t]);
-                    const float lse2 = l > 0.f ? s_ref[t] + log2f(l) : -INFINITY;
-                    if (!s.whole) ws.part_lse[slot_id * rows + t] = lse2;
-                    else if (p.lse_out)
-                        p.lse_out[((long long)s.b * Hq + s.g * r + t % r) * T + t / r] = lse2 * kLn2;
-                }
-                if (!s.whole) {
-                    // last piece of the unit to arrive merges all of them, in CTA order
-                    __threadfence();
+                    for (int i = 0; i < NQ; ++i)
+                        if (i < rows) po[i * kD] = __uint_as_float(o[i]) * s_fac[i];
+                    // publish: the barrier orders the warpgroup's stores before thread 0's fence and flag
                     wg_sync();
-                    if (t == 0) s_tmem[1] = atomicAdd(ws.counters + s.u, 1) == s.cta_last - s.cta_first ? 1u : 0u;
-                    wg_sync();
-                    if (s_tmem[1]) {
+                    if (t == 0) {
                         __threadfence();
-                        const int ps = s_prefix[s.u];
-                        const int nseg = s.cta_last - s.cta_first + 1;
-                        auto slot_of = [&](int c) -> long long { return (long long)c * 2 + (ps <= c * chunk ? 0 : 1); };
-                        if (nseg <= kMergeFast) {
-                            // weights of the pieces, row t by thread t: all normalisers are loaded at once
-                            if (t < rows) {
-                                float l[kMergeFast];
+                        st_release(ws.flags + slot_id, 1);
+                    }
+                } else {
+                    float acc[NQ];
 #pragma unroll
-                                for (int j = 0; j < kMergeFast; ++j)
-                                    l[j] = j < nseg ? __ldcg(ws.part_lse + slot_of(s.cta_first + j) * rows + t) : -INFINITY;
-                                float M = l[0];
+                    for (int i = 0; i < NQ; ++i) acc[i] = __uint_as_float(o[i]) * s_fac[i];
+                    if (merge) {
 #pragma unroll
-                                for (int j = 1; j < kMergeFast; ++j) M = fmaxf(M, l[j]);
-                                float w[kMergeFast], W = 0.f;
-#pragma unroll
-                                for (int j = 0; j < kMergeFast; ++j) {
-                                    w[j] = l[j] == -INFINITY ? 0.f : exp2f(l[j] - M);
-                                    W += w[j];
-                                }
-                                const float inv = W > 0.f ? 1.f / W : 0.f;
-#pragma unroll
-                                for (int j = 0; j < kMergeFast; ++j) s_wgt[j * NQ + t] = w[j] * inv;
-                                if (p.lse_out)
-                                    p.lse_out[((long long)s.b * Hq + s.g * r + t % r) * T + t / r] =
-                                        W > 0.f ? (M + log2f(W)) * kLn2 : -INFINITY;
-                            }
+                        for (int i = 0; i < NQ; ++i) acc[i] = fmaf(s_wgt[i], v1[i], acc[i]);
+                        for (int j = 2; j < nseg; ++j) {   // units cut into more than two pieces (very long sequences)
+                            const long long sid = (long long)(s.cta_first + j) * 2;
                             wg_sync();
-                            float acc[NQ];
-#pragma unroll
-                            for (int i = 0; i < NQ; ++i) acc[i] = 0.f;
-                            for (int j = 0; j < nseg; ++j) {   // pieces in CTA order; the NQ loads of one piece are independent
-                                const float* src = ws.part_o + slot_of(s.cta_first + j) * rows * kD + t;
-                                float v[NQ];
-#pragma unroll
-                                for (int i = 0; i < NQ; ++i) v[i] = i < rows ? __ldcg(src + i * kD) : 0.f;
-#pragma unroll
-                                for (int i = 0; i < NQ; ++i) acc[i] = fmaf(s_wgt[j * NQ + i], v[i], acc[i]);
+                            if (t < rows) {
+                                const float lj = __ldcg(ws.part_lse + sid * rows + t);
+                                s_wgt[t] = lj == -INFINITY ? 0.f : exp2f(lj - M_row) * W_row;
                             }
+                            const float* src = ws.part_o + sid * rows * kD + t;
 #pragma unroll
-                            for (int i = 0; i < NQ; ++i)
-                                if (i < rows) outb[s_rowoff[i]] = __float2bfloat16_rn(acc[i]);
-                        } else {
-                            // a unit cut into many pieces (one very long sequence): plain sequential merge
-                            for (int i = 0; i < rows; ++i) {
-                                float M = -INFINITY;
-                                for (int c = s.cta_first; c <= s.cta_last; ++c)
-                                    M = fmaxf(M, __ldcg(ws.part_lse + slot_of(c) * rows + i));
-                                float W = 0.f, acc = 0.f;
-                                for (int c = s.cta_first; c <= s.cta_last; ++c) {
-                                    const float lse = __ldcg(ws.part_lse + slot_of(c) * rows + i);
-                                    const float w = lse == -INFINITY ? 0.f : exp2f(lse - M);
-                                    acc += w * __ldcg(ws.part_o + (slot_of(c) * rows + i) * kD + t);
-                                    W += w;
-                                }
-                                outb[s_rowoff[i]] = __float2bfloat16_rn(W > 0.f ? acc / W : 0.f);
-                                if (p.lse_out && t == 0)
-                                    p.lse_out[((long long)s.b * Hq + s.g * r + i % r) * T + i / r] =
-                                        W > 0.f ? (M + log2f(W)) * kLn2 : -INFINITY;
-                            }
+                            for (int i = 0; i < NQ; ++i) v1[i] = i < rows ? __ldcg(src + i * kD) : 0.f;
+                            wg_sync();
+#pragma unroll
+                            for (int i = 0; i < NQ; ++i) acc[i] = fmaf(s_wgt[i], v1[i], acc[i]);
                         }
                     }
+#pragma unroll
+                    for (int i = 0; i < NQ; ++i)
+                        if (i < rows) outb[s_rowoff[i]] = __float2bfloat16_rn(acc[i]);
                 }
+                if (t == 0) TS(34 + 4 * (cur.seg_no & 3));
+                if (t == 0) TS(35 + 4 * (cur.seg_no & 3));
                 wg_sync();
                 if (t < NQ) s_ref[t] = kRefInit;
                 wg_sync();
@@ -729,7 +794,8 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
 
     tc_fence_before();
     __syncthreads();
-    if (warp == 4) {
+    if (tid == 0) TS(3);
+    if (warp == 8) {
         tc_fence_after();
         tmem_dealloc(tmem, 512);
     }
@@ -755,7 +821,7 @@ inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 template <int NQ, bool GATHER>
 cudaError_t launch_tc(const AttnParams& p, const TcWs& ws, int grid, cudaStream_t stream) {
     using C = TcCfg<NQ>;
-    constexpr int smem = C::kSmemBytes + 1024;
+    constexpr int smem = C::kSmemBytes;
     static bool attr_done = false;   // per instantiation
     if (!attr_done) {
         cudaError_t e = cudaFuncSetAttribute(attn_tc_kernel<NQ, GATHER>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
@@ -782,8 +848,8 @@ bool attn_tc_usable(int batch, int n_kv_heads, int head_dim, int rows, int max_t
 }
 
 size_t attn_tc_ws_bytes(int batch, int n_kv_heads, int rows) {
-    return align256((size_t)batch * n_kv_heads * sizeof(int)) + 256 + align256((size_t)kMaxGrid * 2 * rows * kD * sizeof(float)) +
-           align256((size_t)kMaxGrid * 2 * rows * sizeof(float));
+    return align256((size_t)kMaxGrid * 2 * sizeof(int)) + 256 + align256((size_t)kMaxGrid * 2 * rows * kD * sizeof(float)) +
+           align256((size_t)kMaxGrid * 2 * rows * sizeof(float)) + (size_t)kMaxGrid * 64 * 8;
 }
 
 cudaError_t launch_attn_tc(const AttnParams& p_in, void* ws_base, cudaStream_t stream) {
@@ -792,11 +858,12 @@ cudaError_t launch_attn_tc(const AttnParams& p_in, void* ws_base, cudaStream_t s
     const size_t units = (size_t)p.batch * p.n_kv_heads;
     char* base = static_cast<char*>(ws_base);
     TcWs ws;
-    ws.counters = reinterpret_cast<int*>(base);
-    const size_t head = align256(units * sizeof(int)) + 256;   // counters, then the zero row
+    ws.flags = reinterpret_cast<int*>(base);
+    const size_t head = align256((size_t)kMaxGrid * 2 * sizeof(int)) + 256;   // flags, then the zero row
     ws.zero_row = base + head - 256;
     ws.part_o = reinterpret_cast<float*>(base + head);
     ws.part_lse = reinterpret_cast<float*>(base + head + align256((size_t)kMaxGrid * 2 * p.rows * kD * sizeof(float)));
+    ws.dbg_ts = (p.dbg & 8) ? reinterpret_cast<unsigned long long*>(reinterpret_cast<char*>(ws.part_lse) + align256((size_t)kMaxGrid * 2 * p.rows * sizeof(float))) : nullptr;
     cudaError_t e = cudaMemsetAsync(base, 0, head, stream);
     if (e != cudaSuccess) return e;
     const int max_tokens = (p.idx ? (p.k_max < p.max_ctx ? p.k_max : p.max_ctx) : p.max_ctx) + p.n_new;
