@@ -84,6 +84,13 @@ int         dustin_version(void);
 const char* dustin_status_string(int status);
 int         dustin_last_cuda_error(void);            /* cudaError_t of the last failed launch on this thread     */
 
+/* Workspace.  The first DUSTIN_WS_HEADER_BYTES of a workspace persist between calls (completion flags of the
+ * attention kernel and a row of zeros): they must be ZERO before the first call that uses the buffer and must not
+ * be written by the caller afterwards; every call that returns DUSTIN_OK and runs to completion leaves them zero
+ * again, so one memset at allocation time serves any number of calls (and CUDA-graph replays).  The rest of the
+ * buffer is plain scratch with no state.  One workspace must not be used by two calls that run concurrently. */
+#define DUSTIN_WS_HEADER_BYTES 4096
+
 /* Scratch (bytes of device memory, 256-byte aligned by the caller) that is enough for every entry point on this
  * shape: the scoring stage with the head subset `head_mask` (0 => sized for all n_q_heads heads) plus the
  * attention stage over at most `k_max` selected rows per list (k_max <= 0 => max_ctx rows, the dense case).

@@ -218,8 +218,9 @@ def workspace_bytes(shape: Shape, head_mask: int = 0, k_max: int = 0) -> int:
 
 
 def alloc_workspace(shape: Shape, head_mask: int = 0, k_max: int = 0, device="cuda") -> torch.Tensor:
-    """A uint8 device buffer of dustin_workspace_bytes (torch allocations are 512-byte aligned)."""
-    return torch.empty(workspace_bytes(shape, head_mask, k_max), dtype=torch.uint8, device=device)
+    """A uint8 device buffer of dustin_workspace_bytes (torch allocations are 512-byte aligned), zeroed: the first
+    DUSTIN_WS_HEADER_BYTES must be zero before the first call (dustin.h, "Workspace")."""
+    return torch.zeros(workspace_bytes(shape, head_mask, k_max), dtype=torch.uint8, device=device)
 
 
 def score_heads(shape: Shape, kv: KV, q: torch.Tensor, head_mask: int, n_lists: int, scores_now: torch.Tensor,

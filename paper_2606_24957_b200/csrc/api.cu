@@ -163,7 +163,7 @@ int run_score(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q,
     rc = build_subset(shape, head_mask, n_lists, &p);
     if (rc) return rc;
     const ScoreWs w = score_ws(shape->batch, p.nsel, shape->max_ctx);
-    if (!ws || ws_bytes < w.total || ((uintptr_t)ws & 255)) return DUSTIN_ERR_WORKSPACE;
+    if (!ws || ws_bytes < kWsHeader + w.total || ((uintptr_t)ws & 255)) return DUSTIN_ERR_WORKSPACE;
     p.q = static_cast<const __nv_bfloat16*>(q);
     p.q_stride_batch = q_stride_batch;
     p.q_stride_head = q_stride_head;
@@ -174,7 +174,7 @@ int run_score(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q,
     p.scale_log2 = scale_log2_of(shape);
     score_plan(p.batch, p.n_groups, p.max_ctx, &p.chunk_tokens, &p.n_chunks);
     p.logit_stride = ((long long)p.max_ctx + 3) & ~3ll;
-    char* base = static_cast<char*>(ws);
+    char* base = static_cast<char*>(ws) + kWsHeader;   // the persistent header belongs to the attention stage
     p.logits = reinterpret_cast<float*>(base + w.logits);
     p.part = reinterpret_cast<float2*>(base + w.part);
     p.stats = reinterpret_cast<float2*>(base + w.stats);
@@ -317,7 +317,7 @@ size_t dustin_workspace_bytes(const dustin_shape_t* shape, uint64_t head_mask, i
     int max_tokens = (k_max > 0 && k_max < shape->max_ctx) ? k_max : shape->max_ctx;
     if (max_tokens < 1) max_tokens = 1;
     const AttnWs aw = attn_ws(shape, max_tokens);
-    return sw.total + aw.total + 256;
+    return kWsHeader + sw.total + aw.total + 256;
 }
 
 int dustin_score_heads(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q, int64_t q_stride_batch,
@@ -374,12 +374,12 @@ int dustin_verify_layer_fused(const dustin_shape_t* shape, const dustin_kv_t* kv
     const ScoreWs sw = score_ws(shape->batch, nsel, shape->max_ctx);
     const int max_tokens = k_max < shape->max_ctx ? k_max : shape->max_ctx;
     const AttnWs aw = attn_ws(shape, max_tokens > 0 ? max_tokens : 1);
-    if (!ws || ((uintptr_t)ws & 255) || ws_bytes < sw.total + aw.total) return DUSTIN_ERR_WORKSPACE;
+    if (!ws || ((uintptr_t)ws & 255) || ws_bytes < kWsHeader + sw.total + aw.total) return DUSTIN_ERR_WORKSPACE;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     char* base = static_cast<char*>(ws);
     // a1 + a2: scores of verify position 0 (reading A3), accumulated straight into hist (Eq. 5)
     rc = run_score(shape, kv, q, (int64_t)shape->n_new * shape->n_q_heads * shape->head_dim, shape->head_dim,
-                   head_mask, select->n_lists, scores_now_out, hist_inout, alpha, base, sw.total, st);
+                   head_mask, select->n_lists, scores_now_out, hist_inout, alpha, ws, ws_bytes, st);
     if (rc) return rc;
     // a3
     rc = run_select(shape->batch, shape->max_ctx, kv->seq_lens, select, s_draft, draft_list_stride, hist_inout,
@@ -387,7 +387,7 @@ int dustin_verify_layer_fused(const dustin_shape_t* shape, const dustin_kv_t* kv
     if (rc) return rc;
     // a4
     return run_attn(shape, kv, q, k_new, v_new, idx_out, cnt_out, select->n_lists, k_max, out, lse_out,
-                    base + sw.total, ws_bytes - sw.total, st);
+                    ws, ws_bytes, st);
 }
 
 }  // extern "C"

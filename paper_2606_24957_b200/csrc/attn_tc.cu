@@ -691,6 +691,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
                     for (int i = 0; i < NQ; ++i) v1[i] = i < rows ? __ldcg(src1 + i * kD) : 0.f;
                     if (t < rows) lse1 = __ldcg(ws.part_lse + sid1 * rows + t);
                 }
+                if (t == 0) TS(56);
                 {
                     int rb = 0;
                     tr_reduce<false, NQ, 0>(lpart, lane, rb);
@@ -733,8 +734,10 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
                             p.lse_out[((long long)s.b * Hq + s.g * r + t % r) * T + t / r] = lse_fin * kLn2;
                     }
                 }
+                if (t == 0) TS(54);
                 mbar_wait(bar(kPvDone), (uint32_t)gj & 1u);   // every P.V of the piece has completed
                 tc_fence_after();
+                if (t == 0) TS(55);
                 uint32_t o[NQ];
 #pragma unroll
                 for (int c = 0; c < NQ / 16; ++c)
@@ -742,6 +745,8 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
                 tmem_wait_ld();
                 tc_fence_before();
                 wg_sync();
+                if (merge && t == 0)   // every thread is past its flag waits: leave the flags zero for the next launch
+                    for (int j = 1; j < nseg; ++j) ws.flags[(long long)(s.cta_first + j) * 2] = 0;
                 if (t == 0) TS(33 + 4 * (cur.seg_no & 3));
                 __nv_bfloat16* outb = p.out + ((long long)s.b * T * Hq + (long long)s.g * r) * kD + t;   // t = dim
                 if (s.pos_lo != 0) {
@@ -777,6 +782,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
                             for (int i = 0; i < NQ; ++i) acc[i] = fmaf(s_wgt[i], v1[i], acc[i]);
                         }
                     }
+                    if (t == 0) TS(53);
 #pragma unroll
                     for (int i = 0; i < NQ; ++i)
                         if (i < rows) outb[s_rowoff[i]] = __float2bfloat16_rn(acc[i]);
@@ -848,7 +854,8 @@ bool attn_tc_usable(int batch, int n_kv_heads, int head_dim, int rows, int max_t
 }
 
 size_t attn_tc_ws_bytes(int batch, int n_kv_heads, int rows) {
-    return align256((size_t)kMaxGrid * 2 * sizeof(int)) + 256 + align256((size_t)kMaxGrid * 2 * rows * kD * sizeof(float)) +
+    static_assert(kMaxGrid * 2 * sizeof(int) + 256 <= kWsHeader, "flags + zero row must fit the persistent header");
+    return kWsHeader + align256((size_t)kMaxGrid * 2 * rows * kD * sizeof(float)) +
            align256((size_t)kMaxGrid * 2 * rows * sizeof(float)) + (size_t)kMaxGrid * 64 * 8;
 }
 
@@ -857,15 +864,15 @@ cudaError_t launch_attn_tc(const AttnParams& p_in, void* ws_base, cudaStream_t s
     { const char* e = getenv("DUSTIN_DBG"); p.dbg = e ? atoi(e) : 0; }
     const size_t units = (size_t)p.batch * p.n_kv_heads;
     char* base = static_cast<char*>(ws_base);
+    (void)stream;
     TcWs ws;
+    // Persistent header (kernels.cuh kWsHeader): flags at 0, the zero row at 2048.  Zero before the first use
+    // (dustin.h); every launch leaves it zero again (the merging piece clears the flags it has consumed).
     ws.flags = reinterpret_cast<int*>(base);
-    const size_t head = align256((size_t)kMaxGrid * 2 * sizeof(int)) + 256;   // flags, then the zero row
-    ws.zero_row = base + head - 256;
-    ws.part_o = reinterpret_cast<float*>(base + head);
-    ws.part_lse = reinterpret_cast<float*>(base + head + align256((size_t)kMaxGrid * 2 * p.rows * kD * sizeof(float)));
+    ws.zero_row = base + 2048;
+    ws.part_o = reinterpret_cast<float*>(base + kWsHeader);
+    ws.part_lse = reinterpret_cast<float*>(base + kWsHeader + align256((size_t)kMaxGrid * 2 * p.rows * kD * sizeof(float)));
     ws.dbg_ts = (p.dbg & 8) ? reinterpret_cast<unsigned long long*>(reinterpret_cast<char*>(ws.part_lse) + align256((size_t)kMaxGrid * 2 * p.rows * sizeof(float))) : nullptr;
-    cudaError_t e = cudaMemsetAsync(base, 0, head, stream);
-    if (e != cudaSuccess) return e;
     const int max_tokens = (p.idx ? (p.k_max < p.max_ctx ? p.k_max : p.max_ctx) : p.max_ctx) + p.n_new;
     long long tiles = ((long long)units * max_tokens + kTile - 1) / kTile;
     int grid = sm_count() < kMaxGrid ? sm_count() : kMaxGrid;
