@@ -141,6 +141,16 @@ __host__ __device__ constexpr uint32_t umma_idesc(int m, int n, int a_mn_major, 
            ((uint32_t)(n >> 3) << 17) | ((uint32_t)(m >> 4) << 24);
 }
 
+// Predicated 2-byte store without a branch (keeps unrolled row loops in one basic block).
+__device__ __forceinline__ void st_bf16_if(__nv_bfloat16* p, float v, bool pred) {
+    const __nv_bfloat16 b = __float2bfloat16_rn(v);
+    asm volatile(
+        "{\n\t.reg .pred q;\n\t"
+        "setp.ne.b32 q, %2, 0;\n\t"
+        "@q st.global.b16 [%0], %1;\n\t}" ::"l"(p),
+        "h"(*reinterpret_cast<const unsigned short*>(&b)), "r"((uint32_t)pred)
+        : "memory");
+}
 __device__ __forceinline__ void st_release(int* p, int v) {
     asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
@@ -686,10 +696,10 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
                 if (merge) {   // second piece = slot 0 of the next CTA: loads in flight during the reductions below
                     const long long sid1 = (long long)(s.cta_first + 1) * 2;
                     wait_flag(ws.flags + sid1);
-                    const float* src1 = ws.part_o + sid1 * rows * kD + t;
+                    const float* src1 = ws.part_o + sid1 * NQ * kD + t;
 #pragma unroll
-                    for (int i = 0; i < NQ; ++i) v1[i] = i < rows ? __ldcg(src1 + i * kD) : 0.f;
-                    if (t < rows) lse1 = __ldcg(ws.part_lse + sid1 * rows + t);
+                    for (int i = 0; i < NQ; ++i) v1[i] = __ldcg(src1 + i * kD);
+                    if (t < rows) lse1 = __ldcg(ws.part_lse + sid1 * NQ + t);
                 }
                 if (t == 0) TS(56);
                 {
@@ -711,13 +721,13 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
                         for (int j = 2; j < nseg; ++j) {
                             const long long sid = (long long)(s.cta_first + j) * 2;
                             wait_flag(ws.flags + sid);
-                            M = fmaxf(M, __ldcg(ws.part_lse + sid * rows + t));
+                            M = fmaxf(M, __ldcg(ws.part_lse + sid * NQ + t));
                         }
                         const float e0 = lse_own == -INFINITY ? 0.f : exp2f(lse_own - M);
                         const float e1 = lse1 == -INFINITY ? 0.f : exp2f(lse1 - M);
                         float W = e0 + e1;
                         for (int j = 2; j < nseg; ++j) {
-                            const float lj = __ldcg(ws.part_lse + ((long long)(s.cta_first + j) * 2) * rows + t);
+                            const float lj = __ldcg(ws.part_lse + ((long long)(s.cta_first + j) * 2) * NQ + t);
                             W += lj == -INFINITY ? 0.f : exp2f(lj - M);
                         }
                         const float invW = W > 0.f ? 1.f / W : 0.f;
@@ -729,7 +739,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
                     }
                     s_fac[t] = scale;
                     if (t < rows) {
-                        if (s.pos_lo != 0) ws.part_lse[slot_id * rows + t] = lse_own;
+                        if (s.pos_lo != 0) ws.part_lse[slot_id * NQ + t] = lse_own;
                         else if (p.lse_out)
                             p.lse_out[((long long)s.b * Hq + s.g * r + t % r) * T + t / r] = lse_fin * kLn2;
                     }
@@ -750,10 +760,9 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
                 if (t == 0) TS(33 + 4 * (cur.seg_no & 3));
                 __nv_bfloat16* outb = p.out + ((long long)s.b * T * Hq + (long long)s.g * r) * kD + t;   // t = dim
                 if (s.pos_lo != 0) {
-                    float* po = ws.part_o + slot_id * rows * kD + t;
+                    float* po = ws.part_o + slot_id * NQ * kD + t;   // padded to NQ rows: no predicate
 #pragma unroll
-                    for (int i = 0; i < NQ; ++i)
-                        if (i < rows) po[i * kD] = __uint_as_float(o[i]) * s_fac[i];
+                    for (int i = 0; i < NQ; ++i) po[i * kD] = __uint_as_float(o[i]) * s_fac[i];
                     // publish: the barrier orders the warpgroup's stores before thread 0's fence and flag
                     wg_sync();
                     if (t == 0) {
@@ -771,21 +780,23 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
                             const long long sid = (long long)(s.cta_first + j) * 2;
                             wg_sync();
                             if (t < rows) {
-                                const float lj = __ldcg(ws.part_lse + sid * rows + t);
+                                const float lj = __ldcg(ws.part_lse + sid * NQ + t);
                                 s_wgt[t] = lj == -INFINITY ? 0.f : exp2f(lj - M_row) * W_row;
                             }
-                            const float* src = ws.part_o + sid * rows * kD + t;
+                            const float* src = ws.part_o + sid * NQ * kD + t;
 #pragma unroll
-                            for (int i = 0; i < NQ; ++i) v1[i] = i < rows ? __ldcg(src + i * kD) : 0.f;
+                            for (int i = 0; i < NQ; ++i) v1[i] = __ldcg(src + i * kD);
                             wg_sync();
 #pragma unroll
                             for (int i = 0; i < NQ; ++i) acc[i] = fmaf(s_wgt[i], v1[i], acc[i]);
                         }
                     }
                     if (t == 0) TS(53);
+                    int ro[NQ];
 #pragma unroll
-                    for (int i = 0; i < NQ; ++i)
-                        if (i < rows) outb[s_rowoff[i]] = __float2bfloat16_rn(acc[i]);
+                    for (int i = 0; i < NQ; ++i) ro[i] = s_rowoff[i];
+#pragma unroll
+                    for (int i = 0; i < NQ; ++i) st_bf16_if(outb + ro[i], acc[i], i < rows);
                 }
                 if (t == 0) TS(34 + 4 * (cur.seg_no & 3));
                 if (t == 0) TS(35 + 4 * (cur.seg_no & 3));
@@ -855,8 +866,9 @@ bool attn_tc_usable(int batch, int n_kv_heads, int head_dim, int rows, int max_t
 
 size_t attn_tc_ws_bytes(int batch, int n_kv_heads, int rows) {
     static_assert(kMaxGrid * 2 * sizeof(int) + 256 <= kWsHeader, "flags + zero row must fit the persistent header");
-    return kWsHeader + align256((size_t)kMaxGrid * 2 * rows * kD * sizeof(float)) +
-           align256((size_t)kMaxGrid * 2 * rows * sizeof(float)) + (size_t)kMaxGrid * 64 * 8;
+    const size_t nq = (size_t)((rows + 15) / 16) * 16;   // partials are padded to the kernel's NQ rows
+    return kWsHeader + align256((size_t)kMaxGrid * 2 * nq * kD * sizeof(float)) +
+           align256((size_t)kMaxGrid * 2 * nq * sizeof(float)) + (size_t)kMaxGrid * 64 * 8;
 }
 
 cudaError_t launch_attn_tc(const AttnParams& p_in, void* ws_base, cudaStream_t stream) {
@@ -871,8 +883,9 @@ cudaError_t launch_attn_tc(const AttnParams& p_in, void* ws_base, cudaStream_t s
     ws.flags = reinterpret_cast<int*>(base);
     ws.zero_row = base + 2048;
     ws.part_o = reinterpret_cast<float*>(base + kWsHeader);
-    ws.part_lse = reinterpret_cast<float*>(base + kWsHeader + align256((size_t)kMaxGrid * 2 * p.rows * kD * sizeof(float)));
-    ws.dbg_ts = (p.dbg & 8) ? reinterpret_cast<unsigned long long*>(reinterpret_cast<char*>(ws.part_lse) + align256((size_t)kMaxGrid * 2 * p.rows * sizeof(float))) : nullptr;
+    const size_t nq = (size_t)((p.rows + 15) / 16) * 16;
+    ws.part_lse = reinterpret_cast<float*>(base + kWsHeader + align256((size_t)kMaxGrid * 2 * nq * kD * sizeof(float)));
+    ws.dbg_ts = (p.dbg & 8) ? reinterpret_cast<unsigned long long*>(reinterpret_cast<char*>(ws.part_lse) + align256((size_t)kMaxGrid * 2 * nq * sizeof(float))) : nullptr;
     const int max_tokens = (p.idx ? (p.k_max < p.max_ctx ? p.k_max : p.max_ctx) : p.max_ctx) + p.n_new;
     long long tiles = ((long long)units * max_tokens + kTile - 1) / kTile;
     int grid = sm_count() < kMaxGrid ? sm_count() : kMaxGrid;
