@@ -85,7 +85,7 @@ const char* dustin_status_string(int status);
 int         dustin_last_cuda_error(void);            /* cudaError_t of the last failed launch on this thread     */
 
 /* Workspace.  The first DUSTIN_WS_HEADER_BYTES of a workspace persist between calls (completion flags of the
- * attention kernel and a row of zeros): they must be ZERO before the first call that uses the buffer and must not
+ * attention kernel): they must be ZERO before the first call that uses the buffer and must not
  * be written by the caller afterwards; every call that returns DUSTIN_OK and runs to completion leaves them zero
  * again, so one memset at allocation time serves any number of calls (and CUDA-graph replays).  The rest of the
  * buffer is plain scratch with no state.  One workspace must not be used by two calls that run concurrently. */

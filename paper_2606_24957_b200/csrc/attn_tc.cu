@@ -215,8 +215,8 @@ struct TcCfg {
     static constexpr int kOffWgt = kOffWarp + 4 * NQ * 4;                 // float [kMergeFast][NQ]: merge weights
     static constexpr int kOffRowTab = (kOffWgt + kMergeFast * NQ * 4 + 15) & ~15;   // {K row, V row} addresses, 4 x 32
     static constexpr int kOffRowOff = kOffRowTab + 128 * 16;              // int row -> element offset inside out[b]
-    static constexpr int kOffScan = kOffRowOff + NQ * 4;                  // int [8] warp totals of the prefix scan
-    static constexpr int kOffBar = (kOffScan + 8 * 4 + 8 + 7) & ~7;       // uint64 barriers
+    static constexpr int kOffScan = kOffRowOff + NQ * 4;                  // int [16] warp totals / maxima of the scan
+    static constexpr int kOffBar = (kOffScan + 16 * 4 + 8 + 7) & ~7;      // uint64 barriers
     static constexpr int kNumBar = 2 * kSlotsN + 10;
     static constexpr int kOffTmem = kOffBar + kNumBar * 8;                // uint32 TMEM base, uint32 combine flag
     static constexpr int kSmemBytes = kOffTmem + 16;
@@ -286,7 +286,6 @@ struct TileCursor {
 struct TcWs {
     int* flags;         // [grid, 2] "partial is in the workspace" flags, zeroed before the launch
     unsigned long long* dbg_ts;   // optional timeline (DUSTIN_DBG & 8): [grid][64] globaltimer samples
-    const void* zero_row;   // 256 zero bytes (zeroed with the counters): source of the rows past the end of a piece
     float* part_o;      // [grid, 2, rows, 128] normalised partial outputs
     float* part_lse;    // [grid, 2, rows] log2-domain normalisers
 };
@@ -340,8 +339,12 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
     // barriers and TMEM first: neither depends on the list lengths, whose loads are in flight meanwhile
     const int per = (n_units + 255) / 256;
     const int u_lo = min(tid * per, n_units), u_hi = tid < 256 ? min(u_lo + per, n_units) : u_lo;
-    int sum = 0;
-    for (int u = u_lo; u < u_hi; ++u) sum += unit_len(u);
+    int sum = 0, longest = 0;
+    for (int u = u_lo; u < u_hi; ++u) {
+        const int l = unit_len(u);
+        sum += l;
+        longest = max(longest, l);
+    }
     if (tid == 0) {
         for (int i = 0; i < NS; ++i) {
             mbar_init(bar(kSlotFull + i), 128);
@@ -365,7 +368,11 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
             const int v = __shfl_up_sync(0xffffffffu, inc, d);
             if (lane >= d) inc += v;
         }
-        if (lane == 31 && warp < 8) s_scan[warp] = inc;
+        longest = __reduce_max_sync(0xffffffffu, longest);
+        if (lane == 31 && warp < 8) {
+            s_scan[warp] = inc;
+            s_scan[8 + warp] = longest;
+        }
         __syncthreads();
         int base = 0;
         for (int w = 0; w < warp && w < 8; ++w) base += s_scan[w];
@@ -388,10 +395,23 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
     constexpr uint32_t kColS = 0, kColO = 256;   // S buffers at columns 0 and 128, O^T at 256
     const int total = s_prefix[n_units];
     const int chunk = (((total + (int)gridDim.x - 1) / (int)gridDim.x) + 31) & ~31;
-    const int lo = (int)blockIdx.x * chunk, hi = min(lo + chunk, total);
+    // Few units of similar length (at most one per CTA, the longest not much above the even share): every CTA
+    // takes one WHOLE unit -- no partials, no merge, one epilogue -- and the memory system, not the idle SMs, sets
+    // the pace.  Otherwise: equal token ranges (stream-K).
+    int longest_all = 0;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) longest_all = max(longest_all, s_scan[8 + w]);
+    const bool whole_mode = n_units <= (int)gridDim.x && longest_all <= total / (int)gridDim.x + 4 * kTile && !(p.dbg & 32);
+    int lo = (int)blockIdx.x * chunk, hi = min(lo + chunk, total);
+    if (whole_mode) {
+        lo = (int)blockIdx.x < n_units ? s_prefix[blockIdx.x] : total;
+        hi = (int)blockIdx.x < n_units ? s_prefix[blockIdx.x + 1] : total;
+    }
     const bool active = lo < hi;   // a CTA past the end of the token space only takes part in the teardown
     int u0 = 0;
-    if (active) {
+    if (whole_mode) {
+        u0 = min((int)blockIdx.x, n_units - 1);
+    } else if (active) {
         int a = 0, bnd = n_units;   // largest u with prefix[u] <= lo
         while (bnd - a > 1) {
             const int m = (a + bnd) >> 1;
@@ -427,10 +447,8 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
             }
             return t;
         };
-        // Absolute addresses of the K row and of the V row of a token code; rows past the end of the piece read
-        // the zeroed row of the workspace, so the copy loop needs no predicate.
+        // Absolute addresses of the K row and of the V row of a token code (0 = past the end of the piece).
         struct RowPtr { unsigned long long k, v; };
-        const unsigned long long zero_row = (unsigned long long)ws.zero_row;
         auto resolve = [&](const Tok& t) -> RowPtr {
             RowPtr a;
             if (t.tok >= 0) {
@@ -438,7 +456,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
                 a.k = (unsigned long long)(p.kv.k + o);
                 a.v = (unsigned long long)(p.kv.v + o);
             } else if (t.tok == -1) {
-                a.k = a.v = zero_row;
+                a.k = a.v = 0ull;   // past the end of the piece: zero-filled by the copy (src-size 0)
             } else {
                 const long long o = (((long long)t.b * T + (-2 - t.tok)) * Hkv + t.g) * kD;
                 a.k = (unsigned long long)(p.k_new + o);
@@ -459,6 +477,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
         ulonglong2* tab = reinterpret_cast<ulonglong2*>(smem + C::kOffRowTab) + 32 * pw;   // this warp's 32 entries
         const ulonglong2* tab_rd = tab + h;
         const unsigned long long coff = (unsigned long long)c * 16;
+        const unsigned long long kdummy = (unsigned long long)p.kv.k;   // never read (src-size 0)
         // K and V tiles of tile gj: items 2gj and 2gj+1 of the slot ring
         auto issue_tile = [&](int gj, const RowPtr& mine) {
             const int ik = 2 * gj, iv = 2 * gj + 1, sk = ik % NS, sv = iv % NS;
@@ -473,8 +492,9 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
             for (int i = 0; i < 16; ++i) {
                 const ulonglong2 a = tab_rd[2 * i];
                 const uint32_t d = dsw[i & 3] + (uint32_t)(i >> 2) * 1024;
-                cp_async16(dk + d, reinterpret_cast<const void*>(a.x + coff), 16);
-                cp_async16(dv + d, reinterpret_cast<const void*>(a.y + coff), 16);
+                const int nb = a.x != 0ull ? 16 : 0;
+                cp_async16(dk + d, reinterpret_cast<const void*>((nb ? a.x : kdummy) + coff), nb);
+                cp_async16(dv + d, reinterpret_cast<const void*>((nb ? a.y : kdummy) + coff), nb);
             }
             cp_async_mbar_arrive_noinc(bar(kSlotFull + sk));
             cp_async_mbar_arrive_noinc(bar(kSlotFull + sv));
@@ -865,7 +885,7 @@ bool attn_tc_usable(int batch, int n_kv_heads, int head_dim, int rows, int max_t
 }
 
 size_t attn_tc_ws_bytes(int batch, int n_kv_heads, int rows) {
-    static_assert(kMaxGrid * 2 * sizeof(int) + 256 <= kWsHeader, "flags + zero row must fit the persistent header");
+    static_assert(kMaxGrid * 2 * sizeof(int) <= kWsHeader, "the flags must fit the persistent header");
     const size_t nq = (size_t)((rows + 15) / 16) * 16;   // partials are padded to the kernel's NQ rows
     return kWsHeader + align256((size_t)kMaxGrid * 2 * nq * kD * sizeof(float)) +
            align256((size_t)kMaxGrid * 2 * nq * sizeof(float)) + (size_t)kMaxGrid * 64 * 8;
@@ -878,10 +898,9 @@ cudaError_t launch_attn_tc(const AttnParams& p_in, void* ws_base, cudaStream_t s
     char* base = static_cast<char*>(ws_base);
     (void)stream;
     TcWs ws;
-    // Persistent header (kernels.cuh kWsHeader): flags at 0, the zero row at 2048.  Zero before the first use
+    // Persistent header (kernels.cuh kWsHeader): the flags.  Zero before the first use
     // (dustin.h); every launch leaves it zero again (the merging piece clears the flags it has consumed).
     ws.flags = reinterpret_cast<int*>(base);
-    ws.zero_row = base + 2048;
     ws.part_o = reinterpret_cast<float*>(base + kWsHeader);
     const size_t nq = (size_t)((p.rows + 15) / 16) * 16;
     ws.part_lse = reinterpret_cast<float*>(base + kWsHeader + align256((size_t)kMaxGrid * 2 * nq * kD * sizeof(float)));

@@ -69,7 +69,7 @@ cudaError_t launch_attn(const AttnParams& p, cudaStream_t stream);
 // Host-side split heuristic shared by workspace sizing and launch.
 void attn_plan(int batch, int n_kv_heads, int max_tokens, int* split_tokens, int* n_splits);
 void attn_set_split_override(int split_tokens);
-// Bytes at the start of every workspace that persist between calls (flags + zero row of attn_tc.cu): zero before
+// Bytes at the start of every workspace that persist between calls (completion flags of attn_tc.cu): zero before
 // the first use, never touched by the other stages, whose scratch starts right after it.
 constexpr size_t kWsHeader = DUSTIN_WS_HEADER_BYTES;
 // tcgen05 kernel (attn_tc.cu): head_dim 128, stream-K over tokens, partials + arrival counters in the workspace.
