@@ -214,22 +214,64 @@ class Dist:
             dist.destroy_process_group()
 
 
-def time_steps(step_fn, steps: int, warmup: int, dist: Dist, device) -> float:
+class CudaTimer:
+    """Device-side clock: two CUDA events on the launching (current) stream."""
+
+    def sync(self):
+        torch.cuda.synchronize()
+
+    def start(self):
+        self.e0, self.e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        self.e0.record()
+
+    def stop_ms(self) -> float:
+        self.e1.record()
+        torch.cuda.synchronize()
+        return self.e0.elapsed_time(self.e1)
+
+
+class HostTimer:
+    """Wall clock; only for the CPU (gloo) tests of the rank plumbing and for the oracle arm."""
+
+    def sync(self):
+        pass
+
+    def start(self):
+        self.t0 = time.perf_counter()
+
+    def stop_ms(self) -> float:
+        return 1e3 * (time.perf_counter() - self.t0)
+
+
+def time_steps(step_fn, steps: int, warmup: int, dist: Dist, device, timer=None) -> float:
     """ms per step: `warmup` untimed steps, then exactly `steps` steps between two CUDA events on the launching
     stream, bracketed by barrier + synchronize; max over ranks."""
+    timer = timer or CudaTimer()
     for _ in range(warmup):
         step_fn()
-    torch.cuda.synchronize()
+    timer.sync()
     dist.barrier()
-    torch.cuda.synchronize()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
+    timer.sync()
+    timer.start()
     for _ in range(steps):
         step_fn()
-    e1.record()
-    torch.cuda.synchronize()
+    ms = timer.stop_ms()
     dist.barrier()
-    return dist.max_float(e0.elapsed_time(e1), device) / steps
+    return dist.max_float(ms, device) / steps
+
+
+def rank_seed(cfg: synth.Config, rank: int) -> synth.Config:
+    """Weak scaling: rank r draws its own batch of the same workload (independent sequences, no data-path
+    collective -- DESIGN.md §9).  Rank 0 keeps the workload's base seed."""
+    import dataclasses
+    return dataclasses.replace(cfg, seed=cfg.seed + 104729 * rank)
+
+
+def aggregate(us_per_layer_max: float, cfg: synth.Config, world: int) -> dict:
+    """Whole-job figures from the max-over-ranks time: every rank verified `cfg.batch` sequences per layer in that
+    time, so the job verified `world * cfg.batch`."""
+    return {"global_batch": cfg.batch * world,
+            "sequences_per_s": cfg.batch * world / (us_per_layer_max * 1e-6) if us_per_layer_max > 0 else 0.0}
 
 
 def profile_steps(api, step_fn, steps: int) -> dict:
@@ -389,14 +431,14 @@ def headline_config(args) -> synth.Config:
     return cfg
 
 
-def workload_config(cfg: synth.Config, n_sets: int, note: str) -> dict:
+def workload_config(cfg: synth.Config, n_sets: int, note: str, world: int = 1) -> dict:
     return {"workload": "BASELINE.json configs[2]: Qwen2.5-72B-shaped verification step "
                         f"(B={cfg.batch}, N={cfg.ctx}, Hq={cfg.n_q_heads}, Hkv={cfg.n_kv_heads}, d={cfg.head_dim}, "
                         f"gamma={cfg.gamma}, k={cfg.budget} incl. {cfg.n_sink} sink + {cfg.n_recent} recent, "
                         f"|H|={len(cfg.heads)} subset heads {'spread one per KV group' if cfg.n_lists > 1 else 'packed in one KV group'}, "
                         f"G={cfg.n_lists} lists per sequence, L={cfg.n_layers} layers)",
             "schedule": "every layer runs a1 scoring -> a2 fusion -> a3 top-k -> a4 sparse attention (north_star)",
-            "global_batch": cfg.batch, "seq_len": cfg.ctx, "layers": cfg.n_layers, "budget": cfg.budget,
+            "global_batch": cfg.batch * world, "batch_per_gpu": cfg.batch, "seq_len": cfg.ctx, "layers": cfg.n_layers, "budget": cfg.budget,
             "distinct_kv_caches": n_sets,
             "l2": "inputs exceed L2: layers cycle over distinct 2.1 GB K/V caches, none is re-read within 126 MB",
             "launch": "one CUDA graph replay per step (the L fused C-ABI calls captured once)", "note": note}
@@ -467,7 +509,7 @@ def main():
         dist.barrier()
     api.lib()
 
-    cfg = headline_config(args)
+    cfg = rank_seed(headline_config(args), dist.rank)
     w, r = measure_workload(api, cfg, args.sets, args.steps, args.warmup, dist, device, True, True)
     by = w.bytes_per_layer()
     peak, peak_src = measured_peak()
@@ -498,7 +540,9 @@ def main():
         "metric": METRIC, "value": round(us_layer, 3), "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": round(r["ms_per_step"], 4), "higher_is_better": False,
         "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-        "config": workload_config(cfg, w.n_sets, "weak scaling: every rank runs this workload on its own batch"),
+        "config": workload_config(cfg, w.n_sets, "weak scaling: every rank runs this workload on its own batch "
+                                  "(value = max-over-ranks us per layer of the whole job's global batch)", dist.world),
+        "aggregate": aggregate(us_layer, cfg, dist.world),
         "clocks": r["clocks"],
         "e2e": {"value": round(1e3 * e2e_ms / L, 3), "unit": UNIT, "h2d_bytes_per_step": e2e.h2d,
                 "d2h_bytes_per_step": e2e.d2h, "ms_per_step": round(e2e_ms, 4),
