@@ -7,10 +7,23 @@
 // sum over its popcounts.  The score rows (<= 512 KB) are re-read from L2 a handful of times; HBM sees them once.
 #include "kernels.cuh"
 
+#include <climits>
+
 namespace dustin {
 
 namespace {
 
+#ifdef SEL_TS
+__device__ unsigned long long g_sel_ts[64];
+__device__ int g_sel_slot;
+__device__ unsigned long long g_blk[1024][4];
+__device__ __forceinline__ unsigned long long gt_now() { unsigned long long t_; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t_)); return t_; }
+#define STS() do { if (blockIdx.x == 3 && blockIdx.y == 5 && threadIdx.x == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t_)); g_sel_ts[g_sel_slot] = t_; g_sel_slot = (g_sel_slot + 1) & 63; } } while (0)
+#define SVAL(v) do { if (blockIdx.x == 3 && blockIdx.y == 5 && threadIdx.x == 0) { g_sel_ts[g_sel_slot] = 1000000000000000000ull + (unsigned long long)(v); g_sel_slot = (g_sel_slot + 1) & 63; } } while (0)
+#else
+#define STS() do {} while (0)
+#define SVAL(v) do {} while (0)
+#endif
 constexpr int kSelThreads = 1024;
 constexpr int kSelWarps = kSelThreads / 32;
 constexpr int kBins = 2048;
@@ -22,6 +35,10 @@ struct SelShared {
     uint32_t warp_tot[kSelWarps + 1];
     uint32_t res_bin, res_rank, res_cnt;
     uint32_t list_n, res_total;
+    // scratch of the sampled path: two copies used alternately (parity of a per-thread phase counter), so one barrier
+    // between a write and its reads is enough
+    uint32_t tot_db[2][kSelWarps], min_db[2][kSelWarps], max_db[2][kSelWarps], res_db[2][4];
+    uint32_t small_n, small_key[32], small_idx[32];
 };
 
 // Exclusive prefix of v over the block in thread order; *total (optional) receives the block sum.
@@ -411,6 +428,296 @@ __device__ void list_select(const SelLayout& L, int n_list, uint32_t rank, int f
     __syncthreads();
 }
 
+// ---- building blocks of the sampled path: one barrier each (double-buffered scratch, use counters in `ph`) ----------
+struct Phase {
+    int scan = 0, mm = 0, res = 0;   // uses so far of tot_db / min_db+max_db / res_db (block-uniform)
+};
+// Block-wide minimum of `tmin` and maximum of `tmax` over the threads with `valid` set (kmin > kmax when none is).
+__device__ __forceinline__ void block_minmax(uint32_t tmin, uint32_t tmax, bool valid, SelShared& sh, Phase& ph,
+                                             uint32_t& kmin, uint32_t& kmax) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, b = ph.mm++ & 1;
+    const uint32_t lo = __reduce_min_sync(0xffffffffu, valid ? tmin : 0xffffffffu);
+    const uint32_t hi = __reduce_max_sync(0xffffffffu, valid ? tmax : 0u);
+    if (lane == 0) {
+        sh.min_db[b][warp] = lo;
+        sh.max_db[b][warp] = hi;
+    }
+    __syncthreads();
+    kmin = __reduce_min_sync(0xffffffffu, sh.min_db[b][lane]);
+    kmax = __reduce_max_sync(0xffffffffu, sh.max_db[b][lane]);
+}
+
+// Exclusive prefix of v over the block in thread order; *total receives the block sum.
+__device__ __forceinline__ uint32_t block_excl_scan_db(uint32_t v, SelShared& sh, Phase& ph, uint32_t* total) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, b = ph.scan++ & 1;
+    uint32_t inc = v;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+        const uint32_t o = __shfl_up_sync(0xffffffffu, inc, off);
+        if (lane >= off) inc += o;
+    }
+    if (lane == 31) sh.tot_db[b][warp] = inc;
+    __syncthreads();
+    const uint32_t t = sh.tot_db[b][lane];   // every warp scans the 32 warp totals redundantly
+    uint32_t ti = t;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+        const uint32_t o = __shfl_up_sync(0xffffffffu, ti, off);
+        if (lane >= off) ti += o;
+    }
+    *total = __shfl_sync(0xffffffffu, ti, 31);
+    return __shfl_sync(0xffffffffu, ti - t, warp) + inc - v;
+}
+
+// Bin of the single-replica histogram that holds rank `rank` (1-based, ascending bin order).  Leaves the histogram
+// ZEROED for its next use.  Returns {bin, rank inside the bin, bin count, total}; bin is valid when rank <= total.
+__device__ __forceinline__ uint4 find_bin_db(uint32_t* hist, uint32_t rank, SelShared& sh, Phase& ph) {
+    const uint2 x = reinterpret_cast<const uint2*>(hist)[threadIdx.x];
+    uint32_t total;
+    const uint32_t excl = block_excl_scan_db(x.x + x.y, sh, ph, &total);
+    reinterpret_cast<uint2*>(hist)[threadIdx.x] = make_uint2(0u, 0u);   // every thread is past its read (barrier above)
+    const int b = ph.res++ & 1;
+    if (excl < rank && rank <= excl + x.x) {
+        sh.res_db[b][0] = 2 * threadIdx.x;
+        sh.res_db[b][1] = rank - excl;
+        sh.res_db[b][2] = x.x;
+    } else if (excl + x.x < rank && rank <= excl + x.x + x.y) {
+        sh.res_db[b][0] = 2 * threadIdx.x + 1;
+        sh.res_db[b][1] = rank - excl - x.x;
+        sh.res_db[b][2] = x.y;
+    }
+    __syncthreads();
+    return make_uint4(sh.res_db[b][0], sh.res_db[b][1], sh.res_db[b][2], total);
+}
+
+// Digit position that spreads the key range [kmin, kmax] over the kBins bins: bucket = (key - kmin) >> shift.
+__device__ __forceinline__ int range_shift(uint32_t kmin, uint32_t kmax) {
+    const int bits = kmax > kmin ? 32 - __clz(kmax - kmin) : 0;
+    return bits > 11 ? bits - 11 : 0;
+}
+
+// Exact selection on the candidate list by an OFFSET radix select: a pass spreads the current key range
+// [klo, khi] (first pass: the list's own minimum and maximum) over the 2048 bins, so the scores of one row -- which
+// share their leading exponent bits -- do not pile up in a handful of bins (same-address shared atomics serialise).
+// A threshold bin of <= 32 entries is then ranked by brute force ((key desc, index asc) order, which also settles
+// ties); a fuller one becomes the range of the next pass.  Admits the `rank` best of the n_list entries.
+template <int kPer>   // entries per thread: n_list <= kPer * kSelThreads
+__device__ void list_select_ranged(const float* __restrict__ s, const SelLayout& L, int n_list, uint32_t rank,
+                                   SelShared& sh, Phase& ph) {
+    // On entry: list_idx[0, n_list) filled, hist (replica 0) all zero, a barrier since both.  Leaves hist zero.
+    uint32_t* hist = L.hist;
+    uint32_t key[kPer], idx[kPer];
+    uint32_t part = 0;        // bit e: entry threadIdx.x + e * kSelThreads is still inside the key range
+    uint32_t lmin = 0xffffffffu, lmax = 0u;
+#pragma unroll
+    for (int e = 0; e < kPer; ++e) {   // the keys come straight from the score row: independent loads, all in flight
+        const int j = threadIdx.x + e * kSelThreads;
+        idx[e] = j < n_list ? L.list_idx[j] : 0u;
+        key[e] = j < n_list ? key_max0(__ldcg(s + idx[e])) : 0u;
+    }
+#pragma unroll
+    for (int e = 0; e < kPer; ++e)
+        if (threadIdx.x + e * kSelThreads < n_list) {
+            part |= 1u << e;
+            lmin = min(lmin, key[e]);
+            lmax = max(lmax, key[e]);
+        }
+    if (threadIdx.x == 0) sh.small_n = 0;
+    uint32_t klo, khi;
+    block_minmax(lmin, lmax, part != 0, sh, ph, klo, khi);
+    uint32_t eq_total = (uint32_t)n_list;
+    uint32_t T = klo, i_star = 0xffffffffu;   // admitted: key > T, or key == T and index <= i_star
+    bool settled = false;
+#pragma unroll 1
+    while (khi > klo) {
+        const int shift = range_shift(klo, khi);
+#pragma unroll
+        for (int e = 0; e < kPer; ++e)
+            if ((part >> e) & 1u) atomicAdd(&hist[kBins - 1 - ((key[e] - klo) >> shift)], 1u);
+        __syncthreads();
+        const uint4 fb = find_bin_db(hist, rank, sh, ph);
+        const uint32_t bucket = (uint32_t)(kBins - 1) - fb.x;
+        rank = fb.y;
+        eq_total = fb.z;
+        // entries above the bucket are in, entries below are out; the bucket itself is what is left to rank
+        const uint32_t nlo = klo + (bucket << shift);
+        const uint32_t nhi = shift == 0 ? nlo : min(khi, nlo + ((1u << shift) - 1u));
+#pragma unroll
+        for (int e = 0; e < kPer; ++e)
+            if (((part >> e) & 1u) && (key[e] < nlo || key[e] > nhi)) part &= ~(1u << e);
+        klo = nlo;
+        khi = nhi;
+        if (eq_total <= 32u) {
+#pragma unroll
+            for (int e = 0; e < kPer; ++e)
+                if ((part >> e) & 1u) {
+                    const uint32_t at = atomicAdd(&sh.small_n, 1u);
+                    sh.small_key[at] = key[e];
+                    sh.small_idx[at] = idx[e];
+                }
+            __syncthreads();
+            const int b = ph.res++ & 1;
+            if (threadIdx.x < eq_total) {
+                const uint32_t mk = sh.small_key[threadIdx.x], mi = sh.small_idx[threadIdx.x];
+                uint32_t ahead = 0;
+                for (uint32_t i = 0; i < eq_total; ++i) {
+                    const uint32_t ok = sh.small_key[i], oi = sh.small_idx[i];
+                    ahead += (ok > mk || (ok == mk && oi < mi)) ? 1u : 0u;
+                }
+                if (ahead == rank - 1u) {
+                    sh.res_db[b][0] = mk;
+                    sh.res_db[b][1] = mi;
+                }
+            }
+            __syncthreads();
+            T = sh.res_db[b][0];
+            i_star = sh.res_db[b][1];
+            settled = true;
+            break;
+        }
+    }
+    if (!settled) {
+        T = klo;
+        const uint32_t need_eq = rank;
+        if (need_eq < eq_total) {
+            // More than 32 equal keys straddle the threshold: i_star = the need_eq-th lowest index among them
+            // (indices < 2^21), by two histogram passes over the index bits.
+#pragma unroll
+            for (int e = 0; e < kPer; ++e)
+                if (((part >> e) & 1u) && key[e] == T) atomicAdd(&hist[idx[e] >> 10], 1u);
+            __syncthreads();
+            const uint4 f1 = find_bin_db(hist, need_eq, sh, ph);
+#pragma unroll
+            for (int e = 0; e < kPer; ++e)
+                if (((part >> e) & 1u) && key[e] == T && (idx[e] >> 10) == f1.x) atomicAdd(&hist[idx[e] & 0x3ffu], 1u);
+            __syncthreads();
+            const uint4 f2 = find_bin_db(hist, f1.y, sh, ph);
+            i_star = (f1.x << 10) | f2.x;
+        }
+    }
+#pragma unroll
+    for (int e = 0; e < kPer; ++e)
+        if (threadIdx.x + e * kSelThreads < n_list && (key[e] > T || (key[e] == T && idx[e] <= i_star)))
+            set_member(L.mem, (int)idx[e]);
+    __syncthreads();
+}
+
+// ---- sampled path on 16-byte loads ---------------------------------------------------------------------------------
+// Thread t holds the vectors v0 + (8c + u) * 1024 + t of the row (chunk c = 32768 elements, u = 0..7).  A row of one
+// chunk stays in registers from the threshold estimate to the compaction; longer rows are re-read from L2 per phase.
+//  (a) 1024 samples spread over the row -> their minimum / maximum -> offset-radix histogram -> the key tau that
+//      the true rank-th key exceeds with overwhelming probability (the sample only decides which path runs);
+//  (b) every candidate with key >= tau goes to the (key, index) list: per-thread counts, one block scan per chunk,
+//      no atomics;  (c) exact selection on the list (list_select_ranged).
+// Returns false (nothing admitted) when the list came out too short or too long; the caller then takes path (2).
+// On entry hist (replica 0) must be all zero; it is left all zero.
+__device__ bool sampled_tier_vec(const float* __restrict__ s, int lo, int hi, int rank, const SelLayout& L,
+                                 SelShared& sh, Phase& ph) {
+    constexpr int kVecPerChunk = 8;
+    const float4* s4 = reinterpret_cast<const float4*>(s);
+    const int t = threadIdx.x;
+    const int v0 = lo >> 2, v_end = (hi + 3) >> 2;
+    const int n_chunks = (v_end - v0 + kVecPerChunk * kSelThreads - 1) / (kVecPerChunk * kSelThreads);
+    const bool one = n_chunks == 1;
+    const int n_cand = hi - lo;
+    float4 x[kVecPerChunk];
+    auto load_chunk = [&](int c) {
+#pragma unroll
+        for (int u = 0; u < kVecPerChunk; ++u) {
+            const int vv = v0 + (c * kVecPerChunk + u) * kSelThreads + t;
+            x[u] = vv < v_end ? __ldcg(s4 + vv) : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+    };
+    // candidate nibble of a vector: bit e clear <=> element 4 * vv + e is a candidate
+    auto nib_of = [&](int vv) -> uint32_t {
+        const int n = vv << 2;
+        return vv < v_end ? (L.mem[n >> 5] >> (n & 31)) & 0xfu : 0xfu;
+    };
+    // ---- (a) threshold from 1024 samples ----
+    uint32_t skey = 0;
+    bool svalid = false;
+    int n_slots;
+    if (one) {
+        load_chunk(0);
+        const int u_s = t & 7, e_s = (t >> 3) & 3;
+        float4 xv = x[0];
+#pragma unroll
+        for (int u = 1; u < kVecPerChunk; ++u)
+            if (u_s == u) xv = x[u];
+        const float f = e_s == 0 ? xv.x : (e_s == 1 ? xv.y : (e_s == 2 ? xv.z : xv.w));
+        skey = key_max0(f);
+        svalid = !((nib_of(v0 + u_s * kSelThreads + t) >> e_s) & 1u);
+        n_slots = min(kSelThreads, (v_end - v0));   // threads whose sampled vector can exist at all (upper bound)
+    } else {
+        const int stride = max(1, n_cand / kSelThreads);
+        n_slots = min(kSelThreads, (n_cand + stride - 1) / stride);
+        const int pos = lo + t * stride;
+        if (t < n_slots) {
+            skey = key_max0(__ldcg(s + pos));
+            svalid = !((L.mem[pos >> 5] >> (pos & 31)) & 1u);
+        }
+    }
+    uint32_t kmin, kmax;
+    STS();
+    block_minmax(skey, skey, svalid, sh, ph, kmin, kmax);
+    STS();
+    uint32_t tau = 0;   // 0: every candidate goes to the list
+    if (kmin <= kmax) {
+        const int shift = range_shift(kmin, kmax);
+        if (svalid) atomicAdd(&L.hist[kBins - 1 - ((skey - kmin) >> shift)], 1u);
+        __syncthreads();
+        // sample rank that the true rank-th key exceeds with overwhelming probability (mean * 1.25 + 3.5 sigma + 4)
+        const float mean = (float)n_slots * (float)rank / (float)n_cand;
+        const uint32_t j = (uint32_t)(mean * 1.25f + 3.5f * sqrtf(mean) + 4.f);
+        const uint4 fb = find_bin_db(L.hist, j, sh, ph);
+        if (j <= fb.w) tau = kmin + (((uint32_t)(kBins - 1) - fb.x) << shift);
+    }
+    // ---- (b) compaction: candidates with key >= tau ----
+    // Signed compare on the raw bits: for s >= 0 it is the key order; negative scores (key 0, reading A15) pass
+    // only when tau == 0, i.e. when every candidate is taken.
+    STS();
+    const int tau_s = tau == 0u ? INT_MIN : (int)tau;
+    const int wsh = ((v0 + t) & 7) * 4;                      // this thread's nibble inside its bitmask words
+    uint32_t base = 0;
+#pragma unroll 1
+    for (int c = 0; c < n_chunks; ++c) {
+        if (!one) load_chunk(c);
+        const int vc = v0 + c * kVecPerChunk * kSelThreads + t;   // vector of u = 0
+        uint32_t hits = 0, taken = 0;   // bit 4u + e: element e of vector u
+#pragma unroll
+        for (int u = 0; u < kVecPerChunk; ++u) {
+            hits |= (__float_as_int(x[u].x) >= tau_s ? 1u : 0u) << (4 * u);
+            hits |= (__float_as_int(x[u].y) >= tau_s ? 2u : 0u) << (4 * u);
+            hits |= (__float_as_int(x[u].z) >= tau_s ? 4u : 0u) << (4 * u);
+            hits |= (__float_as_int(x[u].w) >= tau_s ? 8u : 0u) << (4 * u);
+            const int vv = vc + u * kSelThreads;
+            const uint32_t nib = vv < v_end ? (L.mem[vv >> 3] >> wsh) & 0xfu : 0xfu;
+            taken |= nib << (4 * u);
+        }
+        hits &= ~taken;
+        uint32_t total;
+        uint32_t pos = base + block_excl_scan_db((uint32_t)__popc(hits), sh, ph, &total);
+        base += total;
+        while (hits) {   // ~6 % of the elements; only the index is kept, list_select_ranged gathers the keys
+            const int bit = __ffs(hits) - 1;
+            hits &= hits - 1;
+            if (pos < (uint32_t)L.cap) L.list_idx[pos] = (uint32_t)(((vc + (bit >> 2) * kSelThreads) << 2) + (bit & 3));
+            ++pos;
+        }
+    }
+    __syncthreads();
+    const uint32_t n_list = base;
+    STS();
+    SVAL(n_list);
+    if (n_list < (uint32_t)rank || n_list > (uint32_t)L.cap) return false;
+    if (n_list <= 2u * kSelThreads)
+        list_select_ranged<2>(s, L, (int)n_list, (uint32_t)rank, sh, ph);
+    else
+        list_select_ranged<8>(s, L, (int)n_list, (uint32_t)rank, sh, ph);
+    STS();
+    return true;
+}
+
 // One tier of Eq. 6: admits into `mem` the `rank` best candidates of [lo, hi) by s (ties -> lower index).
 //  (1) sampled path: 1024 strided samples give a conservative threshold on the top 11 key bits; one scan compacts
 //      every candidate at or above it into the list; if the list holds >= rank entries (and fits) the exact answer
@@ -419,13 +726,27 @@ __device__ void list_select(const SelLayout& L, int n_list, uint32_t rank, int f
 //  (3) full-scan path for a threshold bin larger than the list (massive ties).
 template <bool VEC>
 __device__ void select_tier(const float* __restrict__ s, int lo, int hi, int rank, const SelLayout& L, int n_words,
-                            SelShared& sh) {
+                            SelShared& sh, Phase& ph, bool& hist_clean) {
     const int R = L.R, rep = threadIdx.x & (R - 1);
     uint32_t* hist = L.hist;
     const ListAppender app{L.list_key, L.list_idx, &sh.list_n, (uint32_t)L.cap};
     const int n_cand = hi - lo;
+    if (VEC) {
+        STS();
+        if (!hist_clean) {
+            clear_hist(hist, 1);
+            __syncthreads();
+        }
+        hist_clean = true;
+        if (sampled_tier_vec(s, lo, hi, rank, L, sh, ph)) return;
+        hist_clean = false;   // the paths below leave their counts behind
+#ifdef SEL_TS
+        if (threadIdx.x == 0) g_blk[blockIdx.y * gridDim.x + blockIdx.x][2] += 1;
+#endif
+        __syncthreads();
+    }
     // ---- (1) sampled threshold ----
-    {
+    if (!VEC) {
         clear_hist(hist, 1);
         if (threadIdx.x == 0) sh.list_n = 0;
         __syncthreads();
@@ -476,6 +797,13 @@ __global__ void __launch_bounds__(kSelThreads) select_kernel(const SelectParams 
     extern __shared__ __align__(16) uint32_t smem_dyn[];
     __shared__ SelShared sh;
     const int l = blockIdx.x, b = blockIdx.y;
+#ifdef SEL_TS
+    if (blockIdx.x == 3 && blockIdx.y == 5 && threadIdx.x == 0) g_sel_slot = 0;
+#endif
+    STS();
+#ifdef SEL_TS
+    if (threadIdx.x == 0) { g_blk[blockIdx.y * gridDim.x + blockIdx.x][0] = gt_now(); g_blk[blockIdx.y * gridDim.x + blockIdx.x][2] = 0; }
+#endif
     const int N = seq_len_of(p.seq_lens, b, p.max_ctx);
     const int k = p.budgets ? p.budgets[b] : p.budget;
     int* out = p.idx_out + ((long long)b * p.n_lists + l) * p.k_max;
@@ -517,16 +845,20 @@ __global__ void __launch_bounds__(kSelThreads) select_kernel(const SelectParams 
         }
         mem[w] = bits;
     }
+    Phase ph;
+    bool hist_clean = VEC;
+    if (VEC) clear_hist(L.hist, 1);
     __syncthreads();
 
     // tier 0: I_draft = TopK(S_Draft \ I_prot, m);  tier 1: I_target = TopK(S_Target \ (I_prot U I_draft), k-m-|I_prot|)
 #pragma unroll 1
     for (int tier = 0; tier < 2; ++tier) {
         const int want = tier == 0 ? m : c - m;
-        if (want > 0) select_tier<VEC>(tier == 0 ? sd : st, lo, hi, want, L, n_words, sh);
+        if (want > 0) select_tier<VEC>(tier == 0 ? sd : st, lo, hi, want, L, n_words, sh, ph, hist_clean);
     }
     if (threadIdx.x == 0 && (N & 31)) mem[n_words - 1] &= (1u << (N & 31)) - 1u;   // drop the tail bits >= N
     __syncthreads();
+    STS();
     // I_verify in ascending order: prefix sum over the popcounts of the bitmask words.
     const int wpt = (n_words + kSelThreads - 1) / kSelThreads;   // consecutive words per thread
     const int w_lo = threadIdx.x * wpt, w_hi = min(w_lo + wpt, n_words);
@@ -545,6 +877,10 @@ __global__ void __launch_bounds__(kSelThreads) select_kernel(const SelectParams 
     }
     for (int i = (int)total + threadIdx.x; i < p.k_max; i += kSelThreads) out[i] = -1;
     if (threadIdx.x == 0) *cnt_out = (int)total;
+    STS();
+#ifdef SEL_TS
+    if (threadIdx.x == 0) g_blk[blockIdx.y * gridDim.x + blockIdx.x][1] = gt_now();
+#endif
 }
 
 }  // namespace
@@ -565,6 +901,15 @@ size_t select_smem_bytes(int max_ctx) {
     select_plan(max_ctx, &mw, &R, &cap);
     return ((size_t)mw + (size_t)kBins * R + 2 * (size_t)cap) * 4;
 }
+
+#ifdef SEL_TS
+extern "C" int dustin_dbg_sel_ts(unsigned long long* out) {
+    return (int)cudaMemcpyFromSymbol(out, g_sel_ts, sizeof(g_sel_ts));
+}
+extern "C" int dustin_dbg_sel_blk(unsigned long long* out) {
+    return (int)cudaMemcpyFromSymbol(out, g_blk, sizeof(g_blk));
+}
+#endif
 
 cudaError_t launch_select(const SelectParams& p_in, cudaStream_t stream) {
     SelectParams p = p_in;
