@@ -683,25 +683,29 @@ __device__ bool sampled_tier_vec(const float* __restrict__ s, int lo, int hi, in
     for (int c = 0; c < n_chunks; ++c) {
         if (!one) load_chunk(c);
         const int vc = v0 + c * kVecPerChunk * kSelThreads + t;   // vector of u = 0
+        // vectors u < nv of this thread exist; the bitmask words of the others are padding (select_plan), ignored
+        const int nv = min(max((v_end - vc + kSelThreads - 1) / kSelThreads, 0), kVecPerChunk);
+        const uint32_t exist = nv >= 8 ? 0xffffffffu : (1u << (4 * nv)) - 1u;
+        const uint32_t* mrow = L.mem + (vc >> 3);                 // word of vector u: mrow[128 u], same nibble
         uint32_t hits = 0, taken = 0;   // bit 4u + e: element e of vector u
 #pragma unroll
         for (int u = 0; u < kVecPerChunk; ++u) {
-            hits |= (__float_as_int(x[u].x) >= tau_s ? 1u : 0u) << (4 * u);
-            hits |= (__float_as_int(x[u].y) >= tau_s ? 2u : 0u) << (4 * u);
-            hits |= (__float_as_int(x[u].z) >= tau_s ? 4u : 0u) << (4 * u);
-            hits |= (__float_as_int(x[u].w) >= tau_s ? 8u : 0u) << (4 * u);
-            const int vv = vc + u * kSelThreads;
-            const uint32_t nib = vv < v_end ? (L.mem[vv >> 3] >> wsh) & 0xfu : 0xfu;
-            taken |= nib << (4 * u);
+            if (__float_as_int(x[u].x) >= tau_s) hits |= 1u << (4 * u);
+            if (__float_as_int(x[u].y) >= tau_s) hits |= 2u << (4 * u);
+            if (__float_as_int(x[u].z) >= tau_s) hits |= 4u << (4 * u);
+            if (__float_as_int(x[u].w) >= tau_s) hits |= 8u << (4 * u);
+            taken |= ((mrow[128 * u] >> wsh) & 0xfu) << (4 * u);
         }
+        hits &= exist;
         hits &= ~taken;
         uint32_t total;
         uint32_t pos = base + block_excl_scan_db((uint32_t)__popc(hits), sh, ph, &total);
         base += total;
+        const uint32_t n0 = (uint32_t)vc << 2;
         while (hits) {   // ~6 % of the elements; only the index is kept, list_select_ranged gathers the keys
-            const int bit = __ffs(hits) - 1;
-            hits &= hits - 1;
-            if (pos < (uint32_t)L.cap) L.list_idx[pos] = (uint32_t)(((vc + (bit >> 2) * kSelThreads) << 2) + (bit & 3));
+            const uint32_t bit = (uint32_t)__ffs(hits) - 1u;
+            hits &= hits - 1u;
+            if (pos < (uint32_t)L.cap) L.list_idx[pos] = n0 + (bit >> 2) * (4u * kSelThreads) + (bit & 3u);
             ++pos;
         }
     }
@@ -888,7 +892,8 @@ __global__ void __launch_bounds__(kSelThreads) select_kernel(const SelectParams 
 // Shared-memory plan: bitmask (max_ctx / 8 bytes) + kBins * R histogram counters + a 2 * cap word candidate list,
 // shrunk for very long rows so that everything fits the 227 KB of one SM.
 void select_plan(int max_ctx, int* mask_words, int* replicas, int* list_cap) {
-    *mask_words = ((max_ctx + 31) / 32 + 3) & ~3;
+    // + 1024 words of padding: the sampled path reads the words of a whole 32768-element chunk past the row's end
+    *mask_words = (((max_ctx + 31) / 32 + 3) & ~3) + 1024;
     const size_t mask_bytes = (size_t)*mask_words * 4;
     int R = 8, cap = 8192;
     if (mask_bytes > 64 * 1024) R = 4, cap = 4096;   // rows beyond 512k tokens
