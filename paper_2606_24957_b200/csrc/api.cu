@@ -3,6 +3,7 @@
 #include "kernels.cuh"
 
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 
 namespace dustin {
@@ -147,9 +148,11 @@ AttnWs attn_ws(const dustin_shape_t* s, int max_tokens) {
     return w;
 }
 
+// norm_out != nullptr: launch only the logits kernel and describe the pending normalisation + Eq. 5 accumulation for
+// the selection kernel, which then does it row by row (SelectParams::Norm).
 int run_score(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q, int64_t q_stride_batch,
               int64_t q_stride_head, uint64_t head_mask, int32_t n_lists, float* scores_now, float* hist,
-              float alpha, void* ws, size_t ws_bytes, cudaStream_t stream) {
+              float alpha, void* ws, size_t ws_bytes, cudaStream_t stream, SelectParams::Norm* norm_out = nullptr) {
     int rc = check_shape(shape);
     if (rc) return rc;
     ScoreParams p;
@@ -179,8 +182,27 @@ int run_score(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q,
     p.part = reinterpret_cast<float2*>(base + w.part);
     p.stats = reinterpret_cast<float2*>(base + w.stats);
     if (p.max_ctx == 0) return DUSTIN_OK;
-    const cudaError_t e = launch_score(p, scores_now, hist, alpha, stream);
+    if (norm_out) {
+        norm_out->logits = p.logits;
+        norm_out->part = p.part;
+        norm_out->logit_stride = p.logit_stride;
+        norm_out->nsel = p.nsel;
+        norm_out->n_chunks = p.n_chunks;
+        norm_out->alpha = alpha;
+        std::memcpy(norm_out->list_first, p.list_first, sizeof p.list_first);
+        std::memcpy(norm_out->list_cnt, p.list_cnt, sizeof p.list_cnt);
+    }
+    const cudaError_t e = launch_score(p, scores_now, hist, alpha, norm_out != nullptr, stream);
     return e == cudaSuccess ? DUSTIN_OK : fail_cuda(e);
+}
+
+// DUSTIN_FUSED_ROWS=0 keeps the separate stats / normalise kernels in the fused entry point (A/B measurements).
+bool fused_rows_disabled() {
+    static const bool off = [] {
+        const char* e = std::getenv("DUSTIN_FUSED_ROWS");
+        return e && e[0] == '0';
+    }();
+    return off;
 }
 
 int check_select(const dustin_select_t* sel, int32_t k_max) {
@@ -197,7 +219,7 @@ int check_select(const dustin_select_t* sel, int32_t k_max) {
 
 int run_select(int32_t batch, int32_t max_ctx, const int32_t* seq_lens, const dustin_select_t* sel,
                const float* s_draft, int64_t draft_list_stride, const float* s_target, int32_t* idx_out,
-               int32_t* cnt_out, int32_t k_max, cudaStream_t stream) {
+               int32_t* cnt_out, int32_t k_max, cudaStream_t stream, const SelectParams::Norm* norm = nullptr) {
     int rc = check_select(sel, k_max);
     if (rc) return rc;
     if (batch <= 0 || max_ctx < 0 || !s_draft || !s_target || !idx_out || !cnt_out) return DUSTIN_ERR_INVALID_ARG;
@@ -221,6 +243,8 @@ int run_select(int32_t batch, int32_t max_ctx, const int32_t* seq_lens, const du
     p.s_target = s_target;
     p.idx_out = idx_out;
     p.cnt_out = cnt_out;
+    std::memset(&p.norm, 0, sizeof p.norm);
+    if (norm) p.norm = *norm;
     const cudaError_t e = launch_select(p, stream);
     return e == cudaSuccess ? DUSTIN_OK : fail_cuda(e);
 }
@@ -378,12 +402,19 @@ int dustin_verify_layer_fused(const dustin_shape_t* shape, const dustin_kv_t* kv
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     char* base = static_cast<char*>(ws);
     // a1 + a2: scores of verify position 0 (reading A3), accumulated straight into hist (Eq. 5)
+    // With enough rows to fill the GPU the selection kernel normalises and accumulates its own rows (no separate
+    // stats / normalise launches, no extra pass over the scores); it needs 16-byte rows and no scores_now output.
+    SelectParams::Norm norm;
+    const bool rows_in_select = !scores_now_out && (shape->max_ctx & 3) == 0 && shape->max_ctx > 0 &&
+                                (((uintptr_t)hist_inout | (uintptr_t)s_draft) & 15) == 0 &&
+                                (long long)shape->batch * select->n_lists >= 64 && !fused_rows_disabled();
     rc = run_score(shape, kv, q, (int64_t)shape->n_new * shape->n_q_heads * shape->head_dim, shape->head_dim,
-                   head_mask, select->n_lists, scores_now_out, hist_inout, alpha, ws, ws_bytes, st);
+                   head_mask, select->n_lists, scores_now_out, hist_inout, alpha, ws, ws_bytes, st,
+                   rows_in_select ? &norm : nullptr);
     if (rc) return rc;
     // a3
     rc = run_select(shape->batch, shape->max_ctx, kv->seq_lens, select, s_draft, draft_list_stride, hist_inout,
-                    idx_out, cnt_out, k_max, st);
+                    idx_out, cnt_out, k_max, st, rows_in_select ? &norm : nullptr);
     if (rc) return rc;
     // a4
     return run_attn(shape, kv, q, k_new, v_new, idx_out, cnt_out, select->n_lists, k_max, out, lse_out,

@@ -93,4 +93,34 @@ __device__ __forceinline__ float fast_exp2(float x) {
     return y;
 }
 
+// ---- softmax bookkeeping of stage a1 (shared by score.cu and the row materialisation inside select.cu; explicit
+// fma / mul intrinsics so that both compile to the same arithmetic, bit for bit) ----------------------------------
+// Merge (om, os) into the running (m, s): maxima and sums of exp2(l - max) in the log2 domain.
+__device__ __forceinline__ void softmax_merge(float& m, float& s, float om, float os) {
+    const float mn = fmaxf(m, om);
+    s = (mn > -INFINITY) ? __fmaf_rn(s, exp2f(m - mn), __fmul_rn(os, exp2f(om - mn))) : 0.f;
+    m = mn;
+}
+// (M, 1/Z) of one head from its n_chunks per-CTA partials; one warp, every lane receives the result.
+__device__ __forceinline__ float2 fold_stats_warp(const float2* __restrict__ src, int n_chunks, int lane) {
+    float m = -INFINITY, s = 0.f;
+    for (int i = lane; i < n_chunks; i += 32) {
+        const float2 o = __ldcg(src + i);
+        softmax_merge(m, s, o.x, o.y);
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        const float om = __shfl_xor_sync(0xffffffffu, m, off), os = __shfl_xor_sync(0xffffffffu, s, off);
+        softmax_merge(m, s, om, os);
+    }
+    return make_float2(m, s > 0.f ? 1.f / s : 0.f);
+}
+// a += exp2(l - M) / Z for the four logits of one 16-byte load.
+__device__ __forceinline__ void prob_accumulate4(float (&a)[4], const float4 l, const float2 st) {
+    a[0] = __fmaf_rn(exp2f(l.x - st.x), st.y, a[0]);
+    a[1] = __fmaf_rn(exp2f(l.y - st.x), st.y, a[1]);
+    a[2] = __fmaf_rn(exp2f(l.z - st.x), st.y, a[2]);
+    a[3] = __fmaf_rn(exp2f(l.w - st.x), st.y, a[3]);
+}
+
 }  // namespace dustin

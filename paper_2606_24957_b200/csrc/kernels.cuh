@@ -27,7 +27,10 @@ struct ScoreParams {
     float2* stats;                  // ws: [B, nsel] (M, 1/Z)
 };
 
-cudaError_t launch_score(const ScoreParams& p, float* scores_now, float* hist, float alpha, cudaStream_t stream);
+// logits_only: stop after the logits + per-CTA partials; launch_select (SelectParams::norm) then normalises and
+// accumulates each row itself.
+cudaError_t launch_score(const ScoreParams& p, float* scores_now, float* hist, float alpha, bool logits_only,
+                         cudaStream_t stream);
 cudaError_t launch_fuse(int batch, int n_lists, int max_ctx, const int* seq_lens, const float* now, float* hist,
                         float alpha, cudaStream_t stream);
 
@@ -44,6 +47,17 @@ struct SelectParams {
     int* idx_out;
     int* cnt_out;
     int mask_words, replicas, list_cap;   // shared-memory plan, filled by launch_select
+    // Row materialisation (fused entry point): when norm.logits != nullptr the kernel first computes its own target
+    // row, s_target[b,l,n] = alpha * s_target[b,l,n] + sum_j exp2(logit_j[n] - M_j) / Z_j (a1's normalisation and
+    // Eq. 5), from the logits and partials that score_logits_kernel left in the workspace, and writes it back.
+    struct Norm {
+        const float* logits;            // [B, nsel, logit_stride]
+        const float2* part;             // [B, nsel, n_chunks]
+        long long logit_stride;
+        int nsel, n_chunks;
+        float alpha;
+        unsigned char list_first[64], list_cnt[64];
+    } norm;
 };
 cudaError_t launch_select(const SelectParams& p, cudaStream_t stream);
 size_t select_smem_bytes(int max_ctx);

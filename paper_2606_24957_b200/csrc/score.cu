@@ -147,22 +147,8 @@ __global__ void __launch_bounds__(kScoreThreads) score_logits_kernel(const Score
 __global__ void __launch_bounds__(256) score_stats_kernel(const ScoreParams p) {
     const int b = blockIdx.x, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     for (int j = warp; j < p.nsel; j += 8) {
-        const float2* src = p.part + ((long long)b * p.nsel + j) * p.n_chunks;
-        float m = -INFINITY, s = 0.f;
-        for (int i = lane; i < p.n_chunks; i += 32) {
-            const float2 o = __ldcg(src + i);
-            const float mn = fmaxf(m, o.x);
-            s = (mn > -INFINITY) ? s * exp2f(m - mn) + o.y * exp2f(o.x - mn) : 0.f;
-            m = mn;
-        }
-#pragma unroll
-        for (int off = 16; off > 0; off >>= 1) {
-            const float om = __shfl_xor_sync(0xffffffffu, m, off), os = __shfl_xor_sync(0xffffffffu, s, off);
-            const float mn = fmaxf(m, om);
-            s = (mn > -INFINITY) ? s * exp2f(m - mn) + os * exp2f(om - mn) : 0.f;
-            m = mn;
-        }
-        if (lane == 0) p.stats[(long long)b * p.nsel + j] = make_float2(m, s > 0.f ? 1.f / s : 0.f);
+        const float2 st = fold_stats_warp(p.part + ((long long)b * p.nsel + j) * p.n_chunks, p.n_chunks, lane);
+        if (lane == 0) p.stats[(long long)b * p.nsel + j] = st;
     }
 }
 
@@ -185,16 +171,12 @@ __global__ void __launch_bounds__(256) score_normalize_kernel(const ScoreParams 
         for (int i = 0; i < VEC; ++i) a[i] = 0.f;
         if (n < N) {
             for (int j = 0; j < nh; ++j) {
-                const float M = st[j].x, iz = st[j].y;
-                float x[VEC];
-                if (VEC == 4) {
-                    const float4 t = __ldcg(reinterpret_cast<const float4*>(lg + (long long)j * p.logit_stride + n));
-                    x[0] = t.x, x[VEC > 1 ? 1 : 0] = t.y, x[VEC > 2 ? 2 : 0] = t.z, x[VEC > 3 ? 3 : 0] = t.w;
+                if constexpr (VEC == 4) {
+                    prob_accumulate4(a, __ldcg(reinterpret_cast<const float4*>(lg + (long long)j * p.logit_stride + n)),
+                                     st[j]);
                 } else {
-                    x[0] = __ldcg(lg + (long long)j * p.logit_stride + n);
+                    a[0] = __fmaf_rn(exp2f(__ldcg(lg + (long long)j * p.logit_stride + n) - st[j].x), st[j].y, a[0]);
                 }
-#pragma unroll
-                for (int i = 0; i < VEC; ++i) a[i] += exp2f(x[i] - M) * iz;
             }
 #pragma unroll
             for (int i = 1; i < VEC; ++i)
@@ -205,10 +187,10 @@ __global__ void __launch_bounds__(256) score_normalize_kernel(const ScoreParams 
                 *reinterpret_cast<float4*>(scores_now + row + n) = make_float4(a[0], a[VEC > 1 ? 1 : 0], a[VEC > 2 ? 2 : 0], a[VEC > 3 ? 3 : 0]);
             if (hist && n < N) {
                 float4 h = *reinterpret_cast<const float4*>(hist + row + n);
-                h.x = fmaf(alpha, h.x, a[0]);
-                if (n + 1 < N) h.y = fmaf(alpha, h.y, a[VEC > 1 ? 1 : 0]);
-                if (n + 2 < N) h.z = fmaf(alpha, h.z, a[VEC > 2 ? 2 : 0]);
-                if (n + 3 < N) h.w = fmaf(alpha, h.w, a[VEC > 3 ? 3 : 0]);
+                h.x = __fmaf_rn(alpha, h.x, a[0]);
+                if (n + 1 < N) h.y = __fmaf_rn(alpha, h.y, a[VEC > 1 ? 1 : 0]);
+                if (n + 2 < N) h.z = __fmaf_rn(alpha, h.z, a[VEC > 2 ? 2 : 0]);
+                if (n + 3 < N) h.w = __fmaf_rn(alpha, h.w, a[VEC > 3 ? 3 : 0]);
                 *reinterpret_cast<float4*>(hist + row + n) = h;
             }
         } else {
@@ -242,7 +224,8 @@ __global__ void __launch_bounds__(256) fuse_kernel(int max_ctx, const int* __res
 
 }  // namespace
 
-cudaError_t launch_score(const ScoreParams& p, float* scores_now, float* hist, float alpha, cudaStream_t stream) {
+cudaError_t launch_score(const ScoreParams& p, float* scores_now, float* hist, float alpha, bool logits_only,
+                         cudaStream_t stream) {
     dim3 grid(p.n_chunks, p.n_groups, p.batch);
     {
         ProfScope prof(kKernScoreLogits, stream);
@@ -252,7 +235,7 @@ cudaError_t launch_score(const ScoreParams& p, float* scores_now, float* hist, f
             score_logits_kernel<64><<<grid, kScoreThreads, 0, stream>>>(p);
     }
     cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
+    if (e != cudaSuccess || logits_only) return e;   // logits_only: the consumer (select.cu) normalises its own rows
     {
         ProfScope prof(kKernScoreStats, stream);
         score_stats_kernel<<<p.batch, 256, 0, stream>>>(p);

@@ -13,17 +13,6 @@ namespace dustin {
 
 namespace {
 
-#ifdef SEL_TS
-__device__ unsigned long long g_sel_ts[64];
-__device__ int g_sel_slot;
-__device__ unsigned long long g_blk[1024][4];
-__device__ __forceinline__ unsigned long long gt_now() { unsigned long long t_; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t_)); return t_; }
-#define STS() do { if (blockIdx.x == 3 && blockIdx.y == 5 && threadIdx.x == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t_)); g_sel_ts[g_sel_slot] = t_; g_sel_slot = (g_sel_slot + 1) & 63; } } while (0)
-#define SVAL(v) do { if (blockIdx.x == 3 && blockIdx.y == 5 && threadIdx.x == 0) { g_sel_ts[g_sel_slot] = 1000000000000000000ull + (unsigned long long)(v); g_sel_slot = (g_sel_slot + 1) & 63; } } while (0)
-#else
-#define STS() do {} while (0)
-#define SVAL(v) do {} while (0)
-#endif
 constexpr int kSelThreads = 1024;
 constexpr int kSelWarps = kSelThreads / 32;
 constexpr int kBins = 2048;
@@ -39,6 +28,7 @@ struct SelShared {
     // between a write and its reads is enough
     uint32_t tot_db[2][kSelWarps], min_db[2][kSelWarps], max_db[2][kSelWarps], res_db[2][4];
     uint32_t small_n, small_key[32], small_idx[32];
+    float2 stats[64];   // (M, 1/Z) of the heads feeding this row (row materialisation)
 };
 
 // Exclusive prefix of v over the block in thread order; *total (optional) receives the block sum.
@@ -602,6 +592,11 @@ __device__ void list_select_ranged(const float* __restrict__ s, const SelLayout&
     __syncthreads();
 }
 
+__device__ __noinline__ void list_select_ranged_big(const float* __restrict__ s, const SelLayout& L, int n_list,
+                                                    uint32_t rank, SelShared& sh, Phase& ph) {
+    list_select_ranged<8>(s, L, n_list, rank, sh, ph);
+}
+
 // ---- sampled path on 16-byte loads ---------------------------------------------------------------------------------
 // Thread t holds the vectors v0 + (8c + u) * 1024 + t of the row (chunk c = 32768 elements, u = 0..7).  A row of one
 // chunk stays in registers from the threshold estimate to the compaction; longer rows are re-read from L2 per phase.
@@ -658,9 +653,7 @@ __device__ bool sampled_tier_vec(const float* __restrict__ s, int lo, int hi, in
         }
     }
     uint32_t kmin, kmax;
-    STS();
     block_minmax(skey, skey, svalid, sh, ph, kmin, kmax);
-    STS();
     uint32_t tau = 0;   // 0: every candidate goes to the list
     if (kmin <= kmax) {
         const int shift = range_shift(kmin, kmax);
@@ -675,7 +668,6 @@ __device__ bool sampled_tier_vec(const float* __restrict__ s, int lo, int hi, in
     // ---- (b) compaction: candidates with key >= tau ----
     // Signed compare on the raw bits: for s >= 0 it is the key order; negative scores (key 0, reading A15) pass
     // only when tau == 0, i.e. when every candidate is taken.
-    STS();
     const int tau_s = tau == 0u ? INT_MIN : (int)tau;
     const int wsh = ((v0 + t) & 7) * 4;                      // this thread's nibble inside its bitmask words
     uint32_t base = 0;
@@ -711,14 +703,11 @@ __device__ bool sampled_tier_vec(const float* __restrict__ s, int lo, int hi, in
     }
     __syncthreads();
     const uint32_t n_list = base;
-    STS();
-    SVAL(n_list);
     if (n_list < (uint32_t)rank || n_list > (uint32_t)L.cap) return false;
     if (n_list <= 2u * kSelThreads)
         list_select_ranged<2>(s, L, (int)n_list, (uint32_t)rank, sh, ph);
     else
-        list_select_ranged<8>(s, L, (int)n_list, (uint32_t)rank, sh, ph);
-    STS();
+        list_select_ranged_big(s, L, (int)n_list, (uint32_t)rank, sh, ph);
     return true;
 }
 
@@ -728,27 +717,34 @@ __device__ bool sampled_tier_vec(const float* __restrict__ s, int lo, int hi, in
 //      is selected from the list alone.  The sample only decides which path runs, never the result.
 //  (2) histogram path: full histogram of the top 11 bits, second scan admits / compacts the threshold bin.
 //  (3) full-scan path for a threshold bin larger than the list (massive ties).
+// The slower paths of a tier, out of line so that the common path stays compact in the instruction cache.
 template <bool VEC>
-__device__ void select_tier(const float* __restrict__ s, int lo, int hi, int rank, const SelLayout& L, int n_words,
-                            SelShared& sh, Phase& ph, bool& hist_clean) {
-    const int R = L.R, rep = threadIdx.x & (R - 1);
-    uint32_t* hist = L.hist;
-    const ListAppender app{L.list_key, L.list_idx, &sh.list_n, (uint32_t)L.cap};
-    const int n_cand = hi - lo;
+__device__ __noinline__ void fallback_tier(const float* __restrict__ s, int lo, int hi, int rank, const SelLayout& L,
+                                           int n_words, SelShared& sh);
+
+template <bool VEC>
+__device__ __forceinline__ void select_tier(const float* __restrict__ s, int lo, int hi, int rank, const SelLayout& L,
+                                            int n_words, SelShared& sh, Phase& ph, bool& hist_clean) {
     if (VEC) {
-        STS();
         if (!hist_clean) {
-            clear_hist(hist, 1);
+            clear_hist(L.hist, 1);
             __syncthreads();
         }
         hist_clean = true;
         if (sampled_tier_vec(s, lo, hi, rank, L, sh, ph)) return;
         hist_clean = false;   // the paths below leave their counts behind
-#ifdef SEL_TS
-        if (threadIdx.x == 0) g_blk[blockIdx.y * gridDim.x + blockIdx.x][2] += 1;
-#endif
         __syncthreads();
     }
+    fallback_tier<VEC>(s, lo, hi, rank, L, n_words, sh);
+}
+
+template <bool VEC>
+__device__ __noinline__ void fallback_tier(const float* __restrict__ s, int lo, int hi, int rank, const SelLayout& L,
+                                           int n_words, SelShared& sh) {
+    const int R = L.R, rep = threadIdx.x & (R - 1);
+    uint32_t* hist = L.hist;
+    const ListAppender app{L.list_key, L.list_idx, &sh.list_n, (uint32_t)L.cap};
+    const int n_cand = hi - lo;
     // ---- (1) sampled threshold ----
     if (!VEC) {
         clear_hist(hist, 1);
@@ -796,23 +792,76 @@ __device__ void select_tier(const float* __restrict__ s, int lo, int hi, int ran
     list_select(L, (int)sh.list_n, rank1, 1, t1 << 21, sh);
 }
 
+// Row materialisation (fused entry point): a1's softmax normalisation summed over the heads of list l, and Eq. 5
+// (PAPER.md:161-164), for this CTA's own target row -- the same arithmetic as score_stats_kernel +
+// score_normalize_kernel (common.cuh helpers), so the result is bit-identical to the staged calls.  Ends with a
+// barrier; the row is then re-read with ld.cg (L2, where this CTA's stores have landed).
+__device__ __forceinline__ void materialize_row(const SelectParams& p, int b, int l, int N, SelShared& sh) {
+    const int first = p.norm.list_first[l], nh = p.norm.list_cnt[l];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int j = warp; j < nh; j += kSelWarps) {
+        const float2 st = fold_stats_warp(p.norm.part + ((long long)b * p.norm.nsel + first + j) * p.norm.n_chunks,
+                                          p.norm.n_chunks, lane);
+        if (lane == 0) sh.stats[j] = st;
+    }
+    __syncthreads();
+    float4* hrow = reinterpret_cast<float4*>(const_cast<float*>(p.s_target) +
+                                             ((long long)b * p.n_lists + l) * p.max_ctx);
+    const float* lg = p.norm.logits + ((long long)b * p.norm.nsel + first) * p.norm.logit_stride;
+    const float alpha = p.norm.alpha;
+    const int nvec = (N + 3) >> 2;
+    constexpr int kU = 4;   // vectors in flight per thread
+#pragma unroll 1
+    for (int v0 = threadIdx.x; v0 < nvec; v0 += kU * kSelThreads) {
+        float4 h[kU];
+        float a[kU][4];
+#pragma unroll
+        for (int u = 0; u < kU; ++u) {
+            const int v = v0 + u * kSelThreads;
+            h[u] = v < nvec ? hrow[v] : make_float4(0.f, 0.f, 0.f, 0.f);
+            a[u][0] = a[u][1] = a[u][2] = a[u][3] = 0.f;
+        }
+#pragma unroll 1
+        for (int j = 0; j < nh; ++j) {
+            const float2 st = sh.stats[j];
+            const float4* lj = reinterpret_cast<const float4*>(lg + (long long)j * p.norm.logit_stride);
+            float4 x[kU];
+#pragma unroll
+            for (int u = 0; u < kU; ++u) {
+                const int v = v0 + u * kSelThreads;
+                x[u] = v < nvec ? __ldcg(lj + v) : make_float4(0.f, 0.f, 0.f, 0.f);
+            }
+#pragma unroll
+            for (int u = 0; u < kU; ++u) prob_accumulate4(a[u], x[u], st);
+        }
+#pragma unroll
+        for (int u = 0; u < kU; ++u) {
+            const int v = v0 + u * kSelThreads, n = v << 2;
+            if (v < nvec) {
+                float4 r = h[u];
+                r.x = __fmaf_rn(alpha, r.x, a[u][0]);
+                if (n + 1 < N) r.y = __fmaf_rn(alpha, r.y, a[u][1]);
+                if (n + 2 < N) r.z = __fmaf_rn(alpha, r.z, a[u][2]);
+                if (n + 3 < N) r.w = __fmaf_rn(alpha, r.w, a[u][3]);
+                hrow[v] = r;
+            }
+        }
+    }
+    __syncthreads();   // the row is re-read below (ld.cg: L2, where these stores have landed for this CTA)
+}
+
 template <bool VEC>
 __global__ void __launch_bounds__(kSelThreads) select_kernel(const SelectParams p) {
     extern __shared__ __align__(16) uint32_t smem_dyn[];
     __shared__ SelShared sh;
     const int l = blockIdx.x, b = blockIdx.y;
-#ifdef SEL_TS
-    if (blockIdx.x == 3 && blockIdx.y == 5 && threadIdx.x == 0) g_sel_slot = 0;
-#endif
-    STS();
-#ifdef SEL_TS
-    if (threadIdx.x == 0) { g_blk[blockIdx.y * gridDim.x + blockIdx.x][0] = gt_now(); g_blk[blockIdx.y * gridDim.x + blockIdx.x][2] = 0; }
-#endif
     const int N = seq_len_of(p.seq_lens, b, p.max_ctx);
     const int k = p.budgets ? p.budgets[b] : p.budget;
     int* out = p.idx_out + ((long long)b * p.n_lists + l) * p.k_max;
     int* cnt_out = p.cnt_out + (long long)b * p.n_lists + l;
 
+    const bool own_row = VEC && p.norm.logits != nullptr;   // this CTA computes its target row itself
+    if (own_row) materialize_row(p, b, l, N, sh);
     if (k > p.k_max || k < p.n_sink + p.n_recent) {   // argument error on this row (dustin.h)
         for (int i = threadIdx.x; i < p.k_max; i += kSelThreads) out[i] = -1;
         if (threadIdx.x == 0) *cnt_out = 0;
@@ -862,7 +911,6 @@ __global__ void __launch_bounds__(kSelThreads) select_kernel(const SelectParams 
     }
     if (threadIdx.x == 0 && (N & 31)) mem[n_words - 1] &= (1u << (N & 31)) - 1u;   // drop the tail bits >= N
     __syncthreads();
-    STS();
     // I_verify in ascending order: prefix sum over the popcounts of the bitmask words.
     const int wpt = (n_words + kSelThreads - 1) / kSelThreads;   // consecutive words per thread
     const int w_lo = threadIdx.x * wpt, w_hi = min(w_lo + wpt, n_words);
@@ -881,10 +929,6 @@ __global__ void __launch_bounds__(kSelThreads) select_kernel(const SelectParams 
     }
     for (int i = (int)total + threadIdx.x; i < p.k_max; i += kSelThreads) out[i] = -1;
     if (threadIdx.x == 0) *cnt_out = (int)total;
-    STS();
-#ifdef SEL_TS
-    if (threadIdx.x == 0) g_blk[blockIdx.y * gridDim.x + blockIdx.x][1] = gt_now();
-#endif
 }
 
 }  // namespace
@@ -907,14 +951,6 @@ size_t select_smem_bytes(int max_ctx) {
     return ((size_t)mw + (size_t)kBins * R + 2 * (size_t)cap) * 4;
 }
 
-#ifdef SEL_TS
-extern "C" int dustin_dbg_sel_ts(unsigned long long* out) {
-    return (int)cudaMemcpyFromSymbol(out, g_sel_ts, sizeof(g_sel_ts));
-}
-extern "C" int dustin_dbg_sel_blk(unsigned long long* out) {
-    return (int)cudaMemcpyFromSymbol(out, g_blk, sizeof(g_blk));
-}
-#endif
 
 cudaError_t launch_select(const SelectParams& p_in, cudaStream_t stream) {
     SelectParams p = p_in;
