@@ -141,16 +141,6 @@ __host__ __device__ constexpr uint32_t umma_idesc(int m, int n, int a_mn_major, 
            ((uint32_t)(n >> 3) << 17) | ((uint32_t)(m >> 4) << 24);
 }
 
-// Predicated 2-byte store without a branch (keeps unrolled row loops in one basic block).
-__device__ __forceinline__ void st_bf16_if(__nv_bfloat16* p, float v, bool pred) {
-    const __nv_bfloat16 b = __float2bfloat16_rn(v);
-    asm volatile(
-        "{\n\t.reg .pred q;\n\t"
-        "setp.ne.b32 q, %2, 0;\n\t"
-        "@q st.global.b16 [%0], %1;\n\t}" ::"l"(p),
-        "h"(*reinterpret_cast<const unsigned short*>(&b)), "r"((uint32_t)pred)
-        : "memory");
-}
 __device__ __forceinline__ void st_release(int* p, int v) {
     asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
@@ -336,6 +326,16 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
         }
         return c + T;
     };
+    // Producers, whole-unit case (CTA x takes unit x from its first token, decided below): the index entries of tiles
+    // 0 and 1 are requested now, so that their latency overlaps the length loads and the prefix scan.
+    int spec_idx[2] = {-1, -1};
+    if (GATHER && warp >= 4 && warp < 8 && (int)blockIdx.x < n_units) {
+        const int sb = (int)blockIdx.x / Hkv, sl = p.n_lists == 1 ? 0 : (int)blockIdx.x - sb * Hkv;
+        const int* row = p.idx + ((long long)sb * p.n_lists + sl) * p.k_max;
+        const int pos0 = 32 * (warp - 4) + lane;
+        if (pos0 < p.k_max) spec_idx[0] = __ldg(row + pos0);
+        if (pos0 + kTile < p.k_max) spec_idx[1] = __ldg(row + pos0 + kTile);
+    }
     // barriers and TMEM first: neither depends on the list lengths, whose loads are in flight meanwhile
     const int per = (n_units + 255) / 256;
     const int u_lo = min(tid * per, n_units), u_hi = tid < 256 ? min(u_lo + per, n_units) : u_lo;
@@ -432,7 +432,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
         TileCursor pf = cur;   // runs two tiles ahead of `cur`
         struct Tok { int tok, b, g; };
         // token code of row 32*pw + lane of the cursor's tile: >= 0 cache row, -1 none, <= -2 new row (-2 - u)
-        auto load_tok = [&](const TileCursor& c) -> Tok {
+        auto load_tok = [&](const TileCursor& c, int spec = -1) -> Tok {   // spec >= 0: index entry already loaded
             Tok t;
             t.tok = -1; t.b = 0; t.g = 0;
             if (!c.valid) return t;
@@ -441,7 +441,9 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
             const int pos = s.pos_lo + c.ti * kTile + 32 * pw + lane;
             if (pos < s.pos_hi) {
                 if (pos < s.cnt)
-                    t.tok = GATHER ? __ldg(p.idx + ((long long)s.b * p.n_lists + s.list) * p.k_max + pos) : pos;
+                    t.tok = !GATHER ? pos
+                                    : (spec >= 0 ? spec
+                                                 : __ldg(p.idx + ((long long)s.b * p.n_lists + s.list) * p.k_max + pos));
                 else
                     t.tok = -2 - (pos - s.cnt);
             }
@@ -500,30 +502,38 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
             cp_async_mbar_arrive_noinc(bar(kSlotFull + sv));
         };
 
-        const Tok t0 = load_tok(pf);           // tiles 0 and 1: both index loads in flight before the first use
+        if (ptid == 0) TS(40);
+        // The T*r query rows of the cursor's segment (zero-padded to NQ) into Q buffer seg_no % 2.
+        auto issue_q = [&]() {
+            const int k = cur.seg_no, qb = k & 1;
+            mbar_wait(bar(kQEmpty + qb), (((uint32_t)(k >> 1)) & 1u) ^ 1u);
+            const uint32_t qdst = sbase + C::kOffQ + (uint32_t)qb * C::kQBytes;
+            const __nv_bfloat16* qsrc = p.q + ((long long)cur.s.b * T * Hq + (long long)cur.s.g * r) * kD;
+#pragma unroll 1
+            for (int x = ptid; x < NQ * 16; x += 128) {
+                const int rr = x >> 4, cc = x & 15;
+                const bool ok = rr < rows;
+                const __nv_bfloat16* src = ok ? qsrc + s_rowoff[rr] + cc * 8 : p.q;
+                cp_async16(qdst + (uint32_t)(cc >> 3) * (NQ * 128) + (uint32_t)rr * 128 +
+                               (uint32_t)(((cc & 7) ^ (rr & 7)) << 4), src, ok ? 16 : 0);
+            }
+            cp_async_mbar_arrive_noinc(bar(kQFull + qb));
+        };
+        // tiles 0 and 1: both index loads are in flight (or already here, whole-unit case) before the first use, and
+        // the first segment's Q rows are requested while they travel
+        const bool spec = GATHER && whole_mode;
+        const Tok t0 = load_tok(pf, spec ? spec_idx[0] : -1);
         if (pf.valid) pf.advance();
-        Tok t1 = load_tok(pf);
+        Tok t1 = load_tok(pf, spec ? spec_idx[1] : -1);
         if (pf.valid) pf.advance();
+        if (cur.valid) issue_q();
         RowPtr a0 = resolve(t0);
         int gj = 0;
         while (cur.valid) {
             Tok t2 = load_tok(pf);                 // tile gj + 2: index load in flight
             if (pf.valid) pf.advance();
             const RowPtr a1 = resolve(t1);         // tile gj + 1: page-table lookup in flight
-            if (cur.ti == 0) {                     // new segment: its T*r query rows (zero-padded to NQ)
-                const int k = cur.seg_no, qb = k & 1;
-                mbar_wait(bar(kQEmpty + qb), (((uint32_t)(k >> 1)) & 1u) ^ 1u);
-                const uint32_t qdst = sbase + C::kOffQ + (uint32_t)qb * C::kQBytes;
-                const __nv_bfloat16* qsrc = p.q + ((long long)cur.s.b * T * Hq + (long long)cur.s.g * r) * kD;
-                for (int x = ptid; x < NQ * 16; x += 128) {
-                    const int rr = x >> 4, cc = x & 15;
-                    const bool ok = rr < rows;
-                    const __nv_bfloat16* src = ok ? qsrc + s_rowoff[rr] + cc * 8 : p.q;
-                    cp_async16(qdst + (uint32_t)(cc >> 3) * (NQ * 128) + (uint32_t)rr * 128 +
-                                   (uint32_t)(((cc & 7) ^ (rr & 7)) << 4), src, ok ? 16 : 0);
-                }
-                cp_async_mbar_arrive_noinc(bar(kQFull + qb));
-            }
+            if (cur.ti == 0 && gj > 0) issue_q();  // new segment
             issue_tile(gj, a0);
             if (ptid == 0 && gj < 4) TS(4 + gj);
             a0 = a1;
@@ -778,7 +788,6 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
                 if (merge && t == 0)   // every thread is past its flag waits: leave the flags zero for the next launch
                     for (int j = 1; j < nseg; ++j) ws.flags[(long long)(s.cta_first + j) * 2] = 0;
                 if (t == 0) TS(33 + 4 * (cur.seg_no & 3));
-                __nv_bfloat16* outb = p.out + ((long long)s.b * T * Hq + (long long)s.g * r) * kD + t;   // t = dim
                 if (s.pos_lo != 0) {
                     float* po = ws.part_o + slot_id * NQ * kD + t;   // padded to NQ rows: no predicate
 #pragma unroll
@@ -812,11 +821,19 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
                         }
                     }
                     if (t == 0) TS(53);
-                    int ro[NQ];
+                    // bf16 rows staged in the P buffer (idle: every P.V of the piece has completed), then written
+                    // with 16-byte stores: row x / 16, chunk x % 16
+                    __nv_bfloat16* so = reinterpret_cast<__nv_bfloat16*>(smem + C::kOffP);
 #pragma unroll
-                    for (int i = 0; i < NQ; ++i) ro[i] = s_rowoff[i];
-#pragma unroll
-                    for (int i = 0; i < NQ; ++i) st_bf16_if(outb + ro[i], acc[i], i < rows);
+                    for (int i = 0; i < NQ; ++i) so[i * kD + t] = __float2bfloat16_rn(acc[i]);
+                    wg_sync();
+                    __nv_bfloat16* ob = p.out + ((long long)s.b * T * Hq + (long long)s.g * r) * kD;
+#pragma unroll 1
+                    for (int x = t; x < rows * 16; x += 128) {
+                        const int rr = x >> 4, cc = x & 15;
+                        *reinterpret_cast<uint4*>(ob + s_rowoff[rr] + cc * 8) =
+                            *reinterpret_cast<const uint4*>(so + rr * kD + cc * 8);
+                    }
                 }
                 if (t == 0) TS(34 + 4 * (cur.seg_no & 3));
                 if (t == 0) TS(35 + 4 * (cur.seg_no & 3));
