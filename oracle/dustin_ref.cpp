@@ -19,6 +19,10 @@
 //                                 causal among the new tokens).  idx == NULL gives the full-cache
 //                                 verification attention of :248 / :570.
 //
+//   dustin_ref_arr                :72-75 Eq. 1 (Attention Recovery Rate), Eq. 2-4 by composition.
+//   dustin_ref_append_kv          :153 (accepted tokens appended, rejected discarded).
+//   dustin_ref_draft_aggregate    :157-161 Eq. 5, first line (S_Draft = sum over draft heads, layers, lookahead tokens).
+//
 // Pins (tests/test_oracle_pins.py): brute force on tiny inputs, closed forms (uniform softmax, one
 // planted key, constant V, zero K), library cross-checks (torch fp64 softmax / SDPA, full sort),
 // invariants (row sums, membership, thresholds, k = N reproduces dense), printed Eq. 7 arithmetic.
@@ -293,6 +297,117 @@ int dustin_ref_sparse_verify_attn(int batch, int n_q_heads, int n_kv_heads, int 
                 if (lse) lse[((int64_t)b * n_q_heads + h) * T + t] = M + std::log(Z);
             }
         }
+    }
+    return 0;
+}
+
+// ---------------------------------------------------------------------------------------------
+// O5 -- Attention Recovery Rate, Eq. 1: ARR = sum_{j in K} A_j where A is normalised over the
+// valid positions V = [0, N_b) (sum_{j in V} A_j = 1).  `a` arrives as any non-negative weights (e.g. the
+// per-list sums of O1, which add up to the number of heads) and is normalised here: ARR = sum_K a / sum_V a;
+// a row without mass gives 0.  K = the cnt[b,l] DISTINCT entries idx[b,l,:] (a set, as in Eq. 1).
+// The windowed form (Eq. 2) and the SD-oracle bound (Eq. 3-4) follow by passing the window mean of A (Eq. 3's
+// A-bar; a window SUM gives the same ratio) and, for Eq. 4, K = TopK_k(A-bar) from O3 with m = 0, S = W = 0.
+// arr_out: fp64 [batch, n_lists].
+// ---------------------------------------------------------------------------------------------
+int dustin_ref_arr(int batch, int n_lists, int max_ctx, const int32_t* seq_lens, const float* a,
+                   const int32_t* idx, const int32_t* cnt, int k_max, double* arr_out) {
+    for (int b = 0; b < batch; ++b) {
+        const int N = seq_len(seq_lens, b, max_ctx);
+        for (int l = 0; l < n_lists; ++l) {
+            const float* row = a + ((int64_t)b * n_lists + l) * max_ctx;
+            double total = 0.0;
+            for (int n = 0; n < N; ++n) total += (double)row[n];
+            const int32_t* list = idx + ((int64_t)b * n_lists + l) * k_max;
+            int c = cnt[(int64_t)b * n_lists + l];
+            c = c < 0 ? 0 : (c > k_max ? k_max : c);
+            double kept = 0.0;
+            for (int i = 0; i < c; ++i)
+                if (list[i] >= 0 && list[i] < N) kept += (double)row[list[i]];
+            arr_out[(int64_t)b * n_lists + l] = total > 0.0 ? kept / total : 0.0;
+        }
+    }
+    return 0;
+}
+
+// ---------------------------------------------------------------------------------------------
+// O6 -- KV append after verification ("accepted tokens are appended to the KV cache, rejected ones
+// are discarded"; App. C.4 :453-466).  The first n_append[b] rows of the verify block (reading A13: row 0 is the
+// last generated token, rows 1.. the accepted draft tokens) become cache rows N_b, N_b+1, ... of sequence b; rows
+// that would not fit into max_ctx are dropped; seq_lens[b] grows accordingly.  When hist != NULL the accumulated
+// target scores of the new positions start from 0 (Eq. 5 is a sum and nothing has been added yet).
+// ---------------------------------------------------------------------------------------------
+int dustin_ref_append_kv(int batch, int n_kv_heads, int head_dim, int n_new, int max_ctx, uint16_t* k_cache,
+                         uint16_t* v_cache, int64_t stride_seq, int64_t stride_token, int64_t stride_head,
+                         const int32_t* page_table, int page_size, int max_pages, int32_t* seq_lens,
+                         const uint16_t* k_new, const uint16_t* v_new, const int32_t* n_append, float* hist,
+                         int n_lists) {
+    if (!seq_lens || !n_append) return -1;
+    KvView kv{k_cache, v_cache, stride_seq, stride_token, stride_head, page_table, page_size, max_pages};
+    for (int b = 0; b < batch; ++b) {
+        const int N = seq_len(seq_lens, b, max_ctx);
+        int a = n_append[b];
+        a = a < 0 ? 0 : (a > n_new ? n_new : a);
+        if (N + a > max_ctx) a = max_ctx - N;
+        for (int u = 0; u < a; ++u)
+            for (int g = 0; g < n_kv_heads; ++g) {
+                const int64_t dst = row_offset(kv, b, N + u, g);
+                const int64_t src = (((int64_t)b * n_new + u) * n_kv_heads + g) * head_dim;
+                for (int c = 0; c < head_dim; ++c) {
+                    k_cache[dst + c] = k_new[src + c];
+                    v_cache[dst + c] = v_new[src + c];
+                }
+            }
+        if (hist)
+            for (int l = 0; l < n_lists; ++l)
+                for (int u = 0; u < a; ++u) hist[((int64_t)b * n_lists + l) * max_ctx + N + u] = 0.0f;
+        seq_lens[b] = N + a;
+    }
+    return 0;
+}
+
+// ---------------------------------------------------------------------------------------------
+// O7 -- draft-side lookahead aggregation, Eq. 5 first line:
+//   S_Draft[n] = sum_{h in H_d} sum_{l in L_sel} sum_{gamma < Gamma} A^Draft_{h,l,n,gamma},
+// A^Draft_{h,l,.,gamma} = softmax over the N_b cached context tokens (reading A4) of the draft model's query of
+// lookahead token gamma, head h, layer l, against that layer's K cache.  One global vector per sequence
+// (PAPER.md:155).  Layer l's cache and queries are layer_k[l] (same strides / page table for all layers) and
+// layer_q[l] = bf16 [batch, n_gamma, n_q_heads, head_dim].  s_draft: fp32 [batch, max_ctx], written (0 for n >= N_b).
+// ---------------------------------------------------------------------------------------------
+int dustin_ref_draft_aggregate(int batch, int n_q_heads, int n_kv_heads, int head_dim, int n_gamma, int max_ctx,
+                               float sm_scale, int n_layers, const uint16_t* const* layer_k, int64_t stride_seq,
+                               int64_t stride_token, int64_t stride_head, const int32_t* page_table, int page_size,
+                               int max_pages, const int32_t* seq_lens, const uint16_t* const* layer_q,
+                               uint64_t head_mask, float* s_draft) {
+    if (n_q_heads % n_kv_heads != 0) return -1;
+    const int r = n_q_heads / n_kv_heads;
+    const double scale = scale_of(sm_scale, head_dim);
+#pragma omp parallel for schedule(dynamic)
+    for (int b = 0; b < batch; ++b) {
+        const int N = seq_len(seq_lens, b, max_ctx);
+        std::vector<double> sum(N, 0.0), logit(N);
+        for (int l = 0; l < n_layers; ++l) {
+            KvView kv{layer_k[l], nullptr, stride_seq, stride_token, stride_head, page_table, page_size, max_pages};
+            for (int gam = 0; gam < n_gamma; ++gam)
+                for (int h = 0; h < n_q_heads; ++h) {
+                    if (!((head_mask >> h) & 1ull)) continue;
+                    const int g = h / r;
+                    const uint16_t* qh = layer_q[l] + (((int64_t)b * n_gamma + gam) * n_q_heads + h) * head_dim;
+                    double M = -INFINITY;
+                    for (int n = 0; n < N; ++n) {
+                        const uint16_t* krow = layer_k[l] + row_offset(kv, b, n, g);
+                        double acc = 0.0;
+                        for (int c = 0; c < head_dim; ++c) acc += bf16_to_double(qh[c]) * bf16_to_double(krow[c]);
+                        logit[n] = acc * scale;
+                        if (logit[n] > M) M = logit[n];
+                    }
+                    double Z = 0.0;
+                    for (int n = 0; n < N; ++n) Z += std::exp(logit[n] - M);
+                    for (int n = 0; n < N; ++n) sum[n] += std::exp(logit[n] - M) / Z;
+                }
+        }
+        float* dst = s_draft + (int64_t)b * max_ctx;
+        for (int n = 0; n < max_ctx; ++n) dst[n] = n < N ? (float)sum[n] : 0.0f;
     }
     return 0;
 }

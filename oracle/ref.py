@@ -160,3 +160,57 @@ def sparse_verify_attn(kv: KV, q: torch.Tensor, k_new: torch.Tensor, v_new: torc
     if rc != 0:
         raise ValueError(f"dustin_ref_sparse_verify_attn: status {rc}")
     return out, lse
+
+
+def arr(a: torch.Tensor, idx: torch.Tensor, cnt: torch.Tensor, seq_lens=None) -> torch.Tensor:
+    """Eq. 1 (PAPER.md:72-75).  a: fp32 [B, G, N] non-negative weights; idx int32 [B, G, k_max] distinct entries;
+    cnt int32 [B, G].  Returns fp64 [B, G]."""
+    B, G, N = a.shape
+    out = torch.zeros(B, G, dtype=torch.float64)
+    rc = lib().dustin_ref_arr(ctypes.c_int(B), ctypes.c_int(G), ctypes.c_int(N), _p(_i32(seq_lens)), _p(_f32(a)),
+                              _p(_i32(idx)), _p(_i32(cnt)), ctypes.c_int(idx.shape[2]), _p(out))
+    if rc != 0:
+        raise ValueError(f"dustin_ref_arr: status {rc}")
+    return out
+
+
+def append_kv(kv: KV, seq_lens: torch.Tensor, k_new: torch.Tensor, v_new: torch.Tensor, n_append: torch.Tensor,
+              max_ctx: int, hist: Optional[torch.Tensor] = None):
+    """PAPER.md:153.  Writes the first n_append[b] rows of k_new / v_new ([B,T,Hkv,d] bf16) behind sequence b IN PLACE
+    in kv.k / kv.v, zeroes the new positions of hist ([B,G,max_ctx] fp32, in place) and returns the new int32 lengths."""
+    B, T, Hkv, d = k_new.shape
+    lens = seq_lens.to(torch.int32).contiguous().clone()
+    assert kv.k.is_contiguous() and kv.v.is_contiguous() and (hist is None or hist.is_contiguous())
+    pt = _i32(kv.page_table)
+    rc = lib().dustin_ref_append_kv(
+        ctypes.c_int(B), ctypes.c_int(Hkv), ctypes.c_int(d), ctypes.c_int(T), ctypes.c_int(max_ctx),
+        ctypes.c_void_p(kv.k.data_ptr()), ctypes.c_void_p(kv.v.data_ptr()), ctypes.c_int64(kv.stride_seq),
+        ctypes.c_int64(kv.stride_token), ctypes.c_int64(kv.stride_head), _p(pt), ctypes.c_int(kv.page_size),
+        ctypes.c_int(0 if pt is None else pt.shape[1]), _p(lens), _p(_bits(k_new)), _p(_bits(v_new)),
+        _p(_i32(n_append)), _p(hist), ctypes.c_int(0 if hist is None else hist.shape[1]))
+    if rc != 0:
+        raise ValueError(f"dustin_ref_append_kv: status {rc}")
+    return lens
+
+
+def draft_aggregate(layer_k: list, layer_q: list, head_mask: int, n_kv_heads: int, max_ctx: int, stride_seq: int,
+                    stride_token: int, stride_head: int, page_table=None, page_size: int = 0, seq_lens=None,
+                    sm_scale: float = 0.0) -> torch.Tensor:
+    """Eq. 5, first line.  layer_k[l]: bf16 K cache of draft layer l (all layers share the
+    strides / page table); layer_q[l]: bf16 [B, Gamma, Hq, d].  Returns S_Draft fp32 [B, max_ctx]."""
+    B, n_gamma, Hq, d = layer_q[0].shape
+    L = len(layer_k)
+    ks = [_bits(k) for k in layer_k]
+    qs = [_bits(q) for q in layer_q]
+    karr = (ctypes.c_void_p * L)(*[k.data_ptr() for k in ks])
+    qarr = (ctypes.c_void_p * L)(*[q.data_ptr() for q in qs])
+    pt = _i32(page_table)
+    out = torch.zeros(B, max_ctx, dtype=torch.float32)
+    rc = lib().dustin_ref_draft_aggregate(
+        ctypes.c_int(B), ctypes.c_int(Hq), ctypes.c_int(n_kv_heads), ctypes.c_int(d), ctypes.c_int(n_gamma),
+        ctypes.c_int(max_ctx), ctypes.c_float(sm_scale), ctypes.c_int(L), karr, ctypes.c_int64(stride_seq),
+        ctypes.c_int64(stride_token), ctypes.c_int64(stride_head), _p(pt), ctypes.c_int(page_size),
+        ctypes.c_int(0 if pt is None else pt.shape[1]), _p(_i32(seq_lens)), qarr, ctypes.c_uint64(head_mask), _p(out))
+    if rc != 0:
+        raise ValueError(f"dustin_ref_draft_aggregate: status {rc}")
+    return out
