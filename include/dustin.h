@@ -7,6 +7,8 @@
  *   a4 dustin_sparse_verify_attn (gamma+1)-query attention over the selected KV    PAPER.md:153, App. G :568
  *   a5 the same call with idx == NULL is the full-cache verification baseline
  *   a6 dustin_verify_layer_fused a1..a4 enqueued on one stream, no host sync
+ * and the steps either side of it: dustin_arr (Eq. 1-4), dustin_append_kv,
+ * dustin_draft_aggregate (Eq. 5, first line).
  *
  * Conventions (all entry points):
  *  - Every pointer marked "device" is a CUDA device pointer owned by the caller; the library never allocates,
@@ -112,7 +114,7 @@ void dustin_tune_attn_impl(int32_t impl);
  * (and drops earlier records); dustin_profile_enable(0) stops.  dustin_profile_collect is the one call that
  * synchronises: it waits for the recorded events and writes, per kernel id in [0, DUSTIN_N_KERNELS), the summed
  * device time in ms and the number of launches (host arrays), then clears the records.  Process-wide. */
-#define DUSTIN_N_KERNELS 7
+#define DUSTIN_N_KERNELS 9
 uint64_t    dustin_launch_count(void);
 void        dustin_profile_enable(int32_t on);
 int         dustin_profile_collect(double* ms_out, int64_t* launches_out);
@@ -168,6 +170,40 @@ int dustin_verify_layer_fused(const dustin_shape_t* shape, const dustin_kv_t* kv
                               const dustin_select_t* select, int32_t k_max, float* scores_now_out, void* out,
                               float* lse_out, int32_t* idx_out, int32_t* cnt_out, void* ws, size_t ws_bytes,
                               void* stream);
+
+/* ---- steps either side of the layer path ---------------------------------------------------- */
+
+/* Attention Recovery Rate, Eq. 1: the share of the attention mass of row (b,l) that the index list
+ * keeps,  arr[b,l] = sum_{j in idx[b,l,:cnt[b,l]]} a[b,l,j] / sum_{j < N_b} a[b,l,j]   (0 for a row without mass).
+ * `a` is any non-negative weight row (it is normalised here, as Eq. 1 requires sum_V A = 1); the listed indices
+ * must be distinct (a set; dustin_topk_select's output is).  The windowed ARR of Eq. 2 and the SD-oracle bound of
+ * Eq. 3-4 follow by composition: pass the window sum of A (dustin_fuse_scores with alpha = 1) and, for Eq. 4, the
+ * list dustin_topk_select returns for it with m = 0, S = W = 0.
+ *   a: device fp32 [B, n_lists, max_ctx];  idx: device int32 [B, n_lists, k_max];  cnt: device int32 [B, n_lists];
+ *   arr_out: device fp32 [B, n_lists], written. */
+int dustin_arr(int32_t batch, int32_t n_lists, int32_t max_ctx, const int32_t* seq_lens, const float* a,
+               const int32_t* idx, const int32_t* cnt, int32_t k_max, float* arr_out, void* stream);
+
+/* KV append after verification (accepted tokens are appended to the cache, rejected ones discarded).
+ * The first n_append[b] rows (clipped to [0, T] and to the room left below max_ctx) of the verify block k_new /
+ * v_new [B,T,Hkv,d] become cache rows N_b, N_b+1, ... of sequence b (kv->k / kv->v are WRITTEN; in a paged cache the
+ * pages must already be mapped); seq_lens_inout[b] grows by that count.  kv->seq_lens is ignored (the lengths are
+ * seq_lens_inout).  hist_inout (optional, device fp32 [B, n_lists, max_ctx]): the accumulated scores of the new
+ * positions are set to 0 (Eq. 5 is a sum; nothing has been added for them yet).
+ *   seq_lens_inout, n_append: device int32 [B]. */
+int dustin_append_kv(const dustin_shape_t* shape, const dustin_kv_t* kv, int32_t* seq_lens_inout, const void* k_new,
+                     const void* v_new, const int32_t* n_append, float* hist_inout, int32_t n_lists, void* stream);
+
+/* Draft-side lookahead aggregation, Eq. 5 first line:
+ *   s_draft[b,n] = sum_{h in head_mask} sum_{l < n_layers} sum_{gamma < T} softmax_n( sm_scale * q_l[b,gamma,h,:] . K_l[b,n,g(h),:] )
+ * over the N_b cached tokens (reading A4), one vector per sequence.  `shape` describes the DRAFT model
+ * (n_new = the number of lookahead queries per layer).  kv_layers: HOST array of n_layers cache descriptors (only k is
+ * read);  q_layers: HOST array of n_layers device pointers, each bf16 [B, T, Hq, d].  Runs the scoring stage (a1) once
+ * per (layer, lookahead token) on `stream`.   s_draft: device fp32 [B, max_ctx], written (0 for n >= N_b).
+ *   ws: dustin_workspace_bytes(shape, head_mask, 1) bytes. */
+int dustin_draft_aggregate(const dustin_shape_t* shape, const dustin_kv_t* kv_layers, const void* const* q_layers,
+                           int32_t n_layers, uint64_t head_mask, float* s_draft, void* ws, size_t ws_bytes,
+                           void* stream);
 
 #ifdef __cplusplus
 }

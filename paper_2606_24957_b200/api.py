@@ -90,17 +90,24 @@ def lib():
         L.dustin_verify_layer_fused.restype = ctypes.c_int
         L.dustin_verify_layer_fused.argtypes = [sp, kp, vp, vp, vp, u64, vp, i64, vp, f32, selp, i32, vp, vp, vp,
                                                 vp, vp, vp, sz, vp]
+        L.dustin_arr.restype = ctypes.c_int
+        L.dustin_arr.argtypes = [i32, i32, i32, vp, vp, vp, vp, i32, vp, vp]
+        L.dustin_append_kv.restype = ctypes.c_int
+        L.dustin_append_kv.argtypes = [sp, kp, vp, vp, vp, vp, vp, i32, vp]
+        L.dustin_draft_aggregate.restype = ctypes.c_int
+        L.dustin_draft_aggregate.argtypes = [sp, kp, ctypes.POINTER(vp), i32, u64, vp, vp, sz, vp]
         _lib = L
     return _lib
 
 
-N_KERNELS = 7
+N_KERNELS = 9
 
 EXPORTS = ("dustin_version", "dustin_status_string", "dustin_last_cuda_error", "dustin_tune_attn_split_tokens",
            "dustin_tune_attn_impl",
            "dustin_launch_count", "dustin_profile_enable", "dustin_profile_collect", "dustin_kernel_name",
            "dustin_workspace_bytes", "dustin_score_heads", "dustin_fuse_scores", "dustin_topk_select",
-           "dustin_sparse_verify_attn", "dustin_verify_layer_fused")
+           "dustin_sparse_verify_attn", "dustin_verify_layer_fused", "dustin_arr", "dustin_append_kv",
+           "dustin_draft_aggregate")
 
 
 @dataclass
@@ -292,3 +299,37 @@ def verify_layer_fused(shape: Shape, kv: KV, q: torch.Tensor, k_new: torch.Tenso
         None if lse_out is None else _dense(lse_out, torch.float32), _dense(idx_out, torch.int32),
         _dense(cnt_out, torch.int32), _ptr(ws), ws.numel(), _stream())
     _check("dustin_verify_layer_fused", rc)
+
+
+def arr(a: torch.Tensor, idx: torch.Tensor, cnt: torch.Tensor, arr_out: torch.Tensor,
+        seq_lens: Optional[torch.Tensor] = None) -> None:
+    """Eq. 1: a fp32 [B,G,N], idx int32 [B,G,k_max], cnt int32 [B,G] -> arr_out fp32 [B,G]."""
+    B, G, N = a.shape
+    rc = lib().dustin_arr(B, G, N, None if seq_lens is None else _dense(seq_lens, torch.int32),
+                          _dense(a, torch.float32), _dense(idx, torch.int32), _dense(cnt, torch.int32), idx.shape[2],
+                          _dense(arr_out, torch.float32), _stream())
+    _check("dustin_arr", rc)
+
+
+def append_kv(shape: Shape, kv: KV, seq_lens_inout: torch.Tensor, k_new: torch.Tensor, v_new: torch.Tensor,
+              n_append: torch.Tensor, hist_inout: Optional[torch.Tensor] = None) -> None:
+    """the first n_append[b] rows of the verify block go behind sequence b; lengths advance in place."""
+    kvc = kv.c()
+    rc = lib().dustin_append_kv(
+        ctypes.byref(shape), ctypes.byref(kvc), _dense(seq_lens_inout, torch.int32), _dense(k_new, torch.bfloat16),
+        _dense(v_new, torch.bfloat16), _dense(n_append, torch.int32),
+        None if hist_inout is None else _dense(hist_inout, torch.float32),
+        0 if hist_inout is None else hist_inout.shape[1], _stream())
+    _check("dustin_append_kv", rc)
+
+
+def draft_aggregate(shape: Shape, kv_layers: list, q_layers: list, head_mask: int, s_draft: torch.Tensor,
+                    ws: torch.Tensor) -> None:
+    """Eq. 5, first line: kv_layers / q_layers are per-draft-layer KV views and bf16 [B,T,Hq,d]
+    query tensors; s_draft fp32 [B, max_ctx] is written."""
+    L = len(kv_layers)
+    kvs = (_Kv * L)(*[kv.c() for kv in kv_layers])
+    qs = (ctypes.c_void_p * L)(*[_dense(q, torch.bfloat16) for q in q_layers])
+    rc = lib().dustin_draft_aggregate(ctypes.byref(shape), kvs, qs, L, ctypes.c_uint64(head_mask),
+                                      _dense(s_draft, torch.float32), _ptr(ws), ws.numel(), _stream())
+    _check("dustin_draft_aggregate", rc)

@@ -421,4 +421,55 @@ int dustin_verify_layer_fused(const dustin_shape_t* shape, const dustin_kv_t* kv
                     ws, ws_bytes, st);
 }
 
+int dustin_arr(int32_t batch, int32_t n_lists, int32_t max_ctx, const int32_t* seq_lens, const float* a,
+               const int32_t* idx, const int32_t* cnt, int32_t k_max, float* arr_out, void* stream) {
+    if (batch <= 0 || n_lists <= 0 || max_ctx < 0 || k_max <= 0 || !a || !idx || !cnt || !arr_out)
+        return DUSTIN_ERR_INVALID_ARG;
+    if (batch > 65535) return DUSTIN_ERR_UNSUPPORTED;
+    const cudaError_t e = launch_arr(batch, n_lists, max_ctx, seq_lens, a, idx, cnt, k_max, arr_out,
+                                     static_cast<cudaStream_t>(stream));
+    return e == cudaSuccess ? DUSTIN_OK : fail_cuda(e);
+}
+
+int dustin_append_kv(const dustin_shape_t* shape, const dustin_kv_t* kv, int32_t* seq_lens_inout, const void* k_new,
+                     const void* v_new, const int32_t* n_append, float* hist_inout, int32_t n_lists, void* stream) {
+    int rc = check_shape(shape);
+    if (rc) return rc;
+    KvView view;
+    rc = check_kv(shape, kv, true, &view);
+    if (rc) return rc;
+    if (!seq_lens_inout || !k_new || !v_new || !n_append || (hist_inout && n_lists <= 0)) return DUSTIN_ERR_INVALID_ARG;
+    if (((uintptr_t)k_new | (uintptr_t)v_new) & 15) return DUSTIN_ERR_INVALID_ARG;
+    view.seq_lens = seq_lens_inout;
+    const cudaError_t e = launch_append(view, seq_lens_inout, n_append, static_cast<const __nv_bfloat16*>(k_new),
+                                        static_cast<const __nv_bfloat16*>(v_new), shape->batch, shape->n_new,
+                                        shape->n_kv_heads, shape->head_dim, shape->max_ctx, hist_inout, n_lists,
+                                        static_cast<cudaStream_t>(stream));
+    return e == cudaSuccess ? DUSTIN_OK : fail_cuda(e);
+}
+
+int dustin_draft_aggregate(const dustin_shape_t* shape, const dustin_kv_t* kv_layers, const void* const* q_layers,
+                           int32_t n_layers, uint64_t head_mask, float* s_draft, void* ws, size_t ws_bytes,
+                           void* stream) {
+    int rc = check_shape(shape);
+    if (rc) return rc;
+    if (!kv_layers || !q_layers || n_layers <= 0 || !s_draft) return DUSTIN_ERR_INVALID_ARG;
+    for (int l = 0; l < n_layers; ++l)
+        if (!q_layers[l]) return DUSTIN_ERR_INVALID_ARG;
+    const int64_t q_stride_batch = (int64_t)shape->n_new * shape->n_q_heads * shape->head_dim;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    bool first = true;
+    for (int l = 0; l < n_layers; ++l)
+        for (int gam = 0; gam < shape->n_new; ++gam) {
+            const __nv_bfloat16* q = static_cast<const __nv_bfloat16*>(q_layers[l]) +
+                                     (int64_t)gam * shape->n_q_heads * shape->head_dim;
+            // the first term overwrites s_draft (and writes the zeros beyond N_b), the others accumulate (Eq. 5 is a sum)
+            rc = run_score(shape, &kv_layers[l], q, q_stride_batch, shape->head_dim, head_mask, 1,
+                           first ? s_draft : nullptr, first ? nullptr : s_draft, 1.0f, ws, ws_bytes, st);
+            if (rc) return rc;
+            first = false;
+        }
+    return DUSTIN_OK;
+}
+
 }  // extern "C"

@@ -1,0 +1,117 @@
+// extras.cu -- the steps either side of the per-layer path:
+//   arr_kernel          Attention Recovery Rate of an index list, Eq. 1; Eq. 2-4 by composition
+//   append_rows_kernel  accepted rows of the verify block appended to the KV cache, new positions of the
+//   bump_lens_kernel    accumulated scores zeroed, sequence lengths advanced
+// The draft-side lookahead aggregation (Eq. 5, first line) is a host loop over the scoring stage and lives in api.cu.
+#include "kernels.cuh"
+
+namespace dustin {
+
+namespace {
+
+constexpr int kArrThreads = 256;
+
+// One CTA per (list, sequence): total mass of the row over [0, N_b), mass at the listed positions, their ratio.
+// fp64 accumulation in a fixed order (strided per thread, shuffle tree, then the 8 warps in order): deterministic.
+__global__ void __launch_bounds__(kArrThreads) arr_kernel(int max_ctx, int n_lists, const int* __restrict__ seq_lens,
+                                                          const float* __restrict__ a, const int* __restrict__ idx,
+                                                          const int* __restrict__ cnt, int k_max,
+                                                          float* __restrict__ arr_out) {
+    const int l = blockIdx.x, b = blockIdx.y;
+    const int N = seq_len_of(seq_lens, b, max_ctx);
+    const float* row = a + ((long long)b * n_lists + l) * max_ctx;
+    const int* list = idx + ((long long)b * n_lists + l) * k_max;
+    int c = cnt[(long long)b * n_lists + l];
+    c = c < 0 ? 0 : (c > k_max ? k_max : c);
+    double total = 0.0, kept = 0.0;
+    for (int n = threadIdx.x; n < N; n += kArrThreads) total += (double)__ldg(row + n);
+    for (int i = threadIdx.x; i < c; i += kArrThreads) {
+        const int j = __ldg(list + i);
+        if (j >= 0 && j < N) kept += (double)__ldg(row + j);
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        total += __shfl_xor_sync(0xffffffffu, total, off);
+        kept += __shfl_xor_sync(0xffffffffu, kept, off);
+    }
+    __shared__ double s_tot[kArrThreads / 32], s_kept[kArrThreads / 32];
+    if ((threadIdx.x & 31) == 0) {
+        s_tot[threadIdx.x >> 5] = total;
+        s_kept[threadIdx.x >> 5] = kept;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0, k = 0.0;
+        for (int w = 0; w < kArrThreads / 32; ++w) {
+            t += s_tot[w];
+            k += s_kept[w];
+        }
+        arr_out[(long long)b * n_lists + l] = t > 0.0 ? (float)(k / t) : 0.f;
+    }
+}
+
+// Rows to append to sequence b: n_append[b] clipped to [0, T] and to the room left in the cache.
+__device__ __forceinline__ int rows_to_append(const int* seq_lens, const int* n_append, int b, int T, int max_ctx,
+                                              int& N) {
+    N = seq_len_of(seq_lens, b, max_ctx);
+    int a = n_append[b];
+    a = a < 0 ? 0 : (a > T ? T : a);
+    return N + a > max_ctx ? max_ctx - N : a;
+}
+
+// One CTA per (block row u, sequence b); thread = one 16-byte chunk of the Hkv * d elements of that token.
+__global__ void append_rows_kernel(KvView kv, const int* __restrict__ n_append, const __nv_bfloat16* __restrict__ k_new,
+                                   const __nv_bfloat16* __restrict__ v_new, int T, int n_kv_heads, int head_dim,
+                                   int max_ctx, float* __restrict__ hist, int n_lists) {
+    const int u = blockIdx.x, b = blockIdx.y;
+    int N;
+    const int a = rows_to_append(kv.seq_lens, n_append, b, T, max_ctx, N);
+    if (u >= a) return;
+    const int chunks_per_head = head_dim / 8;
+    for (int x = threadIdx.x; x < n_kv_heads * chunks_per_head; x += blockDim.x) {
+        const int g = x / chunks_per_head, c = x - g * chunks_per_head;
+        const long long dst = kv_row_offset(kv, b, N + u, g) + c * 8;
+        const long long src = (((long long)b * T + u) * n_kv_heads + g) * head_dim + c * 8;
+        *reinterpret_cast<uint4*>(const_cast<__nv_bfloat16*>(kv.k) + dst) = *reinterpret_cast<const uint4*>(k_new + src);
+        *reinterpret_cast<uint4*>(const_cast<__nv_bfloat16*>(kv.v) + dst) = *reinterpret_cast<const uint4*>(v_new + src);
+    }
+    if (hist)
+        for (int l = threadIdx.x; l < n_lists; l += blockDim.x) hist[((long long)b * n_lists + l) * max_ctx + N + u] = 0.f;
+}
+
+// Runs after append_rows_kernel on the same stream: every reader of the old lengths is done.
+__global__ void bump_lens_kernel(int* __restrict__ seq_lens, const int* __restrict__ n_append, int batch, int T,
+                                 int max_ctx) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= batch) return;
+    int N;
+    const int a = rows_to_append(seq_lens, n_append, b, T, max_ctx, N);
+    seq_lens[b] = N + a;
+}
+
+}  // namespace
+
+cudaError_t launch_arr(int batch, int n_lists, int max_ctx, const int* seq_lens, const float* a, const int* idx,
+                       const int* cnt, int k_max, float* arr_out, cudaStream_t stream) {
+    ProfScope prof(kKernArr, stream);
+    arr_kernel<<<dim3(n_lists, batch), kArrThreads, 0, stream>>>(max_ctx, n_lists, seq_lens, a, idx, cnt, k_max, arr_out);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_append(const KvView& kv, int* seq_lens, const int* n_append, const __nv_bfloat16* k_new,
+                          const __nv_bfloat16* v_new, int batch, int T, int n_kv_heads, int head_dim, int max_ctx,
+                          float* hist, int n_lists, cudaStream_t stream) {
+    {
+        ProfScope prof(kKernAppend, stream);
+        const int threads = min(256, max(32, n_kv_heads * head_dim / 8));
+        append_rows_kernel<<<dim3(T, batch), threads, 0, stream>>>(kv, n_append, k_new, v_new, T, n_kv_heads, head_dim,
+                                                                  max_ctx, hist, n_lists);
+    }
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    ProfScope prof(kKernAppend, stream);
+    bump_lens_kernel<<<(batch + 127) / 128, 128, 0, stream>>>(seq_lens, n_append, batch, T, max_ctx);
+    return cudaGetLastError();
+}
+
+}  // namespace dustin

@@ -93,9 +93,18 @@ cudaError_t launch_attn_tc(const AttnParams& p, void* ws_base, cudaStream_t stre
 void attn_set_impl(int impl);   // 0 auto, 1 mma.sync cluster kernel, 2 tcgen05 kernel where usable
 int attn_get_impl();
 
+// ---- steps either side of the layer path (extras.cu) -----------------------------------------
+cudaError_t launch_arr(int batch, int n_lists, int max_ctx, const int* seq_lens, const float* a, const int* idx,
+                       const int* cnt, int k_max, float* arr_out, cudaStream_t stream);
+// kv.seq_lens must be seq_lens (the lengths before the append); k / v of the view are written.
+cudaError_t launch_append(const KvView& kv, int* seq_lens, const int* n_append, const __nv_bfloat16* k_new,
+                          const __nv_bfloat16* v_new, int batch, int T, int n_kv_heads, int head_dim, int max_ctx,
+                          float* hist, int n_lists, cudaStream_t stream);
+
 // ---- launch bookkeeping (profile.cu) ----------------------------------------------------------------------------
 enum KernelId {
     kKernScoreLogits = 0, kKernScoreStats, kKernScoreNormalize, kKernFuse, kKernSelect, kKernAttn, kKernAttnCombine,
+    kKernArr, kKernAppend,
     kKernCount
 };
 // Put one on the stack around a kernel launch: counts it and, when profiling is on, brackets it with CUDA events.

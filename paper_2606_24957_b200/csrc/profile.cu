@@ -30,7 +30,8 @@ cudaEvent_t take_event() {
     return e;
 }
 const char* const kNames[kKernCount] = {"score_logits_kernel", "score_stats_kernel", "score_normalize_kernel",
-                                        "fuse_kernel", "select_kernel", "attn_kernel", "attn_combine_kernel"};
+                                        "fuse_kernel", "select_kernel", "attn_kernel", "attn_combine_kernel",
+                                        "arr_kernel", "append_kernel"};
 }  // namespace
 
 ProfScope::ProfScope(int kid, cudaStream_t stream) : kid_(kid), stream_(stream), slot_(-1) {

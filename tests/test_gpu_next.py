@@ -1,0 +1,167 @@
+"""GPU parity of the steps either side of the layer path: dustin_arr (Eq. 1-4), dustin_append_kv
+(PAPER.md:153), dustin_draft_aggregate (Eq. 5, first line) and a multi-step decode loop that chains them with the
+fused layer call.  Every expected value comes from oracle/."""
+import math
+
+import pytest
+import torch
+
+from oracle import ref
+from paper_2606_24957_b200 import api, synth
+from tests import harness as H
+
+pytestmark = pytest.mark.gpu
+
+ARR_ATOL = 2e-6            # fp64 accumulation on both sides, one fp32 rounding of the ratio
+DRAFT_RTOL = 1e-5          # same arithmetic as a1 (DESIGN.md §7 rule 3), a sum of L * Gamma fp32 terms
+
+
+def _rand_bf16(*shape, seed):
+    g = torch.Generator().manual_seed(seed)
+    return torch.randn(*shape, generator=g).to(torch.bfloat16)
+
+
+# ---- dustin_arr -------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("B,G,N,k", [(1, 1, 1024, 128), (3, 4, 5000, 700), (2, 8, 32768, 2048)])
+def test_arr_matches_oracle(B, G, N, k):
+    g = torch.Generator().manual_seed(N)
+    a = torch.rand(B, G, N, generator=g) ** 8                       # a few heavy entries, like attention rows
+    sd = torch.rand(B, G, N, generator=g)
+    lens = torch.randint(k + 1, N + 1, (B,), generator=g, dtype=torch.int32)
+    lens[0] = N
+    idx, cnt = ref.topk_select(sd, a, k, 4, 16, 1, 2, k, lens)
+    want = ref.arr(a, idx, cnt, lens)
+    got = torch.full((B, G), float("nan"), device="cuda")
+    api.arr(a.cuda(), idx.cuda(), cnt.cuda(), got, lens.cuda())
+    assert torch.allclose(got.cpu().double(), want, atol=ARR_ATOL, rtol=0)
+    # empty lists and rows without mass
+    api.arr(torch.zeros(B, G, N, device="cuda"), idx.cuda(), cnt.cuda(), got, lens.cuda())
+    assert torch.all(got == 0)
+    api.arr(a.cuda(), idx.cuda(), torch.zeros_like(cnt).cuda(), got, lens.cuda())
+    assert torch.all(got == 0)
+
+
+def test_sd_oracle_bound_eq4_by_composition_of_select_and_arr():
+    """Eq. 3-4: K = TopK_k of the window sum (dustin_fuse_scores, alpha = 1), ARR evaluated on it; and no policy list
+    of the same size beats it."""
+    B, G, N, k, w = 2, 2, 4096, 256, 4
+    g = torch.Generator().manual_seed(7)
+    steps = [(torch.rand(B, G, N, generator=g) ** 6).cuda() for _ in range(w)]
+    acc = torch.zeros(B, G, N, device="cuda")
+    for s in steps:
+        api.fuse_scores(s, acc, 1.0)
+    idx = torch.empty(B, G, k, dtype=torch.int32, device="cuda")
+    cnt = torch.empty(B, G, dtype=torch.int32, device="cuda")
+    api.topk_select(api.Select(k, 0, 0, 0, 1, G, None), acc, acc, idx, cnt)
+    best = torch.empty(B, G, device="cuda")
+    api.arr(acc, idx, cnt, best)
+    want_idx, want_cnt = ref.topk_select(acc.cpu(), acc.cpu(), k, 0, 0, 0, 1)
+    assert torch.equal(idx.cpu(), want_idx)
+    assert torch.allclose(best.cpu().double(), ref.arr(acc.cpu(), want_idx, want_cnt), atol=ARR_ATOL)
+    other = torch.empty(B, G, device="cuda")
+    api.topk_select(api.Select(k, 0, 0, 0, 1, G, None), steps[0], steps[0], idx, cnt)   # look-back policy, delta = w
+    api.arr(acc, idx, cnt, other)
+    assert torch.all(other <= best + 1e-6)
+
+
+# ---- dustin_append_kv -------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("paged", [False, True])
+def test_append_matches_oracle_bitwise(paged):
+    B, cap, Hkv, Hq, d, T, G, page = 5, 96, 4, 8, 128, 5, 4, 16
+    k, v = _rand_bf16(B, cap, Hkv, d, seed=1), _rand_bf16(B, cap, Hkv, d, seed=2)
+    kn, vn = _rand_bf16(B, T, Hkv, d, seed=3), _rand_bf16(B, T, Hkv, d, seed=4)
+    lens = torch.tensor([10, 93, 0, 96, 47], dtype=torch.int32)
+    na = torch.tensor([5, 5, 1, 3, 0], dtype=torch.int32)
+    hist = torch.rand(B, G, cap)
+    shape = api.Shape(B, Hq, Hkv, d, T, cap, 0.0)
+    if paged:
+        n_pages = B * cap // page
+        table = torch.randperm(n_pages, generator=torch.Generator().manual_seed(5)).to(torch.int32).view(B, cap // page)
+        kp = torch.zeros(n_pages, page, Hkv, d, dtype=torch.bfloat16)
+        vp = torch.zeros_like(kp)
+        for b in range(B):
+            for pg in range(cap // page):
+                kp[table[b, pg]] = k[b, pg * page:(pg + 1) * page]
+                vp[table[b, pg]] = v[b, pg * page:(pg + 1) * page]
+        k, v = kp, vp
+        cpu_kv = ref.KV(k, v, page * Hkv * d, Hkv * d, d, table.contiguous(), page)
+        gk, gv = k.cuda(), v.cuda()
+        gpu_kv = api.KV.paged_nhd(gk, gv, table.contiguous().cuda(), None)
+    else:
+        cpu_kv = ref.KV.contiguous_nhd(k, v)
+        gk, gv = k.cuda(), v.cuda()
+        gpu_kv = api.KV.contiguous_nhd(gk, gv, None)
+    g_lens, g_hist = lens.cuda(), hist.cuda()
+    api.append_kv(shape, gpu_kv, g_lens, kn.cuda(), vn.cuda(), na.cuda(), g_hist)
+    torch.cuda.synchronize()
+    want_lens = ref.append_kv(cpu_kv, lens, kn, vn, na, cap, hist)          # k, v, hist updated in place
+    assert g_lens.cpu().tolist() == want_lens.tolist() == [15, 96, 1, 96, 47]
+    assert torch.equal(gk.cpu().view(torch.int16), k.view(torch.int16))
+    assert torch.equal(gv.cpu().view(torch.int16), v.view(torch.int16))
+    assert torch.equal(g_hist.cpu(), hist)
+
+
+# ---- dustin_draft_aggregate -------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("B,N,Hq,Hkv,d,gamma,L,mask", [
+    (2, 3000, 14, 2, 64, 4, 3, 0b00101000100010),      # Qwen2.5-0.5B-shaped draft: 14/2 heads, d = 64, 3 layers x 4 heads
+    (1, 1024, 8, 8, 128, 2, 2, 0b10000001),
+])
+def test_draft_aggregate_matches_oracle(B, N, Hq, Hkv, d, gamma, L, mask):
+    ks = [_rand_bf16(B, N, Hkv, d, seed=10 + l) for l in range(L)]
+    qs = [_rand_bf16(B, gamma, Hq, d, seed=20 + l) for l in range(L)]
+    lens = torch.tensor([N] + [N - 333] * (B - 1), dtype=torch.int32)
+    want = ref.draft_aggregate(ks, qs, mask, Hkv, N, N * Hkv * d, Hkv * d, d, seq_lens=lens)
+    shape = api.Shape(B, Hq, Hkv, d, gamma, N, 0.0)
+    ws = api.alloc_workspace(shape, mask, 1)
+    gks = [k.cuda() for k in ks]
+    kvs = [api.KV.contiguous_nhd(k, None, lens.cuda()) for k in gks]
+    got = torch.full((B, N), float("nan"), device="cuda")
+    api.draft_aggregate(shape, kvs, [q.cuda() for q in qs], mask, got, ws)
+    torch.cuda.synchronize()
+    H.check_scores(got.cpu().unsqueeze(1), want.unsqueeze(1), "s_draft", DRAFT_RTOL)
+    n_terms = bin(mask).count("1") * L * gamma
+    assert torch.allclose(got.sum(-1).cpu(), torch.full((B,), float(n_terms)), rtol=1e-4)   # Eq. 5 mass
+
+
+# ---- multi-step decode loop: verify -> accept -> append, history carried ----------------------
+def test_multi_step_decode_loop_matches_oracle():
+    """Three speculative steps on one layer.  Each step: the fused layer call (a1..a4) on the GPU and the oracle on the
+    CPU from the SAME state; a seeded acceptance length; dustin_append_kv on both sides.  State carried across steps:
+    cache, lengths, accumulated scores (Eq. 5)."""
+    cfg = synth.shrink(synth.config_llama8b(batch=3, ctx=2048, n_layers=1), budget=256, n_sink=8, n_recent=32)
+    cap = cfg.ctx
+    cpu = synth.make_layer(cfg, 0, "cpu")
+    g = torch.Generator().manual_seed(99)
+    lens = torch.tensor([cap - 40, cap - 400, cap - 2], dtype=torch.int32)       # the last one runs out of room
+    cpu.seq_lens = lens.clone()
+    for b in range(cfg.batch):                                                     # nothing accumulated beyond N_b yet
+        cpu.hist[b, :, int(lens[b]):] = 0
+    dev = cpu.to("cuda")
+    sh = H.shape_of(cfg)
+    ws = api.alloc_workspace(sh, cfg.head_mask, cpu.k_max)
+    for step in range(3):
+        # fresh verify block and draft scores of this step (seeded inputs, same on both sides)
+        cpu.q = _rand_bf16(*cpu.q.shape, seed=100 + step)
+        cpu.k_new = _rand_bf16(*cpu.k_new.shape, seed=200 + step)
+        cpu.v_new = _rand_bf16(*cpu.v_new.shape, seed=300 + step)
+        cpu.s_draft = torch.rand(cpu.s_draft.shape, generator=g)
+        dev.q, dev.k_new, dev.v_new, dev.s_draft = cpu.q.cuda(), cpu.k_new.cuda(), cpu.v_new.cuda(), cpu.s_draft.cuda()
+        got = H.run_gpu_fused(dev)
+        a_ref, h_ref = H.oracle_scores(cpu)
+        H.check_scores(got.hist.cpu(), h_ref, f"hist step {step}")
+        idx_same, cnt_same = H.oracle_select(cpu, got.hist.cpu())
+        assert torch.equal(got.idx.cpu(), idx_same) and torch.equal(got.cnt.cpu(), cnt_same)
+        o_ref, _ = H.oracle_attn(cpu, got.idx.cpu(), got.cnt.cpu())
+        H.check_attn(got.out, o_ref)
+        # accept 1..T rows, append on both sides; the GPU history becomes the state of both (rule 2 of DESIGN.md §7)
+        n_app = torch.randint(1, cfg.n_new + 1, (cfg.batch,), generator=g, dtype=torch.int32)
+        dev.hist = got.hist
+        api.append_kv(sh, H.gpu_kv(dev), dev.seq_lens, dev.k_new, dev.v_new, n_app.cuda(), dev.hist)
+        torch.cuda.synchronize()
+        cpu.hist = got.hist.cpu()
+        cpu.seq_lens = ref.append_kv(H.cpu_kv(cpu), cpu.seq_lens, cpu.k_new, cpu.v_new, n_app, cap, cpu.hist)
+        assert torch.equal(dev.seq_lens.cpu(), cpu.seq_lens)
+        assert torch.equal(dev.k.cpu().view(torch.int16), cpu.k.view(torch.int16))
+        assert torch.equal(dev.v.cpu().view(torch.int16), cpu.v.view(torch.int16))
+        assert torch.equal(dev.hist.cpu(), cpu.hist)
+    assert int(cpu.seq_lens[2]) == cap and int(cpu.seq_lens[0]) > cap - 40
