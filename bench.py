@@ -128,8 +128,9 @@ class Workload:
         self.idx = torch.full((L, B, G, self.k_max), -1, dtype=torch.int32, device=device)
         self.cnt = torch.zeros((L, B, G), dtype=torch.int32, device=device)
         self.shape = api.Shape(B, c.n_q_heads, c.n_kv_heads, c.head_dim, T, N, 0.0)
-        self.select = api.Select(c.budget, c.n_sink, c.n_recent, c.m_num, c.m_den, G, None)
-        self.kv = [api.KV.contiguous_nhd(s.k, s.v, None) for s in self.sets]
+        self.select = api.Select(c.budget, c.n_sink, c.n_recent, c.m_num, c.m_den, G, self.sets[0].budgets)
+        self.kv = [api.KV.paged_nhd(s.k, s.v, s.page_table, s.seq_lens) if s.page_table is not None
+                   else api.KV.contiguous_nhd(s.k, s.v, s.seq_lens) for s in self.sets]
         self.ws = api.alloc_workspace(self.shape, c.head_mask, 0)        # sized for the dense baseline too
         self.dense_out = torch.zeros_like(self.out[0])
 
@@ -153,6 +154,16 @@ class Workload:
             self.api.sparse_verify_attn(self.shape, self.kv[s], self.q[l], self.k_new[l], self.v_new[l],
                                         self.idx[0], self.cnt[0], self.out[l], self.ws)
 
+    def step_score_only(self):
+        """a1 alone in every layer (scores_now written to a scratch tensor): the estimation cost of PAPER.md:297."""
+        if not hasattr(self, "scratch_scores"):
+            self.scratch_scores = torch.empty_like(self.hist[0])
+        T, Hq, d = self.cfg.n_new, self.cfg.n_q_heads, self.cfg.head_dim
+        for l in range(self.L):
+            s = l % self.n_sets
+            self.api.score_heads(self.shape, self.kv[s], self.q[l][:, 0], self.cfg.head_mask, self.cfg.n_lists,
+                                 self.scratch_scores, self.ws)
+
     def step_attn_only(self):
         """a4 alone in every layer, each with the index lists its own fused pass left in idx[l] / cnt[l] (kernel-only
         timing of the gathered attention: the region holds nothing but L launches of that kernel)."""
@@ -171,16 +182,23 @@ class Workload:
     # -- algorithmic bytes per layer ------------------------------------------------
     def bytes_per_layer(self) -> dict:
         c = self.cfg
-        B, N, T, G, d, e = c.batch, c.ctx, c.n_new, c.n_lists, c.head_dim, 2
+        B, T, G, d, e = c.batch, c.n_new, c.n_lists, c.head_dim, 2
+        s0 = self.sets[0]
+        # ragged workloads: B * N stands for sum_b N_b and B * k for sum_b min(k_b, N_b)
+        lens = s0.seq_lens.cpu().tolist() if s0.seq_lens is not None else [c.ctx] * B
+        buds = s0.budgets.cpu().tolist() if s0.budgets is not None else [c.budget] * B
+        BN = sum(lens)
+        Bk = sum(min(k, n) for k, n in zip(buds, lens))
+        N, k = BN / B, Bk / B
         groups = len({h // c.group for h in c.heads})
-        k = min(c.budget, N)
-        a1_k = groups * B * N * d * e
-        a1 = a1_k + B * len(c.heads) * d * e + 4 * G * B * N
-        a2 = 3 * 4 * G * B * N
-        a3 = 4 * B * N * (G if self.s_draft.dim() == 4 else 1) + 4 * G * B * N + 4 * G * B * k
-        a4 = 2 * c.n_kv_heads * B * k * d * e + 2 * B * T * c.n_kv_heads * d * e + 2 * B * T * c.n_q_heads * d * e \
-            + 4 * G * B * k
-        a5 = 2 * c.n_kv_heads * B * N * d * e + 2 * B * T * c.n_kv_heads * d * e + 2 * B * T * c.n_q_heads * d * e
+        a1_k = int(groups * BN * d * e)
+        a1 = a1_k + B * len(c.heads) * d * e + 4 * G * BN
+        a2 = 3 * 4 * G * BN
+        a3 = 4 * BN * (G if self.s_draft.dim() == 4 else 1) + 4 * G * BN + 4 * G * Bk
+        a4 = 2 * c.n_kv_heads * Bk * d * e + 2 * B * T * c.n_kv_heads * d * e + 2 * B * T * c.n_q_heads * d * e \
+            + 4 * G * Bk
+        a5 = 2 * c.n_kv_heads * BN * d * e + 2 * B * T * c.n_kv_heads * d * e + 2 * B * T * c.n_q_heads * d * e
+        N, k = int(N), int(k)
         must_read = a1_k + 2 * 4 * G * B * N + a4          # K stream + hist, s_draft reads + a4
         return {"a1": a1, "a1_k": a1_k + B * len(c.heads) * d * e, "a2": a2, "a3": a3, "a4": a4, "a5": a5,
                 "fused_must_read": must_read}
@@ -482,6 +500,56 @@ def measure_workload(api, cfg: synth.Config, n_sets: int, steps: int, warmup: in
     return w, r
 
 
+def run_sweep(api, args, dist: Dist, device):
+    """BASELINE.json configs[3] (context sweep on the Qwen2.5-72B-shaped layer: N in 4k..128k, batch reduced so the
+    cache fits, budget 2048 and 6.25 % of N, gamma 2 / 4 / 8) and configs[4] (paged, ragged, Llama-3-8B-shaped).  Per
+    point, graph-replayed regions that hold one kind of launch each: scoring (a1) and sparse verification (a4)
+    separately, the fused layer (a1..a4) and the dense baseline (a5).  Rank 0 prints ONE JSON line {"sweep": [...]}."""
+    peak, _ = measured_peak()
+    points = []
+    grid = []
+    for ctx, batch in ((4096, 16), (8192, 16), (16384, 16), (32768, 16), (65536, 8), (131072, 4)):
+        for gamma in (2, 4, 8):
+            grid.append(("fixed-2048", ctx, batch, gamma, 2048))
+        grid.append(("6.25%", ctx, batch, 4, ctx // 16))
+    L, n_sets = 8, 4
+    for label, ctx, batch, gamma, budget in grid:
+        cfg = synth.config_qwen72b(batch=batch, ctx=ctx, n_layers=L, gamma=gamma, budget=budget)
+        points.append(sweep_point(api, cfg, n_sets, dist, device, peak,
+                                  {"series": label, "ctx": ctx, "batch": batch, "gamma": gamma, "budget": budget}))
+        torch.cuda.empty_cache()
+    cfg = synth.config_paged(n_layers=4)
+    points.append(sweep_point(api, cfg, 2, dist, device, peak,
+                              {"series": "paged-ragged (configs[4])", "ctx": "U[8192,65536]", "batch": cfg.batch,
+                               "gamma": cfg.gamma, "budget": "6.25% of N_b", "page_size": cfg.page_size}))
+    if dist.rank == 0:
+        print(json.dumps({"sweep": points, "unit": "us per layer (graph-replayed, CUDA events)",
+                          "peak_gbs": peak, "layers_per_point": L}), flush=True)
+
+
+def sweep_point(api, cfg: synth.Config, n_sets: int, dist: Dist, device, peak: float, tag: dict) -> dict:
+    w = Workload(cfg, n_sets, device)
+    w.step_every_layer()
+    w.step_dense()
+    w.step_score_only()
+    by = w.bytes_per_layer()
+    t = {}
+    for name, fn in (("fused", w.step_every_layer), ("score", w.step_score_only), ("attn", w.step_attn_only),
+                     ("dense", w.step_dense)):
+        t[name] = 1e3 * time_steps(graphed(fn), 3, 3, dist, device) / cfg.n_layers
+    out = dict(tag)
+    out.update({
+        "fused_us": round(t["fused"], 2), "score_us": round(t["score"], 2), "sparse_attn_us": round(t["attn"], 2),
+        "dense_us": round(t["dense"], 2), "speedup_vs_dense": round(t["dense"] / t["fused"], 2),
+        "attn_speedup_vs_dense": round(t["dense"] / t["attn"], 2),
+        "score_gbs": round(by["a1_k"] / t["score"] / 1e3, 1), "sparse_attn_gbs": round(by["a4"] / t["attn"] / 1e3, 1),
+        "dense_gbs": round(by["a5"] / t["dense"] / 1e3, 1),
+        "fused_frac_of_peak": round(by["fused_must_read"] / t["fused"] / 1e3 / peak, 3),
+    })
+    del w
+    return out
+
+
 def stage_table(kernels: dict, layers: int) -> dict:
     """us per layer per kernel: avg launch duration x launches per step / layers."""
     return {k: round(us * n / layers, 3) for k, (us, n) in kernels.items()}
@@ -499,6 +567,7 @@ def main():
     ap.add_argument("--sets", type=int, default=20, help="distinct K/V caches the layers cycle over")
     ap.add_argument("--packed", action="store_true", help="headline on the packed/G=1 subset placement")
     ap.add_argument("--no-extras", action="store_true", help="skip the secondary workloads and the CPU baseline")
+    ap.add_argument("--sweep", action="store_true", help="context / gamma / budget sweep (configs[3]) + paged (configs[4])")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     dist = Dist()
@@ -519,6 +588,10 @@ def main():
         dist.barrier()
     api.lib()
 
+    if args.sweep:
+        run_sweep(api, args, dist, device)
+        dist.finish()
+        return
     cfg = rank_seed(headline_config(args), dist.rank)
     w, r = measure_workload(api, cfg, args.sets, args.steps, args.warmup, dist, device, True, True)
     by = w.bytes_per_layer()
