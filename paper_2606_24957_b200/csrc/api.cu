@@ -60,22 +60,30 @@ float scale_log2_of(const dustin_shape_t* s) {
 }
 
 // ---- scoring plan ---------------------------------------------------------------------------------------------
-// Tokens per scoring CTA: as large as possible while the grid still holds >= 8 CTAs per SM (148 SMs).
-void score_plan(int batch, int n_groups, int max_ctx, int* chunk_tokens, int* n_chunks) {
+// Tokens per scoring CTA (all scored KV groups of those tokens): as large as possible while the grid still holds >= 8
+// CTAs per SM (148 SMs), never below 256.  group_slots = how many groups the 8 warps of a CTA serve side by side;
+// n_parts = softmax partials per (sequence, head) = CTAs per sequence x warps per group.
+void score_plan(int batch, int n_groups, int max_ctx, int* chunk_tokens, int* n_parts, int* group_slots) {
+    int slots = 1;
+    while (slots < n_groups && slots < 8) slots <<= 1;
+    // CTAs per sequence = ceil(max_ctx / chunk): the tiles of a sequence are dealt round-robin to them (score.cu), so
+    // chunk only sets the CTA count: as few as keep >= 8 CTAs per SM (148 SMs) in the grid, at least 256 tokens each.
+    // Measured at config 3 (B = 16, 32k): 128 CTAs per sequence 172 us, 64: 185, 27 (one wave): 188.
     int chunk = 2048;
-    auto ctas = [&](int c) { return (long long)batch * n_groups * ((max_ctx + c - 1) / c); };
+    auto ctas = [&](int c) { return (long long)batch * ((max_ctx + c - 1) / c); };
     while (chunk > 256 && ctas(chunk) < 148 * 8) chunk >>= 1;
     *chunk_tokens = chunk;
-    *n_chunks = max_ctx > 0 ? (max_ctx + chunk - 1) / chunk : 1;
+    *group_slots = slots;
+    *n_parts = (max_ctx > 0 ? (max_ctx + chunk - 1) / chunk : 1) * (8 / slots);
 }
 
 struct ScoreWs {
     size_t logits, part, stats, total;
 };
 ScoreWs score_ws(int batch, int nsel, int max_ctx) {
-    // n_chunks upper bound: the smallest chunk (256 tokens)
+    // upper bound of the partial count: the smallest chunk (256 tokens) x 8 warps of one group
     const size_t stride = ((size_t)max_ctx + 3) & ~(size_t)3;
-    const size_t n_chunks = ((size_t)max_ctx + 255) / 256 + 1;
+    const size_t n_chunks = (((size_t)max_ctx + 255) / 256 + 1) * 8;
     ScoreWs w;
     w.logits = 0;
     w.part = align256(w.logits + (size_t)batch * nsel * stride * sizeof(float));
@@ -175,7 +183,7 @@ int run_score(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q,
     p.max_ctx = shape->max_ctx;
     p.n_lists = n_lists;
     p.scale_log2 = scale_log2_of(shape);
-    score_plan(p.batch, p.n_groups, p.max_ctx, &p.chunk_tokens, &p.n_chunks);
+    score_plan(p.batch, p.n_groups, p.max_ctx, &p.chunk_tokens, &p.n_chunks, &p.group_slots);
     p.logit_stride = ((long long)p.max_ctx + 3) & ~3ll;
     char* base = static_cast<char*>(ws) + kWsHeader;   // the persistent header belongs to the attention stage
     p.logits = reinterpret_cast<float*>(base + w.logits);

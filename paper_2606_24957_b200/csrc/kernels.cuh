@@ -14,7 +14,8 @@ struct ScoreParams {
     float scale_log2;        // sm_scale * log2(e): logits live in the log2 domain
     int nsel;                // |subset|; ordinals follow ascending head index, so a KV group's heads are contiguous
     int n_groups;            // KV groups holding >= 1 subset head (the only K rows that are read)
-    int chunk_tokens, n_chunks;
+    int chunk_tokens, n_chunks;     // tokens per scoring CTA; softmax partials per (sequence, head) = CTAs x sub-ranges
+    int group_slots;                // scored KV groups served side by side by the 8 warps of a CTA: 1, 2, 4 or 8
     unsigned char sel_head[64];     // ordinal -> query head
     unsigned char group_id[64];     // scored group slot -> KV head
     unsigned char group_first[64];  // scored group slot -> first ordinal

@@ -47,100 +47,152 @@ __device__ __forceinline__ void load_tile(KFrag<D>& f, const ScoreParams& p, int
     }
 }
 
+// ---- shared-memory staging of the K stream -----------------------------------------------------------------------
+// A warp owns a private ring of kStages tiles (16 tokens x D bf16).  issue_tile requests one tile with fully
+// coalesced 16-byte cp.async (a warp instruction covers whole rows: 2 rows x 256 B at D = 128), zero-filling rows past
+// N; frag_tile reads the mma A fragments back.  Chunk c of row r sits at chunk c ^ ((r & 1) << 2), which keeps the
+// 16-byte fragment reads of the row pairs (g, g + 1) on disjoint banks.  No block-wide barrier anywhere: the ring is
+// ordered by cp.async groups and __syncwarp.
+constexpr int kStages = 2;
+
 template <int D>
-__global__ void __launch_bounds__(kScoreThreads) score_logits_kernel(const ScoreParams p) {
-    const int chunk = blockIdx.x, gi = blockIdx.y, b = blockIdx.z;
+__device__ __forceinline__ void issue_tile(uint32_t stage, const ScoreParams& p, int b, int grp, int n0, int N, int lane) {
+    constexpr int CPR = D / 8;              // 16-byte chunks per row
+    constexpr int RPI = 32 / CPR;           // rows per warp instruction
+    long long my = -1;                      // lanes 0..15: element offset of row n0 + lane (page table resolved once)
+    if (lane < kTileTokens && n0 + lane < N) my = kv_row_offset(p.kv, b, n0 + lane, grp);
+    const int ch = lane % CPR, r0 = lane / CPR;
+#pragma unroll
+    for (int i = 0; i < kTileTokens / RPI; ++i) {
+        const int row = i * RPI + r0;
+        const long long off = __shfl_sync(0xffffffffu, my, row);
+        const __nv_bfloat16* src = off >= 0 ? p.kv.k + off + ch * 8 : p.kv.k;
+        cp_async16(stage + (uint32_t)row * (D * 2) + (uint32_t)((ch ^ ((row & 1) << 2)) << 4), src, off >= 0 ? 16 : 0);
+    }
+}
+
+template <int D>
+__device__ __forceinline__ void frag_tile(KFrag<D>& f, const unsigned char* stage, int lane) {
+    const int g = lane >> 2, c = lane & 3;
+    const unsigned char* lo = stage + g * (D * 2);
+    const unsigned char* hi = lo + 8 * (D * 2);
+    const int sw = (g & 1) << 2;
+#pragma unroll
+    for (int j = 0; j < D / 32; ++j) {
+        f.lo[j] = *reinterpret_cast<const uint4*>(lo + (((4 * j + c) ^ sw) << 4));
+        f.hi[j] = *reinterpret_cast<const uint4*>(hi + (((4 * j + c) ^ sw) << 4));
+    }
+}
+
+// gridDim = (CTAs per sequence, batch).  Warp w serves scored KV group (w % group_slots) and, when fewer than 8 groups
+// are scored, every n_sub-th tile: at any moment the warps of a CTA read the SAME tokens' records, each its own
+// 256-byte piece.  Each warp streams its tiles through a private two-stage cp.async ring (3 CTAs = 24 warps x 8 KB
+// per SM in flight) and feeds mma.sync from shared memory; no block-wide barrier.
+template <int D>
+__global__ void __launch_bounds__(kScoreThreads, 3) score_logits_kernel(const ScoreParams p) {
+    extern __shared__ __align__(128) unsigned char s_ring[];   // [warp][stage][16 tokens][D] bf16
+    const int chunk = blockIdx.x, b = blockIdx.y;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int g = lane >> 2, c = lane & 3;
-    const int grp = p.group_id[gi], first = p.group_first[gi], nh = p.group_cnt[gi];
     const int N = seq_len_of(p.kv.seq_lens, b, p.max_ctx);
+    const int slots = p.group_slots, n_sub = kScoreWarps / slots;
+    const int ws = warp / slots;                       // which tiles of the range
+    // Tiles are dealt round-robin: CTA `chunk` takes the 16-token tiles chunk * n_sub + ws, + gridDim.x * n_sub, ... of the
+    // sequence, so at any moment the CTAs of a sequence read ONE contiguous window of the cache.  Contiguous per-CTA
+    // ranges put the concurrent streams a fixed stride apart, which loads the DRAM channels unevenly (measured: 174 to
+    // 189 us at config 3 depending on that stride).
+    const int chunk_lo = chunk * (kScoreWarps / p.group_slots) * kTileTokens;
+    const int chunk_hi = N;
 
-    // B fragments: head slot n = g of this KV group (zero beyond the subset), dims j*32 + c*8 .. +8.
-    uint4 qf[D / 32];
+    for (int gi = warp % slots; gi < p.n_groups; gi += slots) {
+        const int grp = p.group_id[gi], first = p.group_first[gi], nh = p.group_cnt[gi];
+        // B fragments: head slot n = g of this KV group (zero beyond the subset), dims j*32 + c*8 .. +8.
+        uint4 qf[D / 32];
 #pragma unroll
-    for (int j = 0; j < D / 32; ++j) qf[j] = make_uint4(0, 0, 0, 0);
-    if (g < nh) {
-        const int h = p.sel_head[first + g];
-        const __nv_bfloat16* qrow = p.q + (long long)b * p.q_stride_batch + (long long)h * p.q_stride_head + c * 8;
+        for (int j = 0; j < D / 32; ++j) qf[j] = make_uint4(0, 0, 0, 0);
+        if (g < nh) {
+            const int h = p.sel_head[first + g];
+            const __nv_bfloat16* qrow = p.q + (long long)b * p.q_stride_batch + (long long)h * p.q_stride_head + c * 8;
 #pragma unroll
-        for (int j = 0; j < D / 32; ++j) qf[j] = *reinterpret_cast<const uint4*>(qrow + j * 32);
-    }
-
-    // this thread's logits: heads 2c, 2c+1 of tokens (g, g+8) of each tile
-    float m0 = -INFINITY, m1 = -INFINITY, s0 = 0.f, s1 = 0.f;
-    const int chunk_lo = chunk * p.chunk_tokens;
-    const int chunk_hi = min(chunk_lo + p.chunk_tokens, N);
-    const bool h0 = 2 * c < nh, h1 = 2 * c + 1 < nh;
-    float* l0 = p.logits + ((long long)b * p.nsel + first + 2 * c) * p.logit_stride;
-    float* l1 = l0 + p.logit_stride;
-
-    KFrag<D> cur, nxt;
-    int n0 = chunk_lo + warp * kTileTokens;
-    if (n0 < chunk_hi) load_tile<D>(cur, p, b, grp, n0, N, lane);
-    for (; n0 < chunk_hi; n0 += kScoreWarps * kTileTokens) {
-        const int n1 = n0 + kScoreWarps * kTileTokens;
-        if (n1 < chunk_hi) load_tile<D>(nxt, p, b, grp, n1, N, lane);
-        float acc[4] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll
-        for (int j = 0; j < D / 32; ++j) {
-            mma_bf16_16816(acc, cur.lo[j].x, cur.hi[j].x, cur.lo[j].y, cur.hi[j].y, qf[j].x, qf[j].y);
-            mma_bf16_16816(acc, cur.lo[j].z, cur.hi[j].z, cur.lo[j].w, cur.hi[j].w, qf[j].z, qf[j].w);
+            for (int j = 0; j < D / 32; ++j) qf[j] = *reinterpret_cast<const uint4*>(qrow + j * 32);
         }
-        const int n_lo = n0 + g, n_hi = n0 + g + 8;
-        const bool v_lo = n_lo < N, v_hi = n_hi < N;
-        const float a0 = v_lo ? acc[0] * p.scale_log2 : -INFINITY;   // (token g    , head 2c  )
-        const float a1 = v_lo ? acc[1] * p.scale_log2 : -INFINITY;   // (token g    , head 2c+1)
-        const float a2 = v_hi ? acc[2] * p.scale_log2 : -INFINITY;   // (token g + 8, head 2c  )
-        const float a3 = v_hi ? acc[3] * p.scale_log2 : -INFINITY;   // (token g + 8, head 2c+1)
-        if (h0) {
-            if (v_lo) l0[n_lo] = a0;
-            if (v_hi) l0[n_hi] = a2;
-            const float mn = fmaxf(m0, fmaxf(a0, a2));
-            if (mn > -INFINITY) {
-                s0 = s0 * exp2f(m0 - mn) + exp2f(a0 - mn) + exp2f(a2 - mn);
-                m0 = mn;
+
+        // this thread's logits: heads 2c, 2c+1 of tokens (g, g+8) of each tile
+        float m0 = -INFINITY, m1 = -INFINITY, s0 = 0.f, s1 = 0.f;
+        const bool h0 = 2 * c < nh, h1 = 2 * c + 1 < nh;
+        float* l0 = p.logits + ((long long)b * p.nsel + first + 2 * c) * p.logit_stride;
+        float* l1 = l0 + p.logit_stride;
+
+        // Two tiles are always on their way: tile t + 1 while t is consumed, t + 2 requested as soon as t's fragments are
+        // in registers (its stage is free then).
+        constexpr int kTileBytes = kTileTokens * D * 2;
+        unsigned char* ring = s_ring + warp * (kStages * kTileBytes);
+        const uint32_t ring_u32 = smem_u32(ring);
+        const int step = (int)gridDim.x * n_sub * kTileTokens;
+        int n0 = chunk_lo + ws * kTileTokens;
+        __syncwarp();                                        // the previous group's reads of the ring are done
+        if (n0 < chunk_hi) issue_tile<D>(ring_u32, p, b, grp, n0, N, lane);
+        cp_async_commit();
+        if (n0 + step < chunk_hi) issue_tile<D>(ring_u32 + kTileBytes, p, b, grp, n0 + step, N, lane);
+        cp_async_commit();
+        KFrag<D> cur;
+        for (int t = 0; n0 < chunk_hi; n0 += step, ++t) {
+            cp_async_wait<1>();                              // tile t has landed (tile t + 1 may still be in flight)
+            __syncwarp();
+            frag_tile<D>(cur, ring + (t & 1) * kTileBytes, lane);
+            __syncwarp();                                    // every lane has read stage t & 1: it can be refilled
+            if (n0 + 2 * step < chunk_hi) issue_tile<D>(ring_u32 + (t & 1) * kTileBytes, p, b, grp, n0 + 2 * step, N, lane);
+            cp_async_commit();
+            float acc[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+            for (int j = 0; j < D / 32; ++j) {
+                mma_bf16_16816(acc, cur.lo[j].x, cur.hi[j].x, cur.lo[j].y, cur.hi[j].y, qf[j].x, qf[j].y);
+                mma_bf16_16816(acc, cur.lo[j].z, cur.hi[j].z, cur.lo[j].w, cur.hi[j].w, qf[j].z, qf[j].w);
+            }
+            const int n_lo = n0 + g, n_hi = n0 + g + 8;
+            const bool v_lo = n_lo < N, v_hi = n_hi < N;
+            const float a0 = v_lo ? acc[0] * p.scale_log2 : -INFINITY;   // (token g    , head 2c  )
+            const float a1 = v_lo ? acc[1] * p.scale_log2 : -INFINITY;   // (token g    , head 2c+1)
+            const float a2 = v_hi ? acc[2] * p.scale_log2 : -INFINITY;   // (token g + 8, head 2c  )
+            const float a3 = v_hi ? acc[3] * p.scale_log2 : -INFINITY;   // (token g + 8, head 2c+1)
+            if (h0) {
+                if (v_lo) l0[n_lo] = a0;
+                if (v_hi) l0[n_hi] = a2;
+                const float mn = fmaxf(m0, fmaxf(a0, a2));
+                if (mn > -INFINITY) {
+                    s0 = s0 * exp2f(m0 - mn) + exp2f(a0 - mn) + exp2f(a2 - mn);
+                    m0 = mn;
+                }
+            }
+            if (h1) {
+                if (v_lo) l1[n_lo] = a1;
+                if (v_hi) l1[n_hi] = a3;
+                const float mn = fmaxf(m1, fmaxf(a1, a3));
+                if (mn > -INFINITY) {
+                    s1 = s1 * exp2f(m1 - mn) + exp2f(a1 - mn) + exp2f(a3 - mn);
+                    m1 = mn;
+                }
             }
         }
-        if (h1) {
-            if (v_lo) l1[n_lo] = a1;
-            if (v_hi) l1[n_hi] = a3;
-            const float mn = fmaxf(m1, fmaxf(a1, a3));
-            if (mn > -INFINITY) {
-                s1 = s1 * exp2f(m1 - mn) + exp2f(a1 - mn) + exp2f(a3 - mn);
-                m1 = mn;
-            }
-        }
-        if (n1 < chunk_hi) cur = nxt;
-    }
 
-    // (max, sum) over the 8 lanes that share c, then over the warps (fixed order => deterministic).
+        cp_async_wait<0>();
+        // (max, sum) over the 8 lanes that share c (fixed order => deterministic); one partial per (warp, head)
 #pragma unroll
-    for (int off = 4; off < 32; off <<= 1) {
-        const float om0 = __shfl_xor_sync(0xffffffffu, m0, off), os0 = __shfl_xor_sync(0xffffffffu, s0, off);
-        const float om1 = __shfl_xor_sync(0xffffffffu, m1, off), os1 = __shfl_xor_sync(0xffffffffu, s1, off);
-        const float n0m = fmaxf(m0, om0), n1m = fmaxf(m1, om1);
-        s0 = (n0m > -INFINITY) ? s0 * exp2f(m0 - n0m) + os0 * exp2f(om0 - n0m) : 0.f;
-        s1 = (n1m > -INFINITY) ? s1 * exp2f(m1 - n1m) + os1 * exp2f(om1 - n1m) : 0.f;
-        m0 = n0m;
-        m1 = n1m;
-    }
-    __shared__ float2 wpart[kScoreWarps][8];
-    if (g == 0) {
-        wpart[warp][2 * c] = make_float2(m0, s0);
-        wpart[warp][2 * c + 1] = make_float2(m1, s1);
-    }
-    __syncthreads();
-    if (threadIdx.x < nh) {
-        float m = -INFINITY, s = 0.f;
-        for (int w = 0; w < kScoreWarps; ++w) {
-            const float2 o = wpart[w][threadIdx.x];
-            const float mn = fmaxf(m, o.x);
-            s = (mn > -INFINITY) ? s * exp2f(m - mn) + o.y * exp2f(o.x - mn) : 0.f;
-            m = mn;
+        for (int off = 4; off < 32; off <<= 1) {
+            const float om0 = __shfl_xor_sync(0xffffffffu, m0, off), os0 = __shfl_xor_sync(0xffffffffu, s0, off);
+            const float om1 = __shfl_xor_sync(0xffffffffu, m1, off), os1 = __shfl_xor_sync(0xffffffffu, s1, off);
+            const float n0m = fmaxf(m0, om0), n1m = fmaxf(m1, om1);
+            s0 = (n0m > -INFINITY) ? s0 * exp2f(m0 - n0m) + os0 * exp2f(om0 - n0m) : 0.f;
+            s1 = (n1m > -INFINITY) ? s1 * exp2f(m1 - n1m) + os1 * exp2f(om1 - n1m) : 0.f;
+            m0 = n0m;
+            m1 = n1m;
         }
-        p.part[((long long)b * p.nsel + first + threadIdx.x) * p.n_chunks + chunk] = make_float2(m, s);
+        if (g == 0) {
+            const long long part = (long long)chunk * n_sub + ws;
+            if (h0) p.part[((long long)b * p.nsel + first + 2 * c) * p.n_chunks + part] = make_float2(m0, s0);
+            if (h1) p.part[((long long)b * p.nsel + first + 2 * c + 1) * p.n_chunks + part] = make_float2(m1, s1);
+        }
     }
-
 }
 
 // (M, 1/Z) of every subset head from the per-CTA partials: one CTA per sequence, one warp per head at a time.
@@ -226,13 +278,21 @@ __global__ void __launch_bounds__(256) fuse_kernel(int max_ctx, const int* __res
 
 cudaError_t launch_score(const ScoreParams& p, float* scores_now, float* hist, float alpha, bool logits_only,
                          cudaStream_t stream) {
-    dim3 grid(p.n_chunks, p.n_groups, p.batch);
+    dim3 grid(p.n_chunks / (kScoreWarps / p.group_slots), p.batch);   // n_chunks counts partials: CTAs x sub-ranges
     {
         ProfScope prof(kKernScoreLogits, stream);
+        const int smem = kScoreWarps * kStages * kTileTokens * p.head_dim * 2;
+        static bool attr_done = false;
+        if (!attr_done) {
+            cudaError_t ea = cudaFuncSetAttribute(score_logits_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                  kScoreWarps * kStages * kTileTokens * 128 * 2);
+            if (ea != cudaSuccess) return ea;
+            attr_done = true;
+        }
         if (p.head_dim == 128)
-            score_logits_kernel<128><<<grid, kScoreThreads, 0, stream>>>(p);
+            score_logits_kernel<128><<<grid, kScoreThreads, smem, stream>>>(p);
         else
-            score_logits_kernel<64><<<grid, kScoreThreads, 0, stream>>>(p);
+            score_logits_kernel<64><<<grid, kScoreThreads, smem, stream>>>(p);
     }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess || logits_only) return e;   // logits_only: the consumer (select.cu) normalises its own rows
