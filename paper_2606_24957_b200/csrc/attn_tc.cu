@@ -610,7 +610,6 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
         const float sl2 = p.scale_log2;
         const float4* ref4 = reinterpret_cast<const float4*>(s_ref);
         const float4* fac4 = reinterpret_cast<const float4*>(s_fac);
-        constexpr bool kKeepX = NQ <= 48;
         float lpart[NQ];   // this token lane's share of the running row sums
 #pragma unroll
         for (int i = 0; i < NQ; ++i) lpart[i] = 0.f;
@@ -621,81 +620,39 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
             mbar_wait(bar(kSFull + sb), ((uint32_t)(gj >> 1)) & 1u);
             tc_fence_after();
             if (t == 0 && gj < 20) TS(12 + gj);
+            uint32_t xs[NQ];
+#pragma unroll
+            for (int c = 0; c < NQ / 16; ++c)
+                tmem_ld16(lane_base + kColS + (uint32_t)sb * 128 + (uint32_t)c * 16,
+                          reinterpret_cast<uint32_t(&)[16]>(xs[c * 16]));
+            tmem_wait_ld();
+            tc_fence_before();
+            mbar_arrive(bar(kSEmpty + sb));
+
             // scale into the log2 domain; mask the tail of the piece and, for a new row u, the query rows of
             // verify positions < u (row i belongs to position i / r, so those are the rows i < u * r)
             const int pos = s.pos_lo + cur.ti * kTile + t;
             const int thr = pos >= s.pos_hi ? INT_MAX : (pos > s.cnt ? (pos - s.cnt) * r : 0);
-            // Columns [c0, c0 + 32) (16 for the last batch of NQ = 80) of this lane's S row, scaled and masked.
-            auto load_batch = [&](int c0, float (&v)[32]) {
-                uint32_t raw[32];
-                tmem_ld16(lane_base + kColS + (uint32_t)sb * 128 + (uint32_t)c0, reinterpret_cast<uint32_t(&)[16]>(raw[0]));
-                if (c0 + 16 < NQ)
-                    tmem_ld16(lane_base + kColS + (uint32_t)sb * 128 + (uint32_t)c0 + 16,
-                              reinterpret_cast<uint32_t(&)[16]>(raw[16]));
-                tmem_wait_ld();
-#pragma unroll
-                for (int i = 0; i < 32; ++i)
-                    v[i] = (c0 + i < NQ) ? (c0 + i < thr ? -INFINITY : __uint_as_float(raw[i]) * sl2) : 0.f;
-            };
-            // NQ <= 48: the whole row stays in registers (x) and the S buffer is released at once.  Wider rows are
-            // read from TMEM twice, 32 columns at a time, so that nothing spills; the buffer is released after the
-            // second pass.
-            float x[kKeepX ? NQ : 1];
+            float x[NQ];
             bool over = false;
-            if constexpr (kKeepX) {
-                uint32_t xs[NQ];
 #pragma unroll
-                for (int c = 0; c < NQ / 16; ++c)
-                    tmem_ld16(lane_base + kColS + (uint32_t)sb * 128 + (uint32_t)c * 16,
-                              reinterpret_cast<uint32_t(&)[16]>(xs[c * 16]));
-                tmem_wait_ld();
-                tc_fence_before();
-                mbar_arrive(bar(kSEmpty + sb));
+            for (int i4 = 0; i4 < NQ / 4; ++i4) {
+                const float4 m = ref4[i4];
+                const float mm[4] = {m.x, m.y, m.z, m.w};
 #pragma unroll
-                for (int i4 = 0; i4 < NQ / 4; ++i4) {
-                    const float4 m = ref4[i4];
-                    const float mm[4] = {m.x, m.y, m.z, m.w};
-#pragma unroll
-                    for (int e = 0; e < 4; ++e) {
-                        const int i = i4 * 4 + e;
-                        const float v = i < thr ? -INFINITY : __uint_as_float(xs[i]) * sl2;
-                        x[i] = v;
-                        over |= v - mm[e] > kRefSlack;
-                    }
-                }
-            } else {
-#pragma unroll
-                for (int c0 = 0; c0 < NQ; c0 += 32) {
-                    float v[32];
-                    load_batch(c0, v);
-#pragma unroll
-                    for (int i4 = 0; i4 < 8; ++i4)
-                        if (c0 + i4 * 4 < NQ) {
-                            const float4 m = ref4[c0 / 4 + i4];
-                            over |= v[i4 * 4 + 0] - m.x > kRefSlack;
-                            over |= v[i4 * 4 + 1] - m.y > kRefSlack;
-                            over |= v[i4 * 4 + 2] - m.z > kRefSlack;
-                            over |= v[i4 * 4 + 3] - m.w > kRefSlack;
-                        }
+                for (int e = 0; e < 4; ++e) {
+                    const int i = i4 * 4 + e;
+                    const float v = i < thr ? -INFINITY : __uint_as_float(xs[i]) * sl2;
+                    x[i] = v;
+                    over |= v - mm[e] > kRefSlack;
                 }
             }
             if (wg_any(over)) {
                 // Move the reference exponents to the running row maxima (rare after the first tile).
                 {
                     float red[NQ];
-                    if constexpr (kKeepX) {
 #pragma unroll
-                        for (int i = 0; i < NQ; ++i) red[i] = x[i];
-                    } else {
-#pragma unroll
-                        for (int c0 = 0; c0 < NQ; c0 += 32) {
-                            float v[32];
-                            load_batch(c0, v);
-#pragma unroll
-                            for (int i = 0; i < 32; ++i)
-                                if (c0 + i < NQ) red[c0 + i] = v[i];
-                        }
-                    }
+                    for (int i = 0; i < NQ; ++i) red[i] = x[i];
                     int rb = 0;
                     tr_reduce<true, NQ, 0>(red, lane, rb);
 #pragma unroll
@@ -738,55 +695,18 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
             // P^T: this token's NQ weights, bf16, row-contiguous -> 16-byte stores at [8-row block][token]
             if (gj > 0) mbar_wait(bar(kPvDone), (uint32_t)(gj - 1) & 1u);   // the previous P.V has read the buffer
             unsigned char* prow = smem + C::kOffP + t * 16;
-            // The reference exponents are subtracted in a loop of their own, BEFORE any store of the batch: a shared
-            // load may not move above a shared store, and with one warp per scheduler nothing else hides its latency.
-            if constexpr (kKeepX) {
 #pragma unroll
-                for (int i4 = 0; i4 < NQ / 4; ++i4) {
-                    const float4 m = ref4[i4];
-                    x[i4 * 4 + 0] -= m.x;
-                    x[i4 * 4 + 1] -= m.y;
-                    x[i4 * 4 + 2] -= m.z;
-                    x[i4 * 4 + 3] -= m.w;
+            for (int jb = 0; jb < NQ / 8; ++jb) {
+                const float4 m0 = ref4[jb * 2], m1 = ref4[jb * 2 + 1];
+                const float mm[8] = {m0.x, m0.y, m0.z, m0.w, m1.x, m1.y, m1.z, m1.w};
+                float pr[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    pr[e] = fast_exp2(x[jb * 8 + e] - mm[e]);
+                    lpart[jb * 8 + e] += pr[e];
                 }
-            }
-#pragma unroll
-            for (int c0 = 0; c0 < NQ; c0 += 32) {
-                float v[32];
-                if constexpr (kKeepX) {
-#pragma unroll
-                    for (int i = 0; i < 32; ++i) v[i] = c0 + i < NQ ? x[c0 + i] : 0.f;
-                } else {
-                    load_batch(c0, v);
-#pragma unroll
-                    for (int i4 = 0; i4 < 8; ++i4)
-                        if (c0 + i4 * 4 < NQ) {
-                            const float4 m = ref4[c0 / 4 + i4];
-                            v[i4 * 4 + 0] -= m.x;
-                            v[i4 * 4 + 1] -= m.y;
-                            v[i4 * 4 + 2] -= m.z;
-                            v[i4 * 4 + 3] -= m.w;
-                        }
-                }
-#pragma unroll
-                for (int j8 = 0; j8 < 4; ++j8) {
-                    const int jb = c0 / 8 + j8;
-                    if (jb * 8 < NQ) {
-                        float pr[8];
-#pragma unroll
-                        for (int e = 0; e < 8; ++e) {
-                            pr[e] = fast_exp2(v[j8 * 8 + e]);
-                            lpart[jb * 8 + e] += pr[e];
-                        }
-                        *reinterpret_cast<uint4*>(prow + jb * 2048) =
-                            make_uint4(pack_bf16(pr[0], pr[1]), pack_bf16(pr[2], pr[3]), pack_bf16(pr[4], pr[5]),
-                                       pack_bf16(pr[6], pr[7]));
-                    }
-                }
-            }
-            if constexpr (!kKeepX) {   // second pass over the S buffer done: hand it back to the MMA issuer
-                tc_fence_before();
-                mbar_arrive(bar(kSEmpty + sb));
+                *reinterpret_cast<uint4*>(prow + jb * 2048) = make_uint4(pack_bf16(pr[0], pr[1]), pack_bf16(pr[2], pr[3]),
+                                                                         pack_bf16(pr[4], pr[5]), pack_bf16(pr[6], pr[7]));
             }
             fence_proxy_async();
             mbar_arrive(bar(kPFull));
@@ -802,18 +722,14 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
                 const bool merge = s.pos_lo == 0 && !s.whole;
                 const int nseg = s.cta_last - s.cta_first + 1;
                 const long long slot_id = (long long)blockIdx.x * 2 + s.slot;
-                float v1[kKeepX ? NQ : 1];
+                float v1[NQ];
                 float lse1 = -INFINITY;
                 if (merge) {   // second piece = slot 0 of the next CTA: loads in flight during the reductions below
                     const long long sid1 = (long long)(s.cta_first + 1) * 2;
                     wait_flag(ws.flags + sid1);
-                    if constexpr (kKeepX) {
-                        const float* src1 = ws.part_o + sid1 * NQ * kD + t;
+                    const float* src1 = ws.part_o + sid1 * NQ * kD + t;
 #pragma unroll
-                        for (int i = 0; i < NQ; ++i) v1[i] = __ldcg(src1 + i * kD);
-                    } else {   // wide rows: every thread acquires every piece now and reads them column batch by batch
-                        for (int j = 2; j < nseg; ++j) wait_flag(ws.flags + (long long)(s.cta_first + j) * 2);
-                    }
+                    for (int i = 0; i < NQ; ++i) v1[i] = __ldcg(src1 + i * kD);
                     if (t < rows) lse1 = __ldcg(ws.part_lse + sid1 * NQ + t);
                 }
                 if (t == 0) TS(56);
@@ -848,10 +764,6 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
                         const float invW = W > 0.f ? 1.f / W : 0.f;
                         scale *= e0 * invW;
                         s_wgt[t] = e1 * invW;
-                        if constexpr (!kKeepX) {   // the wide-row merge recomputes every piece's weight from these
-                            s_wgt[NQ + t] = M;
-                            s_wgt[2 * NQ + t] = invW;
-                        }
                         lse_fin = W > 0.f ? M + log2f(W) : -INFINITY;
                         M_row = M;
                         W_row = invW;
@@ -867,116 +779,61 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
                 mbar_wait(bar(kPvDone), (uint32_t)gj & 1u);   // every P.V of the piece has completed
                 tc_fence_after();
                 if (t == 0) TS(55);
-                if constexpr (kKeepX) {
-                    uint32_t o[NQ];
+                uint32_t o[NQ];
 #pragma unroll
-                    for (int c = 0; c < NQ / 16; ++c)
-                        tmem_ld16(lane_base + kColO + (uint32_t)c * 16, reinterpret_cast<uint32_t(&)[16]>(o[c * 16]));
-                    tmem_wait_ld();
-                    tc_fence_before();
+                for (int c = 0; c < NQ / 16; ++c)
+                    tmem_ld16(lane_base + kColO + (uint32_t)c * 16, reinterpret_cast<uint32_t(&)[16]>(o[c * 16]));
+                tmem_wait_ld();
+                tc_fence_before();
+                wg_sync();
+                if (merge && t == 0)   // every thread is past its flag waits: leave the flags zero for the next launch
+                    for (int j = 1; j < nseg; ++j) ws.flags[(long long)(s.cta_first + j) * 2] = 0;
+                if (t == 0) TS(33 + 4 * (cur.seg_no & 3));
+                if (s.pos_lo != 0) {
+                    float* po = ws.part_o + slot_id * NQ * kD + t;   // padded to NQ rows: no predicate
+#pragma unroll
+                    for (int i = 0; i < NQ; ++i) po[i * kD] = __uint_as_float(o[i]) * s_fac[i];
+                    // publish: the barrier orders the warpgroup's stores before thread 0's fence and flag
                     wg_sync();
-                    if (merge && t == 0)   // every thread is past its flag waits: leave the flags zero for the next launch
-                        for (int j = 1; j < nseg; ++j) ws.flags[(long long)(s.cta_first + j) * 2] = 0;
-                    if (t == 0) TS(33 + 4 * (cur.seg_no & 3));
-                    if (s.pos_lo != 0) {
-                        float* po = ws.part_o + slot_id * NQ * kD + t;   // padded to NQ rows: no predicate
-#pragma unroll
-                        for (int i = 0; i < NQ; ++i) po[i * kD] = __uint_as_float(o[i]) * s_fac[i];
-                        // publish: the barrier orders the warpgroup's stores before thread 0's fence and flag
-                        wg_sync();
-                        if (t == 0) {
-                            __threadfence();
-                            st_release(ws.flags + slot_id, 1);
-                        }
-                    } else {
-                        float acc[NQ];
-#pragma unroll
-                        for (int i = 0; i < NQ; ++i) acc[i] = __uint_as_float(o[i]) * s_fac[i];
-                        if (merge) {
-#pragma unroll
-                            for (int i = 0; i < NQ; ++i) acc[i] = fmaf(s_wgt[i], v1[i], acc[i]);
-                            for (int j = 2; j < nseg; ++j) {   // units cut into more than two pieces (very long sequences)
-                                const long long sid = (long long)(s.cta_first + j) * 2;
-                                wg_sync();
-                                if (t < rows) {
-                                    const float lj = __ldcg(ws.part_lse + sid * NQ + t);
-                                    s_wgt[t] = lj == -INFINITY ? 0.f : exp2f(lj - M_row) * W_row;
-                                }
-                                const float* src = ws.part_o + sid * NQ * kD + t;
-#pragma unroll
-                                for (int i = 0; i < NQ; ++i) v1[i] = __ldcg(src + i * kD);
-                                wg_sync();
-#pragma unroll
-                                for (int i = 0; i < NQ; ++i) acc[i] = fmaf(s_wgt[i], v1[i], acc[i]);
-                            }
-                        }
-                        if (t == 0) TS(53);
-                        // bf16 rows staged in the P buffer (idle: every P.V of the piece has completed), then written
-                        // with 16-byte stores: row x / 16, chunk x % 16
-                        __nv_bfloat16* so = reinterpret_cast<__nv_bfloat16*>(smem + C::kOffP);
-#pragma unroll
-                        for (int i = 0; i < NQ; ++i) so[i * kD + t] = __float2bfloat16_rn(acc[i]);
-                        wg_sync();
-                        __nv_bfloat16* ob = p.out + ((long long)s.b * T * Hq + (long long)s.g * r) * kD;
-#pragma unroll 1
-                        for (int x = t; x < rows * 16; x += 128) {
-                            const int rr = x >> 4, cc = x & 15;
-                            *reinterpret_cast<uint4*>(ob + s_rowoff[rr] + cc * 8) =
-                                *reinterpret_cast<const uint4*>(so + rr * kD + cc * 8);
-                        }
+                    if (t == 0) {
+                        __threadfence();
+                        st_release(ws.flags + slot_id, 1);
                     }
                 } else {
-                    // Wide rows (NQ > 48): O^T is read 16 columns (query rows) at a time; nothing is kept across
-                    // batches, so nothing spills.  Merge weights of piece j, row i: exp2(lse_j[i] - M[i]) / W[i].
-                    wg_sync();   // s_fac / s_wgt of the statistics above; every thread is past its flag waits
-                    __nv_bfloat16* so = reinterpret_cast<__nv_bfloat16*>(smem + C::kOffP);
-                    float* po = ws.part_o + slot_id * NQ * kD + t;
-#pragma unroll 1
-                    for (int c0 = 0; c0 < NQ; c0 += 16) {
-                        uint32_t o[16];
-                        tmem_ld16(lane_base + kColO + (uint32_t)c0, o);
-                        tmem_wait_ld();
-                        float acc[16];
+                    float acc[NQ];
 #pragma unroll
-                        for (int e = 0; e < 16; ++e) acc[e] = __uint_as_float(o[e]) * s_fac[c0 + e];
-                        if (s.pos_lo != 0) {
+                    for (int i = 0; i < NQ; ++i) acc[i] = __uint_as_float(o[i]) * s_fac[i];
+                    if (merge) {
 #pragma unroll
-                            for (int e = 0; e < 16; ++e) po[(c0 + e) * kD] = acc[e];
-                        } else {
-                            if (merge)
-                                for (int j = 1; j < nseg; ++j) {
-                                    const long long sid = (long long)(s.cta_first + j) * 2;
-                                    const float* src = ws.part_o + sid * NQ * kD + (long long)c0 * kD + t;
-                                    const float* lsj = ws.part_lse + sid * NQ + c0;
+                        for (int i = 0; i < NQ; ++i) acc[i] = fmaf(s_wgt[i], v1[i], acc[i]);
+                        for (int j = 2; j < nseg; ++j) {   // units cut into more than two pieces (very long sequences)
+                            const long long sid = (long long)(s.cta_first + j) * 2;
+                            wg_sync();
+                            if (t < rows) {
+                                const float lj = __ldcg(ws.part_lse + sid * NQ + t);
+                                s_wgt[t] = lj == -INFINITY ? 0.f : exp2f(lj - M_row) * W_row;
+                            }
+                            const float* src = ws.part_o + sid * NQ * kD + t;
 #pragma unroll
-                                    for (int e = 0; e < 16; ++e) {
-                                        const float lj = c0 + e < rows ? __ldcg(lsj + e) : -INFINITY;
-                                        const float w = lj == -INFINITY ? 0.f
-                                                                        : exp2f(lj - s_wgt[NQ + c0 + e]) * s_wgt[2 * NQ + c0 + e];
-                                        acc[e] = fmaf(w, __ldcg(src + e * kD), acc[e]);
-                                    }
-                                }
+                            for (int i = 0; i < NQ; ++i) v1[i] = __ldcg(src + i * kD);
+                            wg_sync();
 #pragma unroll
-                            for (int e = 0; e < 16; ++e) so[(c0 + e) * kD + t] = __float2bfloat16_rn(acc[e]);
+                            for (int i = 0; i < NQ; ++i) acc[i] = fmaf(s_wgt[i], v1[i], acc[i]);
                         }
                     }
-                    tc_fence_before();
+                    if (t == 0) TS(53);
+                    // bf16 rows staged in the P buffer (idle: every P.V of the piece has completed), then written
+                    // with 16-byte stores: row x / 16, chunk x % 16
+                    __nv_bfloat16* so = reinterpret_cast<__nv_bfloat16*>(smem + C::kOffP);
+#pragma unroll
+                    for (int i = 0; i < NQ; ++i) so[i * kD + t] = __float2bfloat16_rn(acc[i]);
                     wg_sync();
-                    if (merge && t == 0)   // leave the flags zero for the next launch
-                        for (int j = 1; j < nseg; ++j) ws.flags[(long long)(s.cta_first + j) * 2] = 0;
-                    if (s.pos_lo != 0) {
-                        if (t == 0) {   // publish: the barrier above orders the warpgroup's stores before fence and flag
-                            __threadfence();
-                            st_release(ws.flags + slot_id, 1);
-                        }
-                    } else {
-                        __nv_bfloat16* ob = p.out + ((long long)s.b * T * Hq + (long long)s.g * r) * kD;
+                    __nv_bfloat16* ob = p.out + ((long long)s.b * T * Hq + (long long)s.g * r) * kD;
 #pragma unroll 1
-                        for (int x = t; x < rows * 16; x += 128) {
-                            const int rr = x >> 4, cc = x & 15;
-                            *reinterpret_cast<uint4*>(ob + s_rowoff[rr] + cc * 8) =
-                                *reinterpret_cast<const uint4*>(so + rr * kD + cc * 8);
-                        }
+                    for (int x = t; x < rows * 16; x += 128) {
+                        const int rr = x >> 4, cc = x & 15;
+                        *reinterpret_cast<uint4*>(ob + s_rowoff[rr] + cc * 8) =
+                            *reinterpret_cast<const uint4*>(so + rr * kD + cc * 8);
                     }
                 }
                 if (t == 0) TS(34 + 4 * (cur.seg_no & 3));

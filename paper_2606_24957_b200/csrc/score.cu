@@ -195,13 +195,11 @@ __global__ void __launch_bounds__(kScoreThreads, 3) score_logits_kernel(const Sc
     }
 }
 
-// (M, 1/Z) of every subset head from the per-CTA partials: one CTA per sequence, one warp per head at a time.
-__global__ void __launch_bounds__(256) score_stats_kernel(const ScoreParams p) {
-    const int b = blockIdx.x, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    for (int j = warp; j < p.nsel; j += 8) {
-        const float2 st = fold_stats_warp(p.part + ((long long)b * p.nsel + j) * p.n_chunks, p.n_chunks, lane);
-        if (lane == 0) p.stats[(long long)b * p.nsel + j] = st;
-    }
+// (M, 1/Z) of every subset head from the per-CTA partials: one warp per (head, sequence).
+__global__ void __launch_bounds__(32) score_stats_kernel(const ScoreParams p) {
+    const int j = blockIdx.x, b = blockIdx.y, lane = threadIdx.x;
+    const float2 st = fold_stats_warp(p.part + ((long long)b * p.nsel + j) * p.n_chunks, p.n_chunks, lane);
+    if (lane == 0) p.stats[(long long)b * p.nsel + j] = st;
 }
 
 // p = exp2(l - M) / Z, summed over the heads that feed list l; optional Eq. 5 accumulation into hist.
@@ -298,7 +296,7 @@ cudaError_t launch_score(const ScoreParams& p, float* scores_now, float* hist, f
     if (e != cudaSuccess || logits_only) return e;   // logits_only: the consumer (select.cu) normalises its own rows
     {
         ProfScope prof(kKernScoreStats, stream);
-        score_stats_kernel<<<p.batch, 256, 0, stream>>>(p);
+        score_stats_kernel<<<dim3(p.nsel, p.batch), 32, 0, stream>>>(p);
     }
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
