@@ -172,6 +172,12 @@ class Workload:
             self.api.sparse_verify_attn(self.shape, self.kv[s], self.q[l], self.k_new[l], self.v_new[l],
                                         self.idx[l], self.cnt[l], self.out[l], self.ws)
 
+    def step_gather_probe(self):
+        """The memory side of a4 alone: dustin_probe_gather reads the rows step_attn_only gathers, nothing else."""
+        for l in range(self.L):
+            s = l % self.n_sets
+            self.api.probe_gather(self.shape, self.kv[s], self.idx[l], self.cnt[l], self.ws)
+
     def step_dense(self):
         """a5: full-cache verification attention in every layer (the baseline of PAPER.md Fig. 7/10)."""
         for l in range(self.L):
@@ -489,6 +495,9 @@ def measure_workload(api, cfg: synth.Config, n_sets: int, steps: int, warmup: in
     if with_score_once:
         rp = graphed(w.step_attn_only)
         r["attn_only_us_per_launch"] = 1e3 * time_steps(rp, max(3, steps // 2), warmup, dist, device) / cfg.n_layers
+        w.step_gather_probe()
+        rp = graphed(w.step_gather_probe)
+        r["gather_probe_us_per_launch"] = 1e3 * time_steps(rp, max(3, steps // 2), warmup, dist, device) / cfg.n_layers
         rp = graphed(w.step_score_once)
         r["score_once_us_per_layer"] = 1e3 * time_steps(rp, max(3, steps // 2), warmup, dist, device) / cfg.n_layers
     if with_dense:
@@ -636,6 +645,12 @@ def main():
         "roofline_attn": roof("attn_kernel", by["a4"], r["attn_only_us_per_launch"],
                               "CUDA events around graph replays that hold only this kernel (L launches, one per "
                               "layer, each on its own K/V cache and index lists); time / launches"),
+        "gather_probe": {"us_per_launch": round(r["gather_probe_us_per_launch"], 3),
+                         "gbs": round(by["a4"] / r["gather_probe_us_per_launch"] / 1e3, 1),
+                         "attn_time_over_probe": round(r["attn_only_us_per_launch"] / r["gather_probe_us_per_launch"], 3),
+                         "what": "dustin_probe_gather: plain 16-byte loads of exactly the K/V rows a4 gathers (same lists, "
+                                 "same caches, graph-replayed), no arithmetic -- the practical floor of the 256-byte row "
+                                 "gather on this memory system"},
         "fused_path": {"bytes_it_must_read_per_layer": by["fused_must_read"], "achieved_gbs": round(fused_gbs, 1),
                        "frac_of_measured_peak": round(fused_gbs / peak, 4),
                        "frac_of_8000_nominal": round(fused_gbs / 8000.0, 4)},

@@ -171,6 +171,12 @@ int dustin_verify_layer_fused(const dustin_shape_t* shape, const dustin_kv_t* kv
                               float* lse_out, int32_t* idx_out, int32_t* cnt_out, void* ws, size_t ws_bytes,
                               void* stream);
 
+/* Measurement aid (bench.py): reads exactly the K and V rows that dustin_sparse_verify_attn would gather for these index
+ * lists -- plain 16-byte loads, no arithmetic -- and writes nothing of interest: its duration is the practical floor of
+ * the gather on this memory system.  ws: any scratch of >= 4 * batch * n_kv_heads bytes.  Not counted as a launch. */
+int dustin_probe_gather(const dustin_shape_t* shape, const dustin_kv_t* kv, const int32_t* idx, const int32_t* cnt,
+                        int32_t n_lists, int32_t k_max, void* ws, size_t ws_bytes, void* stream);
+
 /* ---- steps either side of the layer path ---------------------------------------------------- */
 
 /* Attention Recovery Rate, Eq. 1: the share of the attention mass of row (b,l) that the index list

@@ -90,6 +90,8 @@ def lib():
         L.dustin_verify_layer_fused.restype = ctypes.c_int
         L.dustin_verify_layer_fused.argtypes = [sp, kp, vp, vp, vp, u64, vp, i64, vp, f32, selp, i32, vp, vp, vp,
                                                 vp, vp, vp, sz, vp]
+        L.dustin_probe_gather.restype = ctypes.c_int
+        L.dustin_probe_gather.argtypes = [sp, kp, vp, vp, i32, i32, vp, sz, vp]
         L.dustin_arr.restype = ctypes.c_int
         L.dustin_arr.argtypes = [i32, i32, i32, vp, vp, vp, vp, i32, vp, vp]
         L.dustin_append_kv.restype = ctypes.c_int
@@ -106,7 +108,7 @@ EXPORTS = ("dustin_version", "dustin_status_string", "dustin_last_cuda_error", "
            "dustin_tune_attn_impl",
            "dustin_launch_count", "dustin_profile_enable", "dustin_profile_collect", "dustin_kernel_name",
            "dustin_workspace_bytes", "dustin_score_heads", "dustin_fuse_scores", "dustin_topk_select",
-           "dustin_sparse_verify_attn", "dustin_verify_layer_fused", "dustin_arr", "dustin_append_kv",
+           "dustin_sparse_verify_attn", "dustin_verify_layer_fused", "dustin_arr", "dustin_append_kv", "dustin_probe_gather",
            "dustin_draft_aggregate")
 
 
@@ -333,3 +335,11 @@ def draft_aggregate(shape: Shape, kv_layers: list, q_layers: list, head_mask: in
     rc = lib().dustin_draft_aggregate(ctypes.byref(shape), kvs, qs, L, ctypes.c_uint64(head_mask),
                                       _dense(s_draft, torch.float32), _ptr(ws), ws.numel(), _stream())
     _check("dustin_draft_aggregate", rc)
+
+
+def probe_gather(shape: Shape, kv: KV, idx: torch.Tensor, cnt: torch.Tensor, ws: torch.Tensor) -> None:
+    """Measurement aid: reads the K / V rows a4 would gather for these lists and nothing else."""
+    kvc = kv.c()
+    rc = lib().dustin_probe_gather(ctypes.byref(shape), ctypes.byref(kvc), _dense(idx, torch.int32),
+                                   _dense(cnt, torch.int32), idx.shape[1], idx.shape[2], _ptr(ws), ws.numel(), _stream())
+    _check("dustin_probe_gather", rc)

@@ -429,6 +429,20 @@ int dustin_verify_layer_fused(const dustin_shape_t* shape, const dustin_kv_t* kv
                     ws, ws_bytes, st);
 }
 
+int dustin_probe_gather(const dustin_shape_t* shape, const dustin_kv_t* kv, const int32_t* idx, const int32_t* cnt,
+                        int32_t n_lists, int32_t k_max, void* ws, size_t ws_bytes, void* stream) {
+    int rc = check_shape(shape);
+    if (rc) return rc;
+    KvView view;
+    rc = check_kv(shape, kv, true, &view);
+    if (rc) return rc;
+    if (!idx || !cnt || k_max <= 0 || (n_lists != 1 && n_lists != shape->n_kv_heads)) return DUSTIN_ERR_INVALID_ARG;
+    if (!ws || ws_bytes < kWsHeader + 4 * (size_t)shape->batch * shape->n_kv_heads) return DUSTIN_ERR_WORKSPACE;
+    const cudaError_t e = launch_gather_probe(view, idx, cnt, shape->batch, shape->n_kv_heads, shape->head_dim, n_lists,
+                                              k_max, static_cast<char*>(ws) + kWsHeader, static_cast<cudaStream_t>(stream));
+    return e == cudaSuccess ? DUSTIN_OK : fail_cuda(e);
+}
+
 int dustin_arr(int32_t batch, int32_t n_lists, int32_t max_ctx, const int32_t* seq_lens, const float* a,
                const int32_t* idx, const int32_t* cnt, int32_t k_max, float* arr_out, void* stream) {
     if (batch <= 0 || n_lists <= 0 || max_ctx < 0 || k_max <= 0 || !a || !idx || !cnt || !arr_out)

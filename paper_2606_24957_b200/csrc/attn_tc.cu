@@ -326,25 +326,8 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
         }
         return c + T;
     };
-    // Producers, whole-unit case (CTA x takes unit x from its first token, decided below): the index entries of tiles
-    // 0 and 1 are requested now, so that their latency overlaps the length loads and the prefix scan.
-    int spec_idx[2] = {-1, -1};
-    if (GATHER && warp >= 4 && warp < 8 && (int)blockIdx.x < n_units) {
-        const int sb = (int)blockIdx.x / Hkv, sl = p.n_lists == 1 ? 0 : (int)blockIdx.x - sb * Hkv;
-        const int* row = p.idx + ((long long)sb * p.n_lists + sl) * p.k_max;
-        const int pos0 = 32 * (warp - 4) + lane;
-        if (pos0 < p.k_max) spec_idx[0] = __ldg(row + pos0);
-        if (pos0 + kTile < p.k_max) spec_idx[1] = __ldg(row + pos0 + kTile);
-    }
-    // barriers and TMEM first: neither depends on the list lengths, whose loads are in flight meanwhile
-    const int per = (n_units + 255) / 256;
-    const int u_lo = min(tid * per, n_units), u_hi = tid < 256 ? min(u_lo + per, n_units) : u_lo;
-    int sum = 0, longest = 0;
-    for (int u = u_lo; u < u_hi; ++u) {
-        const int l = unit_len(u);
-        sum += l;
-        longest = max(longest, l);
-    }
+    // Barriers and TMEM need nothing from global memory: under programmatic dependent launch this part runs while the
+    // previous kernel drains; pdl_wait() returns when that kernel has completed and its writes are visible.
     if (tid == 0) {
         for (int i = 0; i < NS; ++i) {
             mbar_init(bar(kSlotFull + i), 128);
@@ -361,6 +344,25 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
         fence_mbar_init();
     }
     if (warp == 8) tmem_alloc(smem_u32(s_tmem), 512);
+    pdl_wait();
+    // Producers, whole-unit case (CTA x takes unit x from its first token, decided below): the index entries of tiles
+    // 0 and 1 are requested now, so that their latency overlaps the length loads and the prefix scan.
+    int spec_idx[2] = {-1, -1};
+    if (GATHER && warp >= 4 && warp < 8 && (int)blockIdx.x < n_units) {
+        const int sb = (int)blockIdx.x / Hkv, sl = p.n_lists == 1 ? 0 : (int)blockIdx.x - sb * Hkv;
+        const int* row = p.idx + ((long long)sb * p.n_lists + sl) * p.k_max;
+        const int pos0 = 32 * (warp - 4) + lane;
+        if (pos0 < p.k_max) spec_idx[0] = __ldg(row + pos0);
+        if (pos0 + kTile < p.k_max) spec_idx[1] = __ldg(row + pos0 + kTile);
+    }
+    const int per = (n_units + 255) / 256;
+    const int u_lo = min(tid * per, n_units), u_hi = tid < 256 ? min(u_lo + per, n_units) : u_lo;
+    int sum = 0, longest = 0;
+    for (int u = u_lo; u < u_hi; ++u) {
+        const int l = unit_len(u);
+        sum += l;
+        longest = max(longest, l);
+    }
     {
         int inc = sum;
 #pragma unroll
@@ -847,6 +849,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
         }
     }
 
+    pdl_trigger();
     tc_fence_before();
     __syncthreads();
     if (tid == 0) TS(3);
@@ -884,8 +887,7 @@ cudaError_t launch_tc(const AttnParams& p, const TcWs& ws, int grid, cudaStream_
         attr_done = true;
     }
     ProfScope prof(kKernAttn, stream);
-    attn_tc_kernel<NQ, GATHER><<<grid, kTcThreads, smem, stream>>>(p, ws);
-    return cudaGetLastError();
+    return launch_pdl(attn_tc_kernel<NQ, GATHER>, dim3(grid), dim3(kTcThreads), smem, stream, p, ws);
 }
 
 template <int NQ>

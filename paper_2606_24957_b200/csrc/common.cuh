@@ -93,6 +93,15 @@ __device__ __forceinline__ float fast_exp2(float x) {
     return y;
 }
 
+// ---- programmatic dependent launch (PDL) ---------------------------------------------------------------------------
+// The three kernels of a layer are launched with the programmatic-stream-serialization attribute: a kernel may start
+// while its predecessor drains, runs its prologue (barrier init, TMEM allocation, index math on parameters), and calls
+// pdl_wait() BEFORE its first access to global memory -- the wait returns once the predecessor grid has completed and
+// its writes are visible.  pdl_trigger() at the end of a CTA's work lets the successor's CTAs be scheduled as soon
+// as every CTA of this grid has got that far.  Both are no-ops when the kernel was launched the ordinary way.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // ---- softmax bookkeeping of stage a1 (shared by score.cu and the row materialisation inside select.cu; explicit
 // fma / mul intrinsics so that both compile to the same arithmetic, bit for bit) ----------------------------------
 // Merge (om, os) into the running (m, s): maxima and sums of exp2(l - max) in the log2 domain.
@@ -121,6 +130,24 @@ __device__ __forceinline__ void prob_accumulate4(float (&a)[4], const float4 l, 
     a[1] = __fmaf_rn(exp2f(l.y - st.x), st.y, a[1]);
     a[2] = __fmaf_rn(exp2f(l.z - st.x), st.y, a[2]);
     a[3] = __fmaf_rn(exp2f(l.w - st.x), st.y, a[3]);
+}
+
+// Host side: kernel launch with the PDL attribute (DUSTIN_PDL=0 in the environment: ordinary launches).
+bool pdl_enabled();
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream,
+                              Args&&... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = pdl_enabled() ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
 }
 
 }  // namespace dustin

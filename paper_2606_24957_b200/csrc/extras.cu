@@ -89,7 +89,56 @@ __global__ void bump_lens_kernel(int* __restrict__ seq_lens, const int* __restri
     seq_lens[b] = N + a;
 }
 
+// Measurement aid (bench.py): the memory side of stage a4 and nothing else.  Reads exactly the K and V rows the
+// attention kernel gathers for the same index lists -- 16 lanes per 256-byte row, 8 rows in flight per thread, plain
+// 16-byte loads, no shared memory, no arithmetic beyond an XOR -- so its time is the practical floor of the gather on
+// this memory system (random 256-byte rows reach about two thirds of the sequential-read bandwidth).
+constexpr int kProbeThreads = 512, kProbeIlp = 8;
+__global__ void __launch_bounds__(kProbeThreads) gather_probe_kernel(KvView kv, const int* __restrict__ idx,
+                                                                     const int* __restrict__ cnt, int n_kv_heads,
+                                                                     int n_lists, int k_max, int chunks_per_row,
+                                                                     unsigned int* __restrict__ sink) {
+    const int u = blockIdx.x, b = u / n_kv_heads, g = u - b * n_kv_heads, l = n_lists == 1 ? 0 : g;
+    const int* list = idx + ((long long)b * n_lists + l) * k_max;
+    int c = cnt[(long long)b * n_lists + l];
+    c = c < 0 ? 0 : (c > k_max ? k_max : c);
+    const int ch = threadIdx.x % chunks_per_row, r0 = threadIdx.x / chunks_per_row;
+    const int rows_per_round = kProbeThreads / chunks_per_row;
+    uint4 acc = make_uint4(0, 0, 0, 0);
+    for (int base = 0; base < c; base += rows_per_round * kProbeIlp) {
+        int tok[kProbeIlp];
+#pragma unroll
+        for (int i = 0; i < kProbeIlp; ++i) {
+            const int r = base + i * rows_per_round + r0;
+            tok[i] = r < c ? __ldg(list + r) : -1;
+        }
+        uint4 kk[kProbeIlp], vv[kProbeIlp];
+#pragma unroll
+        for (int i = 0; i < kProbeIlp; ++i) {
+            kk[i] = vv[i] = make_uint4(0, 0, 0, 0);
+            if (tok[i] >= 0) {
+                const long long off = kv_row_offset(kv, b, tok[i], g) + ch * 8;
+                kk[i] = ldg_stream16(kv.k + off);
+                vv[i] = ldg_stream16(kv.v + off);
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < kProbeIlp; ++i) {
+            acc.x ^= kk[i].x ^ vv[i].y;
+            acc.y ^= kk[i].z ^ vv[i].w;
+        }
+    }
+    if ((acc.x ^ acc.y) == 0x9e3779b9u) sink[u] = acc.x;   // keeps the loads alive; practically never taken
+}
+
 }  // namespace
+
+cudaError_t launch_gather_probe(const KvView& kv, const int* idx, const int* cnt, int batch, int n_kv_heads, int head_dim,
+                                int n_lists, int k_max, void* sink, cudaStream_t stream) {
+    gather_probe_kernel<<<batch * n_kv_heads, kProbeThreads, 0, stream>>>(kv, idx, cnt, n_kv_heads, n_lists, k_max,
+                                                                         head_dim / 8, static_cast<unsigned int*>(sink));
+    return cudaGetLastError();
+}
 
 cudaError_t launch_arr(int batch, int n_lists, int max_ctx, const int* seq_lens, const float* a, const int* idx,
                        const int* cnt, int k_max, float* arr_out, cudaStream_t stream) {

@@ -102,6 +102,11 @@ cudaError_t launch_append(const KvView& kv, int* seq_lens, const int* n_append, 
                           const __nv_bfloat16* v_new, int batch, int T, int n_kv_heads, int head_dim, int max_ctx,
                           float* hist, int n_lists, cudaStream_t stream);
 
+// Measurement aid: reads the K / V rows that a4 would gather for these lists and does nothing else (sink: >= batch *
+// n_kv_heads words of scratch).
+cudaError_t launch_gather_probe(const KvView& kv, const int* idx, const int* cnt, int batch, int n_kv_heads, int head_dim,
+                                int n_lists, int k_max, void* sink, cudaStream_t stream);
+
 // ---- launch bookkeeping (profile.cu) ----------------------------------------------------------------------------
 enum KernelId {
     kKernScoreLogits = 0, kKernScoreStats, kKernScoreNormalize, kKernFuse, kKernSelect, kKernAttn, kKernAttnCombine,

@@ -4,6 +4,7 @@
 #include "kernels.cuh"
 
 #include <atomic>
+#include <cstdlib>
 #include <mutex>
 #include <vector>
 
@@ -49,6 +50,14 @@ ProfScope::~ProfScope() {
     if (slot_ < 0) return;
     std::lock_guard<std::mutex> lk(g_mu);
     if (slot_ < (long long)g_recs.size()) cudaEventRecord(g_recs[slot_].b, stream_);
+}
+
+bool pdl_enabled() {
+    static const bool on = [] {
+        const char* e = getenv("DUSTIN_PDL");
+        return !(e && e[0] == '0');
+    }();
+    return on;
 }
 
 unsigned long long prof_launch_count() { return g_launches.load(std::memory_order_relaxed); }

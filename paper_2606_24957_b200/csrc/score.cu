@@ -94,6 +94,7 @@ __global__ void __launch_bounds__(kScoreThreads, 3) score_logits_kernel(const Sc
     const int chunk = blockIdx.x, b = blockIdx.y;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int g = lane >> 2, c = lane & 3;
+    pdl_wait();
     const int N = seq_len_of(p.kv.seq_lens, b, p.max_ctx);
     const int slots = p.group_slots, n_sub = kScoreWarps / slots;
     const int ws = warp / slots;                       // which tiles of the range
@@ -193,6 +194,7 @@ __global__ void __launch_bounds__(kScoreThreads, 3) score_logits_kernel(const Sc
             if (h1) p.part[((long long)b * p.nsel + first + 2 * c + 1) * p.n_chunks + part] = make_float2(m1, s1);
         }
     }
+    pdl_trigger();
 }
 
 // (M, 1/Z) of every subset head from the per-CTA partials: one warp per (head, sequence).
@@ -276,6 +278,7 @@ __global__ void __launch_bounds__(256) fuse_kernel(int max_ctx, const int* __res
 
 cudaError_t launch_score(const ScoreParams& p, float* scores_now, float* hist, float alpha, bool logits_only,
                          cudaStream_t stream) {
+    cudaError_t e0 = cudaSuccess;
     dim3 grid(p.n_chunks / (kScoreWarps / p.group_slots), p.batch);   // n_chunks counts partials: CTAs x sub-ranges
     {
         ProfScope prof(kKernScoreLogits, stream);
@@ -288,11 +291,11 @@ cudaError_t launch_score(const ScoreParams& p, float* scores_now, float* hist, f
             attr_done = true;
         }
         if (p.head_dim == 128)
-            score_logits_kernel<128><<<grid, kScoreThreads, smem, stream>>>(p);
+            e0 = launch_pdl(score_logits_kernel<128>, grid, dim3(kScoreThreads), smem, stream, p);
         else
-            score_logits_kernel<64><<<grid, kScoreThreads, smem, stream>>>(p);
+            e0 = launch_pdl(score_logits_kernel<64>, grid, dim3(kScoreThreads), smem, stream, p);
     }
-    cudaError_t e = cudaGetLastError();
+    cudaError_t e = e0 != cudaSuccess ? e0 : cudaGetLastError();
     if (e != cudaSuccess || logits_only) return e;   // logits_only: the consumer (select.cu) normalises its own rows
     {
         ProfScope prof(kKernScoreStats, stream);

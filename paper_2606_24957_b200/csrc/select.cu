@@ -855,6 +855,7 @@ __global__ void __launch_bounds__(kSelThreads) select_kernel(const SelectParams 
     extern __shared__ __align__(16) uint32_t smem_dyn[];
     __shared__ SelShared sh;
     const int l = blockIdx.x, b = blockIdx.y;
+    pdl_wait();
     const int N = seq_len_of(p.seq_lens, b, p.max_ctx);
     const int k = p.budgets ? p.budgets[b] : p.budget;
     int* out = p.idx_out + ((long long)b * p.n_lists + l) * p.k_max;
@@ -929,6 +930,7 @@ __global__ void __launch_bounds__(kSelThreads) select_kernel(const SelectParams 
     }
     for (int i = (int)total + threadIdx.x; i < p.k_max; i += kSelThreads) out[i] = -1;
     if (threadIdx.x == 0) *cnt_out = (int)total;
+    pdl_trigger();
 }
 
 }  // namespace
@@ -972,10 +974,8 @@ cudaError_t launch_select(const SelectParams& p_in, cudaStream_t stream) {
     }
     ProfScope prof(kKernSelect, stream);
     if (vec)
-        select_kernel<true><<<dim3(p.n_lists, p.batch), kSelThreads, smem, stream>>>(p);
-    else
-        select_kernel<false><<<dim3(p.n_lists, p.batch), kSelThreads, smem, stream>>>(p);
-    return cudaGetLastError();
+        return launch_pdl(select_kernel<true>, dim3(p.n_lists, p.batch), dim3(kSelThreads), smem, stream, p);
+    return launch_pdl(select_kernel<false>, dim3(p.n_lists, p.batch), dim3(kSelThreads), smem, stream, p);
 }
 
 }  // namespace dustin
