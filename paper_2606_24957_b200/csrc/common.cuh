@@ -113,9 +113,13 @@ __device__ __forceinline__ void softmax_merge(float& m, float& s, float om, floa
 // (M, 1/Z) of one head from its n_chunks per-CTA partials; one warp, every lane receives the result.
 __device__ __forceinline__ float2 fold_stats_warp(const float2* __restrict__ src, int n_chunks, int lane) {
     float m = -INFINITY, s = 0.f;
-    for (int i = lane; i < n_chunks; i += 32) {
-        const float2 o = __ldcg(src + i);
-        softmax_merge(m, s, o.x, o.y);
+    for (int i0 = lane; i0 < n_chunks; i0 += 32 * 8) {   // eight loads in flight, merged in index order
+        float2 o[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) o[u] = i0 + 32 * u < n_chunks ? __ldcg(src + i0 + 32 * u) : make_float2(-INFINITY, 0.f);
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+            if (i0 + 32 * u < n_chunks) softmax_merge(m, s, o[u].x, o[u].y);
     }
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) {
