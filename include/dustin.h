@@ -204,9 +204,12 @@ int dustin_append_kv(const dustin_shape_t* shape, const dustin_kv_t* kv, int32_t
  *   s_draft[b,n] = sum_{h in head_mask} sum_{l < n_layers} sum_{gamma < T} softmax_n( sm_scale * q_l[b,gamma,h,:] . K_l[b,n,g(h),:] )
  * over the N_b cached tokens (reading A4), one vector per sequence.  `shape` describes the DRAFT model
  * (n_new = the number of lookahead queries per layer).  kv_layers: HOST array of n_layers cache descriptors (only k is
- * read);  q_layers: HOST array of n_layers device pointers, each bf16 [B, T, Hq, d].  Runs the scoring stage (a1) once
- * per (layer, lookahead token) on `stream`.   s_draft: device fp32 [B, max_ctx], written (0 for n >= N_b).
- *   ws: dustin_workspace_bytes(shape, head_mask, 1) bytes. */
+ * read);  q_layers: HOST array of n_layers device pointers, each bf16 [B, T, Hq, d].  One pass over each layer's K
+ * cache with the T lookahead queries side by side when a KV group holds at most 8 (query, head) pairs and ws has
+ * dustin_draft_workspace_bytes(shape, head_mask) bytes; otherwise one pass per (layer, lookahead token), for which
+ * dustin_workspace_bytes(shape, head_mask, 1) bytes suffice.   s_draft: device fp32 [B, max_ctx], written (0 for
+ * n >= N_b). */
+size_t dustin_draft_workspace_bytes(const dustin_shape_t* shape, uint64_t head_mask);
 int dustin_draft_aggregate(const dustin_shape_t* shape, const dustin_kv_t* kv_layers, const void* const* q_layers,
                            int32_t n_layers, uint64_t head_mask, float* s_draft, void* ws, size_t ws_bytes,
                            void* stream);

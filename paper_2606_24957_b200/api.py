@@ -96,6 +96,8 @@ def lib():
         L.dustin_arr.argtypes = [i32, i32, i32, vp, vp, vp, vp, i32, vp, vp]
         L.dustin_append_kv.restype = ctypes.c_int
         L.dustin_append_kv.argtypes = [sp, kp, vp, vp, vp, vp, vp, i32, vp]
+        L.dustin_draft_workspace_bytes.restype = sz
+        L.dustin_draft_workspace_bytes.argtypes = [sp, u64]
         L.dustin_draft_aggregate.restype = ctypes.c_int
         L.dustin_draft_aggregate.argtypes = [sp, kp, ctypes.POINTER(vp), i32, u64, vp, vp, sz, vp]
         _lib = L
@@ -108,7 +110,7 @@ EXPORTS = ("dustin_version", "dustin_status_string", "dustin_last_cuda_error", "
            "dustin_tune_attn_impl",
            "dustin_launch_count", "dustin_profile_enable", "dustin_profile_collect", "dustin_kernel_name",
            "dustin_workspace_bytes", "dustin_score_heads", "dustin_fuse_scores", "dustin_topk_select",
-           "dustin_sparse_verify_attn", "dustin_verify_layer_fused", "dustin_arr", "dustin_append_kv", "dustin_probe_gather",
+           "dustin_sparse_verify_attn", "dustin_verify_layer_fused", "dustin_arr", "dustin_append_kv", "dustin_probe_gather", "dustin_draft_workspace_bytes",
            "dustin_draft_aggregate")
 
 
@@ -343,3 +345,11 @@ def probe_gather(shape: Shape, kv: KV, idx: torch.Tensor, cnt: torch.Tensor, ws:
     rc = lib().dustin_probe_gather(ctypes.byref(shape), ctypes.byref(kvc), _dense(idx, torch.int32),
                                    _dense(cnt, torch.int32), idx.shape[1], idx.shape[2], _ptr(ws), ws.numel(), _stream())
     _check("dustin_probe_gather", rc)
+
+
+def alloc_draft_workspace(shape: Shape, head_mask: int, device="cuda") -> torch.Tensor:
+    """Zero-initialised workspace for draft_aggregate's one-pass-per-layer path."""
+    n = int(lib().dustin_draft_workspace_bytes(ctypes.byref(shape), ctypes.c_uint64(head_mask)))
+    if n == 0:
+        raise ValueError("dustin_draft_workspace_bytes: invalid shape or empty head mask")
+    return torch.zeros(n, dtype=torch.uint8, device=device)

@@ -160,7 +160,11 @@ AttnWs attn_ws(const dustin_shape_t* s, int max_tokens) {
 // the selection kernel, which then does it row by row (SelectParams::Norm).
 int run_score(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q, int64_t q_stride_batch,
               int64_t q_stride_head, uint64_t head_mask, int32_t n_lists, float* scores_now, float* hist,
-              float alpha, void* ws, size_t ws_bytes, cudaStream_t stream, SelectParams::Norm* norm_out = nullptr) {
+              float alpha, void* ws, size_t ws_bytes, cudaStream_t stream, SelectParams::Norm* norm_out = nullptr,
+              int n_queries = 1, int64_t q_stride_query = 0) {
+    // n_queries > 1 (draft-side aggregation, n_lists == 1): every subset head is scored for n_queries query rows
+    // q_stride_query apart in ONE pass over K -- the (query, head) pairs are the "heads" of the kernel, <= 8 per KV group
+    // and <= 64 in all (DUSTIN_ERR_UNSUPPORTED otherwise; the caller then scores one query row per pass).
     int rc = check_shape(shape);
     if (rc) return rc;
     ScoreParams p;
@@ -173,6 +177,29 @@ int run_score(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q,
     if (!scores_now && !hist) return DUSTIN_ERR_INVALID_ARG;
     rc = build_subset(shape, head_mask, n_lists, &p);
     if (rc) return rc;
+    for (int i = 0; i < p.nsel; ++i) p.sel_qoff[i] = (int)(p.sel_head[i] * q_stride_head);
+    if (n_queries > 1) {
+        if (n_lists != 1 || p.nsel * n_queries > 64 || q_stride_query < 0 || (q_stride_query & 7))
+            return DUSTIN_ERR_UNSUPPORTED;
+        ScoreParams v = p;
+        int ord = 0;
+        for (int gi = 0; gi < p.n_groups; ++gi) {
+            if (p.group_cnt[gi] * n_queries > 8) return DUSTIN_ERR_UNSUPPORTED;
+            v.group_first[gi] = (unsigned char)ord;
+            v.group_cnt[gi] = (unsigned char)(p.group_cnt[gi] * n_queries);
+            for (int qi = 0; qi < n_queries; ++qi)
+                for (int j = 0; j < p.group_cnt[gi]; ++j) {
+                    const int base = p.group_first[gi] + j;
+                    v.sel_head[ord] = p.sel_head[base];
+                    v.sel_qoff[ord] = (int)(qi * q_stride_query) + p.sel_qoff[base];
+                    ++ord;
+                }
+        }
+        v.nsel = ord;
+        v.list_first[0] = 0;
+        v.list_cnt[0] = (unsigned char)ord;
+        p = v;
+    }
     const ScoreWs w = score_ws(shape->batch, p.nsel, shape->max_ctx);
     if (!ws || ws_bytes < kWsHeader + w.total || ((uintptr_t)ws & 255)) return DUSTIN_ERR_WORKSPACE;
     p.q = static_cast<const __nv_bfloat16*>(q);
@@ -479,19 +506,37 @@ int dustin_draft_aggregate(const dustin_shape_t* shape, const dustin_kv_t* kv_la
     for (int l = 0; l < n_layers; ++l)
         if (!q_layers[l]) return DUSTIN_ERR_INVALID_ARG;
     const int64_t q_stride_batch = (int64_t)shape->n_new * shape->n_q_heads * shape->head_dim;
+    const int64_t q_stride_query = (int64_t)shape->n_q_heads * shape->head_dim;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    bool first = true;
-    for (int l = 0; l < n_layers; ++l)
+    bool first = true;   // the first term overwrites s_draft (and writes the zeros beyond N_b), the others accumulate
+    for (int l = 0; l < n_layers; ++l) {
+        // One pass over the layer's K cache with all T lookahead queries side by side (the (query, head) pairs ride the
+        // N axis of the MMA) when they fit -- <= 8 pairs per KV group -- and the workspace holds their logits ...
+        rc = run_score(shape, &kv_layers[l], q_layers[l], q_stride_batch, shape->head_dim, head_mask, 1,
+                       first ? s_draft : nullptr, first ? nullptr : s_draft, 1.0f, ws, ws_bytes, st, nullptr,
+                       shape->n_new, q_stride_query);
+        if (rc == DUSTIN_OK) {
+            first = false;
+            continue;
+        }
+        if (rc != DUSTIN_ERR_UNSUPPORTED && rc != DUSTIN_ERR_WORKSPACE) return rc;
+        // ... otherwise one pass per lookahead token (Eq. 5 is a plain sum).
         for (int gam = 0; gam < shape->n_new; ++gam) {
-            const __nv_bfloat16* q = static_cast<const __nv_bfloat16*>(q_layers[l]) +
-                                     (int64_t)gam * shape->n_q_heads * shape->head_dim;
-            // the first term overwrites s_draft (and writes the zeros beyond N_b), the others accumulate (Eq. 5 is a sum)
+            const __nv_bfloat16* q = static_cast<const __nv_bfloat16*>(q_layers[l]) + (int64_t)gam * q_stride_query;
             rc = run_score(shape, &kv_layers[l], q, q_stride_batch, shape->head_dim, head_mask, 1,
                            first ? s_draft : nullptr, first ? nullptr : s_draft, 1.0f, ws, ws_bytes, st);
             if (rc) return rc;
             first = false;
         }
+    }
     return DUSTIN_OK;
+}
+
+size_t dustin_draft_workspace_bytes(const dustin_shape_t* shape, uint64_t head_mask) {
+    if (check_shape(shape) != DUSTIN_OK || head_mask == 0) return 0;
+    int nsel = popcount64(head_mask) * shape->n_new;
+    if (nsel > 64) nsel = popcount64(head_mask);   // the per-token fallback
+    return kWsHeader + score_ws(shape->batch, nsel, shape->max_ctx).total + 256;
 }
 
 }  // extern "C"

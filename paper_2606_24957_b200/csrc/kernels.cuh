@@ -17,6 +17,7 @@ struct ScoreParams {
     int chunk_tokens, n_chunks;     // tokens per scoring CTA; softmax partials per (sequence, head) = CTAs x sub-ranges
     int group_slots;                // scored KV groups served side by side by the 8 warps of a CTA: 1, 2, 4 or 8
     unsigned char sel_head[64];     // ordinal -> query head
+    int sel_qoff[64];               // ordinal -> element offset of its query row inside q + b * q_stride_batch
     unsigned char group_id[64];     // scored group slot -> KV head
     unsigned char group_first[64];  // scored group slot -> first ordinal
     unsigned char group_cnt[64];    // scored group slot -> number of subset heads (<= 8)

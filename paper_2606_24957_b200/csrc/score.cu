@@ -112,8 +112,7 @@ __global__ void __launch_bounds__(kScoreThreads, 3) score_logits_kernel(const Sc
 #pragma unroll
         for (int j = 0; j < D / 32; ++j) qf[j] = make_uint4(0, 0, 0, 0);
         if (g < nh) {
-            const int h = p.sel_head[first + g];
-            const __nv_bfloat16* qrow = p.q + (long long)b * p.q_stride_batch + (long long)h * p.q_stride_head + c * 8;
+            const __nv_bfloat16* qrow = p.q + (long long)b * p.q_stride_batch + p.sel_qoff[first + g] + c * 8;
 #pragma unroll
             for (int j = 0; j < D / 32; ++j) qf[j] = *reinterpret_cast<const uint4*>(qrow + j * 32);
         }

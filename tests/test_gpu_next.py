@@ -102,22 +102,35 @@ def test_append_matches_oracle_bitwise(paged):
 
 
 # ---- dustin_draft_aggregate -------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("one_pass", [True, False])
 @pytest.mark.parametrize("B,N,Hq,Hkv,d,gamma,L,mask", [
     (2, 3000, 14, 2, 64, 4, 3, 0b00101000100010),      # Qwen2.5-0.5B-shaped draft: 14/2 heads, d = 64, 3 layers x 4 heads
     (1, 1024, 8, 8, 128, 2, 2, 0b10000001),
+    (2, 2048, 8, 2, 128, 4, 2, 0b00000111),            # 3 heads of one KV group x 4 queries > 8 pairs: per-token passes
 ])
-def test_draft_aggregate_matches_oracle(B, N, Hq, Hkv, d, gamma, L, mask):
+def test_draft_aggregate_matches_oracle(B, N, Hq, Hkv, d, gamma, L, mask, one_pass):
     ks = [_rand_bf16(B, N, Hkv, d, seed=10 + l) for l in range(L)]
     qs = [_rand_bf16(B, gamma, Hq, d, seed=20 + l) for l in range(L)]
     lens = torch.tensor([N] + [N - 333] * (B - 1), dtype=torch.int32)
     want = ref.draft_aggregate(ks, qs, mask, Hkv, N, N * Hkv * d, Hkv * d, d, seq_lens=lens)
     shape = api.Shape(B, Hq, Hkv, d, gamma, N, 0.0)
-    ws = api.alloc_workspace(shape, mask, 1)
+    # the larger workspace lets every layer be ONE pass over its K cache; the smaller one forces a pass per token
+    ws = api.alloc_draft_workspace(shape, mask) if one_pass else api.alloc_workspace(shape, mask, 1)
     gks = [k.cuda() for k in ks]
     kvs = [api.KV.contiguous_nhd(k, None, lens.cuda()) for k in gks]
     got = torch.full((B, N), float("nan"), device="cuda")
+    n0 = api.launch_count()
     api.draft_aggregate(shape, kvs, [q.cuda() for q in qs], mask, got, ws)
     torch.cuda.synchronize()
+    launches = api.launch_count() - n0
+    r = Hq // Hkv
+    fits = max(bin((mask >> (g * r)) & ((1 << r) - 1)).count("1") for g in range(Hkv)) * gamma <= 8
+    if not fits:
+        assert launches == 3 * L * gamma
+    elif one_pass:
+        assert launches == 3 * L
+    else:                                  # a generous general workspace may also hold the one-pass logits
+        assert launches in (3 * L, 3 * L * gamma)
     H.check_scores(got.cpu().unsqueeze(1), want.unsqueeze(1), "s_draft", DRAFT_RTOL)
     n_terms = bin(mask).count("1") * L * gamma
     assert torch.allclose(got.sum(-1).cpu(), torch.full((B,), float(n_terms)), rtol=1e-4)   # Eq. 5 mass
