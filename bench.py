@@ -559,6 +559,49 @@ def sweep_point(api, cfg: synth.Config, n_sets: int, dist: Dist, device, peak: f
     return out
 
 
+def run_arr(api, args, dist: Dist, device):
+    """Quality read-out on the synthetic saliency-drift workload (shape of PAPER.md Table 3 /
+    Fig. 4, no datasets): lists are selected at drift step l (history = step l-1's scores, draft = noisy step-l scores)
+    with Dustin-T (m = 0), Dustin-H (m = 1/2) and Dustin-D (m = all), and scored by the Attention Recovery Rate (Eq. 1)
+    against the attention of step l+1; the SD-oracle bound (Eq. 3-4, w = 1) is TopK_k of that future attention itself."""
+    cfg0 = synth.config_qwen72b(batch=args.batch, ctx=args.ctx, n_layers=1)
+    out = {"workload": f"Qwen2.5-72B-shaped, B={cfg0.batch}, N={cfg0.ctx}, k={cfg0.budget}, drift 10 % per step", "steps": []}
+    n_steps = 4
+    acc = {}
+    for l in range(n_steps):
+        cur = synth.make_layer(cfg0, l, device)
+        nxt = synth.make_layer(cfg0, l + 1, device, want_hist_draft=False)
+        B, G, N = cfg0.batch, cfg0.n_lists, cfg0.ctx
+        shape = api.Shape(B, cfg0.n_q_heads, cfg0.n_kv_heads, cfg0.head_dim, cfg0.n_new, N, 0.0)
+        ws = api.alloc_workspace(shape, cfg0.head_mask, cur.k_max)
+        truth = torch.empty(B, G, N, device=device)
+        api.score_heads(shape, api.KV.contiguous_nhd(nxt.k, nxt.v, None), nxt.q[:, 0], cfg0.head_mask, G, truth, ws)
+        idx = torch.empty(B, G, cur.k_max, dtype=torch.int32, device=device)
+        cnt = torch.empty(B, G, dtype=torch.int32, device=device)
+        arr = torch.empty(B, G, device=device)
+        outb = torch.empty_like(cur.q)
+        row = {}
+        for name, (num, den) in (("dustin_T (m=0)", (0, 1)), ("dustin_H (m=1/2)", (1, 2)), ("dustin_D (m=all)", (1, 1))):
+            hist = cur.hist.clone()
+            sel = api.Select(cfg0.budget, cfg0.n_sink, cfg0.n_recent, num, den, G, None)
+            api.verify_layer_fused(shape, api.KV.contiguous_nhd(cur.k, cur.v, None), cur.q, cur.k_new, cur.v_new,
+                                   cfg0.head_mask, cur.s_draft, hist, 1.0, sel, outb, idx, cnt, ws)
+            api.arr(truth, idx, cnt, arr)
+            row[name] = float(arr.mean())
+        sel = api.Select(cfg0.budget, 0, 0, 0, 1, G, None)                      # Eq. 3: TopK_k of the future attention
+        api.topk_select(sel, truth, truth, idx, cnt)
+        api.arr(truth, idx, cnt, arr)
+        row["sd_oracle (Eq. 4)"] = float(arr.mean())
+        out["steps"].append({k: round(v, 4) for k, v in row.items()})
+        for k, v in row.items():
+            acc[k] = acc.get(k, 0.0) + v / n_steps
+        del cur, nxt
+        torch.cuda.empty_cache()
+    out["mean_arr"] = {k: round(v, 4) for k, v in acc.items()}
+    if dist.rank == 0:
+        print(json.dumps({"arr_readout": out}), flush=True)
+
+
 def stage_table(kernels: dict, layers: int) -> dict:
     """us per layer per kernel: avg launch duration x launches per step / layers."""
     return {k: round(us * n / layers, 3) for k, (us, n) in kernels.items()}
@@ -576,6 +619,7 @@ def main():
     ap.add_argument("--sets", type=int, default=20, help="distinct K/V caches the layers cycle over")
     ap.add_argument("--packed", action="store_true", help="headline on the packed/G=1 subset placement")
     ap.add_argument("--no-extras", action="store_true", help="skip the secondary workloads and the CPU baseline")
+    ap.add_argument("--arr", action="store_true", help="ARR read-out of the selection policies on the drift workload")
     ap.add_argument("--sweep", action="store_true", help="context / gamma / budget sweep (configs[3]) + paged (configs[4])")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -597,8 +641,8 @@ def main():
         dist.barrier()
     api.lib()
 
-    if args.sweep:
-        run_sweep(api, args, dist, device)
+    if args.sweep or args.arr:
+        (run_sweep if args.sweep else run_arr)(api, args, dist, device)
         dist.finish()
         return
     cfg = rank_seed(headline_config(args), dist.rank)
