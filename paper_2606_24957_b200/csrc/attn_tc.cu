@@ -528,7 +528,6 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
         if (pf.valid) pf.advance();
         Tok t1 = load_tok(pf, spec ? spec_idx[1] : -1);
         if (pf.valid) pf.advance();
-        if (cur.valid) issue_q();
         RowPtr a0 = resolve(t0);
         int gj = 0;
         while (cur.valid) {
@@ -537,6 +536,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
             const RowPtr a1 = resolve(t1);         // tile gj + 1: page-table lookup in flight
             if (cur.ti == 0 && gj > 0) issue_q();  // new segment
             issue_tile(gj, a0);
+            if (gj == 0) issue_q();                // first segment: its K/V rows (the longer trip) go out before Q
             if (ptid == 0 && gj < 4) TS(4 + gj);
             a0 = a1;
             t1 = t2;

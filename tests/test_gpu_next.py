@@ -178,3 +178,21 @@ def test_multi_step_decode_loop_matches_oracle():
         assert torch.equal(dev.v.cpu().view(torch.int16), cpu.v.view(torch.int16))
         assert torch.equal(dev.hist.cpu(), cpu.hist)
     assert int(cpu.seq_lens[2]) == cap and int(cpu.seq_lens[0]) > cap - 40
+
+
+# ---- dustin_probe_gather (measurement aid) ----------------------------------------------------------------------------
+@pytest.mark.parametrize("paged", [False, True])
+def test_probe_gather_runs_on_the_lists_of_a_fused_layer(paged):
+    """The probe only reads (the K / V rows of the given lists): it must accept what the fused call produced, on
+    contiguous and paged caches, and leave every tensor untouched."""
+    cfg = synth.shrink(synth.config_paged(), batch=3, ctx=4096, ragged_min=1500) if paged else \
+        synth.shrink(synth.config_llama8b(batch=2, ctx=4096, n_layers=1), budget=512)
+    dev = synth.make_layer(cfg, 0, "cuda")
+    got = H.run_gpu_fused(dev, want_scores=False)
+    sh = H.shape_of(cfg)
+    ws = api.alloc_workspace(sh, cfg.head_mask, dev.k_max)
+    k0, idx0 = dev.k.clone(), got.idx.clone()
+    api.probe_gather(sh, H.gpu_kv(dev), got.idx, got.cnt, ws)
+    torch.cuda.synchronize()
+    assert torch.equal(dev.k.view(torch.int16), k0.view(torch.int16)) and torch.equal(got.idx, idx0)
+    assert int(ws[:4096].max()) == 0                     # the persistent header of the workspace stays zero
