@@ -113,17 +113,23 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&v)[16
 __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
-// Named barrier over the 128 softmax threads (id 1); the .red.or form returns the OR of `pred` over them.
-__device__ __forceinline__ void wg_sync() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
-__device__ __forceinline__ bool wg_any(bool pred) {
+// Named barriers of the softmax warpgroups: id 1 + wg over the 128 threads of warpgroup wg (the .red.or form returns
+// the OR of `pred` over them), id 3 over all softmax threads (128 * NWG).
+__device__ __forceinline__ void wg_sync(int wg) { asm volatile("bar.sync %0, 128;" ::"r"(1 + wg) : "memory"); }
+template <int NWG>
+__device__ __forceinline__ void sm_sync() {
+    if constexpr (NWG == 1) asm volatile("bar.sync 1, 128;" ::: "memory");
+    else asm volatile("bar.sync 3, 256;" ::: "memory");
+}
+__device__ __forceinline__ bool wg_any(bool pred, int wg) {
     uint32_t r;
     asm volatile(
         "{\n\t.reg .pred p, q;\n\t"
         "setp.ne.b32 q, %1, 0;\n\t"
-        "bar.red.or.pred p, 1, 128, q;\n\t"
+        "bar.red.or.pred p, %2, 128, q;\n\t"
         "selp.u32 %0, 1, 0, p;\n\t}"
         : "=r"(r)
-        : "r"((uint32_t)pred)
+        : "r"((uint32_t)pred), "r"(1 + wg)
         : "memory");
     return r != 0;
 }
@@ -287,8 +293,8 @@ __device__ __forceinline__ unsigned long long gtimer() {
 }
 #define TS(slot) do { if (ws.dbg_ts) ws.dbg_ts[(size_t)blockIdx.x * 64 + (slot)] = gtimer(); } while (0)
 
-template <int NQ, bool GATHER>
-__global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams p, const TcWs ws) {
+template <int NQ, int NWG, bool GATHER>
+__global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kernel(const AttnParams p, const TcWs ws) {
     using C = TcCfg<NQ>;
     constexpr int NS = C::kSlotsN;
     extern __shared__ __align__(1024) unsigned char smem[];   // 128-byte-swizzled operands need 1 KB alignment
@@ -337,9 +343,9 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
             mbar_init(bar(kQFull + i), 128);
             mbar_init(bar(kQEmpty + i), 1);
             mbar_init(bar(kSFull + i), 1);
-            mbar_init(bar(kSEmpty + i), 128);
+            mbar_init(bar(kSEmpty + i), 128 * NWG);
         }
-        mbar_init(bar(kPFull), 128);
+        mbar_init(bar(kPFull), 128 * NWG);
         mbar_init(bar(kPvDone), 1);
         fence_mbar_init();
     }
@@ -429,7 +435,8 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
 
     if (warp >= 4 && warp < 8) {
         // ================= producers ===========================================================================
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 96;");
+        if constexpr (NWG == 1) asm volatile("setmaxnreg.dec.sync.aligned.u32 96;");
+        else asm volatile("setmaxnreg.dec.sync.aligned.u32 88;");
         const int pw = warp - 4, ptid = tid - 128;
         TileCursor pf = cur;   // runs two tiles ahead of `cur`
         struct Tok { int tok, b, g; };
@@ -543,9 +550,10 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
             cur.advance();
             ++gj;
         }
-    } else if (warp >= 8) {
+    } else if (warp >= 8 && warp < 12) {
         // ================= MMA issuer (one thread of warp 8) =====================================================
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
+        if constexpr (NWG == 1) asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
+        else asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
         if (warp == 8 && lane == 0) {
             constexpr uint32_t idesc_s = umma_idesc(kTile, NQ, 0, 0);    // S^T = K . Q^T : both K-major
             constexpr uint32_t idesc_pv = umma_idesc(kTile, NQ, 1, 1);   // O^T = V^T . P^T : both MN-major
@@ -573,10 +581,27 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
             bool have_prev = false, prev_first = false;
             while (cur.valid) {
                 const int k = cur.seg_no, qb = k & 1;
-                if (cur.ti == 0) mbar_wait(bar(kQFull + qb), ((uint32_t)(k >> 1)) & 1u);
                 const int item = 2 * gj, slot = item % NS, sb = gj & 1;
-                mbar_wait(bar(kSlotFull + slot), ((uint32_t)(item / NS)) & 1u);
-                mbar_wait(bar(kSEmpty + sb), (((uint32_t)(gj >> 1)) & 1u) ^ 1u);
+                // Whichever is ready first goes first: S of this tile (its K rows have landed, an S buffer is free) or
+                // P.V of the previous one (its P is written).  With a short ring the V slot that P.V releases is what
+                // the producers are waiting for, so P.V must not queue behind a K tile that is still in flight.
+                bool pv_pending = have_prev;
+                if constexpr (NS > 4) {   // longer ring: S first, always (P.V of the previous tile follows below)
+                    if (cur.ti == 0) mbar_wait(bar(kQFull + qb), ((uint32_t)(k >> 1)) & 1u);
+                    mbar_wait(bar(kSlotFull + slot), ((uint32_t)(item / NS)) & 1u);
+                    mbar_wait(bar(kSEmpty + sb), (((uint32_t)(gj >> 1)) & 1u) ^ 1u);
+                } else
+                for (;;) {
+                    const bool s_ok = (cur.ti != 0 || mbar_try_wait(bar(kQFull + qb), ((uint32_t)(k >> 1)) & 1u)) &&
+                                      mbar_try_wait(bar(kSlotFull + slot), ((uint32_t)(item / NS)) & 1u) &&
+                                      mbar_try_wait(bar(kSEmpty + sb), (((uint32_t)(gj >> 1)) & 1u) ^ 1u);
+                    if (s_ok) break;
+                    if (pv_pending && mbar_try_wait(bar(kPFull), (uint32_t)(gj - 1) & 1u) &&
+                        mbar_try_wait(bar(kSlotFull + (2 * gj - 1) % NS), ((uint32_t)((2 * gj - 1) / NS)) & 1u)) {
+                        issue_pv(gj - 1, prev_first);
+                        pv_pending = false;
+                    }
+                }
                 fence_proxy_async();
                 tc_fence_after();
                 const uint32_t kb = slots + (uint32_t)slot * kSlotBytes;
@@ -595,7 +620,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
                 umma_commit(bar(kSFull + sb));
                 if (gj < 4) TS(8 + gj);
                 if (cur.last_tile()) umma_commit(bar(kQEmpty + qb));
-                if (have_prev) issue_pv(gj - 1, prev_first);
+                if (pv_pending) issue_pv(gj - 1, prev_first);
                 have_prev = true;
                 prev_first = cur.ti == 0;
                 cur.advance();
@@ -606,15 +631,28 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
         __syncwarp();
     } else {
         // ================= softmax warpgroup: thread = token of the tile = TMEM lane ==============================
-        asm volatile("setmaxnreg.inc.sync.aligned.u32 240;");
-        const int t = tid;
-        const uint32_t lane_base = tmem + ((uint32_t)(warp * 32) << 16);
+        // NWG = 2 (T*r > 48): a second softmax warpgroup (warps 12-15) takes the query rows [NW, 2 NW); the two own
+        // the same TMEM lanes (warp % 4) and disjoint columns, rows of s_ref / s_fac / P / partials, and meet only on
+        // the mbarriers (S consumed, P ready: 128 arrivals each) and where a flag is published or cleared.
+        if constexpr (NWG == 1) asm volatile("setmaxnreg.inc.sync.aligned.u32 240;");
+        else asm volatile("setmaxnreg.inc.sync.aligned.u32 192;");
+        constexpr int NW = NQ / NWG;
+        const int wg = (NWG == 2 && warp >= 12) ? 1 : 0;
+        const int c_off = wg * NW, wq = warp & 3;
+        const int t = tid - wg * 384;
+        const int rows_w = min(max(rows - c_off, 0), NW);
+        const uint32_t lane_base = tmem + ((uint32_t)(wq * 32) << 16) + (uint32_t)c_off;
         const float sl2 = p.scale_log2;
-        const float4* ref4 = reinterpret_cast<const float4*>(s_ref);
-        const float4* fac4 = reinterpret_cast<const float4*>(s_fac);
-        float lpart[NQ];   // this token lane's share of the running row sums
+        float* s_ref_w = s_ref + c_off;
+        float* s_fac_w = s_fac + c_off;
+        float* s_wgt_w = s_wgt + c_off;
+        const int* s_rowoff_w = s_rowoff + c_off;
+        float* s_warp_w = s_warp + wg * 4 * NW;          // [4 warps][NW] per warpgroup
+        const float4* ref4 = reinterpret_cast<const float4*>(s_ref_w);
+        const float4* fac4 = reinterpret_cast<const float4*>(s_fac_w);
+        float lpart[NW];   // this token lane's share of the running row sums
 #pragma unroll
-        for (int i = 0; i < NQ; ++i) lpart[i] = 0.f;
+        for (int i = 0; i < NW; ++i) lpart[i] = 0.f;
         int gj = 0;
         while (cur.valid) {
             const Seg& s = cur.s;
@@ -622,9 +660,9 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
             mbar_wait(bar(kSFull + sb), ((uint32_t)(gj >> 1)) & 1u);
             tc_fence_after();
             if (t == 0 && gj < 20) TS(12 + gj);
-            uint32_t xs[NQ];
+            uint32_t xs[NW];
 #pragma unroll
-            for (int c = 0; c < NQ / 16; ++c)
+            for (int c = 0; c < NW / 16; ++c)
                 tmem_ld16(lane_base + kColS + (uint32_t)sb * 128 + (uint32_t)c * 16,
                           reinterpret_cast<uint32_t(&)[16]>(xs[c * 16]));
             tmem_wait_ld();
@@ -634,11 +672,11 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
             // scale into the log2 domain; mask the tail of the piece and, for a new row u, the query rows of
             // verify positions < u (row i belongs to position i / r, so those are the rows i < u * r)
             const int pos = s.pos_lo + cur.ti * kTile + t;
-            const int thr = pos >= s.pos_hi ? INT_MAX : (pos > s.cnt ? (pos - s.cnt) * r : 0);
-            float x[NQ];
+            const int thr = (pos >= s.pos_hi ? INT_MAX : (pos > s.cnt ? (pos - s.cnt) * r : 0)) - c_off;
+            float x[NW];
             bool over = false;
 #pragma unroll
-            for (int i4 = 0; i4 < NQ / 4; ++i4) {
+            for (int i4 = 0; i4 < NW / 4; ++i4) {
                 const float4 m = ref4[i4];
                 const float mm[4] = {m.x, m.y, m.z, m.w};
 #pragma unroll
@@ -649,28 +687,28 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
                     over |= v - mm[e] > kRefSlack;
                 }
             }
-            if (wg_any(over)) {
+            if (wg_any(over, wg)) {
                 // Move the reference exponents to the running row maxima (rare after the first tile).
                 {
-                    float red[NQ];
+                    float red[NW];
 #pragma unroll
-                    for (int i = 0; i < NQ; ++i) red[i] = x[i];
+                    for (int i = 0; i < NW; ++i) red[i] = x[i];
                     int rb = 0;
-                    tr_reduce<true, NQ, 0>(red, lane, rb);
+                    tr_reduce<true, NW, 0>(red, lane, rb);
 #pragma unroll
-                    for (int i = 0; i < TrFinal<NQ, 0>::value; ++i) s_warp[warp * NQ + rb + i] = red[i];
+                    for (int i = 0; i < TrFinal<NW, 0>::value; ++i) s_warp_w[wq * NW + rb + i] = red[i];
                 }
-                wg_sync();
-                if (t < NQ) {
-                    const float m_old = s_ref[t];
-                    const float m_new = fmaxf(fmaxf(m_old, fmaxf(s_warp[t], s_warp[NQ + t])),
-                                              fmaxf(s_warp[2 * NQ + t], s_warp[3 * NQ + t]));
-                    s_fac[t] = exp2f(m_old - m_new);
-                    s_ref[t] = m_new;
+                wg_sync(wg);
+                if (t < NW) {
+                    const float m_old = s_ref_w[t];
+                    const float m_new = fmaxf(fmaxf(m_old, fmaxf(s_warp_w[t], s_warp_w[NW + t])),
+                                              fmaxf(s_warp_w[2 * NW + t], s_warp_w[3 * NW + t]));
+                    s_fac_w[t] = exp2f(m_old - m_new);
+                    s_ref_w[t] = m_new;
                 }
-                wg_sync();
+                wg_sync(wg);
 #pragma unroll
-                for (int i4 = 0; i4 < NQ / 4; ++i4) {
+                for (int i4 = 0; i4 < NW / 4; ++i4) {
                     const float4 f = fac4[i4];
                     lpart[i4 * 4 + 0] *= f.x;
                     lpart[i4 * 4 + 1] *= f.y;
@@ -681,12 +719,12 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
                     mbar_wait(bar(kPvDone), (uint32_t)(gj - 1) & 1u);
                     tc_fence_after();
 #pragma unroll
-                    for (int c = 0; c < NQ / 16; ++c) {
+                    for (int c = 0; c < NW / 16; ++c) {
                         uint32_t o[16];
                         tmem_ld16(lane_base + kColO + (uint32_t)c * 16, o);
                         tmem_wait_ld();
 #pragma unroll
-                        for (int e = 0; e < 16; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * s_fac[c * 16 + e]);
+                        for (int e = 0; e < 16; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * s_fac_w[c * 16 + e]);
                         tmem_st16(lane_base + kColO + (uint32_t)c * 16, o);
                     }
                     tmem_wait_st();
@@ -694,11 +732,11 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
                 }
             }
 
-            // P^T: this token's NQ weights, bf16, row-contiguous -> 16-byte stores at [8-row block][token]
+            // P^T: this token's NW weights, bf16, row-contiguous -> 16-byte stores at [8-row block][token]
             if (gj > 0) mbar_wait(bar(kPvDone), (uint32_t)(gj - 1) & 1u);   // the previous P.V has read the buffer
-            unsigned char* prow = smem + C::kOffP + t * 16;
+            unsigned char* prow = smem + C::kOffP + (c_off / 8) * 2048 + t * 16;
 #pragma unroll
-            for (int jb = 0; jb < NQ / 8; ++jb) {
+            for (int jb = 0; jb < NW / 8; ++jb) {
                 const float4 m0 = ref4[jb * 2], m1 = ref4[jb * 2 + 1];
                 const float mm[8] = {m0.x, m0.y, m0.z, m0.w, m1.x, m1.y, m1.z, m1.w};
                 float pr[8];
@@ -724,125 +762,125 @@ __global__ void __launch_bounds__(kTcThreads, 1) attn_tc_kernel(const AttnParams
                 const bool merge = s.pos_lo == 0 && !s.whole;
                 const int nseg = s.cta_last - s.cta_first + 1;
                 const long long slot_id = (long long)blockIdx.x * 2 + s.slot;
-                float v1[NQ];
+                float v1[NW];
                 float lse1 = -INFINITY;
                 if (merge) {   // second piece = slot 0 of the next CTA: loads in flight during the reductions below
                     const long long sid1 = (long long)(s.cta_first + 1) * 2;
                     wait_flag(ws.flags + sid1);
-                    const float* src1 = ws.part_o + sid1 * NQ * kD + t;
+                    const float* src1 = ws.part_o + sid1 * NQ * kD + c_off * kD + t;
 #pragma unroll
-                    for (int i = 0; i < NQ; ++i) v1[i] = __ldcg(src1 + i * kD);
-                    if (t < rows) lse1 = __ldcg(ws.part_lse + sid1 * NQ + t);
+                    for (int i = 0; i < NW; ++i) v1[i] = __ldcg(src1 + i * kD);
+                    if (t < rows_w) lse1 = __ldcg(ws.part_lse + sid1 * NQ + c_off + t);
                 }
                 if (t == 0) TS(56);
                 {
                     int rb = 0;
-                    tr_reduce<false, NQ, 0>(lpart, lane, rb);
+                    tr_reduce<false, NW, 0>(lpart, lane, rb);
 #pragma unroll
-                    for (int i = 0; i < TrFinal<NQ, 0>::value; ++i) s_warp[warp * NQ + rb + i] = lpart[i];
+                    for (int i = 0; i < TrFinal<NW, 0>::value; ++i) s_warp_w[wq * NW + rb + i] = lpart[i];
 #pragma unroll
-                    for (int i = 0; i < NQ; ++i) lpart[i] = 0.f;
+                    for (int i = 0; i < NW; ++i) lpart[i] = 0.f;
                 }
-                wg_sync();
+                wg_sync(wg);
                 float M_row = 0.f, W_row = 0.f;   // thread t < rows: merged maximum and weight sum of row t
-                if (t < NQ) {
-                    const float l = (s_warp[t] + s_warp[NQ + t]) + (s_warp[2 * NQ + t] + s_warp[3 * NQ + t]);
-                    const float lse_own = l > 0.f ? s_ref[t] + log2f(l) : -INFINITY;
+                if (t < NW) {
+                    const float l = (s_warp_w[t] + s_warp_w[NW + t]) + (s_warp_w[2 * NW + t] + s_warp_w[3 * NW + t]);
+                    const float lse_own = l > 0.f ? s_ref_w[t] + log2f(l) : -INFINITY;
                     float scale = l > 0.f ? 1.f / l : 0.f, lse_fin = lse_own;
-                    if (merge && t < rows) {
+                    if (merge && t < rows_w) {
                         float M = fmaxf(lse_own, lse1);
                         for (int j = 2; j < nseg; ++j) {
                             const long long sid = (long long)(s.cta_first + j) * 2;
                             wait_flag(ws.flags + sid);
-                            M = fmaxf(M, __ldcg(ws.part_lse + sid * NQ + t));
+                            M = fmaxf(M, __ldcg(ws.part_lse + sid * NQ + c_off + t));
                         }
                         const float e0 = lse_own == -INFINITY ? 0.f : exp2f(lse_own - M);
                         const float e1 = lse1 == -INFINITY ? 0.f : exp2f(lse1 - M);
                         float W = e0 + e1;
                         for (int j = 2; j < nseg; ++j) {
-                            const float lj = __ldcg(ws.part_lse + ((long long)(s.cta_first + j) * 2) * NQ + t);
+                            const float lj = __ldcg(ws.part_lse + ((long long)(s.cta_first + j) * 2) * NQ + c_off + t);
                             W += lj == -INFINITY ? 0.f : exp2f(lj - M);
                         }
                         const float invW = W > 0.f ? 1.f / W : 0.f;
                         scale *= e0 * invW;
-                        s_wgt[t] = e1 * invW;
+                        s_wgt_w[t] = e1 * invW;
                         lse_fin = W > 0.f ? M + log2f(W) : -INFINITY;
                         M_row = M;
                         W_row = invW;
                     }
-                    s_fac[t] = scale;
-                    if (t < rows) {
-                        if (s.pos_lo != 0) ws.part_lse[slot_id * NQ + t] = lse_own;
+                    s_fac_w[t] = scale;
+                    if (t < rows_w) {
+                        if (s.pos_lo != 0) ws.part_lse[slot_id * NQ + c_off + t] = lse_own;
                         else if (p.lse_out)
-                            p.lse_out[((long long)s.b * Hq + s.g * r + t % r) * T + t / r] = lse_fin * kLn2;
+                            p.lse_out[((long long)s.b * Hq + s.g * r + (c_off + t) % r) * T + (c_off + t) / r] = lse_fin * kLn2;
                     }
                 }
                 if (t == 0) TS(54);
                 mbar_wait(bar(kPvDone), (uint32_t)gj & 1u);   // every P.V of the piece has completed
                 tc_fence_after();
                 if (t == 0) TS(55);
-                uint32_t o[NQ];
+                uint32_t o[NW];
 #pragma unroll
-                for (int c = 0; c < NQ / 16; ++c)
+                for (int c = 0; c < NW / 16; ++c)
                     tmem_ld16(lane_base + kColO + (uint32_t)c * 16, reinterpret_cast<uint32_t(&)[16]>(o[c * 16]));
                 tmem_wait_ld();
                 tc_fence_before();
-                wg_sync();
-                if (merge && t == 0)   // every thread is past its flag waits: leave the flags zero for the next launch
+                sm_sync<NWG>();
+                if (merge && t == 0 && wg == 0)   // every thread is past its flag waits: leave the flags zero for the next launch
                     for (int j = 1; j < nseg; ++j) ws.flags[(long long)(s.cta_first + j) * 2] = 0;
                 if (t == 0) TS(33 + 4 * (cur.seg_no & 3));
                 if (s.pos_lo != 0) {
-                    float* po = ws.part_o + slot_id * NQ * kD + t;   // padded to NQ rows: no predicate
+                    float* po = ws.part_o + slot_id * NQ * kD + c_off * kD + t;   // padded to NW rows: no predicate
 #pragma unroll
-                    for (int i = 0; i < NQ; ++i) po[i * kD] = __uint_as_float(o[i]) * s_fac[i];
-                    // publish: the barrier orders the warpgroup's stores before thread 0's fence and flag
-                    wg_sync();
-                    if (t == 0) {
+                    for (int i = 0; i < NW; ++i) po[i * kD] = __uint_as_float(o[i]) * s_fac_w[i];
+                    // publish: the barrier orders the stores of both warpgroups before thread 0's fence and flag
+                    sm_sync<NWG>();
+                    if (t == 0 && wg == 0) {
                         __threadfence();
                         st_release(ws.flags + slot_id, 1);
                     }
                 } else {
-                    float acc[NQ];
+                    float acc[NW];
 #pragma unroll
-                    for (int i = 0; i < NQ; ++i) acc[i] = __uint_as_float(o[i]) * s_fac[i];
+                    for (int i = 0; i < NW; ++i) acc[i] = __uint_as_float(o[i]) * s_fac_w[i];
                     if (merge) {
 #pragma unroll
-                        for (int i = 0; i < NQ; ++i) acc[i] = fmaf(s_wgt[i], v1[i], acc[i]);
+                        for (int i = 0; i < NW; ++i) acc[i] = fmaf(s_wgt_w[i], v1[i], acc[i]);
                         for (int j = 2; j < nseg; ++j) {   // units cut into more than two pieces (very long sequences)
                             const long long sid = (long long)(s.cta_first + j) * 2;
-                            wg_sync();
-                            if (t < rows) {
-                                const float lj = __ldcg(ws.part_lse + sid * NQ + t);
-                                s_wgt[t] = lj == -INFINITY ? 0.f : exp2f(lj - M_row) * W_row;
+                            wg_sync(wg);
+                            if (t < rows_w) {
+                                const float lj = __ldcg(ws.part_lse + sid * NQ + c_off + t);
+                                s_wgt_w[t] = lj == -INFINITY ? 0.f : exp2f(lj - M_row) * W_row;
                             }
-                            const float* src = ws.part_o + sid * NQ * kD + t;
+                            const float* src = ws.part_o + sid * NQ * kD + c_off * kD + t;
 #pragma unroll
-                            for (int i = 0; i < NQ; ++i) v1[i] = __ldcg(src + i * kD);
-                            wg_sync();
+                            for (int i = 0; i < NW; ++i) v1[i] = __ldcg(src + i * kD);
+                            wg_sync(wg);
 #pragma unroll
-                            for (int i = 0; i < NQ; ++i) acc[i] = fmaf(s_wgt[i], v1[i], acc[i]);
+                            for (int i = 0; i < NW; ++i) acc[i] = fmaf(s_wgt_w[i], v1[i], acc[i]);
                         }
                     }
                     if (t == 0) TS(53);
                     // bf16 rows staged in the P buffer (idle: every P.V of the piece has completed), then written
                     // with 16-byte stores: row x / 16, chunk x % 16
-                    __nv_bfloat16* so = reinterpret_cast<__nv_bfloat16*>(smem + C::kOffP);
+                    __nv_bfloat16* so = reinterpret_cast<__nv_bfloat16*>(smem + C::kOffP) + c_off * kD;
 #pragma unroll
-                    for (int i = 0; i < NQ; ++i) so[i * kD + t] = __float2bfloat16_rn(acc[i]);
-                    wg_sync();
+                    for (int i = 0; i < NW; ++i) so[i * kD + t] = __float2bfloat16_rn(acc[i]);
+                    wg_sync(wg);
                     __nv_bfloat16* ob = p.out + ((long long)s.b * T * Hq + (long long)s.g * r) * kD;
 #pragma unroll 1
-                    for (int x = t; x < rows * 16; x += 128) {
+                    for (int x = t; x < rows_w * 16; x += 128) {
                         const int rr = x >> 4, cc = x & 15;
-                        *reinterpret_cast<uint4*>(ob + s_rowoff[rr] + cc * 8) =
+                        *reinterpret_cast<uint4*>(ob + s_rowoff_w[rr] + cc * 8) =
                             *reinterpret_cast<const uint4*>(so + rr * kD + cc * 8);
                     }
                 }
                 if (t == 0) TS(34 + 4 * (cur.seg_no & 3));
                 if (t == 0) TS(35 + 4 * (cur.seg_no & 3));
-                wg_sync();
-                if (t < NQ) s_ref[t] = kRefInit;
-                wg_sync();
+                wg_sync(wg);
+                if (t < NW) s_ref_w[t] = kRefInit;
+                wg_sync(wg);
             }
             cur.advance();
             ++gj;
@@ -876,23 +914,23 @@ int sm_count() {
 
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
-template <int NQ, bool GATHER>
+template <int NQ, int NWG, bool GATHER>
 cudaError_t launch_tc(const AttnParams& p, const TcWs& ws, int grid, cudaStream_t stream) {
     using C = TcCfg<NQ>;
     constexpr int smem = C::kSmemBytes;
     static bool attr_done = false;   // per instantiation
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(attn_tc_kernel<NQ, GATHER>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        cudaError_t e = cudaFuncSetAttribute(attn_tc_kernel<NQ, NWG, GATHER>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
     ProfScope prof(kKernAttn, stream);
-    return launch_pdl(attn_tc_kernel<NQ, GATHER>, dim3(grid), dim3(kTcThreads), smem, stream, p, ws);
+    return launch_pdl(attn_tc_kernel<NQ, NWG, GATHER>, dim3(grid), dim3(kTcThreads + 128 * (NWG - 1)), smem, stream, p, ws);
 }
 
-template <int NQ>
+template <int NQ, int NWG = 1>
 cudaError_t launch_tc_nq(const AttnParams& p, const TcWs& ws, int grid, cudaStream_t stream) {
-    return p.idx ? launch_tc<NQ, true>(p, ws, grid, stream) : launch_tc<NQ, false>(p, ws, grid, stream);
+    return p.idx ? launch_tc<NQ, NWG, true>(p, ws, grid, stream) : launch_tc<NQ, NWG, false>(p, ws, grid, stream);
 }
 
 }  // namespace
@@ -906,7 +944,7 @@ bool attn_tc_usable(int batch, int n_kv_heads, int head_dim, int rows, int max_t
 
 size_t attn_tc_ws_bytes(int batch, int n_kv_heads, int rows) {
     static_assert(kMaxGrid * 2 * sizeof(int) <= kWsHeader, "the flags must fit the persistent header");
-    const size_t nq = (size_t)((rows + 15) / 16) * 16;   // partials are padded to the kernel's NQ rows
+    const size_t nq = rows > 48 ? 96 : (size_t)((rows + 15) / 16) * 16;   // partials are padded to the kernel's NQ rows
     return kWsHeader + align256((size_t)kMaxGrid * 2 * nq * kD * sizeof(float)) +
            align256((size_t)kMaxGrid * 2 * nq * sizeof(float)) + (size_t)kMaxGrid * 64 * 8;
 }
@@ -922,7 +960,7 @@ cudaError_t launch_attn_tc(const AttnParams& p_in, void* ws_base, cudaStream_t s
     // (dustin.h); every launch leaves it zero again (the merging piece clears the flags it has consumed).
     ws.flags = reinterpret_cast<int*>(base);
     ws.part_o = reinterpret_cast<float*>(base + kWsHeader);
-    const size_t nq = (size_t)((p.rows + 15) / 16) * 16;
+    const size_t nq = p.rows > 48 ? 96 : (size_t)((p.rows + 15) / 16) * 16;
     ws.part_lse = reinterpret_cast<float*>(base + kWsHeader + align256((size_t)kMaxGrid * 2 * nq * kD * sizeof(float)));
     ws.dbg_ts = (p.dbg & 8) ? reinterpret_cast<unsigned long long*>(reinterpret_cast<char*>(ws.part_lse) + align256((size_t)kMaxGrid * 2 * nq * sizeof(float))) : nullptr;
     const int max_tokens = (p.idx ? (p.k_max < p.max_ctx ? p.k_max : p.max_ctx) : p.max_ctx) + p.n_new;
@@ -933,9 +971,11 @@ cudaError_t launch_attn_tc(const AttnParams& p_in, void* ws_base, cudaStream_t s
         case 1: return launch_tc_nq<16>(p, ws, grid, stream);
         case 2: return launch_tc_nq<32>(p, ws, grid, stream);
         case 3: return launch_tc_nq<48>(p, ws, grid, stream);
-        case 4: return launch_tc_nq<64>(p, ws, grid, stream);
-        case 5: return launch_tc_nq<80>(p, ws, grid, stream);
-        case 6: return launch_tc_nq<96>(p, ws, grid, stream);
+        // more than 48 query rows: padded to 96 = 2 x 48, one softmax warpgroup per half (a single warpgroup needs
+        // 2.3 us per tile for 80 rows and bounds the kernel; two need about half)
+        case 4:
+        case 5:
+        case 6: return launch_tc_nq<96, 2>(p, ws, grid, stream);
         default: return cudaErrorInvalidValue;
     }
 }
