@@ -198,12 +198,13 @@ __device__ __forceinline__ void tr_reduce(float (&v)[NV], int lane, int& row_bas
 // ---- shared-memory plan --------------------------------------------------------------------------------------------
 template <int NQ>
 struct TcCfg {
-    static constexpr int kSlotsN = NQ <= 32 ? 6 : (NQ <= 64 ? 5 : 4);
+    static constexpr int kSlotsN = NQ <= 32 ? 6 : 5;
+    static constexpr int kQBufs = NQ <= 64 ? 2 : 1;      // wide rows: one Q buffer buys the fifth K/V slot
     static constexpr int kQBytes = NQ * kD * 2;          // one Q buffer, [64-dim half][row][128 B] swizzled
     static constexpr int kPBytes = NQ * kTile * 2;       // P^T, [8-row block][token][16 B]
     static constexpr int kOffSlots = 0;
     static constexpr int kOffQ = kOffSlots + kSlotsN * kSlotBytes;
-    static constexpr int kOffP = kOffQ + 2 * kQBytes;
+    static constexpr int kOffP = kOffQ + kQBufs * kQBytes;
     static constexpr int kOffPrefix = kOffP + kPBytes;                    // int [kMaxUnits + 1]
     static constexpr int kOffRef = kOffPrefix + (kMaxUnits + 4) * 4;      // float m_ref[NQ]
     static constexpr int kOffFac = kOffRef + NQ * 4;                      // float fac[NQ]
@@ -514,8 +515,8 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
         if (ptid == 0) TS(40);
         // The T*r query rows of the cursor's segment (zero-padded to NQ) into Q buffer seg_no % 2.
         auto issue_q = [&]() {
-            const int k = cur.seg_no, qb = k & 1;
-            mbar_wait(bar(kQEmpty + qb), (((uint32_t)(k >> 1)) & 1u) ^ 1u);
+            const int k = cur.seg_no, qb = k % C::kQBufs;
+            mbar_wait(bar(kQEmpty + qb), (((uint32_t)(k / C::kQBufs)) & 1u) ^ 1u);
             const uint32_t qdst = sbase + C::kOffQ + (uint32_t)qb * C::kQBytes;
             const __nv_bfloat16* qsrc = p.q + ((long long)cur.s.b * T * Hq + (long long)cur.s.g * r) * kD;
 #pragma unroll 1
@@ -580,19 +581,20 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
             int gj = 0;
             bool have_prev = false, prev_first = false;
             while (cur.valid) {
-                const int k = cur.seg_no, qb = k & 1;
+                const int k = cur.seg_no, qb = k % C::kQBufs;
+                const uint32_t qpar = ((uint32_t)(k / C::kQBufs)) & 1u;
                 const int item = 2 * gj, slot = item % NS, sb = gj & 1;
                 // Whichever is ready first goes first: S of this tile (its K rows have landed, an S buffer is free) or
                 // P.V of the previous one (its P is written).  With a short ring the V slot that P.V releases is what
                 // the producers are waiting for, so P.V must not queue behind a K tile that is still in flight.
                 bool pv_pending = have_prev;
                 if constexpr (NS > 4) {   // longer ring: S first, always (P.V of the previous tile follows below)
-                    if (cur.ti == 0) mbar_wait(bar(kQFull + qb), ((uint32_t)(k >> 1)) & 1u);
+                    if (cur.ti == 0) mbar_wait(bar(kQFull + qb), qpar);
                     mbar_wait(bar(kSlotFull + slot), ((uint32_t)(item / NS)) & 1u);
                     mbar_wait(bar(kSEmpty + sb), (((uint32_t)(gj >> 1)) & 1u) ^ 1u);
                 } else
                 for (;;) {
-                    const bool s_ok = (cur.ti != 0 || mbar_try_wait(bar(kQFull + qb), ((uint32_t)(k >> 1)) & 1u)) &&
+                    const bool s_ok = (cur.ti != 0 || mbar_try_wait(bar(kQFull + qb), qpar)) &&
                                       mbar_try_wait(bar(kSlotFull + slot), ((uint32_t)(item / NS)) & 1u) &&
                                       mbar_try_wait(bar(kSEmpty + sb), (((uint32_t)(gj >> 1)) & 1u) ^ 1u);
                     if (s_ok) break;
