@@ -584,26 +584,12 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
                 const int k = cur.seg_no, qb = k % C::kQBufs;
                 const uint32_t qpar = ((uint32_t)(k / C::kQBufs)) & 1u;
                 const int item = 2 * gj, slot = item % NS, sb = gj & 1;
-                // Whichever is ready first goes first: S of this tile (its K rows have landed, an S buffer is free) or
-                // P.V of the previous one (its P is written).  With a short ring the V slot that P.V releases is what
-                // the producers are waiting for, so P.V must not queue behind a K tile that is still in flight.
-                bool pv_pending = have_prev;
-                if constexpr (NS > 4) {   // longer ring: S first, always (P.V of the previous tile follows below)
-                    if (cur.ti == 0) mbar_wait(bar(kQFull + qb), qpar);
-                    mbar_wait(bar(kSlotFull + slot), ((uint32_t)(item / NS)) & 1u);
-                    mbar_wait(bar(kSEmpty + sb), (((uint32_t)(gj >> 1)) & 1u) ^ 1u);
-                } else
-                for (;;) {
-                    const bool s_ok = (cur.ti != 0 || mbar_try_wait(bar(kQFull + qb), qpar)) &&
-                                      mbar_try_wait(bar(kSlotFull + slot), ((uint32_t)(item / NS)) & 1u) &&
-                                      mbar_try_wait(bar(kSEmpty + sb), (((uint32_t)(gj >> 1)) & 1u) ^ 1u);
-                    if (s_ok) break;
-                    if (pv_pending && mbar_try_wait(bar(kPFull), (uint32_t)(gj - 1) & 1u) &&
-                        mbar_try_wait(bar(kSlotFull + (2 * gj - 1) % NS), ((uint32_t)((2 * gj - 1) / NS)) & 1u)) {
-                        issue_pv(gj - 1, prev_first);
-                        pv_pending = false;
-                    }
-                }
+                // S of this tile first, then P.V of the previous one.  (Issuing whichever is ready first was measured on
+                // the 4- and 5-slot rings: it only helps when the ring is too short to hold two tiles besides the one
+                // in use, which no variant is any more.)
+                if (cur.ti == 0) mbar_wait(bar(kQFull + qb), qpar);
+                mbar_wait(bar(kSlotFull + slot), ((uint32_t)(item / NS)) & 1u);
+                mbar_wait(bar(kSEmpty + sb), (((uint32_t)(gj >> 1)) & 1u) ^ 1u);
                 fence_proxy_async();
                 tc_fence_after();
                 const uint32_t kb = slots + (uint32_t)slot * kSlotBytes;
@@ -622,7 +608,7 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
                 umma_commit(bar(kSFull + sb));
                 if (gj < 4) TS(8 + gj);
                 if (cur.last_tile()) umma_commit(bar(kQEmpty + qb));
-                if (pv_pending) issue_pv(gj - 1, prev_first);
+                if (have_prev) issue_pv(gj - 1, prev_first);
                 have_prev = true;
                 prev_first = cur.ti == 0;
                 cur.advance();
