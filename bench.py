@@ -460,7 +460,8 @@ def run_reference(args, dist: Dist):
 
 
 def headline_config(args) -> synth.Config:
-    cfg = synth.config_qwen72b(batch=args.batch, ctx=args.ctx, n_layers=args.layers, spread=not args.packed)
+    cfg = synth.config_qwen72b(batch=args.batch, ctx=args.ctx, n_layers=args.layers, spread=not args.packed,
+                               gamma=getattr(args, "gamma", 4))
     return cfg
 
 
@@ -617,6 +618,7 @@ def main():
     ap.add_argument("--batch", type=int, default=16)
     ap.add_argument("--ctx", type=int, default=32768)
     ap.add_argument("--layers", type=int, default=80)
+    ap.add_argument("--gamma", type=int, default=4, help="draft depth (T = gamma + 1 verify positions)")
     ap.add_argument("--sets", type=int, default=20, help="distinct K/V caches the layers cycle over")
     ap.add_argument("--packed", action="store_true", help="headline on the packed/G=1 subset placement")
     ap.add_argument("--no-extras", action="store_true", help="skip the secondary workloads and the CPU baseline")
