@@ -35,7 +35,8 @@ constexpr int kD = 128;               // head_dim served by this kernel
 constexpr int kSlotBytes = kTile * kD * 2;   // 32 KB: one K or V tile
 constexpr int kMaxUnits = 1024;       // prefix array in shared memory
 constexpr float kRefSlack = 16.f;     // log2 units a score may exceed m_ref before the reference is moved
-constexpr float kRefInit = -1.0e30f;
+constexpr float kRefInit = 0.f;        // reference exponent at the start of a piece (the first tile always moves it)
+constexpr float kRefFloor = -1.0e30f;  // lowest reference (rows that have seen nothing but masked tokens)
 constexpr long long kInvalidRow = LLONG_MIN;
 constexpr int kMergeFast = 4;          // pieces of one unit merged with all loads in flight (more: sequential path)
 
@@ -208,7 +209,8 @@ struct TcCfg {
     static constexpr int kOffPrefix = kOffP + kPBytes;                    // int [kMaxUnits + 1]
     static constexpr int kOffRef = kOffPrefix + (kMaxUnits + 4) * 4;      // float m_ref[NQ]
     static constexpr int kOffFac = kOffRef + NQ * 4;                      // float fac[NQ]
-    static constexpr int kOffWarp = kOffFac + NQ * 4;                     // float [4][NQ]: per-warp maxima / sums
+    static constexpr int kOffDlt = kOffFac + NQ * 4;                      // float dlt[NQ]: m_old - m_new of a reference move
+    static constexpr int kOffWarp = kOffDlt + NQ * 4;                     // float [4][NQ]: per-warp maxima / sums
     static constexpr int kOffWgt = kOffWarp + 4 * NQ * 4;                 // float [kMergeFast][NQ]: merge weights
     static constexpr int kOffRowTab = (kOffWgt + kMergeFast * NQ * 4 + 15) & ~15;   // {K row, V row} addresses, 4 x 32
     static constexpr int kOffRowOff = kOffRowTab + 128 * 16;              // int row -> element offset inside out[b]
@@ -304,6 +306,7 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
     int* s_prefix = reinterpret_cast<int*>(smem + C::kOffPrefix);
     float* s_ref = reinterpret_cast<float*>(smem + C::kOffRef);
     float* s_fac = reinterpret_cast<float*>(smem + C::kOffFac);
+    float* s_dlt = reinterpret_cast<float*>(smem + C::kOffDlt);
     float* s_warp = reinterpret_cast<float*>(smem + C::kOffWarp);
     float* s_wgt = reinterpret_cast<float*>(smem + C::kOffWgt);
     int* s_rowoff = reinterpret_cast<int*>(smem + C::kOffRowOff);
@@ -633,6 +636,7 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
         const float sl2 = p.scale_log2;
         float* s_ref_w = s_ref + c_off;
         float* s_fac_w = s_fac + c_off;
+        float* s_dlt_w = s_dlt + c_off;
         float* s_wgt_w = s_wgt + c_off;
         const int* s_rowoff_w = s_rowoff + c_off;
         float* s_warp_w = s_warp + wg * 4 * NW;          // [4 warps][NW] per warpgroup
@@ -661,20 +665,33 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
             // verify positions < u (row i belongs to position i / r, so those are the rows i < u * r)
             const int pos = s.pos_lo + cur.ti * kTile + t;
             const int thr = (pos >= s.pos_hi ? INT_MAX : (pos > s.cnt ? (pos - s.cnt) * r : 0)) - c_off;
+            // x[i] = d_i = s_i * scale - m_ref[i] (one FFMA), the exponent that P needs; the masks cost nothing in the
+            // tiles that have none (cache rows inside the piece: every tile but the last one or two).
             float x[NW];
-            bool over = false;
+            bool over = cur.ti == 0;   // the first tile of a piece always moves the reference to its row maxima
+            if (__all_sync(0xffffffffu, thr <= 0)) {
 #pragma unroll
-            for (int i4 = 0; i4 < NW / 4; ++i4) {
-                const float4 m = ref4[i4];
-                const float mm[4] = {m.x, m.y, m.z, m.w};
+                for (int i4 = 0; i4 < NW / 4; ++i4) {
+                    const float4 m = ref4[i4];
+                    x[i4 * 4 + 0] = fmaf(__uint_as_float(xs[i4 * 4 + 0]), sl2, -m.x);
+                    x[i4 * 4 + 1] = fmaf(__uint_as_float(xs[i4 * 4 + 1]), sl2, -m.y);
+                    x[i4 * 4 + 2] = fmaf(__uint_as_float(xs[i4 * 4 + 2]), sl2, -m.z);
+                    x[i4 * 4 + 3] = fmaf(__uint_as_float(xs[i4 * 4 + 3]), sl2, -m.w);
+                }
+            } else {
 #pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                    const int i = i4 * 4 + e;
-                    const float v = i < thr ? -INFINITY : __uint_as_float(xs[i]) * sl2;
-                    x[i] = v;
-                    over |= v - mm[e] > kRefSlack;
+                for (int i4 = 0; i4 < NW / 4; ++i4) {
+                    const float4 m = ref4[i4];
+                    const float mm[4] = {m.x, m.y, m.z, m.w};
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        const int i = i4 * 4 + e;
+                        x[i] = i < thr ? -INFINITY : fmaf(__uint_as_float(xs[i]), sl2, -mm[e]);
+                    }
                 }
             }
+#pragma unroll
+            for (int i = 0; i < NW; ++i) over |= x[i] > kRefSlack;
             if (wg_any(over, wg)) {
                 // Move the reference exponents to the running row maxima (rare after the first tile).
                 {
@@ -689,12 +706,26 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
                 wg_sync(wg);
                 if (t < NW) {
                     const float m_old = s_ref_w[t];
-                    const float m_new = fmaxf(fmaxf(m_old, fmaxf(s_warp_w[t], s_warp_w[NW + t])),
-                                              fmaxf(s_warp_w[2 * NW + t], s_warp_w[3 * NW + t]));
-                    s_fac_w[t] = exp2f(m_old - m_new);
+                    const float dmax = fmaxf(fmaxf(s_warp_w[t], s_warp_w[NW + t]), fmaxf(s_warp_w[2 * NW + t], s_warp_w[3 * NW + t]));
+                    // first tile: the reference becomes the row maximum itself (nothing has been accumulated yet, so no
+                    // factor); later: it only ever rises
+                    const float m_new = cur.ti == 0 ? fmaxf(m_old + dmax, kRefFloor) : m_old + fmaxf(dmax, 0.f);
+                    s_dlt_w[t] = m_old - m_new;
+                    s_fac_w[t] = cur.ti == 0 ? 1.f : exp2f(m_old - m_new);
                     s_ref_w[t] = m_new;
                 }
                 wg_sync(wg);
+                {
+                    const float4* dlt4 = reinterpret_cast<const float4*>(s_dlt_w);
+#pragma unroll
+                    for (int i4 = 0; i4 < NW / 4; ++i4) {
+                        const float4 d = dlt4[i4];
+                        x[i4 * 4 + 0] += d.x;
+                        x[i4 * 4 + 1] += d.y;
+                        x[i4 * 4 + 2] += d.z;
+                        x[i4 * 4 + 3] += d.w;
+                    }
+                }
 #pragma unroll
                 for (int i4 = 0; i4 < NW / 4; ++i4) {
                     const float4 f = fac4[i4];
@@ -725,12 +756,10 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
             unsigned char* prow = smem + C::kOffP + (c_off / 8) * 2048 + t * 16;
 #pragma unroll
             for (int jb = 0; jb < NW / 8; ++jb) {
-                const float4 m0 = ref4[jb * 2], m1 = ref4[jb * 2 + 1];
-                const float mm[8] = {m0.x, m0.y, m0.z, m0.w, m1.x, m1.y, m1.z, m1.w};
                 float pr[8];
 #pragma unroll
                 for (int e = 0; e < 8; ++e) {
-                    pr[e] = fast_exp2(x[jb * 8 + e] - mm[e]);
+                    pr[e] = fast_exp2(x[jb * 8 + e]);
                     lpart[jb * 8 + e] += pr[e];
                 }
                 *reinterpret_cast<uint4*>(prow + jb * 2048) = make_uint4(pack_bf16(pr[0], pr[1]), pack_bf16(pr[2], pr[3]),
