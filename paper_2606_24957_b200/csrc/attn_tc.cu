@@ -690,8 +690,13 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
                     }
                 }
             }
+            {
+                float mx = x[0];   // three-input maxima: half the instructions of one compare per score
 #pragma unroll
-            for (int i = 0; i < NW; ++i) over |= x[i] > kRefSlack;
+                for (int i = 1; i + 1 < NW; i += 2) mx = fmaxf(mx, fmaxf(x[i], x[i + 1]));
+                mx = fmaxf(mx, x[NW - 1]);
+                over |= mx > kRefSlack;
+            }
             if (wg_any(over, wg)) {
                 // Move the reference exponents to the running row maxima (rare after the first tile).
                 {
