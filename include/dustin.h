@@ -8,7 +8,7 @@
  *   a5 the same call with idx == NULL is the full-cache verification baseline
  *   a6 dustin_verify_layer_fused a1..a4 enqueued on one stream, no host sync
  * and the steps either side of it: dustin_arr (Eq. 1-4), dustin_append_kv,
- * dustin_draft_aggregate (Eq. 5, first line).
+ * dustin_draft_aggregate (Eq. 5, first line).  Measurement / tuning / testing aids live in dustin_debug.h.
  *
  * Conventions (all entry points):
  *  - Every pointer marked "device" is a CUDA device pointer owned by the caller; the library never allocates,
@@ -19,6 +19,9 @@
  *  - bf16 tensors are raw 16-bit patterns; the last (head_dim) dimension is contiguous; 16-byte aligned rows.
  *  - Outputs are fully overwritten; `hist_inout` is the only in/out state.  Identical inputs give
  *    bit-identical outputs (no order-dependent floating-point atomics anywhere).
+ *  - Thread safety: the entry points keep no mutable state of their own (per-device launch attributes are set once
+ *    under std::call_once-style guards; the library reads no environment variable); calls on different streams and
+ *    workspaces may come from different host threads.  Any device of the process may be current.
  *  - Limits: head_dim in {64,128}; n_q_heads <= 64 (the head subset is a 64-bit mask); n_new (T) <= 16;
  *    T * (n_q_heads / n_kv_heads) <= 96 query rows per KV head; at most 8 subset heads per KV group;
  *    max_ctx <= 2^20.  Outside them the call returns DUSTIN_ERR_UNSUPPORTED.
@@ -90,7 +93,14 @@ int         dustin_last_cuda_error(void);            /* cudaError_t of the last 
  * attention kernel): they must be ZERO before the first call that uses the buffer and must not
  * be written by the caller afterwards; every call that returns DUSTIN_OK and runs to completion leaves them zero
  * again, so one memset at allocation time serves any number of calls (and CUDA-graph replays).  The rest of the
- * buffer is plain scratch with no state.  One workspace must not be used by two calls that run concurrently. */
+ * buffer is plain scratch with no state.  One workspace must not be used by two calls that run concurrently.
+ * After a failure (a call returned DUSTIN_ERR_CUDA, or a kernel of this library was aborted: device fault, reset,
+ * cudaDeviceReset) the header may hold flags of the aborted launch: zero it again (cudaMemsetAsync of
+ * DUSTIN_WS_HEADER_BYTES on the same stream) before reusing the buffer.
+ * Forward progress of the attention kernel when one (sequence, KV head) is cut across several CTAs (long or ragged
+ * units): the CTA that merges a unit waits for partial results of CTAs with LOWER block indices only, which the
+ * hardware dispatches no later than the waiting CTA, so the kernel needs no co-residency of its whole grid (it is safe
+ * under MPS partitions, green contexts and concurrent kernels on other streams). */
 #define DUSTIN_WS_HEADER_BYTES 4096
 
 /* Scratch (bytes of device memory, 256-byte aligned by the caller) that is enough for every entry point on this
@@ -98,27 +108,6 @@ int         dustin_last_cuda_error(void);            /* cudaError_t of the last 
  * attention stage over at most `k_max` selected rows per list (k_max <= 0 => max_ctx rows, the dense case).
  * One buffer of this size serves dustin_verify_layer_fused.  Returns 0 on invalid arguments. */
 size_t dustin_workspace_bytes(const dustin_shape_t* shape, uint64_t head_mask, int32_t k_max);
-
-/* Tuning aid (process-wide, not thread-safe, affects performance only): cache rows per attention CTA;
- * 0 restores the built-in heuristic.  Query dustin_workspace_bytes again after changing it. */
-void dustin_tune_attn_split_tokens(int32_t split_tokens);
-
-/* Tuning / testing aid (process-wide, not thread-safe): which attention kernel serves a4/a5.  0 = automatic (the
- * tcgen05 kernel for head_dim 128 and batch * n_kv_heads <= 1024, else the mma.sync cluster kernel), 1 = always the
- * mma.sync cluster kernel, 2 = same as 0.  Results of the two agree within the a4 tolerance, not bitwise.  Query
- * dustin_workspace_bytes again after changing it. */
-void dustin_tune_attn_impl(int32_t impl);
-
-/* Measurement aids (bench.py).  dustin_launch_count: kernels launched by this library in this process so far.
- * dustin_profile_enable(1) starts bracketing every kernel launch with a CUDA event pair on the launching stream
- * (and drops earlier records); dustin_profile_enable(0) stops.  dustin_profile_collect is the one call that
- * synchronises: it waits for the recorded events and writes, per kernel id in [0, DUSTIN_N_KERNELS), the summed
- * device time in ms and the number of launches (host arrays), then clears the records.  Process-wide. */
-#define DUSTIN_N_KERNELS 9
-uint64_t    dustin_launch_count(void);
-void        dustin_profile_enable(int32_t on);
-int         dustin_profile_collect(double* ms_out, int64_t* launches_out);
-const char* dustin_kernel_name(int32_t kernel_id);   /* NULL outside [0, DUSTIN_N_KERNELS) */
 
 /* a1 -- head-subset scoring (PAPER.md:159 "target attention tensor of the last generated token", :218, :391).
  * For every head h with bit h of head_mask set:  p_h[n] = softmax_n( sm_scale * q[b,h,:] . K[b,n,g(h),:] ) over
@@ -170,12 +159,6 @@ int dustin_verify_layer_fused(const dustin_shape_t* shape, const dustin_kv_t* kv
                               const dustin_select_t* select, int32_t k_max, float* scores_now_out, void* out,
                               float* lse_out, int32_t* idx_out, int32_t* cnt_out, void* ws, size_t ws_bytes,
                               void* stream);
-
-/* Measurement aid (bench.py): reads exactly the K and V rows that dustin_sparse_verify_attn would gather for these index
- * lists -- plain 16-byte loads, no arithmetic -- and writes nothing of interest: its duration is the practical floor of
- * the gather on this memory system.  ws: any scratch of >= 4 * batch * n_kv_heads bytes.  Not counted as a launch. */
-int dustin_probe_gather(const dustin_shape_t* shape, const dustin_kv_t* kv, const int32_t* idx, const int32_t* cnt,
-                        int32_t n_lists, int32_t k_max, void* ws, size_t ws_bytes, void* stream);
 
 /* ---- steps either side of the layer path ---------------------------------------------------- */
 

@@ -69,6 +69,14 @@ def lib():
         L.dustin_tune_attn_split_tokens.argtypes = [i32]
         L.dustin_tune_attn_impl.restype = None
         L.dustin_tune_attn_impl.argtypes = [i32]
+        L.dustin_tune_set.restype = None
+        L.dustin_tune_set.argtypes = [i32, i32]
+        L.dustin_tune_get.restype = i32
+        L.dustin_tune_get.argtypes = [i32]
+        L.dustin_debug_trace_buffer.restype = None
+        L.dustin_debug_trace_buffer.argtypes = [vp, sz]
+        L.dustin_debug_occupy.restype = ctypes.c_int
+        L.dustin_debug_occupy.argtypes = [i32, i32, i32, i32, vp]
         L.dustin_launch_count.restype = ctypes.c_uint64
         L.dustin_launch_count.argtypes = []
         L.dustin_profile_enable.restype = None
@@ -104,14 +112,20 @@ def lib():
     return _lib
 
 
-N_KERNELS = 9
+N_KERNELS = 10
 
-EXPORTS = ("dustin_version", "dustin_status_string", "dustin_last_cuda_error", "dustin_tune_attn_split_tokens",
-           "dustin_tune_attn_impl",
-           "dustin_launch_count", "dustin_profile_enable", "dustin_profile_collect", "dustin_kernel_name",
+# include/dustin.h (the product surface) ...
+EXPORTS = ("dustin_version", "dustin_status_string", "dustin_last_cuda_error",
            "dustin_workspace_bytes", "dustin_score_heads", "dustin_fuse_scores", "dustin_topk_select",
-           "dustin_sparse_verify_attn", "dustin_verify_layer_fused", "dustin_arr", "dustin_append_kv", "dustin_probe_gather", "dustin_draft_workspace_bytes",
-           "dustin_draft_aggregate")
+           "dustin_sparse_verify_attn", "dustin_verify_layer_fused", "dustin_arr", "dustin_append_kv",
+           "dustin_draft_workspace_bytes", "dustin_draft_aggregate")
+# ... and include/dustin_debug.h (measurement / tuning / testing aids)
+DEBUG_EXPORTS = ("dustin_tune_attn_split_tokens", "dustin_tune_attn_impl", "dustin_tune_set", "dustin_tune_get",
+                 "dustin_debug_trace_buffer", "dustin_launch_count", "dustin_profile_enable", "dustin_profile_collect",
+                 "dustin_kernel_name", "dustin_probe_gather", "dustin_debug_occupy")
+
+# enum dustin_knob (dustin_debug.h)
+KNOB_PDL, KNOB_FUSED_ROWS, KNOB_ATTN_TRACE, KNOB_SELECT_SPLIT, KNOB_DRAFT_HOIST, KNOB_ATTN_PREFETCH, KNOB_SELECT_TRACE = range(7)
 
 
 @dataclass
@@ -203,6 +217,29 @@ def tune_attn_split_tokens(split_tokens: int) -> None:
 def tune_attn_impl(impl: int) -> None:
     """0 = automatic, 1 = mma.sync cluster kernel, 2 = tcgen05 kernel where usable (dustin_tune_attn_impl)."""
     lib().dustin_tune_attn_impl(int(impl))
+
+
+def tune_set(knob: int, value: int) -> None:
+    """dustin_tune_set (dustin_debug.h): process-wide A/B switch."""
+    lib().dustin_tune_set(int(knob), int(value))
+
+
+def tune_get(knob: int) -> int:
+    return int(lib().dustin_tune_get(int(knob)))
+
+
+def debug_trace_buffer(buf: Optional[torch.Tensor]) -> None:
+    """Attach (or, with None, detach) the device buffer that receives the DUSTIN_KNOB_SELECT_TRACE timestamps."""
+    if buf is None:
+        lib().dustin_debug_trace_buffer(None, 0)
+    else:
+        lib().dustin_debug_trace_buffer(_ptr(buf), buf.numel() * buf.element_size())
+
+
+def debug_occupy(n_ctas: int, threads: int, smem_bytes: int, microseconds: int, stream=None) -> None:
+    """dustin_debug_occupy: CTAs that hold SM resources for a while (occupancy experiments)."""
+    st = ctypes.c_void_p((stream or torch.cuda.current_stream()).cuda_stream)
+    _check("dustin_debug_occupy", lib().dustin_debug_occupy(n_ctas, threads, smem_bytes, microseconds, st))
 
 
 def launch_count() -> int:

@@ -30,7 +30,7 @@ def _nvcc() -> str:
 
 
 def _deps_mtime() -> float:
-    files = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(INCLUDE, "dustin.h"), __file__]
+    files = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(INCLUDE, "dustin.h"), os.path.join(INCLUDE, "dustin_debug.h"), __file__]
     return max(os.path.getmtime(f) for f in files)
 
 

@@ -2,6 +2,8 @@
 // No device memory is allocated, freed, read or synchronised here; every call only enqueues on `stream`.
 #include "kernels.cuh"
 
+#include "../../include/dustin_debug.h"
+
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
@@ -61,20 +63,21 @@ float scale_log2_of(const dustin_shape_t* s) {
 
 // ---- scoring plan ---------------------------------------------------------------------------------------------
 // Tokens per scoring CTA (all scored KV groups of those tokens): as large as possible while the grid still holds >= 8
-// CTAs per SM (148 SMs), never below 256.  group_slots = how many groups the 8 warps of a CTA serve side by side;
+// CTAs per SM (of the current device: 148 on B200), never below 256.  group_slots = how many groups the 8 warps of a CTA serve side by side;
 // n_parts = softmax partials per (sequence, head) = CTAs per sequence x warps per group.
 void score_plan(int batch, int n_groups, int max_ctx, int* chunk_tokens, int* n_parts, int* group_slots) {
     int slots = 1;
     while (slots < n_groups && slots < 8) slots <<= 1;
     // CTAs per sequence = ceil(max_ctx / chunk): the tiles of a sequence are dealt round-robin to them (score.cu), so
-    // chunk only sets the CTA count: as few as keep >= 8 CTAs per SM (148 SMs) in the grid, at least 256 tokens each.
+    // chunk only sets the CTA count: as few as keep >= 8 CTAs per SM in the grid, at least 256 tokens each.
     // Measured at config 3 (B = 16, 32k): 128 CTAs per sequence 172 us, 64: 185, 27 (one wave): 188.
     int chunk = 2048;
+    const int sms = device_sm_count();
     auto ctas = [&](int c) { return (long long)batch * ((max_ctx + c - 1) / c); };
-    while (chunk > 256 && ctas(chunk) < 148 * 8) chunk >>= 1;
+    while (chunk > 256 && ctas(chunk) < sms * 8) chunk >>= 1;
     // A grid a little above one wave (3 resident CTAs per SM) pays a whole second wave for the overhang: between one
     // and three waves use exactly one (measured at B = 16: 8k 64.5 -> 54.6 us, 16k unchanged, 32k stays at 4.6 waves).
-    const long long resident = 148 * 3;
+    const long long resident = (long long)sms * 3;
     if (ctas(chunk) > resident && ctas(chunk) < 3 * resident && batch <= resident) {
         const int per_seq = (int)(resident / batch);
         const int quantum = 16 * (8 / slots);
@@ -142,6 +145,12 @@ int build_subset(const dustin_shape_t* s, uint64_t head_mask, int n_lists, Score
     return DUSTIN_OK;
 }
 
+// Membership bitmasks I_prot U I_draft that the draft-tier selection kernel of the fused call hands to the target-tier
+// kernel: one row of select_mask_words(max_ctx) words per (sequence, list); lives right after the scoring scratch.
+size_t select_ws_bytes(const dustin_shape_t* s) {
+    return align256((size_t)s->batch * s->n_kv_heads * select_mask_words(s->max_ctx) * sizeof(uint32_t));
+}
+
 int popcount64(uint64_t x) {
     int c = 0;
     for (; x; x &= x - 1) ++c;
@@ -170,7 +179,7 @@ AttnWs attn_ws(const dustin_shape_t* s, int max_tokens) {
 int run_score(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q, int64_t q_stride_batch,
               int64_t q_stride_head, uint64_t head_mask, int32_t n_lists, float* scores_now, float* hist,
               float alpha, void* ws, size_t ws_bytes, cudaStream_t stream, SelectParams::Norm* norm_out = nullptr,
-              int n_queries = 1, int64_t q_stride_query = 0) {
+              int n_queries = 1, int64_t q_stride_query = 0, bool defer_wait = false) {
     // n_queries > 1 (draft-side aggregation, n_lists == 1): every subset head is scored for n_queries query rows
     // q_stride_query apart in ONE pass over K -- the (query, head) pairs are the "heads" of the kernel, <= 8 per KV group
     // and <= 64 in all (DUSTIN_ERR_UNSUPPORTED otherwise; the caller then scores one query row per pass).
@@ -219,6 +228,7 @@ int run_score(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q,
     p.max_ctx = shape->max_ctx;
     p.n_lists = n_lists;
     p.scale_log2 = scale_log2_of(shape);
+    p.defer_wait = defer_wait ? 1 : 0;
     score_plan(p.batch, p.n_groups, p.max_ctx, &p.chunk_tokens, &p.n_chunks, &p.group_slots);
     p.logit_stride = ((long long)p.max_ctx + 3) & ~3ll;
     char* base = static_cast<char*>(ws) + kWsHeader;   // the persistent header belongs to the attention stage
@@ -240,14 +250,8 @@ int run_score(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q,
     return e == cudaSuccess ? DUSTIN_OK : fail_cuda(e);
 }
 
-// DUSTIN_FUSED_ROWS=0 keeps the separate stats / normalise kernels in the fused entry point (A/B measurements).
-bool fused_rows_disabled() {
-    static const bool off = [] {
-        const char* e = std::getenv("DUSTIN_FUSED_ROWS");
-        return e && e[0] == '0';
-    }();
-    return off;
-}
+// DUSTIN_KNOB_FUSED_ROWS = 0 keeps the separate stats / normalise kernels in the fused entry point (A/B measurements).
+bool fused_rows_disabled() { return knob(DUSTIN_KNOB_FUSED_ROWS) == 0; }
 
 int check_select(const dustin_select_t* sel, int32_t k_max) {
     if (!sel) return DUSTIN_ERR_INVALID_ARG;
@@ -263,10 +267,12 @@ int check_select(const dustin_select_t* sel, int32_t k_max) {
 
 int run_select(int32_t batch, int32_t max_ctx, const int32_t* seq_lens, const dustin_select_t* sel,
                const float* s_draft, int64_t draft_list_stride, const float* s_target, int32_t* idx_out,
-               int32_t* cnt_out, int32_t k_max, cudaStream_t stream, const SelectParams::Norm* norm = nullptr) {
+               int32_t* cnt_out, int32_t k_max, cudaStream_t stream, const SelectParams::Norm* norm = nullptr,
+               int mode = 0, uint32_t* draft_mask = nullptr) {
     int rc = check_select(sel, k_max);
     if (rc) return rc;
     if (batch <= 0 || max_ctx < 0 || !s_draft || !s_target || !idx_out || !cnt_out) return DUSTIN_ERR_INVALID_ARG;
+    if (mode != 0 && !draft_mask) return DUSTIN_ERR_INVALID_ARG;
     if (draft_list_stride != 0 && draft_list_stride != max_ctx) return DUSTIN_ERR_INVALID_ARG;
     if (max_ctx > (1 << 20) || batch > 65535) return DUSTIN_ERR_UNSUPPORTED;
     SelectParams p;
@@ -289,7 +295,9 @@ int run_select(int32_t batch, int32_t max_ctx, const int32_t* seq_lens, const du
     p.cnt_out = cnt_out;
     std::memset(&p.norm, 0, sizeof p.norm);
     if (norm) p.norm = *norm;
-    const cudaError_t e = launch_select(p, stream);
+    p.draft_mask = draft_mask;
+    p.draft_mask_stride = (long long)select_mask_words(max_ctx);
+    const cudaError_t e = launch_select(p, stream, mode);
     return e == cudaSuccess ? DUSTIN_OK : fail_cuda(e);
 }
 
@@ -364,6 +372,12 @@ void dustin_tune_attn_split_tokens(int32_t split_tokens) { attn_set_split_overri
 
 void dustin_tune_attn_impl(int32_t impl) { attn_set_impl(impl); }
 
+void dustin_tune_set(int32_t knob_id, int32_t value) { knob_set(knob_id, value); }
+
+int32_t dustin_tune_get(int32_t knob_id) { return knob(knob_id); }
+
+void dustin_debug_trace_buffer(void* device_ptr, size_t bytes) { trace_buffer_set(device_ptr, bytes); }
+
 uint64_t dustin_launch_count(void) { return prof_launch_count(); }
 
 void dustin_profile_enable(int32_t on) { prof_enable(on != 0); }
@@ -385,7 +399,7 @@ size_t dustin_workspace_bytes(const dustin_shape_t* shape, uint64_t head_mask, i
     int max_tokens = (k_max > 0 && k_max < shape->max_ctx) ? k_max : shape->max_ctx;
     if (max_tokens < 1) max_tokens = 1;
     const AttnWs aw = attn_ws(shape, max_tokens);
-    return kWsHeader + sw.total + aw.total + 256;
+    return kWsHeader + sw.total + select_ws_bytes(shape) + aw.total + 256;
 }
 
 int dustin_score_heads(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q, int64_t q_stride_batch,
@@ -427,7 +441,8 @@ int dustin_verify_layer_fused(const dustin_shape_t* shape, const dustin_kv_t* kv
                               const dustin_select_t* select, int32_t k_max, float* scores_now_out, void* out,
                               float* lse_out, int32_t* idx_out, int32_t* cnt_out, void* ws, size_t ws_bytes,
                               void* stream) {
-    // Validate everything before the first launch so that an argument error enqueues nothing.
+    // Validate everything before the first launch so that an argument error enqueues nothing (hist_inout, the only
+    // in/out state, is then untouched): the union of the checks of run_score, run_select and run_attn.
     int rc = check_shape(shape);
     if (rc) return rc;
     rc = check_select(select, k_max);
@@ -435,6 +450,16 @@ int dustin_verify_layer_fused(const dustin_shape_t* shape, const dustin_kv_t* kv
     if (!hist_inout || !s_draft || !idx_out || !cnt_out || !out || !q || !k_new || !v_new || !kv || !kv->v ||
         !std::isfinite(alpha))
         return DUSTIN_ERR_INVALID_ARG;
+    {
+        KvView view;
+        rc = check_kv(shape, kv, true, &view);   // strides, 16-byte alignment of k and v, page-table geometry
+        if (rc) return rc;
+        if (((uintptr_t)q | (uintptr_t)k_new | (uintptr_t)v_new | (uintptr_t)out) & 15) return DUSTIN_ERR_INVALID_ARG;
+        ScoreParams probe;
+        std::memset(&probe, 0, sizeof probe);
+        rc = build_subset(shape, head_mask, select->n_lists, &probe);   // mask inside Hq, <= 8 heads per KV group, n_lists
+        if (rc) return rc;
+    }
     if (select->n_lists != 1 && select->n_lists != shape->n_kv_heads) return DUSTIN_ERR_INVALID_ARG;
     if (draft_list_stride != 0 && draft_list_stride != shape->max_ctx) return DUSTIN_ERR_INVALID_ARG;
     const int nsel = popcount64(head_mask);
@@ -442,9 +467,19 @@ int dustin_verify_layer_fused(const dustin_shape_t* shape, const dustin_kv_t* kv
     const ScoreWs sw = score_ws(shape->batch, nsel, shape->max_ctx);
     const int max_tokens = k_max < shape->max_ctx ? k_max : shape->max_ctx;
     const AttnWs aw = attn_ws(shape, max_tokens > 0 ? max_tokens : 1);
-    if (!ws || ((uintptr_t)ws & 255) || ws_bytes < kWsHeader + sw.total + aw.total) return DUSTIN_ERR_WORKSPACE;
+    if (!ws || ((uintptr_t)ws & 255) || ws_bytes < kWsHeader + sw.total + select_ws_bytes(shape) + aw.total)
+        return DUSTIN_ERR_WORKSPACE;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     char* base = static_cast<char*>(ws);
+    // a3, draft tier (Eq. 6: I_draft = TopK(S_Draft \ I_prot, m)) needs nothing that a1 produces: its kernel is launched
+    // FIRST, releases the scoring kernel at once and works beside it; the bitmask I_prot U I_draft waits in the workspace.
+    uint32_t* draft_mask = reinterpret_cast<uint32_t*>(base + kWsHeader + sw.total);
+    const bool hoist = knob(DUSTIN_KNOB_DRAFT_HOIST) != 0 && pdl_enabled() && shape->max_ctx > 0;
+    if (hoist) {
+        rc = run_select(shape->batch, shape->max_ctx, kv->seq_lens, select, s_draft, draft_list_stride, hist_inout,
+                        idx_out, cnt_out, k_max, st, nullptr, 1, draft_mask);
+        if (rc) return rc;
+    }
     // a1 + a2: scores of verify position 0 (reading A3), accumulated straight into hist (Eq. 5)
     // With enough rows to fill the GPU the selection kernel normalises and accumulates its own rows (no separate
     // stats / normalise launches, no extra pass over the scores); it needs 16-byte rows and no scores_now output.
@@ -454,11 +489,11 @@ int dustin_verify_layer_fused(const dustin_shape_t* shape, const dustin_kv_t* kv
                                 (long long)shape->batch * select->n_lists >= 64 && !fused_rows_disabled();
     rc = run_score(shape, kv, q, (int64_t)shape->n_new * shape->n_q_heads * shape->head_dim, shape->head_dim,
                    head_mask, select->n_lists, scores_now_out, hist_inout, alpha, ws, ws_bytes, st,
-                   rows_in_select ? &norm : nullptr);
+                   rows_in_select ? &norm : nullptr, 1, 0, hoist);
     if (rc) return rc;
-    // a3
+    // a3, target tier + list (or both tiers when the draft tier was not hoisted)
     rc = run_select(shape->batch, shape->max_ctx, kv->seq_lens, select, s_draft, draft_list_stride, hist_inout,
-                    idx_out, cnt_out, k_max, st, rows_in_select ? &norm : nullptr);
+                    idx_out, cnt_out, k_max, st, rows_in_select ? &norm : nullptr, hoist ? 2 : 0, draft_mask);
     if (rc) return rc;
     // a4
     return run_attn(shape, kv, q, k_new, v_new, idx_out, cnt_out, select->n_lists, k_max, out, lse_out,
@@ -476,6 +511,13 @@ int dustin_probe_gather(const dustin_shape_t* shape, const dustin_kv_t* kv, cons
     if (!ws || ws_bytes < kWsHeader + 4 * (size_t)shape->batch * shape->n_kv_heads) return DUSTIN_ERR_WORKSPACE;
     const cudaError_t e = launch_gather_probe(view, idx, cnt, shape->batch, shape->n_kv_heads, shape->head_dim, n_lists,
                                               k_max, static_cast<char*>(ws) + kWsHeader, static_cast<cudaStream_t>(stream));
+    return e == cudaSuccess ? DUSTIN_OK : fail_cuda(e);
+}
+
+int dustin_debug_occupy(int32_t n_ctas, int32_t threads, int32_t smem_bytes, int32_t microseconds, void* stream) {
+    if (n_ctas <= 0 || threads <= 0 || threads > 1024 || smem_bytes < 0 || smem_bytes > 227 * 1024 || microseconds < 0)
+        return DUSTIN_ERR_INVALID_ARG;
+    const cudaError_t e = launch_occupy(n_ctas, threads, smem_bytes, microseconds, static_cast<cudaStream_t>(stream));
     return e == cudaSuccess ? DUSTIN_OK : fail_cuda(e);
 }
 

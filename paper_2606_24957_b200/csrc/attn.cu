@@ -69,7 +69,9 @@ __global__ void __launch_bounds__(32 * MT * KS) attn_kernel(const AttnParams p) 
     const int g = lane >> 2, c = lane & 3;
     const int T = p.n_new, r = p.group, rows = p.rows;
     const int list = p.n_lists == 1 ? 0 : gkv;
-    const int n_sel = MODE == kDense ? seq_len_of(p.kv.seq_lens, b, p.max_ctx) : p.cnt[b * p.n_lists + list];
+    // a caller-supplied cnt is clamped to [0, k_max] as in the tcgen05 kernel: the same inputs behave the same in both
+    const int n_sel = MODE == kDense ? seq_len_of(p.kv.seq_lens, b, p.max_ctx)
+                                     : max(0, min(p.cnt[b * p.n_lists + list], p.k_max));
     const int range_lo = split * p.split_tokens;
     const int n_range = max(0, min(p.split_tokens, n_sel - range_lo));
     const int nt = n_range + (split == 0 ? T : 0);        // this CTA's tokens: cache rows, then the new rows
@@ -372,12 +374,11 @@ cudaError_t launch_mode(const AttnParams& p, cudaStream_t stream) {
     using C = AttnCfg<D, MT, KS>;
     const size_t table = MODE == kGatherTable ? (size_t)(p.split_tokens + 16) * sizeof(RowOff) : 0;
     const size_t smem = C::kPipeBytes + table;
-    static bool attr_done = false;   // per instantiation
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(attn_kernel<D, MT, KS, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)(C::kPipeBytes + kMaxTableTokens * sizeof(RowOff)));
+    static DeviceOnce once;   // per instantiation
+    {
+        const cudaError_t e = ensure_dyn_smem(reinterpret_cast<const void*>(attn_kernel<D, MT, KS, MODE>),
+                                              (int)(C::kPipeBytes + kMaxTableTokens * sizeof(RowOff)), once);
         if (e != cudaSuccess) return e;
-        attr_done = true;
     }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(p.n_splits, p.n_kv_heads, p.batch);
@@ -415,17 +416,17 @@ cudaError_t launch_d(const AttnParams& p, cudaStream_t stream) {
     }
 }
 
-int g_split_override = 0;
-int g_impl = 0;
+std::atomic<int> g_split_override{0};
+std::atomic<int> g_impl{0};
 
 }  // namespace
 
-void attn_set_impl(int impl) { g_impl = impl >= 0 && impl <= 2 ? impl : 0; }
-int attn_get_impl() { return g_impl; }
+void attn_set_impl(int impl) { g_impl.store(impl >= 0 && impl <= 2 ? impl : 0, std::memory_order_relaxed); }
+int attn_get_impl() { return g_impl.load(std::memory_order_relaxed); }
 
-void attn_set_split_override(int split_tokens) { g_split_override = split_tokens > 0 ? split_tokens : 0; }
+void attn_set_split_override(int split_tokens) { g_split_override.store(split_tokens > 0 ? split_tokens : 0, std::memory_order_relaxed); }
 
-// CTAs (= cluster size) per (sequence, KV head): as many as fit one wave of 2 resident CTAs per SM on 148 SMs, at
+// CTAs (= cluster size) per (sequence, KV head): as many as fit one wave of 2 resident CTAs per SM (148 SMs on B200), at
 // most the portable cluster size, at least one 64-token tile each; gather lists are cut so that the address table
 // of a CTA stays within kMaxTableTokens when the cluster size allows.
 void attn_plan(int batch, int n_kv_heads, int max_tokens, int* split_tokens, int* n_splits) {
@@ -433,10 +434,11 @@ void attn_plan(int batch, int n_kv_heads, int max_tokens, int* split_tokens, int
     int tiles = (max_tokens + kTileTokens - 1) / kTileTokens;
     if (tiles < 1) tiles = 1;
     int ns;
-    if (g_split_override > 0) {   // dustin_tune_attn_split_tokens
-        ns = (max_tokens + g_split_override - 1) / g_split_override;
+    const int split_override = g_split_override.load(std::memory_order_relaxed);
+    if (split_override > 0) {   // dustin_tune_attn_split_tokens
+        ns = (max_tokens + split_override - 1) / split_override;
     } else {
-        ns = (148 * 2) / units;
+        ns = (device_sm_count() * 2) / units;
         const int ns_table = (max_tokens + kMaxTableTokens - 17) / (kMaxTableTokens - 16);
         if (ns < ns_table) ns = ns_table;
     }

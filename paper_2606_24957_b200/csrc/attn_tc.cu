@@ -22,8 +22,9 @@
 // CTA-uniformly with one bar.red per tile); O^T and the running sums are then rescaled.
 #include "kernels.cuh"
 
+#include "../../include/dustin_debug.h"
+
 #include <climits>
-#include <cstdlib>
 
 namespace dustin {
 
@@ -151,11 +152,16 @@ __host__ __device__ constexpr uint32_t umma_idesc(int m, int n, int a_mn_major, 
 __device__ __forceinline__ void st_release(int* p, int v) {
     asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
+// Spin until *p != 0.  The writer is a CTA with a lower block index than the caller (see the kernel: range ids run
+// against the block indices), i.e. one the hardware has dispatched no later than the caller, so the wait ends without
+// the whole grid being co-resident.  A few quick polls, then back off so a long wait does not steal issue slots.
 __device__ __forceinline__ void wait_flag(const int* p) {
-    int v;
-    do {
+    int v, polls = 0;
+    for (;;) {
         asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    } while (v == 0);
+        if (v != 0) break;
+        if (++polls > 16) __nanosleep(polls > 256 ? 256 : 64);
+    }
 }
 
 // Order-preserving map float <-> int32 (for redux.sync.max.s32); its own inverse.
@@ -232,7 +238,7 @@ struct Seg {
     int n_tiles;
     int whole;            // the piece is the entire unit: the result goes straight to `out`
     int slot;             // partial slot of this CTA (0: the piece continues a unit begun earlier, 1: otherwise)
-    int cta_first, cta_last;   // CTAs that hold pieces of the unit
+    int cta_first, cta_last;   // range ids (gridDim.x - 1 - blockIdx.x) of the CTAs that hold pieces of the unit
 };
 
 struct TileCursor {
@@ -321,6 +327,10 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int T = p.n_new, r = p.group, rows = p.rows, Hkv = p.n_kv_heads, Hq = p.n_q_heads;
     const int n_units = p.batch * Hkv;
+    // Range id of this CTA in the cut of the concatenated token space: it runs AGAINST the block index.  The CTA that
+    // merges a unit (the one holding the unit's first piece, i.e. its lowest range id) then waits for CTAs with higher
+    // range ids = LOWER block indices, which were dispatched no later than itself: no co-residency assumption.
+    const int rid = (int)gridDim.x - 1 - (int)blockIdx.x;
     if (tid == 0) TS(0);
 
     // ---- token-list lengths of all units -> exclusive prefix sums (threads 0..255) --------------------------------
@@ -355,11 +365,11 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
     }
     if (warp == 8) tmem_alloc(smem_u32(s_tmem), 512);
     pdl_wait();
-    // Producers, whole-unit case (CTA x takes unit x from its first token, decided below): the index entries of tiles
+    // Producers, whole-unit case (the CTA of range id x takes unit x from its first token, decided below): the index entries of tiles
     // 0 and 1 are requested now, so that their latency overlaps the length loads and the prefix scan.
     int spec_idx[2] = {-1, -1};
-    if (GATHER && warp >= 4 && warp < 8 && (int)blockIdx.x < n_units) {
-        const int sb = (int)blockIdx.x / Hkv, sl = p.n_lists == 1 ? 0 : (int)blockIdx.x - sb * Hkv;
+    if (GATHER && warp >= 4 && warp < 8 && rid < n_units) {
+        const int sb = rid / Hkv, sl = p.n_lists == 1 ? 0 : rid - sb * Hkv;
         const int* row = p.idx + ((long long)sb * p.n_lists + sl) * p.k_max;
         const int pos0 = 32 * (warp - 4) + lane;
         if (pos0 < p.k_max) spec_idx[0] = __ldg(row + pos0);
@@ -381,8 +391,9 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
             if (lane >= d) inc += v;
         }
         longest = __reduce_max_sync(0xffffffffu, longest);
-        if (lane == 31 && warp < 8) {
-            s_scan[warp] = inc;
+        const int wsum = __shfl_sync(0xffffffffu, inc, 31);   // stored from lane 0 (see block_excl_scan in select_impl.inl)
+        if (lane == 0 && warp < 8) {
+            s_scan[warp] = wsum;
             s_scan[8 + warp] = longest;
         }
         __syncthreads();
@@ -414,15 +425,15 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
 #pragma unroll
     for (int w = 0; w < 8; ++w) longest_all = max(longest_all, s_scan[8 + w]);
     const bool whole_mode = n_units <= (int)gridDim.x && longest_all <= total / (int)gridDim.x + 4 * kTile && !(p.dbg & 32);
-    int lo = (int)blockIdx.x * chunk, hi = min(lo + chunk, total);
+    int lo = rid * chunk, hi = min(lo + chunk, total);
     if (whole_mode) {
-        lo = (int)blockIdx.x < n_units ? s_prefix[blockIdx.x] : total;
-        hi = (int)blockIdx.x < n_units ? s_prefix[blockIdx.x + 1] : total;
+        lo = rid < n_units ? s_prefix[rid] : total;
+        hi = rid < n_units ? s_prefix[rid + 1] : total;
     }
     const bool active = lo < hi;   // a CTA past the end of the token space only takes part in the teardown
     int u0 = 0;
     if (whole_mode) {
-        u0 = min((int)blockIdx.x, n_units - 1);
+        u0 = min(rid, n_units - 1);
     } else if (active) {
         int a = 0, bnd = n_units;   // largest u with prefix[u] <= lo
         while (bnd - a > 1) {
@@ -783,7 +794,7 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
                 // long finished -- and merge them with this CTA's accumulator, own piece first, then in CTA order.
                 const bool merge = s.pos_lo == 0 && !s.whole;
                 const int nseg = s.cta_last - s.cta_first + 1;
-                const long long slot_id = (long long)blockIdx.x * 2 + s.slot;
+                const long long slot_id = (long long)rid * 2 + s.slot;
                 float v1[NW];
                 float lse1 = -INFINITY;
                 if (merge) {   // second piece = slot 0 of the next CTA: loads in flight during the reductions below
@@ -921,30 +932,16 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
 
 constexpr int kMaxGrid = 256;   // workspace is sized for this many CTAs
 
-int sm_count() {
-    static int n = 0;
-    if (n == 0) {
-        int dev = 0, v = 0;
-        if (cudaGetDevice(&dev) == cudaSuccess &&
-            cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0)
-            n = v;
-        else
-            n = 148;
-    }
-    return n;
-}
-
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 template <int NQ, int NWG, bool GATHER>
 cudaError_t launch_tc(const AttnParams& p, const TcWs& ws, int grid, cudaStream_t stream) {
     using C = TcCfg<NQ>;
     constexpr int smem = C::kSmemBytes;
-    static bool attr_done = false;   // per instantiation
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(attn_tc_kernel<NQ, NWG, GATHER>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    static DeviceOnce once;   // per instantiation
+    {
+        const cudaError_t e = ensure_dyn_smem(reinterpret_cast<const void*>(attn_tc_kernel<NQ, NWG, GATHER>), smem, once);
         if (e != cudaSuccess) return e;
-        attr_done = true;
     }
     ProfScope prof(kKernAttn, stream);
     return launch_pdl(attn_tc_kernel<NQ, NWG, GATHER>, dim3(grid), dim3(kTcThreads + 128 * (NWG - 1)), smem, stream, p, ws);
@@ -973,7 +970,7 @@ size_t attn_tc_ws_bytes(int batch, int n_kv_heads, int rows) {
 
 cudaError_t launch_attn_tc(const AttnParams& p_in, void* ws_base, cudaStream_t stream) {
     AttnParams p = p_in;
-    { const char* e = getenv("DUSTIN_DBG"); p.dbg = e ? atoi(e) : 0; }
+    p.dbg = knob(DUSTIN_KNOB_ATTN_TRACE);
     const size_t units = (size_t)p.batch * p.n_kv_heads;
     char* base = static_cast<char*>(ws_base);
     (void)stream;
@@ -987,7 +984,8 @@ cudaError_t launch_attn_tc(const AttnParams& p_in, void* ws_base, cudaStream_t s
     ws.dbg_ts = (p.dbg & 8) ? reinterpret_cast<unsigned long long*>(reinterpret_cast<char*>(ws.part_lse) + align256((size_t)kMaxGrid * 2 * nq * sizeof(float))) : nullptr;
     const int max_tokens = (p.idx ? (p.k_max < p.max_ctx ? p.k_max : p.max_ctx) : p.max_ctx) + p.n_new;
     long long tiles = ((long long)units * max_tokens + kTile - 1) / kTile;
-    int grid = sm_count() < kMaxGrid ? sm_count() : kMaxGrid;
+    const int sms = device_sm_count();
+    int grid = sms < kMaxGrid ? sms : kMaxGrid;
     if (tiles < grid) grid = tiles < 1 ? 1 : (int)tiles;
     switch ((p.rows + 15) / 16) {
         case 1: return launch_tc_nq<16>(p, ws, grid, stream);

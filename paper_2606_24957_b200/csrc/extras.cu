@@ -131,7 +131,27 @@ __global__ void __launch_bounds__(kProbeThreads) gather_probe_kernel(KvView kv, 
     if ((acc.x ^ acc.y) == 0x9e3779b9u) sink[u] = acc.x;   // keeps the loads alive; practically never taken
 }
 
+// Measurement aid (dustin_debug.h): CTAs that only hold their SM resources for a while.
+__global__ void occupy_kernel(unsigned long long ns) {
+    extern __shared__ unsigned char occ_smem[];
+    unsigned long long t0, t;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t0));
+    do {
+        __nanosleep(200);
+        asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+    } while (t - t0 < ns);
+    if (ns == 0xffffffffffffffffull) occ_smem[threadIdx.x] = 0;   // keeps the allocation referenced
+}
+
 }  // namespace
+
+cudaError_t launch_occupy(int n_ctas, int threads, int smem_bytes, int microseconds, cudaStream_t stream) {
+    static DeviceOnce once;
+    cudaError_t e = ensure_dyn_smem(reinterpret_cast<const void*>(occupy_kernel), 227 * 1024, once);
+    if (e != cudaSuccess) return e;
+    occupy_kernel<<<n_ctas, threads, smem_bytes, stream>>>((unsigned long long)microseconds * 1000ull);
+    return cudaGetLastError();
+}
 
 cudaError_t launch_gather_probe(const KvView& kv, const int* idx, const int* cnt, int batch, int n_kv_heads, int head_dim,
                                 int n_lists, int k_max, void* sink, cudaStream_t stream) {

@@ -3,6 +3,8 @@
 
 #include "common.cuh"
 
+#include <atomic>
+
 namespace dustin {
 
 // ---- a1 / a2 ------------------------------------------------------------------------------------------------
@@ -16,6 +18,10 @@ struct ScoreParams {
     int n_groups;            // KV groups holding >= 1 subset head (the only K rows that are read)
     int chunk_tokens, n_chunks;     // tokens per scoring CTA; softmax partials per (sequence, head) = CTAs x sub-ranges
     int group_slots;                // scored KV groups served side by side by the 8 warps of a CTA: 1, 2, 4 or 8
+    int defer_wait;                 // fused call with a hoisted draft tier: the kernel launched just before this one is the
+                                    // draft-tier selection, whose results a1 does not need -- the dependency wait moves from
+                                    // the start of the kernel to its end (it stays, so that "a1 complete" still implies
+                                    // "everything before it complete" for the kernels that follow)
     unsigned char sel_head[64];     // ordinal -> query head
     int sel_qoff[64];               // ordinal -> element offset of its query row inside q + b * q_stride_batch
     unsigned char group_id[64];     // scored group slot -> KV head
@@ -49,6 +55,11 @@ struct SelectParams {
     int* idx_out;
     int* cnt_out;
     int mask_words, replicas, list_cap;   // shared-memory plan, filled by launch_select
+    unsigned long long* trace;            // DUSTIN_KNOB_SELECT_TRACE: [n_ctas][64] %globaltimer samples, else nullptr
+    // Split selection of the fused call (select.cu): membership bitmask I_prot U I_draft per (b, list) row, written by
+    // the draft-tier kernel and read by the target-tier kernel; draft_mask_stride words per row.
+    uint32_t* draft_mask;
+    long long draft_mask_stride;
     // Row materialisation (fused entry point): when norm.logits != nullptr the kernel first computes its own target
     // row, s_target[b,l,n] = alpha * s_target[b,l,n] + sum_j exp2(logit_j[n] - M_j) / Z_j (a1's normalisation and
     // Eq. 5), from the logits and partials that score_logits_kernel left in the workspace, and writes it back.
@@ -61,8 +72,10 @@ struct SelectParams {
         unsigned char list_first[64], list_cnt[64];
     } norm;
 };
-cudaError_t launch_select(const SelectParams& p, cudaStream_t stream);
-size_t select_smem_bytes(int max_ctx);
+// mode: 0 = both tiers + list (staged call), 1 = draft tier only (-> p.draft_mask; launched before the scoring kernel
+// of the fused call, which it releases at once), 2 = target tier + list (reads p.draft_mask).
+cudaError_t launch_select(const SelectParams& p, cudaStream_t stream, int mode = 0);
+size_t select_mask_words(int max_ctx);   // words per row of SelectParams::draft_mask
 
 // ---- a4 / a5 ------------------------------------------------------------------------------------------------
 struct AttnParams {
@@ -108,10 +121,12 @@ cudaError_t launch_append(const KvView& kv, int* seq_lens, const int* n_append, 
 cudaError_t launch_gather_probe(const KvView& kv, const int* idx, const int* cnt, int batch, int n_kv_heads, int head_dim,
                                 int n_lists, int k_max, void* sink, cudaStream_t stream);
 
+cudaError_t launch_occupy(int n_ctas, int threads, int smem_bytes, int microseconds, cudaStream_t stream);
+
 // ---- launch bookkeeping (profile.cu) ----------------------------------------------------------------------------
 enum KernelId {
-    kKernScoreLogits = 0, kKernScoreStats, kKernScoreNormalize, kKernFuse, kKernSelect, kKernAttn, kKernAttnCombine,
-    kKernArr, kKernAppend,
+    kKernScoreLogits = 0, kKernScoreStats, kKernScoreNormalize, kKernFuse, kKernSelect, kKernAttn, kKernSelectDraft,
+    kKernArr, kKernAppend, kKernSelectCluster,
     kKernCount
 };
 // Put one on the stack around a kernel launch: counts it and, when profiling is on, brackets it with CUDA events.
@@ -126,6 +141,18 @@ private:
     cudaStream_t stream_;
     long long slot_;
 };
+// Tuning knobs of dustin_debug.h (ids: enum dustin_knob), the trace buffer, and per-device caches.
+int knob(int id);
+void knob_set(int id, int value);
+void trace_buffer_set(void* p, size_t bytes);
+void* trace_buffer(size_t* bytes);
+int current_device();
+int device_sm_count();                  // SMs of the current device (cached per device)
+struct DeviceOnce {                     // one bit per device ordinal: "attribute already set there"
+    std::atomic<unsigned long long> done{0};
+};
+// cudaFuncAttributeMaxDynamicSharedMemorySize := bytes on the current device, once per (kernel, device); thread-safe.
+cudaError_t ensure_dyn_smem(const void* func, int bytes, DeviceOnce& once);
 unsigned long long prof_launch_count();
 void prof_enable(bool on);
 cudaError_t prof_collect(double* ms_out, long long* launches_out);

@@ -2,11 +2,12 @@
 // PAPER.md:161-164) for sm_100a.
 //
 // a1 is one streaming read of the K rows of every KV group that holds a subset head (HBM-bound: DESIGN.md §4).
-//   score_logits_kernel   K rows go global -> registers with 16-byte loads and straight into mma.sync fragments
-//                         (tokens on M, the <= 8 subset heads of the KV group on N, head_dim on K; the head_dim
-//                         axis is permuted identically for both operands so each thread's 16 B feed two k-steps).
-//                         Writes log2-domain logits [B, nsel, N] (L2-resident scratch) and per-CTA softmax
-//                         partials (max, sum).
+//   score_logits_kernel   every warp streams its 16-token K tiles through a private two-stage cp.async ring in shared
+//                         memory (16-byte copies, whole rows per warp instruction, XOR-swizzled) and feeds mma.sync
+//                         fragments from it (tokens on M, the <= 8 subset heads of the KV group on N, head_dim on K;
+//                         the head_dim axis is permuted identically for both operands so each thread's 16 B feed two
+//                         k-steps).  Writes log2-domain logits [B, nsel, N] (L2-resident scratch) and per-CTA
+//                         softmax partials (max, sum).
 //   score_stats_kernel    folds the partials into (M, 1/Z) per (sequence, head), in a fixed order.
 //   score_normalize_kernel p = exp2(l - M) / Z summed over the heads of each list; optionally fused with the
 //                         Eq. 5 accumulation into hist (the fused entry point never writes scores_now).
@@ -26,27 +27,6 @@ struct KFrag {
     uint4 hi[D / 32];  // row g + 8
 };
 
-template <int D>
-__device__ __forceinline__ void load_tile(KFrag<D>& f, const ScoreParams& p, int b, int grp, int n0, int N, int lane) {
-    const int g = lane >> 2, c = lane & 3;
-    const int n_lo = n0 + g, n_hi = n0 + g + 8;
-#pragma unroll
-    for (int j = 0; j < D / 32; ++j) {
-        f.lo[j] = make_uint4(0, 0, 0, 0);
-        f.hi[j] = make_uint4(0, 0, 0, 0);
-    }
-    if (n_lo < N) {
-        const __nv_bfloat16* row = p.kv.k + kv_row_offset(p.kv, b, n_lo, grp) + c * 8;
-#pragma unroll
-        for (int j = 0; j < D / 32; ++j) f.lo[j] = ldg_stream16(row + j * 32);
-    }
-    if (n_hi < N) {
-        const __nv_bfloat16* row = p.kv.k + kv_row_offset(p.kv, b, n_hi, grp) + c * 8;
-#pragma unroll
-        for (int j = 0; j < D / 32; ++j) f.hi[j] = ldg_stream16(row + j * 32);
-    }
-}
-
 // ---- shared-memory staging of the K stream -----------------------------------------------------------------------
 // A warp owns a private ring of kStages tiles (16 tokens x D bf16).  issue_tile requests one tile with fully
 // coalesced 16-byte cp.async (a warp instruction covers whole rows: 2 rows x 256 B at D = 128), zero-filling rows past
@@ -56,7 +36,8 @@ __device__ __forceinline__ void load_tile(KFrag<D>& f, const ScoreParams& p, int
 constexpr int kStages = 2;
 
 template <int D>
-__device__ __forceinline__ void issue_tile(uint32_t stage, const ScoreParams& p, int b, int grp, int n0, int N, int lane) {
+__device__ __forceinline__ void issue_tile(uint32_t stage, const ScoreParams& p, int b, int grp, int n0, int N, int lane,
+                                           uint64_t policy) {
     constexpr int CPR = D / 8;              // 16-byte chunks per row
     constexpr int RPI = 32 / CPR;           // rows per warp instruction
     long long my = -1;                      // lanes 0..15: element offset of row n0 + lane (page table resolved once)
@@ -67,7 +48,8 @@ __device__ __forceinline__ void issue_tile(uint32_t stage, const ScoreParams& p,
         const int row = i * RPI + r0;
         const long long off = __shfl_sync(0xffffffffu, my, row);
         const __nv_bfloat16* src = off >= 0 ? p.kv.k + off + ch * 8 : p.kv.k;
-        cp_async16(stage + (uint32_t)row * (D * 2) + (uint32_t)((ch ^ ((row & 1) << 2)) << 4), src, off >= 0 ? 16 : 0);
+        cp_async16_hint(stage + (uint32_t)row * (D * 2) + (uint32_t)((ch ^ ((row & 1) << 2)) << 4), src, off >= 0 ? 16 : 0,
+                        policy);
     }
 }
 
@@ -94,7 +76,7 @@ __global__ void __launch_bounds__(kScoreThreads, 3) score_logits_kernel(const Sc
     const int chunk = blockIdx.x, b = blockIdx.y;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int g = lane >> 2, c = lane & 3;
-    pdl_wait();
+    if (!p.defer_wait) pdl_wait();
     const int N = seq_len_of(p.kv.seq_lens, b, p.max_ctx);
     const int slots = p.group_slots, n_sub = kScoreWarps / slots;
     const int ws = warp / slots;                       // which tiles of the range
@@ -102,6 +84,9 @@ __global__ void __launch_bounds__(kScoreThreads, 3) score_logits_kernel(const Sc
     // sequence, so at any moment the CTAs of a sequence read ONE contiguous window of the cache.  Contiguous per-CTA
     // ranges put the concurrent streams a fixed stride apart, which loads the DRAM channels unevenly (measured: 174 to
     // 189 us at config 3 depending on that stride).
+    // K is read exactly once: evict_first keeps the stream from displacing the logits scratch, the score rows and the
+    // selection state that the following kernels (and the draft-tier selection running beside this one) read from L2
+    const uint64_t policy = l2_policy_evict_first();
     const int chunk_lo = chunk * (kScoreWarps / p.group_slots) * kTileTokens;
     const int chunk_hi = N;
 
@@ -131,9 +116,9 @@ __global__ void __launch_bounds__(kScoreThreads, 3) score_logits_kernel(const Sc
         const int step = (int)gridDim.x * n_sub * kTileTokens;
         int n0 = chunk_lo + ws * kTileTokens;
         __syncwarp();                                        // the previous group's reads of the ring are done
-        if (n0 < chunk_hi) issue_tile<D>(ring_u32, p, b, grp, n0, N, lane);
+        if (n0 < chunk_hi) issue_tile<D>(ring_u32, p, b, grp, n0, N, lane, policy);
         cp_async_commit();
-        if (n0 + step < chunk_hi) issue_tile<D>(ring_u32 + kTileBytes, p, b, grp, n0 + step, N, lane);
+        if (n0 + step < chunk_hi) issue_tile<D>(ring_u32 + kTileBytes, p, b, grp, n0 + step, N, lane, policy);
         cp_async_commit();
         KFrag<D> cur;
         for (int t = 0; n0 < chunk_hi; n0 += step, ++t) {
@@ -141,7 +126,7 @@ __global__ void __launch_bounds__(kScoreThreads, 3) score_logits_kernel(const Sc
             __syncwarp();
             frag_tile<D>(cur, ring + (t & 1) * kTileBytes, lane);
             __syncwarp();                                    // every lane has read stage t & 1: it can be refilled
-            if (n0 + 2 * step < chunk_hi) issue_tile<D>(ring_u32 + (t & 1) * kTileBytes, p, b, grp, n0 + 2 * step, N, lane);
+            if (n0 + 2 * step < chunk_hi) issue_tile<D>(ring_u32 + (t & 1) * kTileBytes, p, b, grp, n0 + 2 * step, N, lane, policy);
             cp_async_commit();
             float acc[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
@@ -193,6 +178,10 @@ __global__ void __launch_bounds__(kScoreThreads, 3) score_logits_kernel(const Sc
             if (h1) p.part[((long long)b * p.nsel + first + 2 * c + 1) * p.n_chunks + part] = make_float2(m1, s1);
         }
     }
+    // Fused call with a hoisted draft tier: ONE CTA -- the last of the grid, dispatched in the last wave -- waits for the
+    // draft-tier kernel that runs beside this one, so that "a1 complete" implies "draft tier complete and visible" for the
+    // kernels that follow.  (Every CTA waiting would park the early ones on their SMs until that kernel is done.)
+    if (p.defer_wait && blockIdx.x == gridDim.x - 1 && blockIdx.y == gridDim.y - 1) pdl_wait();
     pdl_trigger();
 }
 
@@ -282,13 +271,10 @@ cudaError_t launch_score(const ScoreParams& p, float* scores_now, float* hist, f
     {
         ProfScope prof(kKernScoreLogits, stream);
         const int smem = kScoreWarps * kStages * kTileTokens * p.head_dim * 2;
-        static bool attr_done = false;
-        if (!attr_done) {
-            cudaError_t ea = cudaFuncSetAttribute(score_logits_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                  kScoreWarps * kStages * kTileTokens * 128 * 2);
-            if (ea != cudaSuccess) return ea;
-            attr_done = true;
-        }
+        static DeviceOnce once;
+        const cudaError_t ea = ensure_dyn_smem(reinterpret_cast<const void*>(score_logits_kernel<128>),
+                                               kScoreWarps * kStages * kTileTokens * 128 * 2, once);
+        if (ea != cudaSuccess) return ea;
         if (p.head_dim == 128)
             e0 = launch_pdl(score_logits_kernel<128>, grid, dim3(kScoreThreads), smem, stream, p);
         else

@@ -8,6 +8,15 @@ constexpr int kBinsPerThread = kBins / kSelThreads;
 
 __device__ __forceinline__ uint32_t key_of(float s) { return s > 0.f ? __float_as_uint(s) : 0u; }
 
+// DUSTIN_KNOB_SELECT_TRACE: thread 0 of every CTA samples %globaltimer at the phase boundaries.
+__device__ __forceinline__ void sel_ts(unsigned long long* row, int slot) {
+    if (row != nullptr && threadIdx.x == 0) {
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+        row[slot] = t;
+    }
+}
+
 struct SelShared {
     uint32_t hist[kBins];
     uint32_t warp_tot[kSelWarps + 1];
@@ -18,6 +27,8 @@ struct SelShared {
     uint32_t tot_db[2][kSelWarps], min_db[2][kSelWarps], max_db[2][kSelWarps], res_db[2][4];
     uint32_t small_n, small_key[32], small_idx[32];
     float2 stats[64];   // (M, 1/Z) of the heads feeding this row (row materialisation)
+    unsigned long long* trace;   // this CTA's 64 timestamp slots, or nullptr (read and written by thread 0 only)
+    int trace_base;              // first slot of the tier in progress
 };
 
 // Exclusive prefix of v over the block in thread order; *total (optional) receives the block sum.
@@ -30,7 +41,10 @@ __device__ __forceinline__ uint32_t block_excl_scan(uint32_t v, SelShared& sh, u
         if (lane >= off) inc += o;
     }
     __syncthreads();   // protects warp_tot against the previous use
-    if (lane == 31) sh.warp_tot[warp] = inc;
+    // The warp total travels to lane 0 before it is stored.  (Storing from lane 31 miscompiles with nvcc 12.9 in the 256-
+    // and 512-thread instantiations: the address is formed as base + (tid >> 3), which is only warp * 4 when lane == 0.)
+    const uint32_t wtot = __shfl_sync(0xffffffffu, inc, 31);
+    if (lane == 0) sh.warp_tot[warp] = wtot;
     __syncthreads();
     const uint32_t t = lane < kSelWarps ? sh.warp_tot[lane] : 0u;   // every warp scans the warp totals redundantly
     uint32_t ti = t;
@@ -443,7 +457,8 @@ __device__ __forceinline__ uint32_t block_excl_scan_db(uint32_t v, SelShared& sh
         const uint32_t o = __shfl_up_sync(0xffffffffu, inc, off);
         if (lane >= off) inc += o;
     }
-    if (lane == 31) sh.tot_db[b][warp] = inc;
+    const uint32_t wtot = __shfl_sync(0xffffffffu, inc, 31);   // stored from lane 0: see block_excl_scan
+    if (lane == 0) sh.tot_db[b][warp] = wtot;
     __syncthreads();
     const uint32_t t = lane < kSelWarps ? sh.tot_db[b][lane] : 0u;   // every warp scans the warp totals redundantly
     uint32_t ti = t;
@@ -518,6 +533,7 @@ __device__ void list_select_ranged(const float* __restrict__ s, const SelLayout&
     if (threadIdx.x == 0) sh.small_n = 0;
     uint32_t klo, khi;
     block_minmax(lmin, lmax, part != 0, sh, ph, klo, khi);
+    if (threadIdx.x == 0) sel_ts(sh.trace, sh.trace_base + 2);   // list keys gathered, range known
     uint32_t eq_total = (uint32_t)n_list;
     uint32_t T = klo, i_star = 0xffffffffu;   // admitted: key > T, or key == T and index <= i_star
     bool settled = false;
@@ -588,6 +604,7 @@ __device__ void list_select_ranged(const float* __restrict__ s, const SelLayout&
             i_star = (f1.x << 10) | f2.x;
         }
     }
+    if (threadIdx.x == 0) sel_ts(sh.trace, sh.trace_base + 3);   // threshold (T, i_star) settled
 #pragma unroll
     for (int e = 0; e < kPer; ++e)
         if (threadIdx.x + e * kSelThreads < n_list && (key[e] > T || (key[e] == T && idx[e] <= i_star)))
@@ -641,9 +658,18 @@ __device__ bool sampled_tier_vec(const float* __restrict__ s, int lo, int hi, in
         const int n = vv << 2;
         return vv < v_end ? (L.mem[n >> 5] >> (n & 31)) & 0xfu : 0xfu;
     };
-    // ---- (a) threshold from 1024 samples ----
-    uint32_t skey = 0;
-    bool svalid = false;
+    // ---- (a) threshold from ~1024 samples ----
+    // One chunk: one sample per thread, out of the registers.  Longer rows: 1024 strided samples whatever the CTA size
+    // (kSampPer per thread): the estimate, and with it the length of the candidate list, must not degrade in the small-CTA
+    // instantiation.
+    constexpr int kSampPer = kSelThreads >= 1024 ? 1 : 1024 / kSelThreads;
+    uint32_t skey[kSampPer];
+    bool svalid[kSampPer];
+#pragma unroll
+    for (int i = 0; i < kSampPer; ++i) {
+        skey[i] = 0;
+        svalid[i] = false;
+    }
     int n_slots;
     if (one) {
         load_chunk(0);
@@ -653,24 +679,42 @@ __device__ bool sampled_tier_vec(const float* __restrict__ s, int lo, int hi, in
         for (int u = 1; u < kVecPerChunk; ++u)
             if (u_s == u) xv = x[u];
         const float f = e_s == 0 ? xv.x : (e_s == 1 ? xv.y : (e_s == 2 ? xv.z : xv.w));
-        skey = key_max0(f);
-        svalid = !((nib_of(v0 + u_s * kSelThreads + t) >> e_s) & 1u);
+        skey[0] = key_max0(f);
+        svalid[0] = !((nib_of(v0 + u_s * kSelThreads + t) >> e_s) & 1u);
         n_slots = min(kSelThreads, (v_end - v0));   // threads whose sampled vector can exist at all (upper bound)
     } else {
-        const int stride = max(1, n_cand / kSelThreads);
-        n_slots = min(kSelThreads, (n_cand + stride - 1) / stride);
-        const int pos = lo + t * stride;
-        if (t < n_slots) {
-            skey = key_max0(__ldcg(s + pos));
-            svalid = !((L.mem[pos >> 5] >> (pos & 31)) & 1u);
+        constexpr int kSamples = kSampPer * kSelThreads;
+        const int stride = max(1, n_cand / kSamples);
+        n_slots = min(kSamples, (n_cand + stride - 1) / stride);
+#pragma unroll
+        for (int i = 0; i < kSampPer; ++i) {
+            const int slot = t + i * kSelThreads;
+            const int pos = lo + slot * stride;
+            if (slot < n_slots) {
+                skey[i] = key_max0(__ldcg(s + pos));
+                svalid[i] = !((L.mem[pos >> 5] >> (pos & 31)) & 1u);
+            }
         }
     }
     uint32_t kmin, kmax;
-    block_minmax(skey, skey, svalid, sh, ph, kmin, kmax);
+    {
+        uint32_t tmin = 0xffffffffu, tmax = 0u;
+        bool any = false;
+#pragma unroll
+        for (int i = 0; i < kSampPer; ++i)
+            if (svalid[i]) {
+                tmin = min(tmin, skey[i]);
+                tmax = max(tmax, skey[i]);
+                any = true;
+            }
+        block_minmax(tmin, tmax, any, sh, ph, kmin, kmax);
+    }
     uint32_t tau = 0;   // 0: every candidate goes to the list
     if (kmin <= kmax) {
         const int shift = range_shift(kmin, kmax);
-        if (svalid) atomicAdd(&L.hist[kBins - 1 - ((skey - kmin) >> shift)], 1u);
+#pragma unroll
+        for (int i = 0; i < kSampPer; ++i)
+            if (svalid[i]) atomicAdd(&L.hist[kBins - 1 - ((skey[i] - kmin) >> shift)], 1u);
         __syncthreads();
         // sample rank that the true rank-th key exceeds with overwhelming probability (mean * 1.25 + 3.5 sigma + 4)
         const float mean = (float)n_slots * (float)rank / (float)n_cand;
@@ -678,6 +722,7 @@ __device__ bool sampled_tier_vec(const float* __restrict__ s, int lo, int hi, in
         const uint4 fb = find_bin_db(L.hist, j, sh, ph);
         if (j <= fb.w) tau = kmin + (((uint32_t)(kBins - 1) - fb.x) << shift);
     }
+    if (threadIdx.x == 0) sel_ts(sh.trace, sh.trace_base + 0);   // threshold estimate done
     // ---- (b) compaction: candidates with key >= tau ----
     // Signed compare on the raw bits: for s >= 0 it is the key order; negative scores (key 0, reading A15) pass
     // only when tau == 0, i.e. when every candidate is taken.
@@ -715,6 +760,7 @@ __device__ bool sampled_tier_vec(const float* __restrict__ s, int lo, int hi, in
         }
     }
     __syncthreads();
+    if (threadIdx.x == 0) sel_ts(sh.trace, sh.trace_base + 1);   // compaction done
     const uint32_t n_list = base;
     if (n_list < (uint32_t)rank || n_list > (uint32_t)L.cap) return false;
     select_from_list(s, L, (int)n_list, (uint32_t)rank, sh, ph);
@@ -815,6 +861,7 @@ __device__ __forceinline__ void materialize_row(const SelectParams& p, int b, in
         if (lane == 0) sh.stats[j] = st;
     }
     __syncthreads();
+    if (threadIdx.x == 0) sel_ts(sh.trace, 7);   // softmax statistics folded
     float4* hrow = reinterpret_cast<float4*>(const_cast<float*>(p.s_target) +
                                              ((long long)b * p.n_lists + l) * p.max_ctx);
     const float* lg = p.norm.logits + ((long long)b * p.norm.nsel + first) * p.norm.logit_stride;
@@ -860,25 +907,35 @@ __device__ __forceinline__ void materialize_row(const SelectParams& p, int b, in
     __syncthreads();   // the row is re-read below (ld.cg: L2, where these stores have landed for this CTA)
 }
 
-template <bool VEC>
-__global__ void __launch_bounds__(kSelThreads) select_kernel(const SelectParams p) {
-    extern __shared__ __align__(16) uint32_t smem_dyn[];
-    __shared__ SelShared sh;
-    const int l = blockIdx.x, b = blockIdx.y;
-    pdl_wait();
+// MODE kSelBoth: both tiers of Eq. 6 and the list (the staged call).  The fused call splits the work so that the
+// draft tier -- which needs nothing from stage a1 -- runs while a1 streams K:
+//   kSelDraft   I_prot and I_draft = TopK(S_Draft \ I_prot, m) only; the membership bitmask goes to p.draft_mask.
+//               Launched BEFORE the scoring kernel, it releases it at once (pdl_trigger right after its own dependency
+//               wait) and works beside it: gridDim.x CTAs walk the rows blockIdx.x, blockIdx.x + gridDim.x, ...
+//               (select.cu picks 256-thread CTAs, one per row, when many rows are in flight).
+//   kSelTarget  picks the bitmask up, (materialises its target row,) runs the target tier and emits the list.
+constexpr int kSelBoth = 0, kSelDraft = 1, kSelTarget = 2;
+
+// One (sequence b, list l) row.  Returns early (uniformly over the CTA) on rows that need no selection.
+template <bool VEC, int MODE>
+__device__ __forceinline__ void select_row(const SelectParams& p, int b, int l, uint32_t* smem_dyn, SelShared& sh,
+                                           Phase& ph, unsigned long long* tr) {
     const int N = seq_len_of(p.seq_lens, b, p.max_ctx);
     const int k = p.budgets ? p.budgets[b] : p.budget;
     int* out = p.idx_out + ((long long)b * p.n_lists + l) * p.k_max;
     int* cnt_out = p.cnt_out + (long long)b * p.n_lists + l;
 
-    const bool own_row = VEC && p.norm.logits != nullptr;   // this CTA computes its target row itself
+    const bool own_row = MODE != kSelDraft && VEC && p.norm.logits != nullptr;   // this CTA computes its target row itself
     if (own_row) materialize_row(p, b, l, N, sh);
+    sel_ts(tr, 2);
     if (k > p.k_max || k < p.n_sink + p.n_recent) {   // argument error on this row (dustin.h)
+        if (MODE == kSelDraft) return;
         for (int i = threadIdx.x; i < p.k_max; i += kSelThreads) out[i] = -1;
         if (threadIdx.x == 0) *cnt_out = 0;
         return;
     }
     if (k >= N) {   // everything is selected (reading A12)
+        if (MODE == kSelDraft) return;
         for (int i = threadIdx.x; i < p.k_max; i += kSelThreads) out[i] = i < N ? i : -1;
         if (threadIdx.x == 0) *cnt_out = N;
         return;
@@ -898,27 +955,38 @@ __global__ void __launch_bounds__(kSelThreads) select_kernel(const SelectParams 
     L.R = p.replicas;
     L.cap = p.list_cap;
     uint32_t* mem = L.mem;
-    // I_prot = I_sink U I_window
-    for (int w = threadIdx.x; w < n_words; w += kSelThreads) {
-        uint32_t bits = 0;
-        const int n0 = w * 32;
-        if (n0 < S) bits |= (S - n0 >= 32) ? 0xffffffffu : ((1u << (S - n0)) - 1u);
-        if (n0 + 32 > hi) {   // window [hi, N) and, for now, the tail [N, 32 * n_words) of the last word
-            const int from = max(hi - n0, 0);
-            bits |= ~((1u << from) - 1u);
+    uint32_t* gmask = p.draft_mask + ((long long)b * p.n_lists + l) * p.draft_mask_stride;
+    if (MODE == kSelTarget) {
+        // I_prot U I_draft as the draft-tier kernel left it (plain loads: that grid has completed and flushed)
+        for (int w = threadIdx.x; w < n_words; w += kSelThreads) mem[w] = gmask[w];
+    } else {
+        // I_prot = I_sink U I_window
+        for (int w = threadIdx.x; w < n_words; w += kSelThreads) {
+            uint32_t bits = 0;
+            const int n0 = w * 32;
+            if (n0 < S) bits |= (S - n0 >= 32) ? 0xffffffffu : ((1u << (S - n0)) - 1u);
+            if (n0 + 32 > hi) {   // window [hi, N) and, for now, the tail [N, 32 * n_words) of the last word
+                const int from = max(hi - n0, 0);
+                bits |= ~((1u << from) - 1u);
+            }
+            mem[w] = bits;
         }
-        mem[w] = bits;
     }
-    Phase ph;
     bool hist_clean = VEC;
     if (VEC) clear_hist(L.hist, 1);
     __syncthreads();
 
     // tier 0: I_draft = TopK(S_Draft \ I_prot, m);  tier 1: I_target = TopK(S_Target \ (I_prot U I_draft), k-m-|I_prot|)
 #pragma unroll 1
-    for (int tier = 0; tier < 2; ++tier) {
+    for (int tier = (MODE == kSelTarget ? 1 : 0); tier < (MODE == kSelDraft ? 1 : 2); ++tier) {
         const int want = tier == 0 ? m : c - m;
+        if (threadIdx.x == 0) sh.trace_base = 16 + 16 * tier;
         if (want > 0) select_tier<VEC>(tier == 0 ? sd : st, lo, hi, want, L, n_words, sh, ph, hist_clean);
+        sel_ts(tr, 3 + tier);
+    }
+    if (MODE == kSelDraft) {
+        for (int w = threadIdx.x; w < n_words; w += kSelThreads) gmask[w] = mem[w];
+        return;
     }
     if (threadIdx.x == 0 && (N & 31)) mem[n_words - 1] &= (1u << (N & 31)) - 1u;   // drop the tail bits >= N
     __syncthreads();
@@ -929,6 +997,7 @@ __global__ void __launch_bounds__(kSelThreads) select_kernel(const SelectParams 
     for (int w = w_lo; w < w_hi; ++w) mine += __popc(mem[w]);
     uint32_t total;
     uint32_t pos = block_excl_scan(mine, sh, &total);
+    sel_ts(tr, 5);
     for (int w = w_lo; w < w_hi; ++w) {
         uint32_t bits = mem[w];
         while (bits) {
@@ -940,6 +1009,37 @@ __global__ void __launch_bounds__(kSelThreads) select_kernel(const SelectParams 
     }
     for (int i = (int)total + threadIdx.x; i < p.k_max; i += kSelThreads) out[i] = -1;
     if (threadIdx.x == 0) *cnt_out = (int)total;
-    pdl_trigger();
 }
 
+template <bool VEC, int MODE>
+__global__ void __launch_bounds__(kSelThreads, kSelThreads <= 256 ? 3 : 1) select_kernel(const SelectParams p) {
+    extern __shared__ __align__(16) uint32_t smem_dyn[];
+    __shared__ SelShared sh;
+    unsigned long long* const tr =
+        p.trace ? p.trace + ((size_t)blockIdx.y * gridDim.x + blockIdx.x + (MODE == kSelDraft ? (size_t)p.n_lists * p.batch : 0)) * 64
+                : nullptr;
+    sel_ts(tr, 0);
+    pdl_wait();
+    if (MODE == kSelDraft) pdl_trigger();   // the scoring kernel may start now: it needs nothing from this one
+    sel_ts(tr, 1);
+    if (threadIdx.x == 0) {
+        sh.trace = tr;
+        sh.trace_base = 8;
+    }
+    Phase ph;
+    if (MODE == kSelDraft) {
+        // a few CTAs walk all rows (grid = (n_ctas, 1)); the trace shows the CTA's first row and its end
+        const int n_rows = p.n_lists * p.batch;
+#pragma unroll 1
+        for (int row = blockIdx.x; row < n_rows; row += gridDim.x) {
+            select_row<VEC, MODE>(p, row / p.n_lists, row % p.n_lists, smem_dyn, sh, ph, row == (int)blockIdx.x ? tr : nullptr);
+            __syncthreads();   // the next row reuses the shared-memory state
+            if (threadIdx.x == 0) sh.trace = nullptr;
+        }
+        sel_ts(tr, 6);
+        return;
+    }
+    select_row<VEC, MODE>(p, blockIdx.y, blockIdx.x, smem_dyn, sh, ph, tr);
+    sel_ts(tr, 6);
+    pdl_trigger();
+}

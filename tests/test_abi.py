@@ -18,8 +18,8 @@ def lib():
     return api.lib()
 
 
-def declared_functions():
-    text = open(os.path.join(ROOT, "include", "dustin.h")).read()
+def declared_functions(header="dustin.h"):
+    text = open(os.path.join(ROOT, "include", header)).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(dustin_[a-z_0-9]+)\s*\(", text)))
 
@@ -29,6 +29,30 @@ def test_every_declared_symbol_is_exported(lib):
     assert set(names) == set(api.EXPORTS)
     for n in names:
         assert hasattr(lib, n), n
+
+
+def test_debug_header_is_separate_and_exported(lib):
+    """Measurement / tuning aids live in dustin_debug.h, none of them in the product header."""
+    names = declared_functions("dustin_debug.h")
+    assert set(names) == set(api.DEBUG_EXPORTS)
+    assert not set(names) & set(declared_functions())
+    for n in names:
+        assert hasattr(lib, n), n
+    assert api.tune_get(api.KNOB_PDL) == 1
+    api.tune_set(api.KNOB_PDL, 0)
+    assert api.tune_get(api.KNOB_PDL) == 0
+    api.tune_set(api.KNOB_PDL, 1)
+    assert api.tune_get(999) == 0
+
+
+def test_library_reads_no_environment_variable(lib):
+    """No object of csrc/ references getenv (the statically linked CUDA runtime does, for its own settings)."""
+    import glob
+    import subprocess
+    objs = sorted(glob.glob(os.path.join(os.path.dirname(api.LIB_PATH), "build", "*.o")))
+    assert objs
+    out = subprocess.run(["nm", "--undefined-only", *objs], capture_output=True, text=True).stdout
+    assert "getenv" not in out
 
 
 def test_version_and_status_strings(lib):
