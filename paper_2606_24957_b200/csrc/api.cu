@@ -64,7 +64,7 @@ float scale_log2_of(const dustin_shape_t* s) {
 // ---- scoring plan ---------------------------------------------------------------------------------------------
 // Tokens per scoring CTA (all scored KV groups of those tokens): as large as possible while the grid still holds >= 8
 // CTAs per SM (of the current device: 148 on B200), never below 256.  group_slots = how many groups the 8 warps of a CTA serve side by side;
-// n_parts = softmax partials per (sequence, head) = CTAs per sequence x warps per group.
+// n_parts = softmax partials per (sequence, head) = CTAs per sequence.
 void score_plan(int batch, int n_groups, int max_ctx, int* chunk_tokens, int* n_parts, int* group_slots) {
     int slots = 1;
     while (slots < n_groups && slots < 8) slots <<= 1;
@@ -78,24 +78,31 @@ void score_plan(int batch, int n_groups, int max_ctx, int* chunk_tokens, int* n_
     // A grid a little above one wave (3 resident CTAs per SM) pays a whole second wave for the overhang: between one
     // and three waves use exactly one (measured at B = 16: 8k 64.5 -> 54.6 us, 16k unchanged, 32k stays at 4.6 waves).
     const long long resident = (long long)sms * 3;
-    if (ctas(chunk) > resident && ctas(chunk) < 3 * resident && batch <= resident) {
+    // One or two scored KV groups (the packed subset): the 8 warps of a CTA share a group, so a 256-token CTA gives each
+    // warp two tiles and the fixed cost per CTA dominates: one wave of larger CTAs (measured, B = 16, 32k, one group:
+    // 38 -> 31 us).
+    if (((ctas(chunk) > resident && ctas(chunk) < 3 * resident) || (slots <= 2 && ctas(chunk) > resident)) &&
+        batch <= resident) {
         const int per_seq = (int)(resident / batch);
         const int quantum = 16 * (8 / slots);
         chunk = ((max_ctx + per_seq - 1) / per_seq + quantum - 1) / quantum * quantum;
         if (chunk < 256) chunk = 256;
     }
+    const int forced = knob(DUSTIN_KNOB_SCORE_CHUNK);   // tuning aid: tokens per scoring CTA (multiple of 128)
+    if (forced >= 128) chunk = (forced + 127) / 128 * 128;
     *chunk_tokens = chunk;
     *group_slots = slots;
-    *n_parts = (max_ctx > 0 ? (max_ctx + chunk - 1) / chunk : 1) * (8 / slots);
+    *n_parts = max_ctx > 0 ? (max_ctx + chunk - 1) / chunk : 1;   // one partial per (CTA, head): the warps of a CTA that
+                                                                  // share a KV group fold theirs before writing
 }
 
 struct ScoreWs {
     size_t logits, part, stats, total;
 };
 ScoreWs score_ws(int batch, int nsel, int max_ctx) {
-    // upper bound of the partial count: the smallest chunk (256 tokens) x 8 warps of one group
+    // upper bound of the partial count: one per CTA at the smallest chunk (256 tokens)
     const size_t stride = ((size_t)max_ctx + 3) & ~(size_t)3;
-    const size_t n_chunks = (((size_t)max_ctx + 255) / 256 + 1) * 8;
+    const size_t n_chunks = ((size_t)max_ctx + 255) / 256 + 1;
     ScoreWs w;
     w.logits = 0;
     w.part = align256(w.logits + (size_t)batch * nsel * stride * sizeof(float));
@@ -297,6 +304,14 @@ int run_select(int32_t batch, int32_t max_ctx, const int32_t* seq_lens, const du
     if (norm) p.norm = *norm;
     p.draft_mask = draft_mask;
     p.draft_mask_stride = (long long)select_mask_words(max_ctx);
+    p.trace = nullptr;
+    if (mode == 2 && norm) {   // few long rows: one thread-block cluster per row (select_cluster.cu)
+        const int C = select_cluster_size(p);
+        if (C > 0) {
+            const cudaError_t e = launch_select_cluster(p, C, stream);
+            return e == cudaSuccess ? DUSTIN_OK : fail_cuda(e);
+        }
+    }
     const cudaError_t e = launch_select(p, stream, mode);
     return e == cudaSuccess ? DUSTIN_OK : fail_cuda(e);
 }
@@ -484,9 +499,21 @@ int dustin_verify_layer_fused(const dustin_shape_t* shape, const dustin_kv_t* kv
     // With enough rows to fill the GPU the selection kernel normalises and accumulates its own rows (no separate
     // stats / normalise launches, no extra pass over the scores); it needs 16-byte rows and no scores_now output.
     SelectParams::Norm norm;
-    const bool rows_in_select = !scores_now_out && (shape->max_ctx & 3) == 0 && shape->max_ctx > 0 &&
-                                (((uintptr_t)hist_inout | (uintptr_t)s_draft) & 15) == 0 &&
-                                (long long)shape->batch * select->n_lists >= 64 && !fused_rows_disabled();
+    bool rows_in_select = !scores_now_out && (shape->max_ctx & 3) == 0 && shape->max_ctx > 0 &&
+                          (((uintptr_t)hist_inout | (uintptr_t)s_draft) & 15) == 0 && !fused_rows_disabled();
+    if (rows_in_select && (long long)shape->batch * select->n_lists < 64) {
+        // few rows: worth it only when a thread-block cluster shares each row (one CTA per row would push the logits of
+        // every head of the list through a single SM)
+        SelectParams probe;
+        std::memset(&probe, 0, sizeof probe);
+        probe.batch = shape->batch;
+        probe.n_lists = select->n_lists;
+        probe.max_ctx = shape->max_ctx;
+        probe.s_target = hist_inout;
+        probe.draft_mask = draft_mask;
+        probe.norm.logits = reinterpret_cast<const float*>(base);   // non-null marker: the rows will be materialised
+        rows_in_select = hoist && select_cluster_size(probe) > 0;
+    }
     rc = run_score(shape, kv, q, (int64_t)shape->n_new * shape->n_q_heads * shape->head_dim, shape->head_dim,
                    head_mask, select->n_lists, scores_now_out, hist_inout, alpha, ws, ws_bytes, st,
                    rows_in_select ? &norm : nullptr, 1, 0, hoist);

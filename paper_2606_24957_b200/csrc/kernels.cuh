@@ -16,7 +16,7 @@ struct ScoreParams {
     float scale_log2;        // sm_scale * log2(e): logits live in the log2 domain
     int nsel;                // |subset|; ordinals follow ascending head index, so a KV group's heads are contiguous
     int n_groups;            // KV groups holding >= 1 subset head (the only K rows that are read)
-    int chunk_tokens, n_chunks;     // tokens per scoring CTA; softmax partials per (sequence, head) = CTAs x sub-ranges
+    int chunk_tokens, n_chunks;     // tokens per scoring CTA; softmax partials per (sequence, head) = CTAs per sequence
     int group_slots;                // scored KV groups served side by side by the 8 warps of a CTA: 1, 2, 4 or 8
     int defer_wait;                 // fused call with a hoisted draft tier: the kernel launched just before this one is the
                                     // draft-tier selection, whose results a1 does not need -- the dependency wait moves from
@@ -76,6 +76,10 @@ struct SelectParams {
 // of the fused call, which it releases at once), 2 = target tier + list (reads p.draft_mask).
 cudaError_t launch_select(const SelectParams& p, cudaStream_t stream, int mode = 0);
 size_t select_mask_words(int max_ctx);   // words per row of SelectParams::draft_mask
+// Few long rows (select_cluster.cu): the target tier (mode 2, with row materialisation) by one thread-block cluster per
+// row.  select_cluster_size: CTAs per row, or 0 when one CTA per row serves better / the shape does not qualify.
+int select_cluster_size(const SelectParams& p);
+cudaError_t launch_select_cluster(const SelectParams& p, int C, cudaStream_t stream);
 
 // ---- a4 / a5 ------------------------------------------------------------------------------------------------
 struct AttnParams {

@@ -73,6 +73,7 @@ __device__ __forceinline__ void frag_tile(KFrag<D>& f, const unsigned char* stag
 template <int D>
 __global__ void __launch_bounds__(kScoreThreads, 3) score_logits_kernel(const ScoreParams p) {
     extern __shared__ __align__(128) unsigned char s_ring[];   // [warp][stage][16 tokens][D] bf16
+    __shared__ float2 s_part[kScoreWarps][8];                   // per-warp softmax partials of the (<= 8) heads of its group
     const int chunk = blockIdx.x, b = blockIdx.y;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int g = lane >> 2, c = lane & 3;
@@ -173,9 +174,28 @@ __global__ void __launch_bounds__(kScoreThreads, 3) score_logits_kernel(const Sc
             m1 = n1m;
         }
         if (g == 0) {
-            const long long part = (long long)chunk * n_sub + ws;
-            if (h0) p.part[((long long)b * p.nsel + first + 2 * c) * p.n_chunks + part] = make_float2(m0, s0);
-            if (h1) p.part[((long long)b * p.nsel + first + 2 * c + 1) * p.n_chunks + part] = make_float2(m1, s1);
+            if (n_sub == 1) {   // one warp per KV group: its partial is the CTA's
+                if (h0) p.part[((long long)b * p.nsel + first + 2 * c) * p.n_chunks + chunk] = make_float2(m0, s0);
+                if (h1) p.part[((long long)b * p.nsel + first + 2 * c + 1) * p.n_chunks + chunk] = make_float2(m1, s1);
+            } else {            // several warps share the group (each took every n_sub-th tile): folded below
+                s_part[warp][2 * c] = make_float2(m0, s0);
+                s_part[warp][2 * c + 1] = make_float2(m1, s1);
+            }
+        }
+    }
+    if (n_sub > 1) {
+        // Fewer than eight scored KV groups: the warps ws = 0 .. n_sub-1 of a group fold their partials in that order, so
+        // that the CTA leaves ONE partial per head (the consumers fold n_chunks of them per head; with a single scored
+        // group that is an eighth of what it would be).  slots >= n_groups here, so the loop above ran at most once.
+        __syncthreads();
+        const int gi = warp;   // warps 0 .. slots-1 (ws == 0) finish the groups 0 .. slots-1
+        if (gi < p.n_groups && gi < slots && lane < p.group_cnt[gi]) {
+            float m = -INFINITY, s = 0.f;
+            for (int i = 0; i < n_sub; ++i) {
+                const float2 o = s_part[gi + slots * i][lane];
+                softmax_merge(m, s, o.x, o.y);
+            }
+            p.part[((long long)b * p.nsel + p.group_first[gi] + lane) * p.n_chunks + chunk] = make_float2(m, s);
         }
     }
     // Fused call with a hoisted draft tier: ONE CTA -- the last of the grid, dispatched in the last wave -- waits for the
@@ -267,7 +287,7 @@ __global__ void __launch_bounds__(256) fuse_kernel(int max_ctx, const int* __res
 cudaError_t launch_score(const ScoreParams& p, float* scores_now, float* hist, float alpha, bool logits_only,
                          cudaStream_t stream) {
     cudaError_t e0 = cudaSuccess;
-    dim3 grid(p.n_chunks / (kScoreWarps / p.group_slots), p.batch);   // n_chunks counts partials: CTAs x sub-ranges
+    dim3 grid(p.n_chunks, p.batch);   // one softmax partial per (CTA, head)
     {
         ProfScope prof(kKernScoreLogits, stream);
         const int smem = kScoreWarps * kStages * kTileTokens * p.head_dim * 2;

@@ -17,6 +17,10 @@ __device__ __forceinline__ void sel_ts(unsigned long long* row, int slot) {
     }
 }
 
+// Threshold bins of at most this many entries are ranked by brute force (list_select_ranged); fuller ones cost another
+// histogram pass (two more block-wide barriers), which showed as the slow tail of the kernel at 32.
+constexpr int kSmallList = 128;
+
 struct SelShared {
     uint32_t hist[kBins];
     uint32_t warp_tot[kSelWarps + 1];
@@ -25,7 +29,7 @@ struct SelShared {
     // scratch of the sampled path: two copies used alternately (parity of a per-thread phase counter), so one barrier
     // between a write and its reads is enough
     uint32_t tot_db[2][kSelWarps], min_db[2][kSelWarps], max_db[2][kSelWarps], res_db[2][4];
-    uint32_t small_n, small_key[32], small_idx[32];
+    uint32_t small_n, small_key[kSmallList], small_idx[kSmallList];
     float2 stats[64];   // (M, 1/Z) of the heads feeding this row (row materialisation)
     unsigned long long* trace;   // this CTA's 64 timestamp slots, or nullptr (read and written by thread 0 only)
     int trace_base;              // first slot of the tier in progress
@@ -507,7 +511,7 @@ __device__ __forceinline__ int range_shift(uint32_t kmin, uint32_t kmax) {
 // Exact selection on the candidate list by an OFFSET radix select: a pass spreads the current key range
 // [klo, khi] (first pass: the list's own minimum and maximum) over the 2048 bins, so the scores of one row -- which
 // share their leading exponent bits -- do not pile up in a handful of bins (same-address shared atomics serialise).
-// A threshold bin of <= 32 entries is then ranked by brute force ((key desc, index asc) order, which also settles
+// A threshold bin of <= kSmallList entries is then ranked by brute force ((key desc, index asc) order, which also settles
 // ties); a fuller one becomes the range of the next pass.  Admits the `rank` best of the n_list entries.
 template <int kPer>   // entries per thread: n_list <= kPer * kSelThreads
 __device__ void list_select_ranged(const float* __restrict__ s, const SelLayout& L, int n_list, uint32_t rank,
@@ -556,7 +560,7 @@ __device__ void list_select_ranged(const float* __restrict__ s, const SelLayout&
             if (((part >> e) & 1u) && (key[e] < nlo || key[e] > nhi)) part &= ~(1u << e);
         klo = nlo;
         khi = nhi;
-        if (eq_total <= 32u) {
+        if (eq_total <= (uint32_t)kSmallList) {
 #pragma unroll
             for (int e = 0; e < kPer; ++e)
                 if ((part >> e) & 1u) {
@@ -621,7 +625,7 @@ __device__ __forceinline__ void select_from_list(const float* __restrict__ s, co
                                                  uint32_t rank, SelShared& sh, Phase& ph) {
     if (n_list <= 2048)
         list_select_ranged<2048 / kSelThreads>(s, L, n_list, rank, sh, ph);
-    else if (kSelThreads < 1024 && n_list <= 3072)
+    else if (n_list <= 3072)   // the tail of the list-length distribution at rank ~900: not worth the 8192-entry variant
         list_select_ranged<3072 / kSelThreads>(s, L, n_list, rank, sh, ph);
     else
         list_select_ranged_big(s, L, n_list, rank, sh, ph);
@@ -636,9 +640,11 @@ __device__ __forceinline__ void select_from_list(const float* __restrict__ s, co
 //      no atomics;  (c) exact selection on the list (list_select_ranged).
 // Returns false (nothing admitted) when the list came out too short or too long; the caller then takes path (2).
 // On entry hist (replica 0) must be all zero; it is left all zero.
+// pre (optional): the row is one chunk and the caller already holds it in registers in exactly this layout
+// (materialize_row<true>): the first read of the row is skipped.
+constexpr int kVecPerChunk = 8;
 __device__ bool sampled_tier_vec(const float* __restrict__ s, int lo, int hi, int rank, const SelLayout& L,
-                                 SelShared& sh, Phase& ph) {
-    constexpr int kVecPerChunk = 8;
+                                 SelShared& sh, Phase& ph, const float4* pre = nullptr) {
     const float4* s4 = reinterpret_cast<const float4*>(s);
     const int t = threadIdx.x;
     const int v0 = lo >> 2, v_end = (hi + 3) >> 2;
@@ -672,7 +678,12 @@ __device__ bool sampled_tier_vec(const float* __restrict__ s, int lo, int hi, in
     }
     int n_slots;
     if (one) {
-        load_chunk(0);
+        if (pre != nullptr) {
+#pragma unroll
+            for (int u = 0; u < kVecPerChunk; ++u) x[u] = pre[u];
+        } else {
+            load_chunk(0);
+        }
         const int u_s = t & 7, e_s = (t >> 3) & 3;
         float4 xv = x[0];
 #pragma unroll
@@ -780,14 +791,15 @@ __device__ __noinline__ void fallback_tier(const float* __restrict__ s, int lo, 
 
 template <bool VEC>
 __device__ __forceinline__ void select_tier(const float* __restrict__ s, int lo, int hi, int rank, const SelLayout& L,
-                                            int n_words, SelShared& sh, Phase& ph, bool& hist_clean) {
+                                            int n_words, SelShared& sh, Phase& ph, bool& hist_clean,
+                                            const float4* pre = nullptr) {
     if (VEC) {
         if (!hist_clean) {
             clear_hist(L.hist, 1);
             __syncthreads();
         }
         hist_clean = true;
-        if (sampled_tier_vec(s, lo, hi, rank, L, sh, ph)) return;
+        if (sampled_tier_vec(s, lo, hi, rank, L, sh, ph, pre)) return;
         hist_clean = false;   // the paths below leave their counts behind
         __syncthreads();
     }
@@ -925,21 +937,8 @@ __device__ __forceinline__ void select_row(const SelectParams& p, int b, int l, 
     int* out = p.idx_out + ((long long)b * p.n_lists + l) * p.k_max;
     int* cnt_out = p.cnt_out + (long long)b * p.n_lists + l;
 
-    const bool own_row = MODE != kSelDraft && VEC && p.norm.logits != nullptr;   // this CTA computes its target row itself
-    if (own_row) materialize_row(p, b, l, N, sh);
-    sel_ts(tr, 2);
-    if (k > p.k_max || k < p.n_sink + p.n_recent) {   // argument error on this row (dustin.h)
-        if (MODE == kSelDraft) return;
-        for (int i = threadIdx.x; i < p.k_max; i += kSelThreads) out[i] = -1;
-        if (threadIdx.x == 0) *cnt_out = 0;
-        return;
-    }
-    if (k >= N) {   // everything is selected (reading A12)
-        if (MODE == kSelDraft) return;
-        for (int i = threadIdx.x; i < p.k_max; i += kSelThreads) out[i] = i < N ? i : -1;
-        if (threadIdx.x == 0) *cnt_out = N;
-        return;
-    }
+    const bool invalid = k > p.k_max || k < p.n_sink + p.n_recent;   // argument error on this row (dustin.h)
+    const bool all = k >= N;                                          // everything is selected (reading A12)
     const int S = min(p.n_sink, N), W = min(p.n_recent, N - S);
     const int lo = S, hi = N - W;                       // candidate range [lo, hi)
     const int c = k - S - W;
@@ -956,24 +955,44 @@ __device__ __forceinline__ void select_row(const SelectParams& p, int b, int l, 
     L.cap = p.list_cap;
     uint32_t* mem = L.mem;
     uint32_t* gmask = p.draft_mask + ((long long)b * p.n_lists + l) * p.draft_mask_stride;
-    if (MODE == kSelTarget) {
-        // I_prot U I_draft as the draft-tier kernel left it (plain loads: that grid has completed and flushed)
-        for (int w = threadIdx.x; w < n_words; w += kSelThreads) mem[w] = gmask[w];
-    } else {
-        // I_prot = I_sink U I_window
-        for (int w = threadIdx.x; w < n_words; w += kSelThreads) {
-            uint32_t bits = 0;
-            const int n0 = w * 32;
-            if (n0 < S) bits |= (S - n0 >= 32) ? 0xffffffffu : ((1u << (S - n0)) - 1u);
-            if (n0 + 32 > hi) {   // window [hi, N) and, for now, the tail [N, 32 * n_words) of the last word
-                const int from = max(hi - n0, 0);
-                bits |= ~((1u << from) - 1u);
+    if (!invalid && !all) {
+        if (MODE == kSelTarget) {
+            // I_prot U I_draft as the draft-tier kernel left it (plain loads: that grid has completed and flushed); requested
+            // before the row is materialised, so the trip overlaps it
+            for (int w = threadIdx.x; w < n_words; w += kSelThreads) mem[w] = gmask[w];
+        } else {
+            // I_prot = I_sink U I_window
+            for (int w = threadIdx.x; w < n_words; w += kSelThreads) {
+                uint32_t bits = 0;
+                const int n0 = w * 32;
+                if (n0 < S) bits |= (S - n0 >= 32) ? 0xffffffffu : ((1u << (S - n0)) - 1u);
+                if (n0 + 32 > hi) {   // window [hi, N) and, for now, the tail [N, 32 * n_words) of the last word
+                    const int from = max(hi - n0, 0);
+                    bits |= ~((1u << from) - 1u);
+                }
+                mem[w] = bits;
             }
-            mem[w] = bits;
         }
+        if (VEC) clear_hist(L.hist, 1);
+    }
+    // Fused call: this CTA computes its target row itself (a1's normalisation + Eq. 5), for every row -- also those
+    // that need no selection.
+    const bool own_row = MODE != kSelDraft && VEC && p.norm.logits != nullptr;
+    if (own_row) materialize_row(p, b, l, N, sh);
+    sel_ts(tr, 2);
+    if (invalid) {
+        if (MODE == kSelDraft) return;
+        for (int i = threadIdx.x; i < p.k_max; i += kSelThreads) out[i] = -1;
+        if (threadIdx.x == 0) *cnt_out = 0;
+        return;
+    }
+    if (all) {
+        if (MODE == kSelDraft) return;
+        for (int i = threadIdx.x; i < p.k_max; i += kSelThreads) out[i] = i < N ? i : -1;
+        if (threadIdx.x == 0) *cnt_out = N;
+        return;
     }
     bool hist_clean = VEC;
-    if (VEC) clear_hist(L.hist, 1);
     __syncthreads();
 
     // tier 0: I_draft = TopK(S_Draft \ I_prot, m);  tier 1: I_target = TopK(S_Target \ (I_prot U I_draft), k-m-|I_prot|)
@@ -981,7 +1000,8 @@ __device__ __forceinline__ void select_row(const SelectParams& p, int b, int l, 
     for (int tier = (MODE == kSelTarget ? 1 : 0); tier < (MODE == kSelDraft ? 1 : 2); ++tier) {
         const int want = tier == 0 ? m : c - m;
         if (threadIdx.x == 0) sh.trace_base = 16 + 16 * tier;
-        if (want > 0) select_tier<VEC>(tier == 0 ? sd : st, lo, hi, want, L, n_words, sh, ph, hist_clean);
+        if (want > 0)
+            select_tier<VEC>(tier == 0 ? sd : st, lo, hi, want, L, n_words, sh, ph, hist_clean);
         sel_ts(tr, 3 + tier);
     }
     if (MODE == kSelDraft) {
@@ -998,16 +1018,34 @@ __device__ __forceinline__ void select_row(const SelectParams& p, int b, int l, 
     uint32_t total;
     uint32_t pos = block_excl_scan(mine, sh, &total);
     sel_ts(tr, 5);
+    // The list is assembled in shared memory (the candidate-list area is free now) and leaves in 16-byte stores; lists
+    // that do not fit there, or unaligned output rows, are written entry by entry.
+    const bool staged = VEC && (uint32_t)p.k_max <= 2u * (uint32_t)L.cap && (p.k_max & 3) == 0 &&
+                        (reinterpret_cast<uintptr_t>(out) & 15) == 0;
+    int* dst = staged ? reinterpret_cast<int*>(L.list_key) : out;
     for (int w = w_lo; w < w_hi; ++w) {
         uint32_t bits = mem[w];
+        if (bits == 0xffffffffu) {   // sink and window words: 32 independent stores instead of a dependent bit chain
+#pragma unroll 8
+            for (int j = 0; j < 32; ++j)
+                if (pos + j < (uint32_t)p.k_max) dst[pos + j] = w * 32 + j;
+            pos += 32;
+            continue;
+        }
         while (bits) {
             const int bit = __ffs(bits) - 1;
             bits &= bits - 1;
-            if (pos < (uint32_t)p.k_max) out[pos] = w * 32 + bit;
+            if (pos < (uint32_t)p.k_max) dst[pos] = w * 32 + bit;
             ++pos;
         }
     }
-    for (int i = (int)total + threadIdx.x; i < p.k_max; i += kSelThreads) out[i] = -1;
+    for (int i = (int)total + threadIdx.x; i < p.k_max; i += kSelThreads) dst[i] = -1;
+    if (staged) {
+        __syncthreads();
+        const int4* src4 = reinterpret_cast<const int4*>(dst);
+        int4* out4 = reinterpret_cast<int4*>(out);
+        for (int i = threadIdx.x; i < p.k_max / 4; i += kSelThreads) out4[i] = src4[i];
+    }
     if (threadIdx.x == 0) *cnt_out = (int)total;
 }
 

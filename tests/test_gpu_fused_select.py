@@ -17,11 +17,16 @@ from tests import harness as H
 pytestmark = pytest.mark.gpu
 
 
-@pytest.fixture(params=["hoist", "no_hoist"])
+@pytest.fixture(params=["hoist", "no_hoist", "cluster2", "cluster4", "cluster8", "no_cluster"])
 def hoist(request):
-    api.tune_set(api.KNOB_DRAFT_HOIST, 1 if request.param == "hoist" else 0)
+    """Which kernels serve the selection of the one-shot call: the draft tier hoisted beside a1 (default) or not; the
+    target tier by one CTA per row or by a thread-block cluster of 2 / 4 / 8 CTAs per row (select_cluster.cu; by default
+    only few-row shapes take it: forced here on every shape)."""
+    api.tune_set(api.KNOB_DRAFT_HOIST, 0 if request.param == "no_hoist" else 1)
+    api.tune_set(api.KNOB_SELECT_SPLIT, {"cluster2": 2, "cluster4": 4, "cluster8": 8, "no_cluster": 1}.get(request.param, 0))
     yield request.param
     api.tune_set(api.KNOB_DRAFT_HOIST, 1)
+    api.tune_set(api.KNOB_SELECT_SPLIT, 0)
 
 
 def many_rows_cases():
