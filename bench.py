@@ -164,6 +164,18 @@ class Workload:
             self.api.score_heads(self.shape, self.kv[s], self.q[l][:, 0], self.cfg.head_mask, self.cfg.n_lists,
                                  self.scratch_scores, self.ws)
 
+    def step_score_all_heads(self):
+        """The Naive estimator of PAPER.md:297-299 (Fig. 8): a1 with EVERY query head in the subset, every layer."""
+        c = self.cfg
+        if not hasattr(self, "scratch_scores"):
+            self.scratch_scores = torch.empty_like(self.hist[0])
+        if not hasattr(self, "ws_all"):
+            self.ws_all = self.api.alloc_workspace(self.shape, (1 << c.n_q_heads) - 1, self.k_max)
+        for l in range(self.L):
+            s = l % self.n_sets
+            self.api.score_heads(self.shape, self.kv[s], self.q[l][:, 0], (1 << c.n_q_heads) - 1, c.n_lists,
+                                 self.scratch_scores, self.ws_all)
+
     def step_attn_only(self):
         """a4 alone in every layer, each with the index lists its own fused pass left in idx[l] / cnt[l] (kernel-only
         timing of the gathered attention: the region holds nothing but L launches of that kernel)."""
@@ -320,21 +332,22 @@ def profile_steps(api, step_fn, steps: int) -> dict:
 
 
 class E2E:
-    """The same step driven from HOST buffers: every step copies each layer's Q / K_new / V_new and the draft
-    scores from pinned host memory, runs the layer, and copies the layer's output (and the last layer's index
-    lists) back to pinned host memory.  Copies run on their own streams and overlap the kernels layer by layer.
-    The KV cache and the historical scores are resident state of the decode loop (like weights), not step inputs."""
+    """The same step driven from HOST buffers: every step copies each layer's Q / K_new / V_new from pinned host
+    memory, runs the layer, and copies the layer's output (and the last layer's index lists) back to pinned host
+    memory.  Copies run on their own streams and overlap the kernels layer by layer.  The KV cache, the historical
+    scores and the draft scores are device-resident state of the decode loop, not step inputs: S_Draft is what
+    dustin_draft_aggregate leaves on the device (Eq. 5, first line), like the cache the draft model wrote."""
 
     def __init__(self, w: Workload):
         self.w = w
         pin = lambda t: torch.empty(t.shape, dtype=t.dtype, device="cpu", pin_memory=True).copy_(t)
-        self.h_q, self.h_kn, self.h_vn, self.h_sd = pin(w.q), pin(w.k_new), pin(w.v_new), pin(w.s_draft)
+        self.h_q, self.h_kn, self.h_vn = pin(w.q), pin(w.k_new), pin(w.v_new)
         self.h_out = torch.empty(w.out.shape, dtype=w.out.dtype, device="cpu", pin_memory=True)
         self.h_idx = torch.empty(w.idx[0].shape, dtype=torch.int32, device="cpu", pin_memory=True)
         self.h_cnt = torch.empty(w.cnt[0].shape, dtype=torch.int32, device="cpu", pin_memory=True)
         self.s_in, self.s_out = torch.cuda.Stream(), torch.cuda.Stream()
         nb = lambda t: t.numel() * t.element_size()
-        self.h2d = nb(self.h_q) + nb(self.h_kn) + nb(self.h_vn) + nb(self.h_sd)
+        self.h2d = nb(self.h_q) + nb(self.h_kn) + nb(self.h_vn)
         self.d2h = nb(self.h_out) + nb(self.h_idx) + nb(self.h_cnt)
 
     def step(self):
@@ -346,8 +359,6 @@ class E2E:
         ready = []
         with torch.cuda.stream(self.s_in):
             for l in range(w.L):
-                if l < w.n_sets:        # the draft scores of set l are first needed by layer l: copy them just in time,
-                    w.s_draft[l].copy_(self.h_sd[l], non_blocking=True)   # so layer 0 does not wait for all of them
                 w.q[l].copy_(self.h_q[l], non_blocking=True)
                 w.k_new[l].copy_(self.h_kn[l], non_blocking=True)
                 w.v_new[l].copy_(self.h_vn[l], non_blocking=True)
@@ -379,12 +390,15 @@ def measured_peak():
 
 
 def ncu_traffic(kernel: str):
-    """DRAM bytes per launch of `kernel` from the committed ncu --set full summary (profiles/traffic.json)."""
+    """(DRAM bytes per launch of `kernel`, commit the capture was taken at) from the committed ncu --set full summary
+    (profiles/traffic.json: dram__bytes_read.sum + dram__bytes_write.sum of one capture; stale once the kernel changes,
+    hence the commit stamp that travels with it)."""
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            return json.load(f).get(kernel)
+            d = json.load(f)
+        return d.get(kernel), d.get("captured_at_commit")
     except Exception:
-        return None
+        return None, None
 
 
 def graphed(step_fn):
@@ -399,33 +413,51 @@ def graphed(step_fn):
 # --------------------------------------------------------------------------------------------------------------
 # CPU baseline: the oracle as it stands, on the host cores, on a bounded sample of the same workload
 # --------------------------------------------------------------------------------------------------------------
-def oracle_layer(ref, cfg: synth.Config, inp: synth.LayerInputs):
-    """One layer of the path through oracle/ (O1 -> O2 -> O3 -> O4).  `inp` on the CPU."""
+def oracle_layer(ref, cfg: synth.Config, inp: synth.LayerInputs, stage_s: dict = None):
+    """One layer of the path through oracle/ (O1 -> O2 -> O3 -> O4).  `inp` on the CPU.  stage_s (optional) receives the
+    wall time of each stage in seconds (appended to lists)."""
+    def timed(name, fn):
+        t0 = time.perf_counter()
+        r = fn()
+        if stage_s is not None:
+            stage_s.setdefault(name, []).append(time.perf_counter() - t0)
+        return r
     kv = ref.KV.contiguous_nhd(inp.k, inp.v, inp.seq_lens)
-    a = ref.score_heads(kv, inp.q[:, 0], cfg.head_mask, cfg.n_lists, cfg.n_kv_heads, cfg.ctx)
-    h = ref.fuse_scores(a, inp.hist, 1.0, inp.seq_lens)
-    idx, cnt = ref.topk_select(inp.s_draft, h, cfg.budget, cfg.n_sink, cfg.n_recent, cfg.m_num, cfg.m_den,
-                               inp.k_max, inp.seq_lens, inp.budgets)
-    out, _ = ref.sparse_verify_attn(kv, inp.q, inp.k_new, inp.v_new, idx, cnt, cfg.ctx)
+    a = timed("O1_score_heads", lambda: ref.score_heads(kv, inp.q[:, 0], cfg.head_mask, cfg.n_lists, cfg.n_kv_heads, cfg.ctx))
+    h = timed("O2_fuse_scores", lambda: ref.fuse_scores(a, inp.hist, 1.0, inp.seq_lens))
+    idx, cnt = timed("O3_topk_select", lambda: ref.topk_select(inp.s_draft, h, cfg.budget, cfg.n_sink, cfg.n_recent,
+                                                               cfg.m_num, cfg.m_den, inp.k_max, inp.seq_lens, inp.budgets))
+    out, _ = timed("O4_sparse_verify_attn", lambda: ref.sparse_verify_attn(kv, inp.q, inp.k_new, inp.v_new, idx, cnt, cfg.ctx))
     return out
 
 
 def cpu_baseline(cfg: synth.Config, inp_cpu: synth.LayerInputs, budget_s: float = 15.0) -> dict:
+    """The oracle as it stands on the host cores: ONE full-size layer, repeated within ~budget_s, median; per-stage
+    medians beside it; the dense full-cache oracle (a5) once (SURVEY.md section 8d "Oracle timing")."""
     from oracle import ref
+    stage_s = {}
     t0 = time.perf_counter()
-    oracle_layer(ref, cfg, inp_cpu)
+    oracle_layer(ref, cfg, inp_cpu, stage_s)
     t1 = time.perf_counter() - t0
     n = max(1, min(8, int(budget_s / max(t1, 1e-3)) - 1))
     times = [t1]
     for _ in range(n):
         t0 = time.perf_counter()
-        oracle_layer(ref, cfg, inp_cpu)
+        oracle_layer(ref, cfg, inp_cpu, stage_s)
         times.append(time.perf_counter() - t0)
     us = 1e6 * statistics.median(times)
+    kv = ref.KV.contiguous_nhd(inp_cpu.k, inp_cpu.v, inp_cpu.seq_lens)
+    t0 = time.perf_counter()
+    ref.sparse_verify_attn(kv, inp_cpu.q, inp_cpu.k_new, inp_cpu.v_new, None, None, cfg.ctx)
+    dense_us = 1e6 * (time.perf_counter() - t0)
     return {"value": us, "unit": UNIT, "cores": ref.threads(), "kind": "oracle",
             "sample": f"{len(times)} repetitions of ONE full-size layer (all {cfg.batch} sequences, N={cfg.ctx}; "
                       f"O1 scoring -> O2 fusion -> O3 selection -> O4 attention), median; a step is "
-                      f"{cfg.n_layers} such layers"}
+                      f"{cfg.n_layers} such layers",
+            "stages_us_per_layer": {k: round(1e6 * statistics.median(v), 1) for k, v in stage_s.items()},
+            "dense_us_per_layer": round(dense_us, 1),
+            "dense_sample": "the dense full-cache oracle (O4 with idx = NULL) on the same layer, timed once",
+            "build": "g++ -O2 -fopenmp (oracle/ref.py), fp64, as it stands"}
 
 
 def run_reference(args, dist: Dist):
@@ -450,7 +482,8 @@ def run_reference(args, dist: Dist):
         "impl": "reference", "metric": METRIC, "value": us, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": us / 1e3, "higher_is_better": False, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": workload_config(cfg, 1, "oracle: one layer per step (bounded sample of the L-layer step)"),
+        "config": workload_config(cfg, 1),
+        "run": {"sample": "oracle: ONE full-size layer per step (a bounded sample of the L-layer step)"},
         "cpu_baseline": {"value": us, "unit": UNIT, "cores": ref.threads(), "kind": "oracle",
                          "sample": "each step = ONE full-size layer of the workload through oracle/ (O1..O4)"},
         "e2e": {"value": us, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -465,17 +498,24 @@ def headline_config(args) -> synth.Config:
     return cfg
 
 
-def workload_config(cfg: synth.Config, n_sets: int, note: str, world: int = 1) -> dict:
+def workload_config(cfg: synth.Config, world: int = 1) -> dict:
+    """What is measured -- the same dict in both arms (ours and --impl reference); how each arm runs it is in `run`."""
     return {"workload": "BASELINE.json configs[2]: Qwen2.5-72B-shaped verification step "
                         f"(B={cfg.batch}, N={cfg.ctx}, Hq={cfg.n_q_heads}, Hkv={cfg.n_kv_heads}, d={cfg.head_dim}, "
                         f"gamma={cfg.gamma}, k={cfg.budget} incl. {cfg.n_sink} sink + {cfg.n_recent} recent, "
                         f"|H|={len(cfg.heads)} subset heads {'spread one per KV group' if cfg.n_lists > 1 else 'packed in one KV group'}, "
                         f"G={cfg.n_lists} lists per sequence, L={cfg.n_layers} layers)",
             "schedule": "every layer runs a1 scoring -> a2 fusion -> a3 top-k -> a4 sparse attention (north_star)",
-            "global_batch": cfg.batch * world, "batch_per_gpu": cfg.batch, "seq_len": cfg.ctx, "layers": cfg.n_layers, "budget": cfg.budget,
-            "distinct_kv_caches": n_sets,
-            "l2": "inputs exceed L2: layers cycle over distinct 2.1 GB K/V caches, none is re-read within 126 MB",
-            "launch": "one CUDA graph replay per step (the L fused C-ABI calls captured once)", "note": note}
+            "global_batch": cfg.batch * world, "batch_per_gpu": cfg.batch, "seq_len": cfg.ctx, "layers": cfg.n_layers,
+            "budget": cfg.budget,
+            "l2": "inputs exceed L2: every layer has a 2.1 GB K/V cache, none is re-read within 126 MB"}
+
+
+def run_info(n_sets: int, world: int) -> dict:
+    return {"distinct_kv_caches": n_sets,
+            "launch": "one CUDA graph replay per step (the L fused C-ABI calls captured once)",
+            "scaling": "weak: every rank runs this workload on its own batch (value = max-over-ranks us per layer of the "
+                       "whole job's global batch)", "world": world}
 
 
 def measure_workload(api, cfg: synth.Config, n_sets: int, steps: int, warmup: int, dist: Dist, device,
@@ -527,7 +567,8 @@ def run_sweep(api, args, dist: Dist, device):
     for label, ctx, batch, gamma, budget in grid:
         cfg = synth.config_qwen72b(batch=batch, ctx=ctx, n_layers=L, gamma=gamma, budget=budget)
         points.append(sweep_point(api, cfg, n_sets, dist, device, peak,
-                                  {"series": label, "ctx": ctx, "batch": batch, "gamma": gamma, "budget": budget}))
+                                  {"series": label, "ctx": ctx, "batch": batch, "gamma": gamma, "budget": budget},
+                                  naive=(label == "fixed-2048" and gamma == 4)))
         torch.cuda.empty_cache()
     cfg = synth.config_paged(n_layers=4)
     points.append(sweep_point(api, cfg, 2, dist, device, peak,
@@ -535,20 +576,50 @@ def run_sweep(api, args, dist: Dist, device):
                                "gamma": cfg.gamma, "budget": "6.25% of N_b", "page_size": cfg.page_size}))
     if dist.rank == 0:
         print(json.dumps({"sweep": points, "unit": "us per layer (graph-replayed, CUDA events)",
-                          "peak_gbs": peak, "layers_per_point": L}), flush=True)
+                          "peak_gbs": peak, "layers_per_point": L, "crossover": crossover(points)}), flush=True)
 
 
-def sweep_point(api, cfg: synth.Config, n_sets: int, dist: Dist, device, peak: float, tag: dict) -> dict:
+def crossover(points) -> dict:
+    """Context length at which the fused sparse layer costs what the dense baseline costs (log-linear interpolation of
+    dense/fused over the context points of one series at gamma = 4): below it the method's fixed costs lose."""
+    out = {}
+    for series in ("fixed-2048", "6.25%"):
+        pts = sorted((p["ctx"], p["speedup_vs_dense"]) for p in points
+                     if p.get("series") == series and p.get("gamma") == 4 and isinstance(p.get("ctx"), int))
+        x = None
+        for (c0, r0), (c1, r1) in zip(pts, pts[1:]):
+            if (r0 - 1.0) * (r1 - 1.0) <= 0 and r0 != r1:
+                import math
+                x = int(round(math.exp(math.log(c0) + (1.0 - r0) / (r1 - r0) * (math.log(c1) - math.log(c0)))))
+                break
+        out[series] = {"fused_equals_dense_at_ctx": x,
+                       "note": None if x else ("fused faster than dense at every point" if pts and pts[0][1] > 1
+                                               else "no crossing inside the sweep")}
+    return out
+
+
+def sweep_point(api, cfg: synth.Config, n_sets: int, dist: Dist, device, peak: float, tag: dict,
+                naive: bool = False) -> dict:
+    """One workload point: graph-replayed regions that hold one kind of launch each -- the fused layer (a1..a4), scoring
+    alone (a1), sparse verification alone (a4, on the lists of the fused pass), the dense baseline (a5) and, with
+    naive=True, scoring with EVERY head in the subset (the Naive estimator of PAPER.md:297-299)."""
     w = Workload(cfg, n_sets, device)
     w.step_every_layer()
     w.step_dense()
     w.step_score_only()
     by = w.bytes_per_layer()
     t = {}
-    for name, fn in (("fused", w.step_every_layer), ("score", w.step_score_only), ("attn", w.step_attn_only),
-                     ("dense", w.step_dense)):
+    legs = [("fused", w.step_every_layer), ("score", w.step_score_only), ("attn", w.step_attn_only),
+            ("dense", w.step_dense)]
+    if naive:
+        w.step_score_all_heads()
+        legs.append(("score_all_heads", w.step_score_all_heads))
+    for name, fn in legs:
         t[name] = 1e3 * time_steps(graphed(fn), 3, 3, dist, device) / cfg.n_layers
     out = dict(tag)
+    if naive:
+        out["score_all_heads_us"] = round(t["score_all_heads"], 2)
+        out["score_all_heads_over_dense"] = round(t["score_all_heads"] / t["dense"], 3)
     out.update({
         "fused_us": round(t["fused"], 2), "score_us": round(t["score"], 2), "sparse_attn_us": round(t["attn"], 2),
         "dense_us": round(t["dense"], 2), "speedup_vs_dense": round(t["dense"] / t["fused"], 2),
@@ -559,6 +630,100 @@ def sweep_point(api, cfg: synth.Config, n_sets: int, dist: Dist, device, peak: f
     })
     del w
     return out
+
+
+def run_loop(api, args, dist: Dist, device):
+    """Multi-step decode loop (PAPER.md:153 accept -> append -> next step): per speculative
+    step, on the device with no host synchronisation inside a step,
+      dustin_draft_aggregate (S_Draft from a Qwen2.5-0.5B-shaped draft: 14 / 2 heads, d = 64, 3 layers x 4 heads, Gamma
+      lookahead queries -- PAPER.md:395)  ->  dustin_verify_layer_fused in each of L target layers (history H carried per
+      layer)  ->  dustin_append_kv of the accepted rows into every target-layer cache and every draft-layer cache.
+    Accept lengths are seeded synthetic draws with mean ~2.2 tokens per step (tau of PAPER.md:315-319, Table 2); the
+    context N_b grows by them.  Reports attention-path us per step, per layer and per accepted token."""
+    L, n_steps, B = args.loop_layers, args.loop_steps, args.batch
+    cfg = synth.config_qwen72b(B, args.ctx, L)
+    T, G, Hkv, d = cfg.n_new, cfg.n_lists, cfg.n_kv_heads, cfg.head_dim
+    N0 = args.ctx - n_steps * T                              # room for every step's appends below max_ctx
+    g = torch.Generator(device=device)
+    g.manual_seed(cfg.seed + 77)
+    layers = []
+    for l in range(L):
+        inp = synth.make_layer(cfg, l, device)
+        inp.planted = None
+        layers.append(inp)
+    shape = api.Shape(B, cfg.n_q_heads, Hkv, d, T, cfg.ctx, 0.0)
+    select = api.Select(cfg.budget, cfg.n_sink, cfg.n_recent, cfg.m_num, cfg.m_den, G, None)
+    seq_lens = torch.full((B,), N0, dtype=torch.int32, device=device)
+    kvs = [api.KV.contiguous_nhd(x.k, x.v, seq_lens) for x in layers]
+    hist = torch.stack([x.hist for x in layers])
+    for x in layers:
+        x.hist = None
+    ws = api.alloc_workspace(shape, cfg.head_mask, layers[0].k_max)
+    out = torch.zeros_like(layers[0].q)
+    idx = torch.full((B, G, layers[0].k_max), -1, dtype=torch.int32, device=device)
+    cnt = torch.zeros((B, G), dtype=torch.int32, device=device)
+    # draft model (PAPER.md:395): 3 selected layers x 4 heads, Gamma lookahead queries, its own K caches
+    dHq, dHkv, dd, dL, dmask = 14, 2, 64, 3, 0b00101000100010
+    dshape = api.Shape(B, dHq, dHkv, dd, cfg.gamma, cfg.ctx, 0.0)
+    dk = [torch.randn(B, cfg.ctx, dHkv, dd, device=device, generator=g).bfloat16() for _ in range(dL)]
+    dq = [torch.randn(B, cfg.gamma, dHq, dd, device=device, generator=g).bfloat16() for _ in range(dL)]
+    dkn = torch.randn(B, T, dHkv, dd, device=device, generator=g).bfloat16()
+    dkvs = [api.KV.contiguous_nhd(k, k, seq_lens) for k in dk]          # V of the draft is not read by this path
+    dws = api.alloc_draft_workspace(dshape, dmask)
+    s_draft = torch.zeros(B, cfg.ctx, device=device)
+    # accept lengths: 1 + Binomial(Gamma, p) with mean 2.2 accepted tokens per step (the bonus token always lands)
+    p_acc = (2.2 - 1.0) / cfg.gamma
+    accepts = (1 + (torch.rand(n_steps, B, cfg.gamma, device=device, generator=g) < p_acc).sum(-1)).to(torch.int32)
+    n_app = torch.zeros(B, dtype=torch.int32, device=device)
+    scratch = torch.zeros_like(seq_lens)
+    dshape_T = api.Shape(B, dHq, dHkv, dd, T, cfg.ctx, 0.0)      # the draft's verify block has T rows too
+
+    def step():
+        api.draft_aggregate(dshape, dkvs, dq, dmask, s_draft, dws)
+        for l in range(L):
+            x = layers[l]
+            api.verify_layer_fused(shape, kvs[l], x.q, x.k_new, x.v_new, cfg.head_mask, s_draft, hist[l], 1.0, select,
+                                   out, idx, cnt, ws)
+        # accept -> append (PAPER.md:153).  dustin_append_kv advances the lengths it is given; all caches share one set of
+        # lengths, so every call but the last works on a scratch copy and the last one advances the live lengths.
+        caches = [(shape, api.KV.contiguous_nhd(x.k, x.v, None), x.k_new, x.v_new, hist[l]) for l, x in enumerate(layers)]
+        caches += [(dshape_T, api.KV.contiguous_nhd(k, k, None), dkn, dkn, None) for k in dk]
+        for i, (sh_, kv_, kn_, vn_, h_) in enumerate(caches):
+            if i < len(caches) - 1:
+                scratch.copy_(seq_lens)
+                api.append_kv(sh_, kv_, scratch, kn_, vn_, n_app, h_)
+            else:
+                api.append_kv(sh_, kv_, seq_lens, kn_, vn_, n_app, h_)
+
+    # warm-up step on a scratch copy of the lengths is not possible without touching the caches: the first step is
+    # simply not timed
+    per_step = []
+    total_acc = 0
+    for sidx in range(n_steps):
+        n_app.copy_(accepts[sidx])
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        step()
+        e1.record()
+        torch.cuda.synchronize()
+        if sidx >= 1:
+            per_step.append(1e3 * e0.elapsed_time(e1))
+            total_acc += int(accepts[sidx].sum())
+    lens_end = seq_lens.cpu().tolist()
+    med = statistics.median(per_step)
+    res = {"decode_loop": {
+        "workload": f"Qwen2.5-72B-shaped target ({L} layers with their own caches), Qwen2.5-0.5B-shaped draft (3 layers x 4 "
+                    f"heads, Gamma={cfg.gamma}), B={B}, N_b {N0} -> {lens_end[0]}..{max(lens_end)}, k={cfg.budget}",
+        "steps_timed": len(per_step), "accepted_tokens_per_step_per_sequence": round(total_acc / len(per_step) / B, 3),
+        "us_per_step": round(med, 1), "us_per_step_min_max": [round(min(per_step), 1), round(max(per_step), 1)],
+        "us_per_layer": round(med / L, 2),
+        "us_per_accepted_token": round(med * len(per_step) / max(total_acc / B, 1e-9), 1),
+        "what": "draft_aggregate + L x verify_layer_fused + (L + 3) x append_kv per step, eager launches on one stream, CUDA "
+                "events around each step, the first step untimed; acceptance is a seeded draw (no models here)"}}
+    if dist.rank == 0:
+        print(json.dumps(res), flush=True)
+    return res
 
 
 def run_arr(api, args, dist: Dist, device):
@@ -624,6 +789,9 @@ def main():
     ap.add_argument("--no-extras", action="store_true", help="skip the secondary workloads and the CPU baseline")
     ap.add_argument("--arr", action="store_true", help="ARR read-out of the selection policies on the drift workload")
     ap.add_argument("--sweep", action="store_true", help="context / gamma / budget sweep (configs[3]) + paged (configs[4])")
+    ap.add_argument("--loop", action="store_true", help="multi-step decode loop: draft aggregate -> L fused layers -> append")
+    ap.add_argument("--loop-layers", type=int, default=8)
+    ap.add_argument("--loop-steps", type=int, default=12)
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     dist = Dist()
@@ -644,8 +812,8 @@ def main():
         dist.barrier()
     api.lib()
 
-    if args.sweep or args.arr:
-        (run_sweep if args.sweep else run_arr)(api, args, dist, device)
+    if args.sweep or args.arr or args.loop:
+        (run_sweep if args.sweep else (run_arr if args.arr else run_loop))(api, args, dist, device)
         dist.finish()
         return
     cfg = rank_seed(headline_config(args), dist.rank)
@@ -669,10 +837,13 @@ def main():
     def roof(kernel, nbytes, us=None, how="CUDA event pair around each launch, second pass over the same steps"):
         us = kern[kernel][0] if us is None else us
         ach = nbytes / us / 1e3
+        traffic, traffic_commit = ncu_traffic(kernel)
         return {"kernel": kernel, "bound": "hbm", "achieved": round(ach, 1), "peak": peak, "unit": "GB/s",
-                "frac": round(ach / peak, 4), "traffic": ncu_traffic(kernel), "peak_source": peak_src,
+                "frac": round(ach / peak, 4), "traffic": traffic, "traffic_commit": traffic_commit,
+                "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": nbytes, "avg_launch_us": round(us, 3),
-                "share_of_step": round(share[kernel] / sum(share.values()), 4),
+                # share of the GRAPH-timed step: this kernel's launches x its average duration over the step time
+                "share_of_step": round(kern[kernel][0] * kern[kernel][1] / (1e3 * r["ms_per_step"]), 4),
                 "timed_with": how}
     roofline = roof(dom, kbytes.get(dom, by["a1_k"]))
     fused_gbs = by["fused_must_read"] / us_layer / 1e3
@@ -681,14 +852,15 @@ def main():
         "metric": METRIC, "value": round(us_layer, 3), "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": round(r["ms_per_step"], 4), "higher_is_better": False,
         "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-        "config": workload_config(cfg, w.n_sets, "weak scaling: every rank runs this workload on its own batch "
-                                  "(value = max-over-ranks us per layer of the whole job's global batch)", dist.world),
+        "config": workload_config(cfg, dist.world),
+        "run": run_info(w.n_sets, dist.world),
         "aggregate": aggregate(us_layer, cfg, dist.world),
         "clocks": r["clocks"],
         "e2e": {"value": round(1e3 * e2e_ms / L, 3), "unit": UNIT, "h2d_bytes_per_step": e2e.h2d,
                 "d2h_bytes_per_step": e2e.d2h, "ms_per_step": round(e2e_ms, 4),
-                "what": "Q/K_new/V_new of every layer + draft scores copied from pinned host memory, outputs of "
-                        "every layer + last index lists copied back, copy streams overlapped with the kernels"},
+                "what": "Q/K_new/V_new of every layer copied from pinned host memory, outputs of every layer + last "
+                        "index lists copied back, copy streams overlapped with the kernels; KV cache, history and draft "
+                        "scores (what dustin_draft_aggregate leaves on the device) are device-resident state"},
         "gpu_launches": int(r["launches_per_step"] * args.steps),
         "roofline": roofline,
         "roofline_attn": roof("attn_kernel", by["a4"], r["attn_only_us_per_launch"],
@@ -751,6 +923,22 @@ def main():
             }
             del w2
             torch.cuda.empty_cache()
+        # BASELINE.json configs[3] (the two ends of the context sweep, gamma 8 once, the Naive all-head estimator at 4k
+        # and 32k) and configs[4] (paged, ragged): 8 layers over 4 distinct caches each, graph-replayed per leg.
+        # The full grid is `bench.py --sweep` (profiles/r02_sweep.json).
+        pts = []
+        for tag, c, naive in (
+                ({"point": "configs[3] 4k, B=16, gamma 4, k=2048"}, synth.config_qwen72b(16, 4096, 8), True),
+                ({"point": "configs[3] 32k, B=16, gamma 8, k=2048"}, synth.config_qwen72b(16, 32768, 8, gamma=8), False),
+                ({"point": "configs[3] 32k, B=16, gamma 4, k=2048 (+ all-head scoring)"}, synth.config_qwen72b(16, 32768, 8), True),
+                ({"point": "configs[3] 128k, B=4, gamma 4, k=2048"}, synth.config_qwen72b(4, 131072, 8), False),
+                ({"point": "configs[3] 128k, B=4, gamma 4, k=8192 (6.25 %)"}, synth.config_qwen72b(4, 131072, 8, budget=8192), False)):
+            pts.append(sweep_point(api, c, 4, dist, device, peak, tag, naive=naive))
+            torch.cuda.empty_cache()
+        pts.append(sweep_point(api, synth.config_paged(n_layers=4), 2, dist, device, peak,
+                               {"point": "configs[4] paged (page 16) ragged U[8k,64k], B=32, Llama-3-8B-shaped, k_b = 6.25 % of N_b"}))
+        torch.cuda.empty_cache()
+        extras["sweep_points"] = pts
         line["other_workloads"] = extras
 
     if dist.rank == 0:

@@ -88,8 +88,12 @@ __global__ void __launch_bounds__(kScoreThreads, 3) score_logits_kernel(const Sc
     // K is read exactly once: evict_first keeps the stream from displacing the logits scratch, the score rows and the
     // selection state that the following kernels (and the draft-tier selection running beside this one) read from L2
     const uint64_t policy = l2_policy_evict_first();
+    // Ragged batches: a sequence of N tokens is shared by only as many of its gridDim.x CTAs as it has chunk_tokens-sized
+    // pieces (the others find no tile and just leave their empty partials), so that a short sequence does not shrink the
+    // work per CTA to a tile or two (measured on the paged ragged workload: 5.0 TB/s against 6.0 contiguous).
+    const int n_active = max(1, min((int)gridDim.x, (N + p.chunk_tokens - 1) / p.chunk_tokens));
     const int chunk_lo = chunk * (kScoreWarps / p.group_slots) * kTileTokens;
-    const int chunk_hi = N;
+    const int chunk_hi = chunk < n_active ? N : 0;
 
     for (int gi = warp % slots; gi < p.n_groups; gi += slots) {
         const int grp = p.group_id[gi], first = p.group_first[gi], nh = p.group_cnt[gi];
@@ -114,7 +118,7 @@ __global__ void __launch_bounds__(kScoreThreads, 3) score_logits_kernel(const Sc
         constexpr int kTileBytes = kTileTokens * D * 2;
         unsigned char* ring = s_ring + warp * (kStages * kTileBytes);
         const uint32_t ring_u32 = smem_u32(ring);
-        const int step = (int)gridDim.x * n_sub * kTileTokens;
+        const int step = n_active * n_sub * kTileTokens;
         int n0 = chunk_lo + ws * kTileTokens;
         __syncwarp();                                        // the previous group's reads of the ring are done
         if (n0 < chunk_hi) issue_tile<D>(ring_u32, p, b, grp, n0, N, lane, policy);

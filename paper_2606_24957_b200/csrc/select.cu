@@ -86,7 +86,8 @@ cudaError_t launch_select(const SelectParams& p_in, cudaStream_t stream, int mod
     // row is in flight at once and a CTA leaves room for two scoring CTAs on its SM (measured: CTAs of that footprint cost
     // a1 ~1 us of 171; so do up to 32 whole SMs taken away).  With few rows, the fast 1024-thread kernel, one SM per row.
     const int n_rows = p.n_lists * p.batch;
-    const bool light = mode == 1 && n_rows > device_sm_count() / 6 && p.max_ctx <= (1 << 18);
+    // (up to 32 SMs given up cost the scoring kernel 1-2 us; 48 cost it 13)
+    const bool light = mode == 1 && n_rows > 32 && p.max_ctx <= (1 << 18);
     select_plan(p.max_ctx, light, &p.mask_words, &p.replicas, &p.list_cap);
     const size_t smem = select_smem_bytes(p.max_ctx, light);
     p.trace = nullptr;

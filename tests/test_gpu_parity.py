@@ -103,6 +103,28 @@ def test_dense_baseline_matches_oracle(name):
     assert torch.allclose(lse.cpu().double(), lse_ref, atol=2e-3, rtol=0)
 
 
+@pytest.mark.parametrize("shape_name,n_lists", [("qwen", 8), ("qwen", 1), ("llama", 8), ("llama", 1)])
+def test_naive_all_head_estimator_matches_oracle(shape_name, n_lists):
+    """The Naive estimator of PAPER.md:297-299 (Fig. 8: scores materialised from ALL heads) is stage a1 with a full head
+    mask: 64 heads / 8 KV groups (Qwen2.5-72B shape) and 32 / 8 (Llama-3-8B shape), per-KV-head and global lists."""
+    from oracle import ref
+    base = synth.config_qwen72b() if shape_name == "qwen" else synth.config_llama8b()
+    cfg = synth.shrink(base, batch=2, ctx=2600, budget=300, n_sink=8, n_recent=32, heads=tuple(range(base.n_q_heads)),
+                       n_lists=n_lists)
+    cpu, dev = _both(cfg)
+    assert cfg.head_mask == (1 << cfg.n_q_heads) - 1
+    sh = H.shape_of(cfg)
+    ws = api.alloc_workspace(sh, cfg.head_mask, dev.k_max)
+    scores = torch.full((cfg.batch, n_lists, cfg.ctx), float("nan"), device="cuda")
+    api.score_heads(sh, H.gpu_kv(dev), dev.q[:, 0], cfg.head_mask, n_lists, scores, ws)
+    torch.cuda.synchronize()
+    want = ref.score_heads(H.cpu_kv(cpu), cpu.q[:, 0], cfg.head_mask, n_lists, cfg.n_kv_heads, cfg.ctx)
+    H.check_scores(scores, want, "all-head scores")
+    # every head's softmax row sums to one: a list's scores sum to the number of heads that feed it
+    heads_per_list = cfg.n_q_heads if n_lists == 1 else cfg.group
+    assert torch.allclose(scores.sum(-1).cpu(), torch.full((cfg.batch, n_lists), float(heads_per_list)), rtol=1e-4)
+
+
 def test_budget_equal_context_reproduces_dense():
     """k = N: the sparse call with the full index list must equal the dense call (PAPER.md:92 ARR = 1)."""
     cfg = synth.shrink(CASES["llama_spread"], ctx=1111, budget=1111, n_sink=4, n_recent=8)
