@@ -134,6 +134,14 @@ class Workload:
         self.ws = api.alloc_workspace(self.shape, c.head_mask, 0)        # sized for the dense baseline too
         self.dense_out = torch.zeros_like(self.out[0])
 
+    def cnt_arg(self, l: int):
+        """List lengths for a stand-alone a4 call.  One budget k <= N for all sequences and no ragged lengths: every list
+        holds exactly k entries, which is what cnt = NULL states (dustin.h) -- the fused call derives the same fact from
+        its select parameters.  Otherwise the lengths the selection wrote."""
+        s0 = self.sets[0]
+        uniform = s0.seq_lens is None and s0.budgets is None and self.k_max <= self.cfg.ctx and self.cfg.budget == self.k_max
+        return None if uniform else self.cnt[l]
+
     # -- schedules ---------------------------------------------------------------------------------------------
     def layer_fused(self, l: int):
         s = l % self.n_sets
@@ -152,7 +160,7 @@ class Workload:
         for l in range(1, self.L):
             s = l % self.n_sets
             self.api.sparse_verify_attn(self.shape, self.kv[s], self.q[l], self.k_new[l], self.v_new[l],
-                                        self.idx[0], self.cnt[0], self.out[l], self.ws)
+                                        self.idx[0], self.cnt_arg(0), self.out[l], self.ws)
 
     def step_score_only(self):
         """a1 alone in every layer (scores_now written to a scratch tensor): the estimation cost of PAPER.md:297."""
@@ -182,7 +190,7 @@ class Workload:
         for l in range(self.L):
             s = l % self.n_sets
             self.api.sparse_verify_attn(self.shape, self.kv[s], self.q[l], self.k_new[l], self.v_new[l],
-                                        self.idx[l], self.cnt[l], self.out[l], self.ws)
+                                        self.idx[l], self.cnt_arg(l), self.out[l], self.ws)
 
     def step_gather_probe(self):
         """The memory side of a4 alone: dustin_probe_gather reads the rows step_attn_only gathers, nothing else."""

@@ -144,7 +144,9 @@ int dustin_topk_select(int32_t batch, int32_t max_ctx, const int32_t* seq_lens, 
  * (causal among the T new tokens, self included), scale sm_scale;  out = sum p * V.
  * idx == NULL: all N_b cached rows (full-cache verification attention, the dense baseline).
  *   q: device bf16 [B,T,Hq,d];  k_new, v_new: device bf16 [B,T,Hkv,d];  idx: device int32 [B,n_lists,k_max]
- *   (entries in [0,N_b), any order);  cnt: device int32 [B,n_lists];  out: device bf16 [B,T,Hq,d];
+ *   (entries in [0,N_b), any order);  cnt: device int32 [B,n_lists], or NULL = every list holds exactly k_max entries
+ *   (needs k_max <= max_ctx and kv->seq_lens == NULL; the kernel then plans its work without reading a length from
+ *   memory, which shortens its start);  out: device bf16 [B,T,Hq,d];
  *   lse_out: device fp32 [B,Hq,T] natural-log normaliser, or NULL. */
 int dustin_sparse_verify_attn(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q, const void* k_new,
                               const void* v_new, const int32_t* idx, const int32_t* cnt, int32_t n_lists,

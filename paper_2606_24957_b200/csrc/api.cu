@@ -318,7 +318,7 @@ int run_select(int32_t batch, int32_t max_ctx, const int32_t* seq_lens, const du
 
 int run_attn(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q, const void* k_new,
              const void* v_new, const int32_t* idx, const int32_t* cnt, int32_t n_lists, int32_t k_max, void* out,
-             float* lse_out, void* ws, size_t ws_bytes, cudaStream_t stream) {
+             float* lse_out, void* ws, size_t ws_bytes, cudaStream_t stream, int uniform_cnt = -1) {
     int rc = check_shape(shape);
     if (rc) return rc;
     AttnParams p;
@@ -328,10 +328,15 @@ int run_attn(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q, 
     if (!q || !k_new || !v_new || !out) return DUSTIN_ERR_INVALID_ARG;
     if (((uintptr_t)q | (uintptr_t)k_new | (uintptr_t)v_new | (uintptr_t)out) & 15) return DUSTIN_ERR_INVALID_ARG;
     if (idx) {
-        if (!cnt || k_max <= 0 || (n_lists != 1 && n_lists != shape->n_kv_heads)) return DUSTIN_ERR_INVALID_ARG;
+        if (k_max <= 0 || (n_lists != 1 && n_lists != shape->n_kv_heads)) return DUSTIN_ERR_INVALID_ARG;
+        if (!cnt) {   // cnt == NULL: every list holds exactly k_max entries (dustin.h)
+            if (k_max > shape->max_ctx || kv->seq_lens) return DUSTIN_ERR_INVALID_ARG;
+            uniform_cnt = k_max;
+        }
     } else {
         n_lists = 1;
         k_max = 0;
+        uniform_cnt = kv->seq_lens ? -1 : shape->max_ctx;   // dense baseline over full-length sequences
     }
     const int max_tokens = idx ? (k_max < shape->max_ctx ? k_max : shape->max_ctx) : shape->max_ctx;
     const AttnWs w = attn_ws(shape, max_tokens > 0 ? max_tokens : 1);
@@ -341,6 +346,7 @@ int run_attn(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q, 
     p.v_new = static_cast<const __nv_bfloat16*>(v_new);
     p.idx = idx;
     p.cnt = cnt;
+    p.uniform_cnt = uniform_cnt;
     p.batch = shape->batch;
     p.n_q_heads = shape->n_q_heads;
     p.n_kv_heads = shape->n_kv_heads;
@@ -522,9 +528,12 @@ int dustin_verify_layer_fused(const dustin_shape_t* shape, const dustin_kv_t* kv
     rc = run_select(shape->batch, shape->max_ctx, kv->seq_lens, select, s_draft, draft_list_stride, hist_inout,
                     idx_out, cnt_out, k_max, st, rows_in_select ? &norm : nullptr, hoist ? 2 : 0, draft_mask);
     if (rc) return rc;
-    // a4
+    // a4.  One budget for all sequences and no ragged lengths: every list will hold min(k, N) entries (Eq. 6 with the
+    // clipping of reading A12), which the attention kernel then need not read back to plan its work.
+    const int uniform_cnt = (!select->budgets && !kv->seq_lens)
+                                ? (select->budget < shape->max_ctx ? select->budget : shape->max_ctx) : -1;
     return run_attn(shape, kv, q, k_new, v_new, idx_out, cnt_out, select->n_lists, k_max, out, lse_out,
-                    ws, ws_bytes, st);
+                    ws, ws_bytes, st, uniform_cnt);
 }
 
 int dustin_probe_gather(const dustin_shape_t* shape, const dustin_kv_t* kv, const int32_t* idx, const int32_t* cnt,

@@ -71,7 +71,7 @@ __global__ void __launch_bounds__(32 * MT * KS) attn_kernel(const AttnParams p) 
     const int list = p.n_lists == 1 ? 0 : gkv;
     // a caller-supplied cnt is clamped to [0, k_max] as in the tcgen05 kernel: the same inputs behave the same in both
     const int n_sel = MODE == kDense ? seq_len_of(p.kv.seq_lens, b, p.max_ctx)
-                                     : max(0, min(p.cnt[b * p.n_lists + list], p.k_max));
+                                     : (p.cnt ? max(0, min(p.cnt[b * p.n_lists + list], p.k_max)) : p.uniform_cnt);
     const int range_lo = split * p.split_tokens;
     const int n_range = max(0, min(p.split_tokens, n_sel - range_lo));
     const int nt = n_range + (split == 0 ? T : 0);        // this CTA's tokens: cache rows, then the new rows

@@ -2,8 +2,9 @@
 // Sparse verification attention over the selected KV (App. G :568) and, with idx == nullptr, the
 // full-cache verification baseline.  DESIGN.md section 5.1.
 //
-// Decomposition ("stream-K" over tokens).  A unit is one (sequence b, KV head g): its token list is the cnt[b,l]
-// selected cache rows followed by the T new draft rows.  The token lists of all units are laid end to end and cut
+// Decomposition ("stream-K" over tokens).  A unit is one (sequence b, KV head g): its token list is the tile of the T new
+// draft rows (needs no index list, so it is worked through while the first gathered rows travel) followed by the cnt[b,l]
+// selected cache rows.  The token lists of all units are laid end to end and cut
 // into gridDim.x equal ranges, one persistent CTA per SM; a CTA therefore works on a few SEGMENTS (pieces of
 // units).  A unit that lies inside one CTA is written straight to `out`; otherwise each piece leaves a normalised
 // partial (o, lse) in the workspace and the LAST piece to finish (a per-unit arrival counter) merges them in
@@ -30,7 +31,8 @@ namespace dustin {
 
 namespace {
 
-constexpr int kTcThreads = 384;        // three warpgroups: softmax | producers | MMA issuer (+ 3 idle warps)
+constexpr int kTcThreads = 384;        // three warpgroups: softmax | producers | MMA issuer + resolvers (+ 1 idle warp);
+                                       // wide rows: a fourth, the second softmax warpgroup
 constexpr int kTile = 128;            // tokens per tile (UMMA M)
 constexpr int kD = 128;               // head_dim served by this kernel
 constexpr int kSlotBytes = kTile * kD * 2;   // 32 KB: one K or V tile
@@ -205,8 +207,8 @@ __device__ __forceinline__ void tr_reduce(float (&v)[NV], int lane, int& row_bas
 // ---- shared-memory plan --------------------------------------------------------------------------------------------
 template <int NQ>
 struct TcCfg {
-    static constexpr int kSlotsN = NQ <= 32 ? 6 : 5;
-    static constexpr int kQBufs = NQ <= 64 ? 2 : 1;      // wide rows: one Q buffer buys the fifth K/V slot
+    static constexpr int kSlotsN = NQ <= 48 ? 6 : 5;
+    static constexpr int kQBufs = NQ <= 32 ? 2 : 1;      // 48 rows and more: one Q buffer buys another K/V slot
     static constexpr int kQBytes = NQ * kD * 2;          // one Q buffer, [64-dim half][row][128 B] swizzled
     static constexpr int kPBytes = NQ * kTile * 2;       // P^T, [8-row block][token][16 B]
     static constexpr int kOffSlots = 0;
@@ -218,13 +220,14 @@ struct TcCfg {
     static constexpr int kOffDlt = kOffFac + NQ * 4;                      // float dlt[NQ]: m_old - m_new of a reference move
     static constexpr int kOffWarp = kOffDlt + NQ * 4;                     // float [4][NQ]: per-warp maxima / sums
     static constexpr int kOffWgt = kOffWarp + 4 * NQ * 4;                 // float [kMergeFast][NQ]: merge weights
-    static constexpr int kOffRowTab = (kOffWgt + kMergeFast * NQ * 4 + 15) & ~15;   // {K row, V row} addresses, 4 x 32
-    static constexpr int kOffRowOff = kOffRowTab + 128 * 16;              // int row -> element offset inside out[b]
+    static constexpr int kOffRowTab = (kOffWgt + kMergeFast * NQ * 4 + 15) & ~15;   // {K row, V row} addresses, 2 tiles
+    static constexpr int kOffRowOff = kOffRowTab + 2 * kTile * 16;        // int row -> element offset inside out[b]
     static constexpr int kOffScan = kOffRowOff + NQ * 4;                  // int [16] warp totals / maxima of the scan
     static constexpr int kOffBar = (kOffScan + 16 * 4 + 8 + 7) & ~7;      // uint64 barriers
-    static constexpr int kNumBar = 2 * kSlotsN + 10;
+    static constexpr int kNumBar = 2 * kSlotsN + 14;
     static constexpr int kOffTmem = kOffBar + kNumBar * 8;                // uint32 TMEM base, uint32 combine flag
-    static constexpr int kSmemBytes = kOffTmem + 16;
+    static constexpr int kOffTs = kOffTmem + 16;                          // uint32 [64] timeline samples (trace knob)
+    static constexpr int kSmemBytes = kOffTs + 256;
     static_assert(kSmemBytes <= 232448, "shared-memory plan exceeds 227 KB");
     static_assert(kOffQ % 1024 == 0 && kQBytes % 1024 == 0 && kOffP % 1024 == 0, "UMMA operands need 1 KB alignment");
 };
@@ -233,7 +236,8 @@ struct TcCfg {
 // Piece of one unit's token list that falls into this CTA's range of the concatenated token space.
 struct Seg {
     int u, b, g, list;
-    int cnt;              // cache rows of the unit (its token list is cnt cache rows, then T new rows)
+    int cnt;              // cache rows of the unit.  Its token list: positions [0, kTile) = the tile of the T new rows
+                          // (the rest of it padding), positions kTile + j = cache row j of the list
     int pos_lo, pos_hi;   // this piece: token positions [pos_lo, pos_hi) of the unit
     int n_tiles;
     int whole;            // the piece is the entire unit: the result goes straight to `out`
@@ -243,7 +247,7 @@ struct Seg {
 
 struct TileCursor {
     const int* prefix;
-    int n_units, n_kv, n_lists, n_new, lo, hi, chunk;
+    int n_units, n_kv, n_lists, lo, hi, chunk;
     int next_u;
     Seg s;
     int ti;        // tile index inside the segment
@@ -259,25 +263,28 @@ struct TileCursor {
         s.b = next_u / n_kv;
         s.g = next_u - s.b * n_kv;
         s.list = n_lists == 1 ? 0 : s.g;
-        s.cnt = pe - ps - n_new;
+        s.cnt = pe - ps - kTile;
         s.pos_lo = max(lo, ps) - ps;
         s.pos_hi = min(hi, pe) - ps;
         s.n_tiles = (s.pos_hi - s.pos_lo + kTile - 1) / kTile;
         s.whole = (s.pos_lo == 0 && s.pos_hi == pe - ps) ? 1 : 0;
         s.slot = ps <= lo ? 0 : 1;
-        s.cta_first = ps / chunk;
+        s.cta_first = (ps + kTile - 1) / chunk;   // cuts inside the new-row tile are moved to the unit's start (snap_cut)
         s.cta_last = (pe - 1) / chunk;
         ++next_u;
         return true;
     }
-    __device__ __forceinline__ void init(const int* prefix_, int n_units_, int n_kv_, int n_lists_, int n_new_, int lo_,
-                                         int hi_, int chunk_, int u0) {
-        prefix = prefix_; n_units = n_units_; n_kv = n_kv_; n_lists = n_lists_; n_new = n_new_;
+    __device__ __forceinline__ void init(const int* prefix_, int n_units_, int n_kv_, int n_lists_, int lo_, int hi_,
+                                         int chunk_, int u0) {
+        prefix = prefix_; n_units = n_units_; n_kv = n_kv_; n_lists = n_lists_;
         lo = lo_; hi = hi_; chunk = chunk_; next_u = u0;
         ti = 0; seg_no = 0;
         valid = load_seg();
     }
     __device__ __forceinline__ bool last_tile() const { return ti == s.n_tiles - 1; }
+    // The tile of the unit's new rows (positions [0, kTile)): no piece starts inside it (make_plan), so it is exactly the
+    // first tile of a piece that starts its unit.  Every other tile holds gathered cache rows only.
+    __device__ __forceinline__ bool new_tile() const { return s.pos_lo == 0 && ti == 0; }
     __device__ __forceinline__ void advance() {
         if (++ti >= s.n_tiles) {
             ti = 0;
@@ -286,6 +293,44 @@ struct TileCursor {
         }
     }
 };
+
+// ---- plan -------------------------------------------------------------------------------------------------------
+// Range [lo, hi) of the concatenated token space that the CTA of range id `rid` works through, and the first unit in
+// it.  prefix(u) = start of unit u (prefix(n_units) = total); unit_of(x) = largest u with prefix(u) <= x.
+struct Plan {
+    int lo, hi, u0, chunk;
+    bool whole;   // every CTA takes one whole unit
+};
+template <class PrefixFn, class UnitOfFn>
+__device__ __forceinline__ Plan make_plan(PrefixFn prefix, UnitOfFn unit_of, int n_units, int longest, int grid, int rid,
+                                          bool force_stream) {
+    Plan pl;
+    const int total = prefix(n_units);
+    pl.chunk = (((total + grid - 1) / grid) + 31) & ~31;
+    // Few units of similar length (at most one per CTA, the longest not much above the even share): every CTA
+    // takes one WHOLE unit -- no partials, no merge, one epilogue -- and the memory system, not the idle SMs, sets
+    // the pace.  Otherwise: equal token ranges (stream-K).
+    pl.whole = n_units <= grid && longest <= total / grid + 4 * kTile && !force_stream;
+    pl.u0 = 0;
+    if (pl.whole) {
+        pl.lo = rid < n_units ? prefix(rid) : total;
+        pl.hi = rid < n_units ? prefix(rid + 1) : total;
+        pl.u0 = min(rid, n_units - 1);
+    } else {
+        // A cut that falls inside the new-row tile of a unit moves down to the unit's start, so that no piece begins in
+        // the padding of that tile (its first tile would hold nothing visible to some query rows).  Seg::cta_first agrees.
+        auto snap_cut = [&](long long x) -> int {
+            if (x >= total) return total;
+            const int ps = prefix(unit_of((int)x));
+            return (int)x - ps < kTile ? ps : (int)x;
+        };
+        const long long c0 = (long long)rid * pl.chunk;
+        pl.lo = snap_cut(c0);
+        pl.hi = snap_cut(c0 + pl.chunk);
+        if (pl.lo < pl.hi) pl.u0 = unit_of(pl.lo);
+    }
+    return pl;
+}
 
 // ---- kernel -----------------------------------------------------------------------------------------------------
 struct TcWs {
@@ -300,12 +345,23 @@ __device__ __forceinline__ unsigned long long gtimer() {
     asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
     return t;
 }
-#define TS(slot) do { if (ws.dbg_ts) ws.dbg_ts[(size_t)blockIdx.x * 64 + (slot)] = gtimer(); } while (0)
+__device__ __forceinline__ uint32_t clock32() {
+    uint32_t t;
+    asm volatile("mov.u32 %0, %clock;" : "=r"(t));
+    return t;
+}
+// Timeline samples (DUSTIN_KNOB_ATTN_TRACE & 8): SM clock into shared memory (a %globaltimer read is far too slow to sit on
+// the paths it is meant to time), copied to the workspace tail when the CTA ends; slot 63 holds %globaltimer at the start.
+#define TS(slot) do { if (p.dbg & 8) s_ts[(slot)] = clock32(); } while (0)
 
 template <int NQ, int NWG, bool GATHER>
 __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kernel(const AttnParams p, const TcWs ws) {
     using C = TcCfg<NQ>;
     constexpr int NS = C::kSlotsN;
+    // Producer warpgroups: one (warps 4-7 copy the K and the V tiles).  A second one for the V tiles (warps 12-15 when
+    // there is a single softmax warpgroup) was measured: the copies are bound by the SM's cp.async path (one 512-byte
+    // warp instruction per ~20 cycles, whoever issues it), eight warps only contend for it -- 1.49 instead of 1.31 us a tile.
+    constexpr int NPW = 1;
     extern __shared__ __align__(1024) unsigned char smem[];   // 128-byte-swizzled operands need 1 KB alignment
     const uint32_t sbase = smem_u32(smem);
     if (sbase & 1023u) __trap();
@@ -322,7 +378,9 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
     auto bar = [&](int i) -> uint32_t { return bar0 + 8u * (uint32_t)i; };
     // barrier indices
     constexpr int kSlotFull = 0, kSlotEmpty = NS, kQFull = 2 * NS, kQEmpty = 2 * NS + 2, kSFull = 2 * NS + 4,
-                  kSEmpty = 2 * NS + 6, kPFull = 2 * NS + 8, kPvDone = 2 * NS + 9;
+                  kSEmpty = 2 * NS + 6, kPFull = 2 * NS + 8, kPvDone = 2 * NS + 9, kTabFull = 2 * NS + 10,
+                  kTabEmpty = 2 * NS + 12;
+    constexpr int kTabs = 2;   // tiles of row addresses in the table ring
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int T = p.n_new, r = p.group, rows = p.rows, Hkv = p.n_kv_heads, Hq = p.n_q_heads;
@@ -331,23 +389,59 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
     // merges a unit (the one holding the unit's first piece, i.e. its lowest range id) then waits for CTAs with higher
     // range ids = LOWER block indices, which were dispatched no later than itself: no co-residency assumption.
     const int rid = (int)gridDim.x - 1 - (int)blockIdx.x;
+    uint32_t* s_ts = reinterpret_cast<uint32_t*>(smem + C::kOffTs);
+    if (p.dbg & 8) {
+        if (tid < 64) s_ts[tid] = 0;
+        __syncthreads();
+        if (tid == 0 && ws.dbg_ts) ws.dbg_ts[(size_t)blockIdx.x * 64 + 63] = gtimer();
+    }
     if (tid == 0) TS(0);
-
+    // Let the next kernel's CTAs be scheduled from now on (they take an SM as soon as its CTA of this grid exits, run
+    // their prologue and stop at their own dependency wait, which still waits for this whole grid to complete).  The
+    // hardware holds them back until every CTA of this grid has started, so they cannot take an SM this grid needs.
+    pdl_trigger();
     // ---- token-list lengths of all units -> exclusive prefix sums (threads 0..255) --------------------------------
+    // A unit's token list is the tile of its T new rows (kTile virtual positions, see Seg) followed by its cache rows.
+    // The new rows need no index list and come first: their tile is worked through while the first gathered rows are
+    // still on their way, instead of costing a nearly empty tile at the end of the unit.
     auto unit_len = [&](int u) -> int {
         const int b = u / Hkv;
         int c;
-        if (GATHER) {
+        if (p.uniform_cnt >= 0) {
+            c = p.uniform_cnt;
+        } else if (GATHER) {
             const int list = p.n_lists == 1 ? 0 : u - b * Hkv;
             c = __ldg(p.cnt + b * p.n_lists + list);
             c = c < 0 ? 0 : (c > p.k_max ? p.k_max : c);
         } else {
             c = seq_len_of(p.kv.seq_lens, b, p.max_ctx);
         }
-        return c + T;
+        return c + kTile;
     };
     // Barriers and TMEM need nothing from global memory: under programmatic dependent launch this part runs while the
     // previous kernel drains; pdl_wait() returns when that kernel has completed and its writes are visible.
+    // Lengths known on the host (uniform budget over full-length sequences; the dense baseline without seq_lens): the
+    // whole plan is arithmetic and is laid out before the dependency wait.  Otherwise the lengths are read after it.
+    const bool uniform = p.uniform_cnt >= 0;
+    Plan pl;
+    // Uniform lengths, one whole unit per CTA, gathered rows (the shape of the headline workload): the resolver warps ask
+    // for the index entries of the first two gathered tiles right here, in as few instructions as possible (at the
+    // start of a launch every line of code is an instruction-cache miss), so that their trip overlaps the rest of the
+    // prologue.  The conditions restate make_plan's for this case.
+    int early_tok[4] = {-1, -1, -1, -1};
+    bool early = false;
+    if (GATHER && uniform && (warp == 9 || warp == 10) && rid < n_units && n_units <= (int)gridDim.x && !(p.dbg & 32)) {
+        const int len = p.uniform_cnt + kTile;
+        if (len <= (n_units * len) / (int)gridDim.x + 4 * kTile) {
+            const int first = (warp - 9) * kTile + lane;   // cache position of this lane's first row
+            const int* lrow = p.idx + (long long)(p.n_lists == 1 ? rid / Hkv : rid) * p.k_max + first;
+            early = true;
+            pdl_wait();
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+                if (first + 32 * i < p.uniform_cnt) early_tok[i] = __ldg(lrow + 32 * i);
+        }
+    }
     if (tid == 0) {
         for (int i = 0; i < NS; ++i) {
             mbar_init(bar(kSlotFull + i), 128);
@@ -361,29 +455,30 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
         }
         mbar_init(bar(kPFull), 128 * NWG);
         mbar_init(bar(kPvDone), 1);
+        for (int i = 0; i < kTabs; ++i) {
+            mbar_init(bar(kTabFull + i), 1);    // the resolver warp of the table
+            mbar_init(bar(kTabEmpty + i), 4 * NPW);   // the producer warps
+        }
         fence_mbar_init();
     }
     if (warp == 8) tmem_alloc(smem_u32(s_tmem), 512);
-    pdl_wait();
-    // Producers, whole-unit case (the CTA of range id x takes unit x from its first token, decided below): the index entries of tiles
-    // 0 and 1 are requested now, so that their latency overlaps the length loads and the prefix scan.
-    int spec_idx[2] = {-1, -1};
-    if (GATHER && warp >= 4 && warp < 8 && rid < n_units) {
-        const int sb = rid / Hkv, sl = p.n_lists == 1 ? 0 : rid - sb * Hkv;
-        const int* row = p.idx + ((long long)sb * p.n_lists + sl) * p.k_max;
-        const int pos0 = 32 * (warp - 4) + lane;
-        if (pos0 < p.k_max) spec_idx[0] = __ldg(row + pos0);
-        if (pos0 + kTile < p.k_max) spec_idx[1] = __ldg(row + pos0 + kTile);
+    if (!uniform) {
+        pdl_wait();
+        if (tid == 0) TS(57);
     }
     const int per = (n_units + 255) / 256;
     const int u_lo = min(tid * per, n_units), u_hi = tid < 256 ? min(u_lo + per, n_units) : u_lo;
-    int sum = 0, longest = 0;
-    for (int u = u_lo; u < u_hi; ++u) {
-        const int l = unit_len(u);
-        sum += l;
-        longest = max(longest, l);
-    }
-    {
+    if (uniform) {
+        const int len = p.uniform_cnt + kTile;
+        for (int u = u_lo; u < u_hi; ++u) s_prefix[u] = u * len;
+        if (tid == 255) s_prefix[n_units] = n_units * len;
+    } else {
+        int sum = 0, longest = 0;
+        for (int u = u_lo; u < u_hi; ++u) {
+            const int l = unit_len(u);
+            sum += l;
+            longest = max(longest, l);
+        }
         int inc = sum;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
@@ -405,91 +500,54 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
             run += unit_len(u);
         }
         if (tid == 255) s_prefix[n_units] = run;
-        if (tid < NQ) {
-            s_ref[tid] = kRefInit;
-            s_rowoff[tid] = ((tid / r) * Hq + tid % r) * kD;
-        }
-        tc_fence_before();
-        __syncthreads();
-        tc_fence_after();
     }
+    if (tid < NQ) {
+        s_ref[tid] = kRefInit;
+        s_rowoff[tid] = ((tid / r) * Hq + tid % r) * kD;
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
     if (tid == 0) TS(1);
     const uint32_t tmem = *s_tmem;
     constexpr uint32_t kColS = 0, kColO = 256;   // S buffers at columns 0 and 128, O^T at 256
-    const int total = s_prefix[n_units];
-    const int chunk = (((total + (int)gridDim.x - 1) / (int)gridDim.x) + 31) & ~31;
-    // Few units of similar length (at most one per CTA, the longest not much above the even share): every CTA
-    // takes one WHOLE unit -- no partials, no merge, one epilogue -- and the memory system, not the idle SMs, sets
-    // the pace.  Otherwise: equal token ranges (stream-K).
-    int longest_all = 0;
+    if (uniform) {
+        const int len = p.uniform_cnt + kTile;
+        pl = make_plan([&](int u) { return u * len; }, [&](int x) { return min(x / len, n_units - 1); }, n_units, len,
+                       (int)gridDim.x, rid, (p.dbg & 32) != 0);
+    } else {
+        int longest_all = 0;
 #pragma unroll
-    for (int w = 0; w < 8; ++w) longest_all = max(longest_all, s_scan[8 + w]);
-    const bool whole_mode = n_units <= (int)gridDim.x && longest_all <= total / (int)gridDim.x + 4 * kTile && !(p.dbg & 32);
-    int lo = rid * chunk, hi = min(lo + chunk, total);
-    if (whole_mode) {
-        lo = rid < n_units ? s_prefix[rid] : total;
-        hi = rid < n_units ? s_prefix[rid + 1] : total;
+        for (int w = 0; w < 8; ++w) longest_all = max(longest_all, s_scan[8 + w]);
+        pl = make_plan([&](int u) { return s_prefix[u]; },
+                       [&](int x) {
+                           int a = 0, bnd = n_units;
+                           while (bnd - a > 1) {
+                               const int m = (a + bnd) >> 1;
+                               if (s_prefix[m] <= x) a = m; else bnd = m;
+                           }
+                           return a;
+                       },
+                       n_units, longest_all, (int)gridDim.x, rid, (p.dbg & 32) != 0);
     }
+    const int lo = pl.lo, hi = pl.hi, u0 = pl.u0, chunk = pl.chunk;
     const bool active = lo < hi;   // a CTA past the end of the token space only takes part in the teardown
-    int u0 = 0;
-    if (whole_mode) {
-        u0 = min(rid, n_units - 1);
-    } else if (active) {
-        int a = 0, bnd = n_units;   // largest u with prefix[u] <= lo
-        while (bnd - a > 1) {
-            const int m = (a + bnd) >> 1;
-            if (s_prefix[m] <= lo) a = m; else bnd = m;
-        }
-        u0 = a;
-    }
     if (tid == 0) TS(2);
+    if (uniform) {
+        pdl_wait();
+        if (tid == 0) TS(57);
+    }
 
     TileCursor cur;
-    cur.init(s_prefix, n_units, Hkv, p.n_lists, T, lo, hi, chunk, u0);
+    cur.init(s_prefix, n_units, Hkv, p.n_lists, lo, hi, chunk, u0);
     if (!active) cur.valid = false;
 
-    if (warp >= 4 && warp < 8) {
+    if ((warp >= 4 && warp < 8) || (NPW == 2 && warp >= 12)) {
         // ================= producers ===========================================================================
         if constexpr (NWG == 1) asm volatile("setmaxnreg.dec.sync.aligned.u32 96;");
         else asm volatile("setmaxnreg.dec.sync.aligned.u32 88;");
-        const int pw = warp - 4, ptid = tid - 128;
-        TileCursor pf = cur;   // runs two tiles ahead of `cur`
-        struct Tok { int tok, b, g; };
-        // token code of row 32*pw + lane of the cursor's tile: >= 0 cache row, -1 none, <= -2 new row (-2 - u)
-        auto load_tok = [&](const TileCursor& c, int spec = -1) -> Tok {   // spec >= 0: index entry already loaded
-            Tok t;
-            t.tok = -1; t.b = 0; t.g = 0;
-            if (!c.valid) return t;
-            const Seg& s = c.s;
-            t.b = s.b; t.g = s.g;
-            const int pos = s.pos_lo + c.ti * kTile + 32 * pw + lane;
-            if (pos < s.pos_hi) {
-                if (pos < s.cnt)
-                    t.tok = !GATHER ? pos
-                                    : (spec >= 0 ? spec
-                                                 : __ldg(p.idx + ((long long)s.b * p.n_lists + s.list) * p.k_max + pos));
-                else
-                    t.tok = -2 - (pos - s.cnt);
-            }
-            return t;
-        };
-        // Absolute addresses of the K row and of the V row of a token code (0 = past the end of the piece).
-        struct RowPtr { unsigned long long k, v; };
-        auto resolve = [&](const Tok& t) -> RowPtr {
-            RowPtr a;
-            if (t.tok >= 0) {
-                const long long o = kv_row_offset(p.kv, t.b, t.tok, t.g);
-                a.k = (unsigned long long)(p.kv.k + o);
-                a.v = (unsigned long long)(p.kv.v + o);
-            } else if (t.tok == -1) {
-                a.k = a.v = 0ull;   // past the end of the piece: zero-filled by the copy (src-size 0)
-            } else {
-                const long long o = (((long long)t.b * T + (-2 - t.tok)) * Hkv + t.g) * kD;
-                a.k = (unsigned long long)(p.k_new + o);
-                a.v = (unsigned long long)(p.v_new + o);
-            }
-            return a;
-        };
+        const bool do_k = warp < 8, do_v = NPW == 1 || warp >= 12;
+        const int pw = warp & 3, ptid = do_k ? tid - 128 : -1;
         // lane = 16-byte chunk c of rows 2i + h (h = lane / 16), i = 0..15, of this warp's 32 rows of the tile.
         // Destination inside a slot: [64-dim half c/8][row][128 B], chunk XOR (row & 7); rows 2i + h and
         // 2(i + 4) + h share the swizzle term and lie 1 KB apart.
@@ -500,42 +558,78 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
             const int row = 32 * pw + 2 * q + h;
             dsw[q] = (uint32_t)(c >> 3) * (kTile * 128) + (uint32_t)row * 128 + (uint32_t)(((c & 7) ^ (row & 7)) << 4);
         }
-        ulonglong2* tab = reinterpret_cast<ulonglong2*>(smem + C::kOffRowTab) + 32 * pw;   // this warp's 32 entries
-        const ulonglong2* tab_rd = tab + h;
+        const ulonglong2* tab_rd = reinterpret_cast<const ulonglong2*>(smem + C::kOffRowTab) + 32 * pw + h;
         const unsigned long long coff = (unsigned long long)c * 16;
         const unsigned long long kdummy = (unsigned long long)p.kv.k;   // never read (src-size 0)
-        // K and V tiles of tile gj: items 2gj and 2gj+1 of the slot ring
-        auto issue_tile = [&](int gj, const RowPtr& mine) {
+        // K and V tiles of tile gj: items 2gj and 2gj+1 of the slot ring; row addresses from the resolver warps' table
+        auto issue_tile = [&](int gj, int ord) {   // ord: ordinal of the tile among the CTA's gathered tiles
+            const int ik = 2 * gj, iv = 2 * gj + 1, sk = ik % NS, sv = iv % NS, tb = ord % kTabs;
+            mbar_wait(bar(kTabFull + tb), ((uint32_t)(ord / kTabs)) & 1u);
+            if (do_k) mbar_wait(bar(kSlotEmpty + sk), (((uint32_t)(ik / NS)) & 1u) ^ 1u);
+            if (do_v) mbar_wait(bar(kSlotEmpty + sv), (((uint32_t)(iv / NS)) & 1u) ^ 1u);
+            const uint32_t dk = sbase + C::kOffSlots + (uint32_t)sk * kSlotBytes;
+            const uint32_t dv = sbase + C::kOffSlots + (uint32_t)sv * kSlotBytes;
+            const ulonglong2* trow = tab_rd + tb * kTile;
+            // (unrolled by 4, not 16: the first pass through this code is an instruction-cache miss per line, and it sits
+            // between the launch and the first request for cache rows)
+#pragma unroll 1
+            for (int i4 = 0; i4 < 4; ++i4) {
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const ulonglong2 a = trow[2 * (4 * i4 + q)];
+                    const uint32_t d = dsw[q] + (uint32_t)i4 * 1024;
+                    const int nb = a.x != 0ull ? 16 : 0;
+                    if (NPW == 1 || do_k) cp_async16(dk + d, reinterpret_cast<const void*>((nb ? a.x : kdummy) + coff), nb);
+                    if (NPW == 1 || do_v) cp_async16(dv + d, reinterpret_cast<const void*>((nb ? a.y : kdummy) + coff), nb);
+                }
+            }
+            if (do_k) cp_async_mbar_arrive_noinc(bar(kSlotFull + sk));
+            if (do_v) cp_async_mbar_arrive_noinc(bar(kSlotFull + sv));
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar(kTabEmpty + tb));   // this warp has read its 32 entries
+        };
+
+        // The tile of a unit's new rows: row u < T of the tile is new row u; the rest is padding, zeroed with plain stores
+        // (the copy path is the SM's scarcest resource: a tile of zero-filling copies would cost as much of it as a tile of
+        // cache rows).  K padding only has to be there; V padding must be finite, since it meets P = 0 in the MMA.
+        auto issue_new = [&](int gj) {
             const int ik = 2 * gj, iv = 2 * gj + 1, sk = ik % NS, sv = iv % NS;
-            __syncwarp();
-            tab[lane] = make_ulonglong2(mine.k, mine.v);
-            __syncwarp();
             mbar_wait(bar(kSlotEmpty + sk), (((uint32_t)(ik / NS)) & 1u) ^ 1u);
             mbar_wait(bar(kSlotEmpty + sv), (((uint32_t)(iv / NS)) & 1u) ^ 1u);
             const uint32_t dk = sbase + C::kOffSlots + (uint32_t)sk * kSlotBytes;
             const uint32_t dv = sbase + C::kOffSlots + (uint32_t)sv * kSlotBytes;
+            const long long o0 = (((long long)cur.s.b * T + (32 * pw + h)) * Hkv + cur.s.g) * kD + c * 8;   // row 32 pw + h
+#pragma unroll 1
+            for (int i4 = 0; i4 < 4; ++i4) {
 #pragma unroll
-            for (int i = 0; i < 16; ++i) {
-                const ulonglong2 a = tab_rd[2 * i];
-                const uint32_t d = dsw[i & 3] + (uint32_t)(i >> 2) * 1024;
-                const int nb = a.x != 0ull ? 16 : 0;
-                cp_async16(dk + d, reinterpret_cast<const void*>((nb ? a.x : kdummy) + coff), nb);
-                cp_async16(dv + d, reinterpret_cast<const void*>((nb ? a.y : kdummy) + coff), nb);
+                for (int q = 0; q < 4; ++q) {
+                    const int i = 4 * i4 + q;
+                    const uint32_t d = dsw[q] + (uint32_t)i4 * 1024;
+                    if (32 * pw + 2 * i + h < T) {
+                        const long long o = o0 + (long long)(2 * i) * Hkv * kD;
+                        cp_async16(dk + d, p.k_new + o, 16);
+                        cp_async16(dv + d, p.v_new + o, 16);
+                    } else {
+                        asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(dk + d), "r"(0) : "memory");
+                        asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(dv + d), "r"(0) : "memory");
+                    }
+                }
             }
+            fence_proxy_async();   // the plain stores, before the arrivals that hand the slots to the MMA
             cp_async_mbar_arrive_noinc(bar(kSlotFull + sk));
             cp_async_mbar_arrive_noinc(bar(kSlotFull + sv));
         };
 
-        if (ptid == 0) TS(40);
-        // The T*r query rows of the cursor's segment (zero-padded to NQ) into Q buffer seg_no % 2.
+        if (ptid == 0) TS(58);
+        // The T*r query rows of the cursor's segment (zero-padded to NQ) into Q buffer seg_no % kQBufs.
         auto issue_q = [&]() {
             const int k = cur.seg_no, qb = k % C::kQBufs;
             mbar_wait(bar(kQEmpty + qb), (((uint32_t)(k / C::kQBufs)) & 1u) ^ 1u);
             const uint32_t qdst = sbase + C::kOffQ + (uint32_t)qb * C::kQBytes;
             const __nv_bfloat16* qsrc = p.q + ((long long)cur.s.b * T * Hq + (long long)cur.s.g * r) * kD;
 #pragma unroll 1
-            for (int x = ptid; x < NQ * 16; x += 128) {
-                const int rr = x >> 4, cc = x & 15;
+            for (int x0 = 0; x0 < NQ * 16; x0 += 128) {
+                const int x = x0 + ptid, rr = x >> 4, cc = x & 15;
                 const bool ok = rr < rows;
                 const __nv_bfloat16* src = ok ? qsrc + s_rowoff[rr] + cc * 8 : p.q;
                 cp_async16(qdst + (uint32_t)(cc >> 3) * (NQ * 128) + (uint32_t)rr * 128 +
@@ -543,33 +637,97 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
             }
             cp_async_mbar_arrive_noinc(bar(kQFull + qb));
         };
-        // tiles 0 and 1: both index loads are in flight (or already here, whole-unit case) before the first use, and
-        // the first segment's Q rows are requested while they travel
-        const bool spec = GATHER && whole_mode;
-        const Tok t0 = load_tok(pf, spec ? spec_idx[0] : -1);
-        if (pf.valid) pf.advance();
-        Tok t1 = load_tok(pf, spec ? spec_idx[1] : -1);
-        if (pf.valid) pf.advance();
-        RowPtr a0 = resolve(t0);
-        int gj = 0;
+        int gj = 0, ord = 0;
+#pragma unroll 1
         while (cur.valid) {
-            Tok t2 = load_tok(pf);                 // tile gj + 2: index load in flight
-            if (pf.valid) pf.advance();
-            const RowPtr a1 = resolve(t1);         // tile gj + 1: page-table lookup in flight
-            if (cur.ti == 0 && gj > 0) issue_q();  // new segment
-            issue_tile(gj, a0);
-            if (gj == 0) issue_q();                // first segment: its K/V rows (the longer trip) go out before Q
-            if (ptid == 0 && gj < 4) TS(4 + gj);
-            a0 = a1;
-            t1 = t2;
+            if (cur.ti == 0 && do_k) issue_q();    // new segment: its query rows
+            if (cur.new_tile()) {
+                issue_new(gj);
+            } else {
+                issue_tile(gj, ord);
+                ++ord;
+            }
+            if (ptid == 0 && gj < 3) TS(4 + gj);
             cur.advance();
             ++gj;
         }
     } else if (warp >= 8 && warp < 12) {
         // ================= MMA issuer (one thread of warp 8) =====================================================
-        if constexpr (NWG == 1) asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
+        if constexpr (NWG == 1) asm volatile("setmaxnreg.dec.sync.aligned.u32 96;");
         else asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
-        if (warp == 8 && lane == 0) {
+        if (warp > 8) {
+            // ================= resolver warps 9 and 10: warp 9 + w serves the gathered tiles of ordinal w, w + 2, ... ====
+            // index entry -> (page table ->) absolute addresses of the K and the V row, for the 128 rows of a tile of
+            // cache rows (4 per lane, all loads of a tile in flight together), into table w of two in shared memory, which
+            // the producers read.  Each warp has two tile periods for its chain of dependent loads, so the producers do not
+            // wait for an index in the steady state; in the whole-unit case the entries of the first two tiles were
+            // requested at the top of the kernel.  (One warp per table: a warp then waits on consecutive phases of its
+            // table's barrier and cannot run a phase ahead.)  The new-row tiles need no table: the producers address them.
+            const int rw = warp - 9;
+            if (rw < kTabs) {
+                ulonglong2* tabw = reinterpret_cast<ulonglong2*>(smem + C::kOffRowTab) + rw * kTile;
+                // cache rows (token indices) of rows lane + 32 i of the cursor's tile; -1 = past the end of the piece
+                auto load4 = [&](const TileCursor& c, int (&tok)[4]) {
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) tok[i] = -1;
+                    if (!c.valid) return;
+                    const Seg& sg = c.s;
+                    const int pos0 = sg.pos_lo + c.ti * kTile + lane;
+                    const int* lrow = GATHER ? p.idx + ((long long)sg.b * p.n_lists + sg.list) * p.k_max - kTile : nullptr;
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        const int pos = pos0 + 32 * i;
+                        if (pos < sg.pos_hi) tok[i] = GATHER ? __ldg(lrow + pos) : pos - kTile;
+                    }
+                };
+                if (rw == 0 && lane == 0) TS(62);
+                TileCursor rc = cur;
+                int ord = 0, want = rw;   // ord: gathered tiles before the cursor's; want: the ordinal this warp serves next
+                auto seek = [&]() {
+                    while (rc.valid) {
+                        if (!rc.new_tile()) {
+                            if (ord == want) return;
+                            ++ord;
+                        }
+                        rc.advance();
+                    }
+                };
+                seek();
+                int tok[4];
+                if (early) {   // whole unit: requested at the top of the kernel
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) tok[i] = early_tok[i];
+                } else {
+                    load4(rc, tok);
+                }
+                int use = 0;   // how many times this warp has filled its table
+#pragma unroll 1
+                while (rc.valid) {
+                    const int sb_ = rc.s.b, sg_ = rc.s.g;
+                    ulonglong2 a[4];
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        a[i].x = a[i].y = 0ull;   // past the end of the piece: zero-filled by the copy (src-size 0)
+                        if (tok[i] >= 0) {
+                            const long long off = kv_row_offset(p.kv, sb_, tok[i], sg_);
+                            a[i].x = (unsigned long long)(p.kv.k + off);
+                            a[i].y = (unsigned long long)(p.kv.v + off);
+                        }
+                    }
+                    mbar_wait(bar(kTabEmpty + rw), ((uint32_t)use & 1u) ^ 1u);
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) tabw[lane + 32 * i] = a[i];
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(bar(kTabFull + rw));
+                    if (rw == 0 && lane == 0 && use == 0) TS(50);
+                    if (rw == 0 && lane == 0 && use == 1) TS(7);
+                    want += kTabs;
+                    seek();
+                    load4(rc, tok);   // this warp's next tile
+                    ++use;
+                }
+            }
+        } else if (lane == 0) {
             constexpr uint32_t idesc_s = umma_idesc(kTile, NQ, 0, 0);    // S^T = K . Q^T : both K-major
             constexpr uint32_t idesc_pv = umma_idesc(kTile, NQ, 1, 1);   // O^T = V^T . P^T : both MN-major
             const uint32_t slots = sbase + C::kOffSlots, pbuf = sbase + C::kOffP;
@@ -641,7 +799,7 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
         constexpr int NW = NQ / NWG;
         const int wg = (NWG == 2 && warp >= 12) ? 1 : 0;
         const int c_off = wg * NW, wq = warp & 3;
-        const int t = tid - wg * 384;
+        const int t = tid - wg * 384;   // (warps 12-15 are the second softmax warpgroup only when NWG == 2)
         const int rows_w = min(max(rows - c_off, 0), NW);
         const uint32_t lane_base = tmem + ((uint32_t)(wq * 32) << 16) + (uint32_t)c_off;
         const float sl2 = p.scale_log2;
@@ -672,10 +830,10 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
             tc_fence_before();
             mbar_arrive(bar(kSEmpty + sb));
 
-            // scale into the log2 domain; mask the tail of the piece and, for a new row u, the query rows of
-            // verify positions < u (row i belongs to position i / r, so those are the rows i < u * r)
+            // scale into the log2 domain; mask the tail of the piece, the padding of the new-row tile and, for a new row
+            // u, the query rows of verify positions < u (row i belongs to position i / r, so those are the rows i < u * r)
             const int pos = s.pos_lo + cur.ti * kTile + t;
-            const int thr = (pos >= s.pos_hi ? INT_MAX : (pos > s.cnt ? (pos - s.cnt) * r : 0)) - c_off;
+            const int thr = (pos >= s.pos_hi ? INT_MAX : (pos >= kTile ? 0 : (pos < T ? pos * r : INT_MAX))) - c_off;
             // x[i] = d_i = s_i * scale - m_ref[i] (one FFMA), the exponent that P needs; the masks cost nothing in the
             // tiles that have none (cache rows inside the piece: every tile but the last one or two).
             float x[NW];
@@ -920,10 +1078,13 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
         }
     }
 
-    pdl_trigger();
     tc_fence_before();
     __syncthreads();
     if (tid == 0) TS(3);
+    if ((p.dbg & 8) && ws.dbg_ts) {
+        __syncthreads();
+        if (tid < 63) ws.dbg_ts[(size_t)blockIdx.x * 64 + tid] = s_ts[tid];
+    }
     if (warp == 8) {
         tc_fence_after();
         tmem_dealloc(tmem, 512);
@@ -958,7 +1119,8 @@ bool attn_tc_usable(int batch, int n_kv_heads, int head_dim, int rows, int max_t
     if (head_dim != kD || rows > 96 || rows < 1) return false;
     const long long units = (long long)batch * n_kv_heads;
     if (units > kMaxUnits) return false;
-    return units * ((long long)max_tokens + n_new) < (1ll << 31) - (1 << 20);
+    (void)n_new;   // the new rows of a unit take one whole tile of its token space
+    return units * ((long long)max_tokens + kTile) < (1ll << 31) - (1 << 20);
 }
 
 size_t attn_tc_ws_bytes(int batch, int n_kv_heads, int rows) {
@@ -982,7 +1144,7 @@ cudaError_t launch_attn_tc(const AttnParams& p_in, void* ws_base, cudaStream_t s
     const size_t nq = p.rows > 48 ? 96 : (size_t)((p.rows + 15) / 16) * 16;
     ws.part_lse = reinterpret_cast<float*>(base + kWsHeader + align256((size_t)kMaxGrid * 2 * nq * kD * sizeof(float)));
     ws.dbg_ts = (p.dbg & 8) ? reinterpret_cast<unsigned long long*>(reinterpret_cast<char*>(ws.part_lse) + align256((size_t)kMaxGrid * 2 * nq * sizeof(float))) : nullptr;
-    const int max_tokens = (p.idx ? (p.k_max < p.max_ctx ? p.k_max : p.max_ctx) : p.max_ctx) + p.n_new;
+    const int max_tokens = (p.idx ? (p.k_max < p.max_ctx ? p.k_max : p.max_ctx) : p.max_ctx) + kTile;
     long long tiles = ((long long)units * max_tokens + kTile - 1) / kTile;
     const int sms = device_sm_count();
     int grid = sms < kMaxGrid ? sms : kMaxGrid;

@@ -88,7 +88,10 @@ struct AttnParams {
     const __nv_bfloat16* k_new;   // [B,T,Hkv,d]
     const __nv_bfloat16* v_new;
     const int* idx;               // [B,G,k_max] or nullptr (dense)
-    const int* cnt;               // [B,G]
+    const int* cnt;               // [B,G]; may be nullptr when uniform_cnt >= 0
+    int uniform_cnt;              // >= 0: every unit holds exactly this many cache rows, known on the host (uniform budget
+                                  // and full-length sequences, or the dense baseline without seq_lens): the kernels plan
+                                  // without reading a length from memory.  -1: read cnt / seq_lens.
     int batch, n_q_heads, n_kv_heads, group, head_dim, n_new, max_ctx, n_lists, k_max;
     float scale_log2;
     int rows;                     // T * group query rows per KV head

@@ -147,7 +147,9 @@ def test_attn_and_fused_reject(lib):
     attn = lambda idx=FAKE, cnt=FAKE, n_lists=1, k_max=512, out=FAKE, ws=FAKE, wsb=1 << 40, kvv=k, s=sh: \
         lib.dustin_sparse_verify_attn(ctypes.byref(s), ctypes.byref(kvv), FAKE, FAKE, FAKE, idx, cnt, n_lists, k_max,
                                       out, None, ws, wsb, None)
-    assert attn(cnt=None) == api.ERR_INVALID_ARG
+    # cnt == NULL states "every list holds k_max entries": refused where that cannot hold
+    assert attn(cnt=None, kvv=kv(seq_lens=FAKE)) == api.ERR_INVALID_ARG
+    assert attn(cnt=None, k_max=4097) == api.ERR_INVALID_ARG
     assert attn(n_lists=3) == api.ERR_INVALID_ARG
     assert attn(out=None) == api.ERR_INVALID_ARG
     assert attn(kvv=kv(v=None)) == api.ERR_INVALID_ARG

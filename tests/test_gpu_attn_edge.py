@@ -121,3 +121,33 @@ def test_query_row_counts(T, r):
     out, lse, o_ref, lse_ref = _run_both(x, idx, cnt, N)
     H.check_attn(out, o_ref)
     assert torch.allclose(lse.cpu().double(), lse_ref, atol=2e-3, rtol=0)
+
+
+@pytest.mark.parametrize("B,Hkv,k", [(2, 2, 300), (16, 8, 257), (1, 1, 2048)])
+def test_cnt_null_means_full_lists(B, Hkv, k):
+    """cnt == NULL (dustin.h: every list holds exactly k_max entries; the kernel plans without reading a length):
+    bitwise the result of the same call with cnt = k_max everywhere, in whole-unit and in cut-unit decompositions, and
+    against the oracle; refused when the lists could be shorter (ragged sequences, k_max > max_ctx)."""
+    N, Hq, d, T = 4096, 4 * Hkv, 128, 5
+    x = _inputs(B, N, Hq, Hkv, d, T, 77)
+    idx, cnt = _lists(B, Hkv, N, [k], k, 78)
+    out_c, lse_c, o_ref, lse_ref = _run_both(x, idx, cnt, N)
+    sh = api.Shape(B, Hq, Hkv, d, T, N, 0.0)
+    dev = {n: t.cuda() for n, t in x.items()}
+    ws = api.alloc_workspace(sh, 1, k)
+    out_n = torch.full_like(dev["q"], float("nan"))
+    lse_n = torch.full((B, Hq, T), float("nan"), device="cuda")
+    api.sparse_verify_attn(sh, api.KV.contiguous_nhd(dev["k"], dev["v"], None), dev["q"], dev["k_new"], dev["v_new"],
+                           idx.cuda(), None, out_n, ws, lse_n)
+    torch.cuda.synchronize()
+    assert torch.equal(out_c, out_n) and torch.equal(lse_c, lse_n)
+    H.check_attn(out_n, o_ref)
+    assert torch.allclose(lse_n.cpu().double(), lse_ref, atol=1e-2, rtol=1e-5)
+    lens = torch.full((B,), N, dtype=torch.int32, device="cuda")
+    with pytest.raises(api.DustinError):
+        api.sparse_verify_attn(sh, api.KV.contiguous_nhd(dev["k"], dev["v"], lens), dev["q"], dev["k_new"],
+                               dev["v_new"], idx.cuda(), None, torch.empty_like(dev["q"]), ws)
+    wide = torch.zeros((B, Hkv, N + 8), dtype=torch.int32, device="cuda")
+    with pytest.raises(api.DustinError):
+        api.sparse_verify_attn(sh, api.KV.contiguous_nhd(dev["k"], dev["v"], None), dev["q"], dev["k_new"],
+                               dev["v_new"], wide, None, torch.empty_like(dev["q"]), ws)
