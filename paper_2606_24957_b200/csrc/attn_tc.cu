@@ -41,7 +41,9 @@ constexpr float kRefSlack = 16.f;     // log2 units a score may exceed m_ref bef
 constexpr float kRefInit = 0.f;        // reference exponent at the start of a piece (the first tile always moves it)
 constexpr float kRefFloor = -1.0e30f;  // lowest reference (rows that have seen nothing but masked tokens)
 constexpr long long kInvalidRow = LLONG_MIN;
-constexpr int kMergeFast = 4;          // pieces of one unit merged with all loads in flight (more: sequential path)
+constexpr int kMergeFast = 4;          // rows of the merge-weight array in shared memory (s_wgt)
+constexpr int kMergeBatch = 8;         // pieces of one unit (the merging CTA's own included) merged with batched loads: their
+                                       // weights live in s_wgt (kMergeFast rows) and in the idle per-warp scratch (3 more)
 
 // ---- PTX wrappers ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
@@ -151,6 +153,11 @@ __host__ __device__ constexpr uint32_t umma_idesc(int m, int n, int a_mn_major, 
            ((uint32_t)(n >> 3) << 17) | ((uint32_t)(m >> 4) << 24);
 }
 
+__device__ __forceinline__ int ld_relaxed(const int* p) {
+    int v;
+    asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
 __device__ __forceinline__ void st_release(int* p, int v) {
     asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
@@ -956,15 +963,32 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
                 const bool merge = s.pos_lo == 0 && !s.whole;
                 const int nseg = s.cta_last - s.cta_first + 1;
                 const long long slot_id = (long long)rid * 2 + s.slot;
+                // The pieces 1 .. nb-1 of the unit (slot 0 of the following CTAs) are merged with their loads batched: one
+                // round trip for all flags, one for all normalisers, and the partial outputs double-buffered; units cut
+                // into more than kMergeBatch pieces (one very long sequence on the whole machine) finish piece by piece.
+                const int nb = merge ? min(nseg, kMergeBatch) : 1;
                 float v1[NW];
-                float lse1 = -INFINITY;
-                if (merge) {   // second piece = slot 0 of the next CTA: loads in flight during the reductions below
+                float lj[kMergeBatch];
+#pragma unroll
+                for (int j = 0; j < kMergeBatch; ++j) lj[j] = -INFINITY;
+                if (merge) {
+                    uint32_t pend = 0;
+#pragma unroll
+                    for (int j = 1; j < kMergeBatch; ++j)
+                        if (j < nb && ld_relaxed(ws.flags + (long long)(s.cta_first + j) * 2) == 0) pend |= 1u << j;
+#pragma unroll 1
+                    for (int j = 1; j < nb; ++j)
+                        if ((pend >> j) & 1u) wait_flag(ws.flags + (long long)(s.cta_first + j) * 2);
+                    __threadfence();   // acquire: the loads below come after the flags have been seen
                     const long long sid1 = (long long)(s.cta_first + 1) * 2;
-                    wait_flag(ws.flags + sid1);
                     const float* src1 = ws.part_o + sid1 * NQ * kD + c_off * kD + t;
 #pragma unroll
-                    for (int i = 0; i < NW; ++i) v1[i] = __ldcg(src1 + i * kD);
-                    if (t < rows_w) lse1 = __ldcg(ws.part_lse + sid1 * NQ + c_off + t);
+                    for (int i = 0; i < NW; ++i) v1[i] = __ldcg(src1 + i * kD);   // in flight during the reductions below
+                    if (t < rows_w) {
+#pragma unroll
+                        for (int j = 1; j < kMergeBatch; ++j)
+                            if (j < nb) lj[j] = __ldcg(ws.part_lse + ((long long)(s.cta_first + j) * 2) * NQ + c_off + t);
+                    }
                 }
                 if (t == 0) TS(56);
                 {
@@ -982,22 +1006,35 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
                     const float lse_own = l > 0.f ? s_ref_w[t] + log2f(l) : -INFINITY;
                     float scale = l > 0.f ? 1.f / l : 0.f, lse_fin = lse_own;
                     if (merge && t < rows_w) {
-                        float M = fmaxf(lse_own, lse1);
-                        for (int j = 2; j < nseg; ++j) {
+                        float M = lse_own;
+#pragma unroll
+                        for (int j = 1; j < kMergeBatch; ++j) M = fmaxf(M, lj[j]);
+                        for (int j = kMergeBatch; j < nseg; ++j) {
                             const long long sid = (long long)(s.cta_first + j) * 2;
                             wait_flag(ws.flags + sid);
                             M = fmaxf(M, __ldcg(ws.part_lse + sid * NQ + c_off + t));
                         }
                         const float e0 = lse_own == -INFINITY ? 0.f : exp2f(lse_own - M);
-                        const float e1 = lse1 == -INFINITY ? 0.f : exp2f(lse1 - M);
-                        float W = e0 + e1;
-                        for (int j = 2; j < nseg; ++j) {
-                            const float lj = __ldcg(ws.part_lse + ((long long)(s.cta_first + j) * 2) * NQ + c_off + t);
-                            W += lj == -INFINITY ? 0.f : exp2f(lj - M);
+                        float W = e0;
+                        float e[kMergeBatch];
+#pragma unroll
+                        for (int j = 1; j < kMergeBatch; ++j) {   // same order as before: piece 1, 2, ...
+                            e[j] = lj[j] == -INFINITY ? 0.f : exp2f(lj[j] - M);
+                            W += e[j];
+                        }
+                        for (int j = kMergeBatch; j < nseg; ++j) {
+                            const float l_j = __ldcg(ws.part_lse + ((long long)(s.cta_first + j) * 2) * NQ + c_off + t);
+                            W += l_j == -INFINITY ? 0.f : exp2f(l_j - M);
                         }
                         const float invW = W > 0.f ? 1.f / W : 0.f;
                         scale *= e0 * invW;
-                        s_wgt_w[t] = e1 * invW;
+                        // weights of the batched pieces: piece j at s_wgt[j - 1] for j <= kMergeFast, the rest in this
+                        // thread's own column of s_warp (read just above, free now)
+#pragma unroll
+                        for (int j = 1; j < kMergeBatch; ++j) {
+                            if (j <= kMergeFast) s_wgt_w[(j - 1) * NQ + t] = e[j] * invW;
+                            else s_warp_w[(j - 1 - kMergeFast) * NW + t] = e[j] * invW;
+                        }
                         lse_fin = W > 0.f ? M + log2f(W) : -INFINITY;
                         M_row = M;
                         W_row = invW;
@@ -1038,9 +1075,30 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
 #pragma unroll
                     for (int i = 0; i < NW; ++i) acc[i] = __uint_as_float(o[i]) * s_fac_w[i];
                     if (merge) {
+                        // batched pieces: the next piece's partial is requested before the current one is folded in
+                        float v2[NW];
+#pragma unroll 1
+                        for (int j = 1; j < nb; j += 2) {
+                            if (j + 1 < nb) {
+                                const float* src = ws.part_o + ((long long)(s.cta_first + j + 1) * 2) * NQ * kD + c_off * kD + t;
 #pragma unroll
-                        for (int i = 0; i < NW; ++i) acc[i] = fmaf(s_wgt_w[i], v1[i], acc[i]);
-                        for (int j = 2; j < nseg; ++j) {   // units cut into more than two pieces (very long sequences)
+                                for (int i = 0; i < NW; ++i) v2[i] = __ldcg(src + i * kD);
+                            }
+                            const float* wa = j <= kMergeFast ? s_wgt_w + (j - 1) * NQ : s_warp_w + (j - 1 - kMergeFast) * NW;
+#pragma unroll
+                            for (int i = 0; i < NW; ++i) acc[i] = fmaf(wa[i], v1[i], acc[i]);
+                            if (j + 1 < nb) {
+                                if (j + 2 < nb) {
+                                    const float* src = ws.part_o + ((long long)(s.cta_first + j + 2) * 2) * NQ * kD + c_off * kD + t;
+#pragma unroll
+                                    for (int i = 0; i < NW; ++i) v1[i] = __ldcg(src + i * kD);
+                                }
+                                const float* wb = j + 1 <= kMergeFast ? s_wgt_w + j * NQ : s_warp_w + (j - kMergeFast) * NW;
+#pragma unroll
+                                for (int i = 0; i < NW; ++i) acc[i] = fmaf(wb[i], v2[i], acc[i]);
+                            }
+                        }
+                        for (int j = kMergeBatch; j < nseg; ++j) {   // beyond the batch (very long sequences): piece by piece
                             const long long sid = (long long)(s.cta_first + j) * 2;
                             wg_sync(wg);
                             if (t < rows_w) {
