@@ -51,6 +51,10 @@ int check_kv(const dustin_shape_t* s, const dustin_kv_t* kv, bool need_v, KvView
     out->stride_head = kv->stride_head;
     out->page_table = kv->page_table;
     out->page_size = kv->page_table ? kv->page_size : 1;
+    out->page_shift = -1;
+    if ((out->page_size & (out->page_size - 1)) == 0)
+        for (int s2 = 0; s2 < 31; ++s2)
+            if ((1 << s2) == out->page_size) out->page_shift = s2;
     out->max_pages = kv->page_table ? kv->max_pages : 0;
     out->seq_lens = kv->seq_lens;
     return DUSTIN_OK;

@@ -20,6 +20,7 @@ struct KvView {
     long long stride_seq, stride_token, stride_head;
     const int* page_table;
     int page_size, max_pages;
+    int page_shift;   // log2(page_size) when it is a power of two (the usual case: shift and mask, no division), else -1
     const int* seq_lens;
 };
 
@@ -33,7 +34,7 @@ __device__ __forceinline__ int seq_len_of(const int* seq_lens, int b, int max_ct
 __device__ __forceinline__ long long kv_row_offset(const KvView& kv, int b, int n, int g) {
     if (kv.page_table == nullptr)
         return (long long)b * kv.stride_seq + (long long)n * kv.stride_token + (long long)g * kv.stride_head;
-    const int pg = n / kv.page_size;
+    const int pg = kv.page_shift >= 0 ? n >> kv.page_shift : n / kv.page_size;
     const int page = __ldg(kv.page_table + (long long)b * kv.max_pages + pg);
     return (long long)page * kv.stride_seq + (long long)(n - pg * kv.page_size) * kv.stride_token +
            (long long)g * kv.stride_head;
