@@ -624,7 +624,13 @@ def sweep_point(api, cfg: synth.Config, n_sets: int, dist: Dist, device, peak: f
         legs.append(("score_all_heads", w.step_score_all_heads))
     for name, fn in legs:
         t[name] = 1e3 * time_steps(graphed(fn), 3, 3, dist, device) / cfg.n_layers
+    # the streaming kernel of a1 alone (event pairs inside the library): "score" above is the whole staged a1 stage --
+    # score_logits_kernel + the stats and normalise launches that write scores_now
+    kern = profile_steps(api, w.step_score_only, 2).get("score_logits_kernel")
     out = dict(tag)
+    if kern:
+        out["score_logits_kernel_us"] = round(kern[0], 2)
+        out["score_logits_kernel_gbs"] = round(by["a1_k"] / kern[0] / 1e3, 1)
     if naive:
         out["score_all_heads_us"] = round(t["score_all_heads"], 2)
         out["score_all_heads_over_dense"] = round(t["score_all_heads"] / t["dense"], 3)
@@ -873,7 +879,9 @@ def main():
         "roofline": roofline,
         "roofline_attn": roof("attn_kernel", by["a4"], r["attn_only_us_per_launch"],
                               "CUDA events around graph replays that hold only this kernel (L launches, one per "
-                              "layer, each on its own K/V cache and index lists); time / launches"),
+                              "layer, each on its own K/V cache and index lists; cnt = NULL: one budget <= N for all "
+                              "sequences, so every list holds k entries -- the fact the fused call derives from its select "
+                              "parameters); time / launches"),
         "gather_probe": {"us_per_launch": round(r["gather_probe_us_per_launch"], 3),
                          "gbs": round(by["a4"] / r["gather_probe_us_per_launch"] / 1e3, 1),
                          "attn_time_over_probe": round(r["attn_only_us_per_launch"] / r["gather_probe_us_per_launch"], 3),

@@ -39,10 +39,6 @@ typedef enum dustin_knob {
     DUSTIN_KNOB_SCORE_CHUNK = 5,    /* tokens per CTA of the scoring kernel (multiple of 128); 0 (default) = heuristic      */
     DUSTIN_KNOB_SELECT_TRACE = 6,   /* 1: selection kernels write %globaltimer samples per phase into the buffer given to
                                        dustin_debug_trace_buffer                                                           */
-    DUSTIN_KNOB_L2_HYGIENE = 7,     /* bit mask, fused call (default 1): 1 = the selection kernel discards the logits scratch
-                                       from L2 once read (when every row of it has a single reader), 2 = it stores the
-                                       accumulated score rows write-through; 0 leaves ~35 MB of dirty lines per layer to
-                                       be written back while the attention kernel gathers                                 */
     DUSTIN_KNOB_COUNT = 16
 } dustin_knob;
 void    dustin_tune_set(int32_t knob, int32_t value);

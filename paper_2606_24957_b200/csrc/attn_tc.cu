@@ -369,6 +369,9 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
     // there is a single softmax warpgroup) was measured: the copies are bound by the SM's cp.async path (one 512-byte
     // warp instruction per ~20 cycles, whoever issues it), eight warps only contend for it -- 1.49 instead of 1.31 us a tile.
     constexpr int NPW = 1;
+    // pieces of a cut unit merged with batched loads: 8 with one softmax warpgroup, 2 (the head's own and the next) with
+    // two, whose 192 registers per thread have no room for the batch's normalisers and weights
+    constexpr int kMB = NWG == 1 ? kMergeBatch : 2;
     extern __shared__ __align__(1024) unsigned char smem[];   // 128-byte-swizzled operands need 1 KB alignment
     const uint32_t sbase = smem_u32(smem);
     if (sbase & 1023u) __trap();
@@ -965,16 +968,16 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
                 const long long slot_id = (long long)rid * 2 + s.slot;
                 // The pieces 1 .. nb-1 of the unit (slot 0 of the following CTAs) are merged with their loads batched: one
                 // round trip for all flags, one for all normalisers, and the partial outputs double-buffered; units cut
-                // into more than kMergeBatch pieces (one very long sequence on the whole machine) finish piece by piece.
-                const int nb = merge ? min(nseg, kMergeBatch) : 1;
+                // into more than kMB pieces (one very long sequence on the whole machine) finish piece by piece.
+                const int nb = merge ? min(nseg, kMB) : 1;
                 float v1[NW];
-                float lj[kMergeBatch];
+                float lj[kMB];
 #pragma unroll
-                for (int j = 0; j < kMergeBatch; ++j) lj[j] = -INFINITY;
+                for (int j = 0; j < kMB; ++j) lj[j] = -INFINITY;
                 if (merge) {
                     uint32_t pend = 0;
 #pragma unroll
-                    for (int j = 1; j < kMergeBatch; ++j)
+                    for (int j = 1; j < kMB; ++j)
                         if (j < nb && ld_relaxed(ws.flags + (long long)(s.cta_first + j) * 2) == 0) pend |= 1u << j;
 #pragma unroll 1
                     for (int j = 1; j < nb; ++j)
@@ -986,7 +989,7 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
                     for (int i = 0; i < NW; ++i) v1[i] = __ldcg(src1 + i * kD);   // in flight during the reductions below
                     if (t < rows_w) {
 #pragma unroll
-                        for (int j = 1; j < kMergeBatch; ++j)
+                        for (int j = 1; j < kMB; ++j)
                             if (j < nb) lj[j] = __ldcg(ws.part_lse + ((long long)(s.cta_first + j) * 2) * NQ + c_off + t);
                     }
                 }
@@ -1008,21 +1011,21 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
                     if (merge && t < rows_w) {
                         float M = lse_own;
 #pragma unroll
-                        for (int j = 1; j < kMergeBatch; ++j) M = fmaxf(M, lj[j]);
-                        for (int j = kMergeBatch; j < nseg; ++j) {
+                        for (int j = 1; j < kMB; ++j) M = fmaxf(M, lj[j]);
+                        for (int j = kMB; j < nseg; ++j) {
                             const long long sid = (long long)(s.cta_first + j) * 2;
                             wait_flag(ws.flags + sid);
                             M = fmaxf(M, __ldcg(ws.part_lse + sid * NQ + c_off + t));
                         }
                         const float e0 = lse_own == -INFINITY ? 0.f : exp2f(lse_own - M);
                         float W = e0;
-                        float e[kMergeBatch];
+                        float e[kMB];
 #pragma unroll
-                        for (int j = 1; j < kMergeBatch; ++j) {   // same order as before: piece 1, 2, ...
+                        for (int j = 1; j < kMB; ++j) {   // same order as before: piece 1, 2, ...
                             e[j] = lj[j] == -INFINITY ? 0.f : exp2f(lj[j] - M);
                             W += e[j];
                         }
-                        for (int j = kMergeBatch; j < nseg; ++j) {
+                        for (int j = kMB; j < nseg; ++j) {
                             const float l_j = __ldcg(ws.part_lse + ((long long)(s.cta_first + j) * 2) * NQ + c_off + t);
                             W += l_j == -INFINITY ? 0.f : exp2f(l_j - M);
                         }
@@ -1031,7 +1034,7 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
                         // weights of the batched pieces: piece j at s_wgt[j - 1] for j <= kMergeFast, the rest in this
                         // thread's own column of s_warp (read just above, free now)
 #pragma unroll
-                        for (int j = 1; j < kMergeBatch; ++j) {
+                        for (int j = 1; j < kMB; ++j) {
                             if (j <= kMergeFast) s_wgt_w[(j - 1) * NQ + t] = e[j] * invW;
                             else s_warp_w[(j - 1 - kMergeFast) * NW + t] = e[j] * invW;
                         }
@@ -1075,30 +1078,52 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
 #pragma unroll
                     for (int i = 0; i < NW; ++i) acc[i] = __uint_as_float(o[i]) * s_fac_w[i];
                     if (merge) {
-                        // batched pieces: the next piece's partial is requested before the current one is folded in
-                        float v2[NW];
+                        // batched pieces.  One softmax warpgroup (240 registers): the next piece's partial is requested
+                        // before the current one is folded in; two (192 registers): one partial at a time, or the
+                        // second buffer spills into the tile loop.
+                        auto wgt_of = [&](int j) -> const float* {
+                            return j <= kMergeFast ? s_wgt_w + (j - 1) * NQ : s_warp_w + (j - 1 - kMergeFast) * NW;
+                        };
+                        auto part_of = [&](int j) -> const float* {
+                            return ws.part_o + ((long long)(s.cta_first + j) * 2) * NQ * kD + c_off * kD + t;
+                        };
+                        if constexpr (NWG == 1) {
+                            float v2[NW];
 #pragma unroll 1
-                        for (int j = 1; j < nb; j += 2) {
-                            if (j + 1 < nb) {
-                                const float* src = ws.part_o + ((long long)(s.cta_first + j + 1) * 2) * NQ * kD + c_off * kD + t;
+                            for (int j = 1; j < nb; j += 2) {
+                                if (j + 1 < nb) {
+                                    const float* src = part_of(j + 1);
 #pragma unroll
-                                for (int i = 0; i < NW; ++i) v2[i] = __ldcg(src + i * kD);
+                                    for (int i = 0; i < NW; ++i) v2[i] = __ldcg(src + i * kD);
+                                }
+                                const float* wa = wgt_of(j);
+#pragma unroll
+                                for (int i = 0; i < NW; ++i) acc[i] = fmaf(wa[i], v1[i], acc[i]);
+                                if (j + 1 < nb) {
+                                    if (j + 2 < nb) {
+                                        const float* src = part_of(j + 2);
+#pragma unroll
+                                        for (int i = 0; i < NW; ++i) v1[i] = __ldcg(src + i * kD);
+                                    }
+                                    const float* wb = wgt_of(j + 1);
+#pragma unroll
+                                    for (int i = 0; i < NW; ++i) acc[i] = fmaf(wb[i], v2[i], acc[i]);
+                                }
                             }
-                            const float* wa = j <= kMergeFast ? s_wgt_w + (j - 1) * NQ : s_warp_w + (j - 1 - kMergeFast) * NW;
-#pragma unroll
-                            for (int i = 0; i < NW; ++i) acc[i] = fmaf(wa[i], v1[i], acc[i]);
-                            if (j + 1 < nb) {
-                                if (j + 2 < nb) {
-                                    const float* src = ws.part_o + ((long long)(s.cta_first + j + 2) * 2) * NQ * kD + c_off * kD + t;
+                        } else {
+#pragma unroll 1
+                            for (int j = 1; j < nb; ++j) {
+                                if (j > 1) {
+                                    const float* src = part_of(j);
 #pragma unroll
                                     for (int i = 0; i < NW; ++i) v1[i] = __ldcg(src + i * kD);
                                 }
-                                const float* wb = j + 1 <= kMergeFast ? s_wgt_w + j * NQ : s_warp_w + (j - kMergeFast) * NW;
+                                const float* wa = wgt_of(j);
 #pragma unroll
-                                for (int i = 0; i < NW; ++i) acc[i] = fmaf(wb[i], v2[i], acc[i]);
+                                for (int i = 0; i < NW; ++i) acc[i] = fmaf(wa[i], v1[i], acc[i]);
                             }
                         }
-                        for (int j = kMergeBatch; j < nseg; ++j) {   // beyond the batch (very long sequences): piece by piece
+                        for (int j = kMB; j < nseg; ++j) {   // beyond the batch (very long sequences): piece by piece
                             const long long sid = (long long)(s.cta_first + j) * 2;
                             wg_sync(wg);
                             if (t < rows_w) {

@@ -68,9 +68,6 @@ struct SelectParams {
         const float2* part;             // [B, nsel, n_chunks]
         long long logit_stride;
         int nsel, n_chunks;
-        int l2_hygiene;                 // bit 0: each logits row has ONE reader (this row's CTA): its lines are discarded
-                                        // from L2 once read, instead of being written back to HBM under the attention
-                                        // kernel's gather; bit 1: the finished score row is stored write-through
         float alpha;
         unsigned char list_first[64], list_cnt[64];
     } norm;

@@ -879,8 +879,6 @@ __device__ __forceinline__ void materialize_row(const SelectParams& p, int b, in
     const float* lg = p.norm.logits + ((long long)b * p.norm.nsel + first) * p.norm.logit_stride;
     const float alpha = p.norm.alpha;
     const int nvec = (N + 3) >> 2;
-    const bool discard = (p.norm.l2_hygiene & 1) != 0, wt = (p.norm.l2_hygiene & 2) != 0;
-    const int line_vecs = (int)(p.norm.logit_stride >> 2);   // whole lines only (logit_stride % 32 == 0 when discard is set)
     constexpr int kU = 4;   // vectors in flight per thread
 #pragma unroll 1
     for (int v0 = threadIdx.x; v0 < nvec; v0 += kU * kSelThreads) {
@@ -904,16 +902,6 @@ __device__ __forceinline__ void materialize_row(const SelectParams& p, int b, in
             }
 #pragma unroll
             for (int u = 0; u < kU; ++u) prob_accumulate4(a[u], x[u], st);
-            if (discard) {
-                // this warp has consumed its four lines of the row (the accumulation above needed every lane's data):
-                // lane 0 of each 8 drops the line from L2 -- nobody reads it again, and the scoring kernel of the next
-                // layer rewrites it
-#pragma unroll
-                for (int u = 0; u < kU; ++u) {
-                    const int v = v0 + u * kSelThreads;
-                    if ((threadIdx.x & 7) == 0 && v + 8 <= line_vecs) l2_discard128(lj + v);
-                }
-            }
         }
 #pragma unroll
         for (int u = 0; u < kU; ++u) {
@@ -924,8 +912,7 @@ __device__ __forceinline__ void materialize_row(const SelectParams& p, int b, in
                 if (n + 1 < N) r.y = __fmaf_rn(alpha, r.y, a[u][1]);
                 if (n + 2 < N) r.z = __fmaf_rn(alpha, r.z, a[u][2]);
                 if (n + 3 < N) r.w = __fmaf_rn(alpha, r.w, a[u][3]);
-                if (wt) st_wt16(hrow + v, r);
-                else hrow[v] = r;
+                hrow[v] = r;
             }
         }
     }
