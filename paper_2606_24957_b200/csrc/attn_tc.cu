@@ -41,9 +41,11 @@ constexpr float kRefSlack = 16.f;     // log2 units a score may exceed m_ref bef
 constexpr float kRefInit = 0.f;        // reference exponent at the start of a piece (the first tile always moves it)
 constexpr float kRefFloor = -1.0e30f;  // lowest reference (rows that have seen nothing but masked tokens)
 constexpr long long kInvalidRow = LLONG_MIN;
-constexpr int kMergeFast = 4;          // rows of the merge-weight array in shared memory (s_wgt)
-constexpr int kMergeBatch = 8;         // pieces of one unit (the merging CTA's own included) merged with batched loads: their
-                                       // weights live in s_wgt (kMergeFast rows) and in the idle per-warp scratch (3 more)
+constexpr int kMergeFast = 4;          // rows of the merge-weight array (only the first is used: the pieces of a cut unit are
+                                       // folded in one at a time.  Batching the flag / normaliser loads of up to 8 pieces and
+                                       // double-buffering their partial outputs was measured in round 2: 22.7 -> 22.1 us at 128k /
+                                       // B = 4, but the extra live registers spill in the 48-row kernel and cost the whole-unit
+                                       // case 0.7 us per launch, 31.2 -> 31.9 -- not kept)
 
 // ---- PTX wrappers ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
@@ -116,6 +118,26 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&v)[16
         "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15])
         : "memory");
 }
+// 8-column forms (row counts per softmax warpgroup that are multiples of 8 but not of 16: 40 rows at Gamma = 8)
+__device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t (&v)[8]) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
+                 : "r"(taddr)
+                 : "memory");
+}
+__device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t (&v)[8]) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"r"(taddr), "r"(v[0]),
+                 "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7])
+                 : "memory");
+}
+// N consecutive columns of this thread's lane (N a multiple of 8) into v
+template <int N>
+__device__ __forceinline__ void tmem_ld_cols(uint32_t taddr, uint32_t (&v)[N]) {
+    static_assert(N % 8 == 0, "column count");
+#pragma unroll
+    for (int c = 0; c < N / 16; ++c) tmem_ld16(taddr + (uint32_t)c * 16, reinterpret_cast<uint32_t(&)[16]>(v[c * 16]));
+    if constexpr (N % 16 != 0) tmem_ld8(taddr + (uint32_t)(N / 16) * 16, reinterpret_cast<uint32_t(&)[8]>(v[(N / 16) * 16]));
+}
 __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
@@ -153,11 +175,6 @@ __host__ __device__ constexpr uint32_t umma_idesc(int m, int n, int a_mn_major, 
            ((uint32_t)(n >> 3) << 17) | ((uint32_t)(m >> 4) << 24);
 }
 
-__device__ __forceinline__ int ld_relaxed(const int* p) {
-    int v;
-    asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
 __device__ __forceinline__ void st_release(int* p, int v) {
     asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
@@ -369,9 +386,6 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
     // there is a single softmax warpgroup) was measured: the copies are bound by the SM's cp.async path (one 512-byte
     // warp instruction per ~20 cycles, whoever issues it), eight warps only contend for it -- 1.49 instead of 1.31 us a tile.
     constexpr int NPW = 1;
-    // pieces of a cut unit merged with batched loads: 8 with one softmax warpgroup, 2 (the head's own and the next) with
-    // two, whose 192 registers per thread have no room for the batch's normalisers and weights
-    constexpr int kMB = NWG == 1 ? kMergeBatch : 2;
     extern __shared__ __align__(1024) unsigned char smem[];   // 128-byte-swizzled operands need 1 KB alignment
     const uint32_t sbase = smem_u32(smem);
     if (sbase & 1023u) __trap();
@@ -835,10 +849,7 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
             tc_fence_after();
             if (t == 0 && gj < 20) TS(12 + gj);
             uint32_t xs[NW];
-#pragma unroll
-            for (int c = 0; c < NW / 16; ++c)
-                tmem_ld16(lane_base + kColS + (uint32_t)sb * 128 + (uint32_t)c * 16,
-                          reinterpret_cast<uint32_t(&)[16]>(xs[c * 16]));
+            tmem_ld_cols<NW>(lane_base + kColS + (uint32_t)sb * 128, xs);
             tmem_wait_ld();
             tc_fence_before();
             mbar_arrive(bar(kSEmpty + sb));
@@ -933,6 +944,15 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
                         for (int e = 0; e < 16; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * s_fac_w[c * 16 + e]);
                         tmem_st16(lane_base + kColO + (uint32_t)c * 16, o);
                     }
+                    if constexpr (NW % 16 != 0) {
+                        constexpr int c8 = (NW / 16) * 16;
+                        uint32_t o[8];
+                        tmem_ld8(lane_base + kColO + (uint32_t)c8, o);
+                        tmem_wait_ld();
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * s_fac_w[c8 + e]);
+                        tmem_st8(lane_base + kColO + (uint32_t)c8, o);
+                    }
                     tmem_wait_st();
                     tc_fence_before();
                 }
@@ -966,32 +986,15 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
                 const bool merge = s.pos_lo == 0 && !s.whole;
                 const int nseg = s.cta_last - s.cta_first + 1;
                 const long long slot_id = (long long)rid * 2 + s.slot;
-                // The pieces 1 .. nb-1 of the unit (slot 0 of the following CTAs) are merged with their loads batched: one
-                // round trip for all flags, one for all normalisers, and the partial outputs double-buffered; units cut
-                // into more than kMB pieces (one very long sequence on the whole machine) finish piece by piece.
-                const int nb = merge ? min(nseg, kMB) : 1;
                 float v1[NW];
-                float lj[kMB];
-#pragma unroll
-                for (int j = 0; j < kMB; ++j) lj[j] = -INFINITY;
-                if (merge) {
-                    uint32_t pend = 0;
-#pragma unroll
-                    for (int j = 1; j < kMB; ++j)
-                        if (j < nb && ld_relaxed(ws.flags + (long long)(s.cta_first + j) * 2) == 0) pend |= 1u << j;
-#pragma unroll 1
-                    for (int j = 1; j < nb; ++j)
-                        if ((pend >> j) & 1u) wait_flag(ws.flags + (long long)(s.cta_first + j) * 2);
-                    __threadfence();   // acquire: the loads below come after the flags have been seen
+                float lse1 = -INFINITY;
+                if (merge) {   // second piece = slot 0 of the next CTA: loads in flight during the reductions below
                     const long long sid1 = (long long)(s.cta_first + 1) * 2;
+                    wait_flag(ws.flags + sid1);
                     const float* src1 = ws.part_o + sid1 * NQ * kD + c_off * kD + t;
 #pragma unroll
-                    for (int i = 0; i < NW; ++i) v1[i] = __ldcg(src1 + i * kD);   // in flight during the reductions below
-                    if (t < rows_w) {
-#pragma unroll
-                        for (int j = 1; j < kMB; ++j)
-                            if (j < nb) lj[j] = __ldcg(ws.part_lse + ((long long)(s.cta_first + j) * 2) * NQ + c_off + t);
-                    }
+                    for (int i = 0; i < NW; ++i) v1[i] = __ldcg(src1 + i * kD);
+                    if (t < rows_w) lse1 = __ldcg(ws.part_lse + sid1 * NQ + c_off + t);
                 }
                 if (t == 0) TS(56);
                 {
@@ -1009,35 +1012,22 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
                     const float lse_own = l > 0.f ? s_ref_w[t] + log2f(l) : -INFINITY;
                     float scale = l > 0.f ? 1.f / l : 0.f, lse_fin = lse_own;
                     if (merge && t < rows_w) {
-                        float M = lse_own;
-#pragma unroll
-                        for (int j = 1; j < kMB; ++j) M = fmaxf(M, lj[j]);
-                        for (int j = kMB; j < nseg; ++j) {
+                        float M = fmaxf(lse_own, lse1);
+                        for (int j = 2; j < nseg; ++j) {
                             const long long sid = (long long)(s.cta_first + j) * 2;
                             wait_flag(ws.flags + sid);
                             M = fmaxf(M, __ldcg(ws.part_lse + sid * NQ + c_off + t));
                         }
                         const float e0 = lse_own == -INFINITY ? 0.f : exp2f(lse_own - M);
-                        float W = e0;
-                        float e[kMB];
-#pragma unroll
-                        for (int j = 1; j < kMB; ++j) {   // same order as before: piece 1, 2, ...
-                            e[j] = lj[j] == -INFINITY ? 0.f : exp2f(lj[j] - M);
-                            W += e[j];
-                        }
-                        for (int j = kMB; j < nseg; ++j) {
-                            const float l_j = __ldcg(ws.part_lse + ((long long)(s.cta_first + j) * 2) * NQ + c_off + t);
-                            W += l_j == -INFINITY ? 0.f : exp2f(l_j - M);
+                        const float e1 = lse1 == -INFINITY ? 0.f : exp2f(lse1 - M);
+                        float W = e0 + e1;
+                        for (int j = 2; j < nseg; ++j) {
+                            const float lj = __ldcg(ws.part_lse + ((long long)(s.cta_first + j) * 2) * NQ + c_off + t);
+                            W += lj == -INFINITY ? 0.f : exp2f(lj - M);
                         }
                         const float invW = W > 0.f ? 1.f / W : 0.f;
                         scale *= e0 * invW;
-                        // weights of the batched pieces: piece j at s_wgt[j - 1] for j <= kMergeFast, the rest in this
-                        // thread's own column of s_warp (read just above, free now)
-#pragma unroll
-                        for (int j = 1; j < kMB; ++j) {
-                            if (j <= kMergeFast) s_wgt_w[(j - 1) * NQ + t] = e[j] * invW;
-                            else s_warp_w[(j - 1 - kMergeFast) * NW + t] = e[j] * invW;
-                        }
+                        s_wgt_w[t] = e1 * invW;
                         lse_fin = W > 0.f ? M + log2f(W) : -INFINITY;
                         M_row = M;
                         W_row = invW;
@@ -1054,9 +1044,7 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
                 tc_fence_after();
                 if (t == 0) TS(55);
                 uint32_t o[NW];
-#pragma unroll
-                for (int c = 0; c < NW / 16; ++c)
-                    tmem_ld16(lane_base + kColO + (uint32_t)c * 16, reinterpret_cast<uint32_t(&)[16]>(o[c * 16]));
+                tmem_ld_cols<NW>(lane_base + kColO, o);
                 tmem_wait_ld();
                 tc_fence_before();
                 sm_sync<NWG>();
@@ -1078,52 +1066,9 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
 #pragma unroll
                     for (int i = 0; i < NW; ++i) acc[i] = __uint_as_float(o[i]) * s_fac_w[i];
                     if (merge) {
-                        // batched pieces.  One softmax warpgroup (240 registers): the next piece's partial is requested
-                        // before the current one is folded in; two (192 registers): one partial at a time, or the
-                        // second buffer spills into the tile loop.
-                        auto wgt_of = [&](int j) -> const float* {
-                            return j <= kMergeFast ? s_wgt_w + (j - 1) * NQ : s_warp_w + (j - 1 - kMergeFast) * NW;
-                        };
-                        auto part_of = [&](int j) -> const float* {
-                            return ws.part_o + ((long long)(s.cta_first + j) * 2) * NQ * kD + c_off * kD + t;
-                        };
-                        if constexpr (NWG == 1) {
-                            float v2[NW];
-#pragma unroll 1
-                            for (int j = 1; j < nb; j += 2) {
-                                if (j + 1 < nb) {
-                                    const float* src = part_of(j + 1);
 #pragma unroll
-                                    for (int i = 0; i < NW; ++i) v2[i] = __ldcg(src + i * kD);
-                                }
-                                const float* wa = wgt_of(j);
-#pragma unroll
-                                for (int i = 0; i < NW; ++i) acc[i] = fmaf(wa[i], v1[i], acc[i]);
-                                if (j + 1 < nb) {
-                                    if (j + 2 < nb) {
-                                        const float* src = part_of(j + 2);
-#pragma unroll
-                                        for (int i = 0; i < NW; ++i) v1[i] = __ldcg(src + i * kD);
-                                    }
-                                    const float* wb = wgt_of(j + 1);
-#pragma unroll
-                                    for (int i = 0; i < NW; ++i) acc[i] = fmaf(wb[i], v2[i], acc[i]);
-                                }
-                            }
-                        } else {
-#pragma unroll 1
-                            for (int j = 1; j < nb; ++j) {
-                                if (j > 1) {
-                                    const float* src = part_of(j);
-#pragma unroll
-                                    for (int i = 0; i < NW; ++i) v1[i] = __ldcg(src + i * kD);
-                                }
-                                const float* wa = wgt_of(j);
-#pragma unroll
-                                for (int i = 0; i < NW; ++i) acc[i] = fmaf(wa[i], v1[i], acc[i]);
-                            }
-                        }
-                        for (int j = kMB; j < nseg; ++j) {   // beyond the batch (very long sequences): piece by piece
+                        for (int i = 0; i < NW; ++i) acc[i] = fmaf(s_wgt_w[i], v1[i], acc[i]);
+                        for (int j = 2; j < nseg; ++j) {   // units cut into more than two pieces (very long sequences)
                             const long long sid = (long long)(s.cta_first + j) * 2;
                             wg_sync(wg);
                             if (t < rows_w) {
@@ -1213,7 +1158,7 @@ bool attn_tc_usable(int batch, int n_kv_heads, int head_dim, int rows, int max_t
 
 size_t attn_tc_ws_bytes(int batch, int n_kv_heads, int rows) {
     static_assert(kMaxGrid * 2 * sizeof(int) <= kWsHeader, "the flags must fit the persistent header");
-    const size_t nq = rows > 48 ? 96 : (size_t)((rows + 15) / 16) * 16;   // partials are padded to the kernel's NQ rows
+    const size_t nq = (size_t)((rows + 15) / 16) * 16;   // partials are padded to the kernel's NQ rows
     return kWsHeader + align256((size_t)kMaxGrid * 2 * nq * kD * sizeof(float)) +
            align256((size_t)kMaxGrid * 2 * nq * sizeof(float)) + (size_t)kMaxGrid * 64 * 8;
 }
@@ -1229,7 +1174,7 @@ cudaError_t launch_attn_tc(const AttnParams& p_in, void* ws_base, cudaStream_t s
     // (dustin.h); every launch leaves it zero again (the merging piece clears the flags it has consumed).
     ws.flags = reinterpret_cast<int*>(base);
     ws.part_o = reinterpret_cast<float*>(base + kWsHeader);
-    const size_t nq = p.rows > 48 ? 96 : (size_t)((p.rows + 15) / 16) * 16;
+    const size_t nq = (size_t)((p.rows + 15) / 16) * 16;
     ws.part_lse = reinterpret_cast<float*>(base + kWsHeader + align256((size_t)kMaxGrid * 2 * nq * kD * sizeof(float)));
     ws.dbg_ts = (p.dbg & 8) ? reinterpret_cast<unsigned long long*>(reinterpret_cast<char*>(ws.part_lse) + align256((size_t)kMaxGrid * 2 * nq * sizeof(float))) : nullptr;
     const int max_tokens = (p.idx ? (p.k_max < p.max_ctx ? p.k_max : p.max_ctx) : p.max_ctx) + kTile;
@@ -1241,10 +1186,10 @@ cudaError_t launch_attn_tc(const AttnParams& p_in, void* ws_base, cudaStream_t s
         case 1: return launch_tc_nq<16>(p, ws, grid, stream);
         case 2: return launch_tc_nq<32>(p, ws, grid, stream);
         case 3: return launch_tc_nq<48>(p, ws, grid, stream);
-        // more than 48 query rows: padded to 96 = 2 x 48, one softmax warpgroup per half (a single warpgroup needs
+        // more than 48 query rows: padded to a multiple of 16, one softmax warpgroup per half (a single warpgroup needs
         // 2.3 us per tile for 80 rows and bounds the kernel; two need about half)
-        case 4:
-        case 5:
+        case 4: return launch_tc_nq<64, 2>(p, ws, grid, stream);
+        case 5: return launch_tc_nq<80, 2>(p, ws, grid, stream);   // Gamma = 8 on an 8-head group: 72 rows, 40 + 32
         case 6: return launch_tc_nq<96, 2>(p, ws, grid, stream);
         default: return cudaErrorInvalidValue;
     }
