@@ -112,9 +112,10 @@ def test_global_list_and_repeated_indices():
     assert torch.allclose(lse.cpu().double(), lse_ref, atol=2e-3, rtol=0)
 
 
-@pytest.mark.parametrize("T,r", [(1, 1), (3, 2), (16, 4), (12, 8), (2, 16)])
+@pytest.mark.parametrize("T,r", [(1, 1), (3, 2), (16, 4), (12, 8), (2, 16), (13, 4), (9, 8), (10, 8), (11, 8)])
 def test_query_row_counts(T, r):
-    """T * r from 1 to 96 query rows per KV head: every NQ instantiation of the tcgen05 kernel."""
+    """T * r from 1 to 96 query rows per KV head: every NQ instantiation of the tcgen05 kernel (16, 32, 48 rows on one
+    softmax warpgroup; 52 -> 64 = 2 x 32, 72 and 80 -> 80 = 2 x 40 with the 8-column TMEM loads, 88 and 96 -> 2 x 48)."""
     B, N, Hkv, d = 2, 900, 2, 128
     x = _inputs(B, N, Hkv * r, Hkv, d, T, 16 + T)
     idx, cnt = _lists(B, Hkv, N, [333, 500], 500, 8)
@@ -151,3 +152,17 @@ def test_cnt_null_means_full_lists(B, Hkv, k):
     with pytest.raises(api.DustinError):
         api.sparse_verify_attn(sh, api.KV.contiguous_nhd(dev["k"], dev["v"], None), dev["q"], dev["k_new"],
                                dev["v_new"], wide, None, torch.empty_like(dev["q"]), ws)
+
+
+def test_cuts_inside_the_new_row_tile_move_to_the_unit_start():
+    """Short lists on a grid of as many CTAs as tiles: the equal cuts of the concatenated token space fall inside the
+    new-row tiles (128 virtual positions at the head of every unit) and must move down to the unit's start -- no piece
+    may begin in the padding of that tile.  Several list lengths so that one, two and three cuts
+    land in one tile, with and without cache rows behind it."""
+    B, N, Hkv, d, T, r = 3, 700, 2, 128, 5, 4
+    x = _inputs(B, N, Hkv * r, Hkv, d, T, 91)
+    for counts in ([40], [0, 40, 300], [7, 129, 0, 64, 511, 1], [200, 0, 0, 3]):
+        idx, cnt = _lists(B, Hkv, N, counts, 512, 92)
+        out, lse, o_ref, lse_ref = _run_both(x, idx, cnt, N)
+        H.check_attn(out, o_ref)
+        assert torch.allclose(lse.cpu().double(), lse_ref, atol=2e-3, rtol=0)
