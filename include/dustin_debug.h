@@ -36,7 +36,7 @@ typedef enum dustin_knob {
     DUSTIN_KNOB_SELECT_SPLIT = 3,   /* CTAs per selection row (thread-block cluster): 0 (default) = heuristic, 1/2/4/8    */
     DUSTIN_KNOB_DRAFT_HOIST = 4,    /* 1 (default): the fused call runs the draft tier of Eq. 6 (I_draft) in a kernel of its
                                        own beside the K stream of a1; 0: both tiers after a1                               */
-    DUSTIN_KNOB_SCORE_CHUNK = 5,    /* tokens per CTA of the scoring kernel (multiple of 128); 0 (default) = heuristic      */
+    DUSTIN_KNOB_SCORE_CHUNK = 5,    /* tokens per CTA of the scoring kernel (multiple of 16, >= 64); 0 (default) = score_plan */
     DUSTIN_KNOB_SELECT_TRACE = 6,   /* 1: selection kernels write %globaltimer samples per phase into the buffer given to
                                        dustin_debug_trace_buffer                                                           */
     DUSTIN_KNOB_COUNT = 16

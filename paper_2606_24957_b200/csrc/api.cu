@@ -60,40 +60,37 @@ int check_kv(const dustin_shape_t* s, const dustin_kv_t* kv, bool need_v, KvView
     return DUSTIN_OK;
 }
 
+constexpr int kMinScoreChunk = 64;   // fewest tokens per scoring CTA (the workspace holds one softmax partial per CTA and head)
+
 float scale_log2_of(const dustin_shape_t* s) {
     const float sc = s->sm_scale == 0.f ? (float)(1.0 / std::sqrt((double)s->head_dim)) : s->sm_scale;
     return sc * kLog2e;
 }
 
 // ---- scoring plan ---------------------------------------------------------------------------------------------
-// Tokens per scoring CTA (all scored KV groups of those tokens): as large as possible while the grid still holds >= 8
-// CTAs per SM (of the current device: 148 on B200), never below 256.  group_slots = how many groups the 8 warps of a CTA serve side by side;
-// n_parts = softmax partials per (sequence, head) = CTAs per sequence.
-void score_plan(int batch, int n_groups, int max_ctx, int* chunk_tokens, int* n_parts, int* group_slots) {
+// Tokens per scoring CTA = CTAs per sequence (the 16-token tiles of a sequence are dealt round-robin to its CTAs, score.cu,
+// so the chunk only sets the CTA count).  group_slots = how many scored KV groups the 8 warps of a CTA serve side by side;
+// the 8 / group_slots warps that share a group take every (8 / group_slots)-th tile each.  n_parts = softmax partials per
+// (sequence, head) = CTAs per sequence.
+// The rule is "a fixed number of tiles per warp", whatever the grid then is -- measured in round 2 on every workload of
+// bench.py (fused layer, us; tiles per warp 4 / 8 / 16 / 32 where it was tried):
+//   8 scored groups (Qwen spread):  32k B=16  226.3 / 224.2 / 228.6 / 236.4;  16k  148.2 / 147.6 / 149.6 / 155.8;
+//                                   8k  108.1 / 107.2 / 110.7 / 116.3;  4k  91.7 / 91.7 / 93.9 / 97.8;  32k B=4  - / 93.4 / 100.9 / 99.4
+//   4 scored groups (Llama spread): 32k  156.5 / 154.9 / 158.0 / -;  16k  112.6 / 114.2 / 114.5 / -;  8k  89.6 / 90.0 / 95.2 / -
+//   1 scored group (packed):        32k  95.2 / 95.7 / 88.8 (16 tiles) ;  128k B=4  97.1 / 96.3 / 92.3;  8k  77.2 / 75.6 / 76.9
+//   paged ragged (4 groups):        380.4 / 344.6 / 338.0 / 344.2
+// i.e. 8 tiles per warp, 16 when the CTA's warps share one or two groups or the cache is paged.  Round 1 used >= 256 tokens
+// per CTA and cut grids of one to three waves down to exactly one wave: at 8 groups that is 16 tiles per warp or more --
+// config 3 loses 4 us per layer to it, 16k 14 us, 32k at batch 4 13 us.
+void score_plan(int batch, int n_groups, int max_ctx, bool paged, int* chunk_tokens, int* n_parts, int* group_slots) {
+    (void)batch;
     int slots = 1;
     while (slots < n_groups && slots < 8) slots <<= 1;
-    // CTAs per sequence = ceil(max_ctx / chunk): the tiles of a sequence are dealt round-robin to them (score.cu), so
-    // chunk only sets the CTA count: as few as keep >= 8 CTAs per SM in the grid, at least 256 tokens each.
-    // Measured at config 3 (B = 16, 32k): 128 CTAs per sequence 172 us, 64: 185, 27 (one wave): 188.
-    int chunk = 2048;
-    const int sms = device_sm_count();
-    auto ctas = [&](int c) { return (long long)batch * ((max_ctx + c - 1) / c); };
-    while (chunk > 256 && ctas(chunk) < sms * 8) chunk >>= 1;
-    // A grid a little above one wave (3 resident CTAs per SM) pays a whole second wave for the overhang: between one
-    // and three waves use exactly one (measured at B = 16: 8k 64.5 -> 54.6 us, 16k unchanged, 32k stays at 4.6 waves).
-    const long long resident = (long long)sms * 3;
-    // One or two scored KV groups (the packed subset): the 8 warps of a CTA share a group, so a 256-token CTA gives each
-    // warp two tiles and the fixed cost per CTA dominates: one wave of larger CTAs (measured, B = 16, 32k, one group:
-    // 38 -> 31 us).
-    if (((ctas(chunk) > resident && ctas(chunk) < 3 * resident) || (slots <= 2 && ctas(chunk) > resident)) &&
-        batch <= resident) {
-        const int per_seq = (int)(resident / batch);
-        const int quantum = 16 * (8 / slots);
-        chunk = ((max_ctx + per_seq - 1) / per_seq + quantum - 1) / quantum * quantum;
-        if (chunk < 256) chunk = 256;
-    }
-    const int forced = knob(DUSTIN_KNOB_SCORE_CHUNK);   // tuning aid: tokens per scoring CTA (multiple of 128)
-    if (forced >= 128) chunk = (forced + 127) / 128 * 128;
+    const int n_sub = 8 / slots;
+    const int tiles_per_warp = (slots <= 2 || paged) ? 16 : 8;
+    int chunk = 16 * n_sub * tiles_per_warp;
+    const int forced = knob(DUSTIN_KNOB_SCORE_CHUNK);   // tuning aid: tokens per scoring CTA (multiple of 16)
+    if (forced >= kMinScoreChunk) chunk = (forced + 15) / 16 * 16;
     *chunk_tokens = chunk;
     *group_slots = slots;
     *n_parts = max_ctx > 0 ? (max_ctx + chunk - 1) / chunk : 1;   // one partial per (CTA, head): the warps of a CTA that
@@ -104,9 +101,9 @@ struct ScoreWs {
     size_t logits, part, stats, total;
 };
 ScoreWs score_ws(int batch, int nsel, int max_ctx) {
-    // upper bound of the partial count: one per CTA at the smallest chunk (256 tokens)
+    // upper bound of the partial count: one per CTA at the smallest chunk
     const size_t stride = ((size_t)max_ctx + 3) & ~(size_t)3;
-    const size_t n_chunks = ((size_t)max_ctx + 255) / 256 + 1;
+    const size_t n_chunks = ((size_t)max_ctx + kMinScoreChunk - 1) / kMinScoreChunk + 1;   // score_plan never goes below it
     ScoreWs w;
     w.logits = 0;
     w.part = align256(w.logits + (size_t)batch * nsel * stride * sizeof(float));
@@ -240,7 +237,7 @@ int run_score(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q,
     p.n_lists = n_lists;
     p.scale_log2 = scale_log2_of(shape);
     p.defer_wait = defer_wait ? 1 : 0;
-    score_plan(p.batch, p.n_groups, p.max_ctx, &p.chunk_tokens, &p.n_chunks, &p.group_slots);
+    score_plan(p.batch, p.n_groups, p.max_ctx, p.kv.page_table != nullptr, &p.chunk_tokens, &p.n_chunks, &p.group_slots);
     p.logit_stride = ((long long)p.max_ctx + 3) & ~3ll;
     char* base = static_cast<char*>(ws) + kWsHeader;   // the persistent header belongs to the attention stage
     p.logits = reinterpret_cast<float*>(base + w.logits);
