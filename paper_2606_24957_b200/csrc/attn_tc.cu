@@ -10,7 +10,9 @@
 // partial (o, lse) in the workspace and the LAST piece to finish (a per-unit arrival counter) merges them in
 // segment order, so the result does not depend on which CTA happens to be last.
 //
-// Roles inside a CTA (384 threads; setmaxnreg moves registers from the other warpgroups to the softmax one):
+// Roles inside a CTA (384 threads; setmaxnreg moves registers from the other warpgroups to the softmax one: 240 / 96 / 96;
+// with two softmax warpgroups, 512 threads: 200 / 200 / 56 / 56 -- measured: resolvers or producers below 56 registers
+// spill into their loops and cost 2-4 us per launch, 208 for the softmax leaves them 48):
 //   warps 0-3  softmax warpgroup: thread = one token of the 128-token tile = one TMEM lane
 //   warp  8    MMA issuer (one thread) and TMEM allocation (warps 9-11 only donate their registers)
 //   warps 4-7  producers: resolve index -> (page table ->) row address, stream K and V tiles with 16-byte cp.async
@@ -569,7 +571,7 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
     if ((warp >= 4 && warp < 8) || (NPW == 2 && warp >= 12)) {
         // ================= producers ===========================================================================
         if constexpr (NWG == 1) asm volatile("setmaxnreg.dec.sync.aligned.u32 96;");
-        else asm volatile("setmaxnreg.dec.sync.aligned.u32 88;");
+        else asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
         const bool do_k = warp < 8, do_v = NPW == 1 || warp >= 12;
         const int pw = warp & 3, ptid = do_k ? tid - 128 : -1;
         // lane = 16-byte chunk c of rows 2i + h (h = lane / 16), i = 0..15, of this warp's 32 rows of the tile.
@@ -681,7 +683,7 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
     } else if (warp >= 8 && warp < 12) {
         // ================= MMA issuer (one thread of warp 8) =====================================================
         if constexpr (NWG == 1) asm volatile("setmaxnreg.dec.sync.aligned.u32 96;");
-        else asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
+        else asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
         if (warp > 8) {
             // ================= resolver warps 9 and 10: warp 9 + w serves the gathered tiles of ordinal w, w + 2, ... ====
             // index entry -> (page table ->) absolute addresses of the K and the V row, for the 128 rows of a tile of
@@ -822,7 +824,7 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
         // the same TMEM lanes (warp % 4) and disjoint columns, rows of s_ref / s_fac / P / partials, and meet only on
         // the mbarriers (S consumed, P ready: 128 arrivals each) and where a flag is published or cleared.
         if constexpr (NWG == 1) asm volatile("setmaxnreg.inc.sync.aligned.u32 240;");
-        else asm volatile("setmaxnreg.inc.sync.aligned.u32 192;");
+        else asm volatile("setmaxnreg.inc.sync.aligned.u32 200;");
         constexpr int NW = NQ / NWG;
         const int wg = (NWG == 2 && warp >= 12) ? 1 : 0;
         const int c_off = wg * NW, wq = warp & 3;
