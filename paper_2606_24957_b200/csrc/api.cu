@@ -288,7 +288,7 @@ int check_select(const dustin_select_t* sel, int32_t k_max) {
 int run_select(int32_t batch, int32_t max_ctx, const int32_t* seq_lens, const dustin_select_t* sel,
                const float* s_draft, int64_t draft_list_stride, const float* s_target, int32_t* idx_out,
                int32_t* cnt_out, int32_t k_max, cudaStream_t stream, const SelectParams::Norm* norm = nullptr,
-               int mode = 0, uint32_t* draft_mask = nullptr) {
+               int mode = 0, uint32_t* draft_mask = nullptr, int draft_rows_per_cta = 1) {
     int rc = check_select(sel, k_max);
     if (rc) return rc;
     if (batch <= 0 || max_ctx < 0 || !s_draft || !s_target || !idx_out || !cnt_out) return DUSTIN_ERR_INVALID_ARG;
@@ -317,6 +317,7 @@ int run_select(int32_t batch, int32_t max_ctx, const int32_t* seq_lens, const du
     if (norm) p.norm = *norm;
     p.draft_mask = draft_mask;
     p.draft_mask_stride = (long long)select_mask_words(max_ctx);
+    p.draft_rows_per_cta = draft_rows_per_cta;
     p.trace = nullptr;
     if (mode == 2 && norm) {   // few long rows: one thread-block cluster per row (select_cluster.cu)
         const int C = select_cluster_size(p);
@@ -510,8 +511,27 @@ int dustin_verify_layer_fused(const dustin_shape_t* shape, const dustin_kv_t* kv
     uint32_t* draft_mask = reinterpret_cast<uint32_t*>(base + kWsHeader + sw.total);
     const bool hoist = knob(DUSTIN_KNOB_DRAFT_HOIST) != 0 && pdl_enabled() && shape->max_ctx > 0;
     if (hoist) {
+        // Rows per draft-tier CTA (select.cu: fewer CTAs let the scoring kernel start earlier).  The draft tier must stay
+        // well inside the K stream it hides under: a row of N tokens takes it about 13 us + 0.6 ns per token there, the
+        // stream groups * B * N * 256 B at ~6.4 TB/s; rows per CTA = three quarters of that ratio, at most 4 (measured, fused
+        // layer, us, 1 / 2 / 3 / 4 / 6 rows: 32k B=16  224.3 / 224.0 / 222.7 / 222.5 / 251.0;  16k  147.7 / 146.3 / 146.0 /
+        // 154.9 / 179;  8k  107.4 / 107.5 / 117.8 / 128 / 149;  64k B=8  226.3 / 226.5 / 247 / 279 / 339).  Ragged batches
+        // keep one row per CTA: the lengths are device data, and a stream shorter than estimated would expose the tier.
+        int rpc = 1;
+        if (!kv->seq_lens) {
+            int n_groups = 0;
+            const int r = shape->n_q_heads / shape->n_kv_heads;
+            for (int g = 0; g < shape->n_kv_heads; ++g) {
+                const uint64_t gm = (r >= 64 ? ~0ull : ((1ull << r) - 1ull)) << (g * r);
+                if (head_mask & gm) ++n_groups;
+            }
+            const double t_row = 13.0 + 0.6e-3 * shape->max_ctx;
+            const double t_a1 = (double)n_groups * shape->batch * shape->max_ctx * shape->head_dim * 2.0 / 6.4e6;
+            rpc = (int)(0.75 * t_a1 / t_row);
+            rpc = rpc < 1 ? 1 : (rpc > 4 ? 4 : rpc);
+        }
         rc = run_select(shape->batch, shape->max_ctx, kv->seq_lens, select, s_draft, draft_list_stride, hist_inout,
-                        idx_out, cnt_out, k_max, st, nullptr, 1, draft_mask);
+                        idx_out, cnt_out, k_max, st, nullptr, 1, draft_mask, rpc);
         if (rc) return rc;
     }
     // a1 + a2: scores of verify position 0 (reading A3), accumulated straight into hist (Eq. 5)

@@ -60,6 +60,7 @@ struct SelectParams {
     // the draft-tier kernel and read by the target-tier kernel; draft_mask_stride words per row.
     uint32_t* draft_mask;
     long long draft_mask_stride;
+    int draft_rows_per_cta;   // draft-tier kernel of the fused call: rows that one of its CTAs walks (0 / 1: one row each)
     // Row materialisation (fused entry point): when norm.logits != nullptr the kernel first computes its own target
     // row, s_target[b,l,n] = alpha * s_target[b,l,n] + sum_j exp2(logit_j[n] - M_j) / Z_j (a1's normalisation and
     // Eq. 5), from the logits and partials that score_logits_kernel left in the workspace, and writes it back.

@@ -103,7 +103,12 @@ cudaError_t launch_select(const SelectParams& p_in, cudaStream_t stream, int mod
     const dim3 rows(p.n_lists, p.batch);
     if (mode == 1) {
         // grid.x CTAs walk the rows blockIdx.x, blockIdx.x + gridDim.x, ...: here one row each
-        const dim3 flat(n_rows);
+        // Fewer CTAs than rows when the scoring kernel beside it runs long enough (api.cu): the scoring kernel can only
+        // start once EVERY CTA of this grid has started, and at the end of the previous layer's attention kernel only the
+        // SMs that kernel left idle can take them early -- 43 CTAs of three rows instead of 128 of one: 224.3 -> 222.7 us
+        // per layer at config 3 (six rows: 251 us, the draft tier then outlasts the K stream).
+        const int rpc = light && p.draft_rows_per_cta > 1 ? p.draft_rows_per_cta : 1;
+        const dim3 flat((n_rows + rpc - 1) / rpc);
         if (light)
             return vec ? launch_one<sel256::select_kernel<true, sel256::kSelDraft>>(p, flat, 256, smem, kKernSelectDraft, stream)
                        : launch_one<sel256::select_kernel<false, sel256::kSelDraft>>(p, flat, 256, smem, kKernSelectDraft, stream);
