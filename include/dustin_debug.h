@@ -39,6 +39,9 @@ typedef enum dustin_knob {
     DUSTIN_KNOB_SCORE_CHUNK = 5,    /* tokens per CTA of the scoring kernel (multiple of 16, >= 64); 0 (default) = score_plan */
     DUSTIN_KNOB_SELECT_TRACE = 6,   /* 1: selection kernels write %globaltimer samples per phase into the buffer given to
                                        dustin_debug_trace_buffer                                                           */
+    DUSTIN_KNOB_L2_HYGIENE = 7,     /* fused call, 1 (default): a selection CTA drops the logits scratch of its row from L2
+                                       (discard.global.L2) when it is done, where every logits row has a single reader; 0: the
+                                       17 MB of dirty lines per layer are written back while the attention kernel gathers    */
     DUSTIN_KNOB_COUNT = 16
 } dustin_knob;
 void    dustin_tune_set(int32_t knob, int32_t value);

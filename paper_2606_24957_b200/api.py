@@ -125,7 +125,8 @@ DEBUG_EXPORTS = ("dustin_tune_attn_split_tokens", "dustin_tune_attn_impl", "dust
                  "dustin_kernel_name", "dustin_probe_gather", "dustin_debug_occupy")
 
 # enum dustin_knob (dustin_debug.h)
-KNOB_PDL, KNOB_FUSED_ROWS, KNOB_ATTN_TRACE, KNOB_SELECT_SPLIT, KNOB_DRAFT_HOIST, KNOB_SCORE_CHUNK, KNOB_SELECT_TRACE = range(7)
+(KNOB_PDL, KNOB_FUSED_ROWS, KNOB_ATTN_TRACE, KNOB_SELECT_SPLIT, KNOB_DRAFT_HOIST, KNOB_SCORE_CHUNK, KNOB_SELECT_TRACE,
+ KNOB_L2_HYGIENE) = range(8)
 
 
 @dataclass

@@ -263,6 +263,10 @@ int run_score(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q,
         norm_out->nsel = p.nsel;
         norm_out->n_chunks = p.n_chunks;
         norm_out->alpha = alpha;
+        // one reader per logits row: one list per sequence, or every KV group has a subset head of its own (no empty group
+        // that would read all rows, reading A2); rows made of whole 128-byte lines
+        norm_out->discard_logits = (n_lists == 1 || p.n_groups == shape->n_kv_heads) && (p.logit_stride & 31) == 0 &&
+                                   knob(DUSTIN_KNOB_L2_HYGIENE) != 0;
         std::memcpy(norm_out->list_first, p.list_first, sizeof p.list_first);
         std::memcpy(norm_out->list_cnt, p.list_cnt, sizeof p.list_cnt);
     }

@@ -41,6 +41,12 @@ __device__ __forceinline__ long long kv_row_offset(const KvView& kv, int b, int 
 }
 
 // ---- memory -------------------------------------------------------------------------------------------------
+// The 128-byte line at p (aligned) is no longer needed: L2 may drop it without writing it back.  Its content is
+// undefined afterwards.
+__device__ __forceinline__ void l2_discard128(const void* p) {
+    asm volatile("discard.global.L2 [%0], 128;" ::"l"(p) : "memory");
+}
+
 // 16-byte streaming load that does not pollute L1 (the K stream is read exactly once).
 __device__ __forceinline__ uint4 ldg_stream16(const void* p) {
     uint4 r;

@@ -69,6 +69,9 @@ struct SelectParams {
         const float2* part;             // [B, nsel, n_chunks]
         long long logit_stride;
         int nsel, n_chunks;
+        int discard_logits;             // every logits row has ONE reader (the CTA of the list it feeds) and is made of whole
+                                        // 128-byte lines: that CTA drops the row from L2 when it is done (the lines are dirty
+                                        // scratch: left alone they are written back to HBM under the attention kernel's gather)
         float alpha;
         unsigned char list_first[64], list_cnt[64];
     } norm;

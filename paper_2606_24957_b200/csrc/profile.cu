@@ -60,7 +60,7 @@ ProfScope::~ProfScope() {
 // ---- knobs (dustin_debug.h) ---------------------------------------------------------------------------------------
 namespace {
 constexpr int kKnobDefaults[DUSTIN_KNOB_COUNT] = {/*PDL*/ 1, /*FUSED_ROWS*/ 1, /*ATTN_TRACE*/ 0, /*SELECT_SPLIT*/ 0,
-                                                  /*DRAFT_HOIST*/ 1, /*SCORE_CHUNK*/ 0, /*SELECT_TRACE*/ 0};
+                                                  /*DRAFT_HOIST*/ 1, /*SCORE_CHUNK*/ 0, /*SELECT_TRACE*/ 0, /*L2_HYGIENE*/ 1};
 std::atomic<int> g_knob[DUSTIN_KNOB_COUNT];
 std::atomic<bool> g_knob_set[DUSTIN_KNOB_COUNT];
 std::atomic<void*> g_trace_ptr{nullptr};

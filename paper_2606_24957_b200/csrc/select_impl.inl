@@ -1047,6 +1047,17 @@ __device__ __forceinline__ void select_row(const SelectParams& p, int b, int l, 
         for (int i = threadIdx.x; i < p.k_max / 4; i += kSelThreads) out4[i] = src4[i];
     }
     if (threadIdx.x == 0) *cnt_out = (int)total;
+    // The logits of the heads that feed this row are scratch nobody reads again (one reader per logits row, whole lines:
+    // api.cu): drop them from L2, or their dirty lines are written back to HBM while the attention kernel gathers.  Every
+    // thread of the CTA is long past its last read of them (the barrier that ends materialize_row).
+    if (own_row && p.norm.discard_logits) {
+        const int first = p.norm.list_first[l], nh = p.norm.list_cnt[l];
+        const int lines = (int)(p.norm.logit_stride >> 5);
+        for (int j = 0; j < nh; ++j) {
+            const float* row = p.norm.logits + ((long long)b * p.norm.nsel + first + j) * p.norm.logit_stride;
+            for (int i = threadIdx.x; i < lines; i += kSelThreads) l2_discard128(row + (long long)i * 32);
+        }
+    }
 }
 
 template <bool VEC, int MODE>
