@@ -854,6 +854,9 @@ def main():
         traffic, traffic_commit = ncu_traffic(kernel)
         return {"kernel": kernel, "bound": "hbm", "achieved": round(ach, 1), "peak": peak, "unit": "GB/s",
                 "frac": round(ach / peak, 4), "traffic": traffic, "traffic_commit": traffic_commit,
+                # the measured peak is a COPY (read + write) bandwidth; a read-only stream can run a few per cent above it
+                **({"frac_note": "above 1: the peak is the measured copy (read+write) bandwidth, this kernel only reads"}
+                   if ach > peak else {}),
                 "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": nbytes, "avg_launch_us": round(us, 3),
                 # share of the GRAPH-timed step: this kernel's launches x its average duration over the step time
