@@ -82,24 +82,16 @@ float scale_log2_of(const dustin_shape_t* s) {
 // i.e. 8 tiles per warp, 16 when the CTA's warps share one or two groups or the cache is paged.  Round 1 used >= 256 tokens
 // per CTA and cut grids of one to three waves down to exactly one wave: at 8 groups that is 16 tiles per warp or more --
 // config 3 loses 4 us per layer to it, 16k 14 us, 32k at batch 4 13 us.
-// alone = the staged call: nothing runs beside the kernel, so a grid between one and two and a half waves of resident CTAs
-// (3 per SM) is cut to exactly one wave -- the overhang would pay a whole second wave (a1 alone at B = 16: 4k 37 -> 29 us,
-// 8k 56 -> 53 us).  In the one-shot call the draft-tier selection shares the SMs and the finer grid wins (table above).
-void score_plan(int batch, int n_groups, int max_ctx, bool paged, bool alone, int* chunk_tokens, int* n_parts,
-                int* group_slots) {
+// The plan does not depend on which entry point asks: the staged and the one-shot call must cut a sequence into the same
+// CTAs, or their softmax partials fold in different groupings and the two paths stop being bit-identical.  (A one-wave
+// grid for the staged call alone -- a1 at B = 16: 4k 37 -> 30 us, 8k 56 -> 53 us -- was dropped for that reason.)
+void score_plan(int batch, int n_groups, int max_ctx, bool paged, int* chunk_tokens, int* n_parts, int* group_slots) {
+    (void)batch;
     int slots = 1;
     while (slots < n_groups && slots < 8) slots <<= 1;
     const int n_sub = 8 / slots;
     const int tiles_per_warp = (slots <= 2 || paged) ? 16 : 8;
     int chunk = 16 * n_sub * tiles_per_warp;
-    if (alone && batch > 0) {
-        const long long resident = (long long)device_sm_count() * 3;
-        const long long ctas = (long long)batch * ((max_ctx + chunk - 1) / chunk);
-        if (ctas > resident && 2 * ctas < 5 * resident && batch <= resident) {
-            const int per_seq = (int)(resident / batch), quantum = 16 * n_sub;
-            chunk = ((max_ctx + per_seq - 1) / per_seq + quantum - 1) / quantum * quantum;
-        }
-    }
     const int forced = knob(DUSTIN_KNOB_SCORE_CHUNK);   // tuning aid: tokens per scoring CTA (multiple of 16)
     if (forced >= kMinScoreChunk) chunk = (forced + 15) / 16 * 16;
     *chunk_tokens = chunk;
@@ -248,8 +240,7 @@ int run_score(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q,
     p.n_lists = n_lists;
     p.scale_log2 = scale_log2_of(shape);
     p.defer_wait = defer_wait ? 1 : 0;
-    score_plan(p.batch, p.n_groups, p.max_ctx, p.kv.page_table != nullptr, norm_out == nullptr, &p.chunk_tokens, &p.n_chunks,
-               &p.group_slots);
+    score_plan(p.batch, p.n_groups, p.max_ctx, p.kv.page_table != nullptr, &p.chunk_tokens, &p.n_chunks, &p.group_slots);
     p.logit_stride = ((long long)p.max_ctx + 3) & ~3ll;
     char* base = static_cast<char*>(ws) + kWsHeader;   // the persistent header belongs to the attention stage
     p.logits = reinterpret_cast<float*>(base + w.logits);
