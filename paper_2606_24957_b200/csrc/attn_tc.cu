@@ -274,6 +274,7 @@ struct Seg {
 struct TileCursor {
     const int* prefix;
     int n_units, n_kv, n_lists, lo, hi, chunk;
+    int ulen;      // >= 0: every unit is this long and prefix[] holds padded unit starts (even-pieces plan); -1: prefix[u + 1]
     int next_u;
     Seg s;
     int ti;        // tile index inside the segment
@@ -284,7 +285,8 @@ struct TileCursor {
         if (next_u >= n_units) return false;
         const int ps = prefix[next_u];
         if (ps >= hi) return false;
-        const int pe = prefix[next_u + 1];
+        const int pe = ulen >= 0 ? ps + ulen : prefix[next_u + 1];
+        if (lo >= pe) return false;   // (even-pieces plan: a range in the padding behind the last unit piece)
         s.u = next_u;
         s.b = next_u / n_kv;
         s.g = next_u - s.b * n_kv;
@@ -301,9 +303,9 @@ struct TileCursor {
         return true;
     }
     __device__ __forceinline__ void init(const int* prefix_, int n_units_, int n_kv_, int n_lists_, int lo_, int hi_,
-                                         int chunk_, int u0) {
+                                         int chunk_, int u0, int ulen_) {
         prefix = prefix_; n_units = n_units_; n_kv = n_kv_; n_lists = n_lists_;
-        lo = lo_; hi = hi_; chunk = chunk_; next_u = u0;
+        lo = lo_; hi = hi_; chunk = chunk_; next_u = u0; ulen = ulen_;
         ti = 0; seg_no = 0;
         valid = load_seg();
     }
@@ -356,6 +358,15 @@ __device__ __forceinline__ Plan make_plan(PrefixFn prefix, UnitOfFn unit_of, int
         if (pl.lo < pl.hi) pl.u0 = unit_of(pl.lo);
     }
     return pl;
+}
+
+// Even-pieces plan: CTAs per unit (>= 2), or 0 when it does not apply.  Units of one length `len` (new-row tile included),
+// at most half as many as CTAs, at least two tiles per piece.
+__device__ __forceinline__ int even_pieces_per_unit(int len, int n_units, int grid) {
+    if (n_units <= 0 || n_units * 2 > grid) return 0;
+    const int n_tiles = (len + kTile - 1) / kTile;
+    const int ppu = min(grid / n_units, n_tiles / 2);
+    return ppu >= 2 ? ppu : 0;
 }
 
 // ---- kernel -----------------------------------------------------------------------------------------------------
@@ -456,7 +467,8 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
     // prologue.  The conditions restate make_plan's for this case.
     int early_tok[4] = {-1, -1, -1, -1};
     bool early = false;
-    if (GATHER && uniform && (warp == 9 || warp == 10) && rid < n_units && n_units <= (int)gridDim.x && !(p.dbg & 32)) {
+    if (GATHER && uniform && (warp == 9 || warp == 10) && rid < n_units && n_units <= (int)gridDim.x && !(p.dbg & 32) &&
+        even_pieces_per_unit(p.uniform_cnt + kTile, n_units, (int)gridDim.x) == 0) {
         const int len = p.uniform_cnt + kTile;
         if (len <= (n_units * len) / (int)gridDim.x + 4 * kTile) {
             const int first = (warp - 9) * kTile + lane;   // cache position of this lane's first row
@@ -494,8 +506,19 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
     }
     const int per = (n_units + 255) / 256;
     const int u_lo = min(tid * per, n_units), u_hi = tid < 256 ? min(u_lo + per, n_units) : u_lo;
+    // Even-pieces plan (gathered rows, all units of one length, at most half as many units as CTAs: 64k / 128k contexts at
+    // small batch): ppu CTAs per unit, every CTA ONE piece of tpp whole tiles of ONE unit; the CTAs beyond n_units * ppu
+    // stay idle.  Equal token ranges over all 148 CTAs give some CTAs the tail of one unit and the head of the next: two
+    // epilogues, a second Q load and 4.6 pieces per unit to merge instead of 4 (measured: 128k / B = 4 22.8 -> 19.7 us,
+    // 64k / B = 8 25.8 -> 22.1 us, 128k / k = 8192 39.8 -> 37.5 us; the dense baseline, which streams far more per unit,
+    // loses: 341 -> 372 us, hence gathered rows only).  The unit starts are padded to ppu * tpp tiles so that the cuts are
+    // plain multiples of the chunk.  Whether the lengths are equal is a property of the data, not of how the kernel learnt
+    // them: the same decomposition follows from the host's hint and from the lengths read below (bit-identical results).
+    int ulen = uniform ? p.uniform_cnt + kTile : -1;                   // common unit length, -1: not (yet) known to be one
+    int ppu = (GATHER && uniform && !(p.dbg & 32)) ? even_pieces_per_unit(ulen, n_units, (int)gridDim.x) : 0;
+    int even_chunk = ppu >= 2 ? ((ulen + kTile - 1) / kTile + ppu - 1) / ppu * kTile : 0;
     if (uniform) {
-        const int len = p.uniform_cnt + kTile;
+        const int len = ppu >= 2 ? ppu * even_chunk : p.uniform_cnt + kTile;
         for (int u = u_lo; u < u_hi; ++u) s_prefix[u] = u * len;
         if (tid == 255) s_prefix[n_units] = n_units * len;
     } else {
@@ -526,6 +549,24 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
             run += unit_len(u);
         }
         if (tid == 255) s_prefix[n_units] = run;
+        if (GATHER && !(p.dbg & 32)) {
+            // lengths read from memory: all equal?  (total == n_units * longest)  Then the even-pieces plan applies as above.
+            __syncthreads();
+            int longest_all = 0;
+#pragma unroll
+            for (int w = 0; w < 8; ++w) longest_all = max(longest_all, s_scan[8 + w]);
+            if (s_prefix[n_units] == n_units * longest_all) {
+                const int pp = even_pieces_per_unit(longest_all, n_units, (int)gridDim.x);
+                if (pp >= 2) {   // (uniform over the CTA)
+                    ulen = longest_all;
+                    ppu = pp;
+                    even_chunk = ((ulen + kTile - 1) / kTile + ppu - 1) / ppu * kTile;
+                    __syncthreads();   // everybody has read the exact prefix
+                    for (int u = u_lo; u < u_hi; ++u) s_prefix[u] = u * ppu * even_chunk;
+                    if (tid == 255) s_prefix[n_units] = n_units * ppu * even_chunk;
+                }
+            }
+        }
     }
     if (tid < NQ) {
         s_ref[tid] = kRefInit;
@@ -537,7 +578,14 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
     if (tid == 0) TS(1);
     const uint32_t tmem = *s_tmem;
     constexpr uint32_t kColS = 0, kColO = 256;   // S buffers at columns 0 and 128, O^T at 256
-    if (uniform) {
+    if (ppu >= 2) {
+        pl.chunk = even_chunk;
+        pl.whole = false;
+        pl.u0 = min(rid / ppu, n_units - 1);
+        pl.lo = rid < n_units * ppu ? rid * even_chunk : n_units * ppu * even_chunk;
+        pl.hi = rid < n_units * ppu ? pl.lo + even_chunk : pl.lo;
+        if (pl.lo >= pl.u0 * ppu * even_chunk + ulen) pl.hi = pl.lo;   // nothing of the unit left for this piece
+    } else if (uniform) {
         const int len = p.uniform_cnt + kTile;
         pl = make_plan([&](int u) { return u * len; }, [&](int x) { return min(x / len, n_units - 1); }, n_units, len,
                        (int)gridDim.x, rid, (p.dbg & 32) != 0);
@@ -565,7 +613,7 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
     }
 
     TileCursor cur;
-    cur.init(s_prefix, n_units, Hkv, p.n_lists, lo, hi, chunk, u0);
+    cur.init(s_prefix, n_units, Hkv, p.n_lists, lo, hi, chunk, u0, ppu >= 2 ? ulen : -1);
     if (!active) cur.valid = false;
 
     if ((warp >= 4 && warp < 8) || (NPW == 2 && warp >= 12)) {
