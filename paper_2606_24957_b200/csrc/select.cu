@@ -35,6 +35,14 @@ namespace sel256 {
 #undef SEL_NT
 }  // namespace sel256
 
+// The target tier when there are more rows than SMs but at most twice as many (the paged ragged workload: 256 rows): 512
+// threads, two CTAs per SM, so that all rows run in ONE wave instead of a full wave and a straggling one.
+namespace sel512 {
+#define SEL_NT 512
+#include "select_impl.inl"
+#undef SEL_NT
+}  // namespace sel512
+
 // Shared-memory plan: bitmask (max_ctx / 8 bytes) + kBins * R histogram counters + a 2 * cap word candidate list,
 // shrunk for very long rows so that everything fits the 227 KB of one SM.  light: the 256-thread draft-tier kernel
 // (one histogram replica: ~90 KB at 32k tokens, beside two scoring CTAs of 64 KB).
@@ -87,7 +95,10 @@ cudaError_t launch_select(const SelectParams& p_in, cudaStream_t stream, int mod
     // a1 ~1 us of 171; so do up to 32 whole SMs taken away).  With few rows, the fast 1024-thread kernel, one SM per row.
     const int n_rows = p.n_lists * p.batch;
     // (up to 32 SMs given up cost the scoring kernel 1-2 us; 48 cost it 13)
-    const bool light = mode == 1 && n_rows > 32 && p.max_ctx <= (1 << 18);
+    const int sms = device_sm_count();
+    const bool half = mode == 2 && n_rows > sms && n_rows <= 2 * sms && p.max_ctx <= (1 << 18) &&
+                      knob(DUSTIN_KNOB_SELECT_SPLIT) != 1;
+    const bool light = (mode == 1 && n_rows > 32 && p.max_ctx <= (1 << 18)) || half;
     select_plan(p.max_ctx, light, &p.mask_words, &p.replicas, &p.list_cap);
     const size_t smem = select_smem_bytes(p.max_ctx, light);
     p.trace = nullptr;
@@ -115,6 +126,8 @@ cudaError_t launch_select(const SelectParams& p_in, cudaStream_t stream, int mod
         return vec ? launch_one<select_kernel<true, kSelDraft>>(p, flat, 1024, smem, kKernSelectDraft, stream)
                    : launch_one<select_kernel<false, kSelDraft>>(p, flat, 1024, smem, kKernSelectDraft, stream);
     }
+    if (mode == 2 && half && vec)
+        return launch_one<sel512::select_kernel<true, sel512::kSelTarget>>(p, rows, 512, smem, kKernSelect, stream);
     if (mode == 2)
         return vec ? launch_one<select_kernel<true, kSelTarget>>(p, rows, 1024, smem, kKernSelect, stream)
                    : launch_one<select_kernel<false, kSelTarget>>(p, rows, 1024, smem, kKernSelect, stream);

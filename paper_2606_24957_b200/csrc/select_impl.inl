@@ -1061,7 +1061,8 @@ __device__ __forceinline__ void select_row(const SelectParams& p, int b, int l, 
 }
 
 template <bool VEC, int MODE>
-__global__ void __launch_bounds__(kSelThreads, kSelThreads <= 256 ? 3 : 1) select_kernel(const SelectParams p) {
+__global__ void __launch_bounds__(kSelThreads, kSelThreads <= 256 ? 3 : (kSelThreads <= 512 ? 2 : 1))
+    select_kernel(const SelectParams p) {
     extern __shared__ __align__(16) uint32_t smem_dyn[];
     __shared__ SelShared sh;
     unsigned long long* const tr =

@@ -35,6 +35,8 @@ def many_rows_cases():
     return {
         # 64 rows, 16-byte rows: select kernels materialise their own rows; the light draft-tier kernel runs
         "llama_64rows": synth.shrink(llama, batch=8, ctx=2048, budget=300, n_sink=8, n_recent=40),
+        # 160 rows: more rows than SMs, at most twice as many -- the 512-thread target-tier kernel (two CTAs per SM)
+        "llama_160rows": synth.shrink(llama, batch=20, ctx=2048, budget=300, n_sink=8, n_recent=40),
         # ragged lengths + per-sequence budgets (one of them made invalid below), paged cache
         "paged_96rows": synth.shrink(synth.config_paged(), batch=12, ctx=3072, ragged_min=700, n_sink=4, n_recent=16),
         # few rows (1024-thread draft-tier kernel, separate normalisation launches), G = 1
@@ -96,6 +98,7 @@ def _tie_heavy_inputs(cfg, seed, device="cuda"):
 
 
 @pytest.mark.parametrize("name,m", [("llama_64rows", (1, 2)), ("llama_64rows", (0, 1)), ("llama_64rows", (1, 1)),
+                                    ("llama_160rows", (1, 2)), ("llama_160rows", (2, 3)),
                                     ("paged_96rows", (1, 3)), ("qwen_packed_4rows", (1, 2)), ("qwen_72rows_odd", (2, 3))])
 def test_fused_selection_is_the_oracles_under_heavy_ties(name, m, hoist):
     cfg = dataclasses.replace(CASES[name], m_num=m[0], m_den=m[1])
