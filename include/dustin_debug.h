@@ -30,9 +30,11 @@ typedef enum dustin_knob {
     DUSTIN_KNOB_PDL = 0,            /* 1 (default): programmatic dependent launch between the kernels of a layer; 0: plain */
     DUSTIN_KNOB_FUSED_ROWS = 1,     /* 1 (default): the fused call normalises + accumulates rows inside the selection
                                        kernels; 0: separate stats / normalise launches as in the staged calls            */
-    DUSTIN_KNOB_ATTN_TRACE = 2,     /* bit mask, tcgen05 attention kernel: 8 = %globaltimer samples per role into the
-                                       workspace tail, 32 = force stream-K even when whole-unit mode applies, 1 / 2 = skip
-                                       the P.V / S MMAs (timing experiments only: results are then wrong)                 */
+    DUSTIN_KNOB_ATTN_TRACE = 2,     /* bit mask, tcgen05 attention kernel: 8 = timeline samples per role (SM clock, via shared
+                                       memory) into the workspace tail, [63] / [62] = %globaltimer at the CTA's start / end;
+                                       32 = force equal token ranges (stream-K) even when the whole-unit or even-pieces plan
+                                       applies; 64 = griddepcontrol.launch_dependents at the end of the kernel instead of its
+                                       start; 1 / 2 = skip the P.V / S MMAs (timing experiments only: results are then wrong) */
     DUSTIN_KNOB_SELECT_SPLIT = 3,   /* CTAs per selection row (thread-block cluster): 0 (default) = heuristic, 1/2/4/8    */
     DUSTIN_KNOB_DRAFT_HOIST = 4,    /* 1 (default): the fused call runs the draft tier of Eq. 6 (I_draft) in a kernel of its
                                        own beside the K stream of a1; 0: both tiers after a1                               */
