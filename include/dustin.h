@@ -43,7 +43,9 @@ typedef enum dustin_status {
     DUSTIN_ERR_INVALID_ARG = -1,   /* null pointer, negative size, Hq % Hkv != 0, S + W > k, empty head mask ...  */
     DUSTIN_ERR_UNSUPPORTED = -2,   /* a documented limit above is exceeded                                         */
     DUSTIN_ERR_WORKSPACE = -3,     /* ws == NULL or ws_bytes < dustin_workspace_bytes(...)                          */
-    DUSTIN_ERR_CUDA = -4           /* a launch failed; see dustin_last_cuda_error()                                 */
+    DUSTIN_ERR_CUDA = -4,          /* a launch failed; see dustin_last_cuda_error()                                 */
+    DUSTIN_ERR_STATIC_SCRATCH = -5 /* dustin_score_heads_static only: the shape needs more scratch than
+                                      DUSTIN_STATIC_SCRATCH_BYTES; nothing was enqueued                             */
 } dustin_status;
 
 /* Problem shape of one layer call.  T = n_new = gamma + 1 verify positions (reading A13). */
@@ -198,6 +200,43 @@ size_t dustin_draft_workspace_bytes(const dustin_shape_t* shape, uint64_t head_m
 int dustin_draft_aggregate(const dustin_shape_t* shape, const dustin_kv_t* kv_layers, const void* const* q_layers,
                            int32_t n_layers, uint64_t head_mask, float* s_draft, void* ws, size_t ws_bytes,
                            void* stream);
+
+/* ---- a1 without a workspace argument --------------------------------------------------------------------------------
+ * dustin_score_heads_static computes exactly what dustin_score_heads computes (same arguments, same kernels, same
+ * bits in scores_now) but takes no `ws`: its scratch is a fixed array of DUSTIN_STATIC_SCRATCH_BYTES that is built into
+ * the library.  The call allocates nothing -- no cudaMalloc / cudaFree, no memory pool, no allocating library routine.
+ *
+ * Who needs this.  Every other entry point asks the caller for a workspace, and some callers have no way to make one:
+ *   - code running under a serving engine whose memory manager claimed (nearly) all of HBM at start-up, so that a
+ *     cudaMalloc made behind the engine's back fails or eats into the KV-cache budget the engine thinks it owns;
+ *   - an operator plugged into a host runtime whose operator signature carries inputs and outputs only, with no slot
+ *     for a scratch buffer and no handle on the runtime's allocator;
+ *   - a decode step that must not stall: cudaMalloc and cudaFree may synchronise the whole device, which a
+ *     latency-bound loop cannot afford in the middle of a step.
+ * Such a caller passes the inputs and the output as usual and nothing else.
+ *
+ * Limit.  The scratch the shape needs -- about 4 * batch * |head_mask| * max_ctx bytes of logits plus a few per cent of
+ * softmax partials; dustin_workspace_bytes(shape, head_mask, 1) is a safe upper bound -- must not exceed
+ * DUSTIN_STATIC_SCRATCH_BYTES (16 MiB: e.g. B = 4, 8 subset heads, 64k context).  A larger shape returns
+ * DUSTIN_ERR_STATIC_SCRATCH before anything touches the device; use dustin_score_heads with your own workspace there.
+ * The array costs its 16 MiB on every GPU on which the library's device code is loaded, from then until the process
+ * exits, whether this entry point is ever called or not.
+ *
+ * First call on a device.  The first call made with a given device current does a one-time set-up for that device: it
+ * makes the CUDA runtime load the library's device code there if it has not yet (that is when the array gets its memory)
+ * and asks it for the array's device address (cudaGetSymbolAddress; a failure returns DUSTIN_ERR_CUDA).  Make that first
+ * call during start-up, outside any stream capture; later calls on the same device only enqueue kernels.  The address is
+ * kept for the life of the process: after cudaDeviceReset it is stale, do not call this entry point again then.
+ *
+ * Sharing.  There is ONE array per GPU and every call on that GPU uses it, whatever the stream or host thread: two calls
+ * whose kernels may overlap on the GPU race on it and both get garbage -- keep them on one stream or order them with
+ * events.  The array keeps what the last call wrote; no call depends on that (nothing in it needs to start at zero: each
+ * call writes every word it later reads), so calls of different shapes may follow each other freely.
+ * Arguments, layouts and the other error codes: see dustin_score_heads. */
+#define DUSTIN_STATIC_SCRATCH_BYTES (16 * 1024 * 1024)
+int dustin_score_heads_static(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q,
+                              int64_t q_stride_batch, int64_t q_stride_head, uint64_t head_mask, int32_t n_lists,
+                              float* scores_now, void* stream);
 
 #ifdef __cplusplus
 }

@@ -18,7 +18,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libdustin.so")
 _lib = None
 
-OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_WORKSPACE, ERR_CUDA = 0, -1, -2, -3, -4
+OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_WORKSPACE, ERR_CUDA, ERR_STATIC_SCRATCH = 0, -1, -2, -3, -4, -5
+STATIC_SCRATCH_BYTES = 16 * 1024 * 1024     # DUSTIN_STATIC_SCRATCH_BYTES (dustin.h)
 
 
 class DustinError(RuntimeError):
@@ -89,6 +90,8 @@ def lib():
         L.dustin_workspace_bytes.argtypes = [sp, u64, i32]
         L.dustin_score_heads.restype = ctypes.c_int
         L.dustin_score_heads.argtypes = [sp, kp, vp, i64, i64, u64, i32, vp, vp, sz, vp]
+        L.dustin_score_heads_static.restype = ctypes.c_int
+        L.dustin_score_heads_static.argtypes = [sp, kp, vp, i64, i64, u64, i32, vp, vp]
         L.dustin_fuse_scores.restype = ctypes.c_int
         L.dustin_fuse_scores.argtypes = [i32, i32, i32, vp, vp, vp, f32, vp]
         L.dustin_topk_select.restype = ctypes.c_int
@@ -118,7 +121,7 @@ N_KERNELS = 10
 EXPORTS = ("dustin_version", "dustin_status_string", "dustin_last_cuda_error",
            "dustin_workspace_bytes", "dustin_score_heads", "dustin_fuse_scores", "dustin_topk_select",
            "dustin_sparse_verify_attn", "dustin_verify_layer_fused", "dustin_arr", "dustin_append_kv",
-           "dustin_draft_workspace_bytes", "dustin_draft_aggregate")
+           "dustin_draft_workspace_bytes", "dustin_draft_aggregate", "dustin_score_heads_static")
 # ... and include/dustin_debug.h (measurement / tuning / testing aids)
 DEBUG_EXPORTS = ("dustin_tune_attn_split_tokens", "dustin_tune_attn_impl", "dustin_tune_set", "dustin_tune_get",
                  "dustin_debug_trace_buffer", "dustin_launch_count", "dustin_profile_enable", "dustin_profile_collect",
@@ -282,6 +285,22 @@ def score_heads(shape: Shape, kv: KV, q: torch.Tensor, head_mask: int, n_lists: 
                                   q.stride(1), ctypes.c_uint64(head_mask), n_lists,
                                   _dense(scores_now, torch.float32), _ptr(ws), ws.numel(), _stream())
     _check("dustin_score_heads", rc)
+
+
+def score_heads_static(shape: Shape, kv: KV, q: torch.Tensor, head_mask: int, n_lists: int,
+                       scores_now: torch.Tensor) -> None:
+    """score_heads for a caller that cannot hand over a workspace (its process may not allocate device memory: the
+    serving engine around it owns all of HBM, or its operator interface passes inputs and outputs only).  Same
+    arguments minus `ws`, same result bit for bit; the scratch is the library's built-in array of STATIC_SCRATCH_BYTES
+    per GPU, so shapes that need more raise DustinError(ERR_STATIC_SCRATCH).  All calls on a GPU share that array:
+    keep them on one stream.  The first call on each device does a one-time set-up (dustin.h)."""
+    if q.dim() != 3 or q.stride(2) != 1:
+        raise ValueError("q must be a [B, Hq, d] view with a contiguous last dimension")
+    kvc = kv.c()
+    rc = lib().dustin_score_heads_static(ctypes.byref(shape), ctypes.byref(kvc), _ptr(q, torch.bfloat16), q.stride(0),
+                                         q.stride(1), ctypes.c_uint64(head_mask), n_lists,
+                                         _dense(scores_now, torch.float32), _stream())
+    _check("dustin_score_heads_static", rc)
 
 
 def fuse_scores(scores_now: torch.Tensor, hist_inout: torch.Tensor, alpha: float,

@@ -7,6 +7,7 @@
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 
 namespace dustin {
 namespace {
@@ -392,6 +393,8 @@ const char* dustin_status_string(int status) {
         case DUSTIN_ERR_UNSUPPORTED: return "unsupported shape (see the limits in dustin.h)";
         case DUSTIN_ERR_WORKSPACE: return "workspace missing, misaligned or too small";
         case DUSTIN_ERR_CUDA: return "CUDA launch error (see dustin_last_cuda_error)";
+        case DUSTIN_ERR_STATIC_SCRATCH:
+            return "shape needs more scratch than DUSTIN_STATIC_SCRATCH_BYTES: use dustin_score_heads with your own workspace";
         default: return "unknown status";
     }
 }
@@ -652,6 +655,62 @@ size_t dustin_draft_workspace_bytes(const dustin_shape_t* shape, uint64_t head_m
     int nsel = popcount64(head_mask) * shape->n_new;
     if (nsel > 64) nsel = popcount64(head_mask);   // the per-token fallback
     return kWsHeader + score_ws(shape->batch, nsel, shape->max_ctx).total + 256;
+}
+
+}  // extern "C"
+
+// ---- dustin_score_heads_static: a1 for callers that have no device memory to give (dustin.h) ------------------------
+// The scratch of the scoring kernels (log2-domain logits, per-CTA softmax partials, per-head statistics) lives in this
+// array instead of a caller-provided workspace.  It is part of the library image: the driver places it on every GPU on
+// which the library's code gets loaded and it stays there until the process exits -- DUSTIN_STATIC_SCRATCH_BYTES per GPU,
+// used or not.  In host code the name `g_static_scratch` is only a handle for the runtime, NOT a device address: the
+// address a kernel can use is asked for below, once per device, with cudaGetSymbolAddress.
+static __device__ __align__(256) unsigned char g_static_scratch[DUSTIN_STATIC_SCRATCH_BYTES];
+
+namespace {
+constexpr int kStaticMaxDev = 64;
+std::mutex g_static_mu;
+void* g_static_ptr[kStaticMaxDev];   // device ordinal -> device address of g_static_scratch there (nullptr: not asked yet)
+
+// Device address of the array on the CURRENT device.  The first call per device is the set-up step: it makes the
+// runtime load the library's device code there (which is when the array gets its memory) and looks the symbol up.
+cudaError_t static_scratch_here(void** out) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kStaticMaxDev) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lk(g_static_mu);
+    if (!g_static_ptr[dev]) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_static_scratch);
+        if (e != cudaSuccess) return e;
+        if (!p) return cudaErrorInvalidSymbol;
+        g_static_ptr[dev] = p;
+    }
+    *out = g_static_ptr[dev];
+    return cudaSuccess;
+}
+}  // namespace
+
+extern "C" {
+
+int dustin_score_heads_static(const dustin_shape_t* shape, const dustin_kv_t* kv, const void* q, int64_t q_stride_batch,
+                              int64_t q_stride_head, uint64_t head_mask, int32_t n_lists, float* scores_now,
+                              void* stream) {
+    if (!scores_now) return DUSTIN_ERR_INVALID_ARG;
+    // Size first, from host values alone: a shape that cannot fit is refused before the device is touched.
+    if (check_shape(shape) == DUSTIN_OK && head_mask != 0) {
+        const size_t need = kWsHeader + score_ws(shape->batch, popcount64(head_mask), shape->max_ctx).total;
+        if (need > (size_t)DUSTIN_STATIC_SCRATCH_BYTES) return DUSTIN_ERR_STATIC_SCRATCH;
+    }
+    void* scratch = nullptr;
+    const cudaError_t e = static_scratch_here(&scratch);
+    if (e != cudaSuccess) return fail_cuda(e);
+    // Same validation, plan and kernels as dustin_score_heads; only the scratch pointer differs.  Nothing in the scratch
+    // has to start at zero (the kernels write every logit, partial and statistic before they read it), so whatever the
+    // previous call left behind is harmless and nothing is cleared here.
+    return run_score(shape, kv, q, q_stride_batch, q_stride_head, head_mask, n_lists, scores_now, nullptr, 0.f, scratch,
+                     (size_t)DUSTIN_STATIC_SCRATCH_BYTES, static_cast<cudaStream_t>(stream));
 }
 
 }  // extern "C"
