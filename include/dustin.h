@@ -96,13 +96,19 @@ int         dustin_last_cuda_error(void);            /* cudaError_t of the last 
  * be written by the caller afterwards; every call that returns DUSTIN_OK and runs to completion leaves them zero
  * again, so one memset at allocation time serves any number of calls (and CUDA-graph replays).  The rest of the
  * buffer is plain scratch with no state.  One workspace must not be used by two calls that run concurrently.
- * After a failure (a call returned DUSTIN_ERR_CUDA, or a kernel of this library was aborted: device fault, reset,
- * cudaDeviceReset) the header may hold flags of the aborted launch: zero it again (cudaMemsetAsync of
+ * After a failure (a call returned DUSTIN_ERR_CUDA, or a kernel of this library was aborted by a fault that left the
+ * context usable) the header may hold flags of the aborted launch: zero it again (cudaMemsetAsync of
  * DUSTIN_WS_HEADER_BYTES on the same stream) before reusing the buffer.
+ * cudaDeviceReset is NOT a supported recovery: the library remembers, per device and for the life of the process, that
+ * it has raised its kernels' dynamic shared-memory limits there (and, for dustin_score_heads_static, a device address);
+ * a reset silently undoes the former and invalidates the latter, after which launches fail with DUSTIN_ERR_CUDA.
+ * Restart the process (or unload and reload the library) after a device reset.
  * Forward progress of the attention kernel when one (sequence, KV head) is cut across several CTAs (long or ragged
- * units): the CTA that merges a unit waits for partial results of CTAs with LOWER block indices only, which the
- * hardware dispatches no later than the waiting CTA, so the kernel needs no co-residency of its whole grid (it is safe
- * under MPS partitions, green contexts and concurrent kernels on other streams). */
+ * units): the CTA that merges a unit waits for partial results of CTAs with LOWER block indices only.  That the kernel
+ * then needs no co-residency of its whole grid (MPS partitions, green contexts, concurrent kernels on other streams)
+ * rests on an IMPLEMENTATION ASSUMPTION, not on a documented CUDA guarantee: that CTAs of a grid are dispatched in
+ * ascending block-index order, as on every current GPU (decoupled look-back scans and stream-K GEMMs rely on the same
+ * behaviour).  On hardware that dispatched out of order the wait could stall a partially resident grid. */
 #define DUSTIN_WS_HEADER_BYTES 4096
 
 /* Scratch (bytes of device memory, 256-byte aligned by the caller) that is enough for every entry point on this

@@ -34,7 +34,8 @@ typedef enum dustin_knob {
                                        memory) into the workspace tail, [63] / [62] = %globaltimer at the CTA's start / end;
                                        32 = force equal token ranges (stream-K) even when the whole-unit or even-pieces plan
                                        applies; 64 = griddepcontrol.launch_dependents at the end of the kernel instead of its
-                                       start; 1 / 2 = skip the P.V / S MMAs (timing experiments only: results are then wrong) */
+                                       start; 1 / 2 = skip the P.V / S MMAs (timing experiments only, results are then wrong: these two
+                                       bits act only in a library built with -DDUSTIN_DEBUG_BUILD, the shipped one ignores them) */
     DUSTIN_KNOB_SELECT_SPLIT = 3,   /* CTAs per selection row (thread-block cluster): 0 (default) = heuristic, 1/2/4/8    */
     DUSTIN_KNOB_DRAFT_HOIST = 4,    /* 1 (default): the fused call runs the draft tier of Eq. 6 (I_draft) in a kernel of its
                                        own beside the K stream of a1; 0: both tiers after a1                               */
@@ -72,6 +73,13 @@ int dustin_probe_gather(const dustin_shape_t* shape, const dustin_kv_t* kv, cons
 /* Occupancy experiments: n_ctas CTAs of `threads` threads and `smem_bytes` of dynamic shared memory that do nothing but
  * hold their SM resources for `microseconds` (they poll %globaltimer).  Launched on `stream`; not counted as a launch. */
 int dustin_debug_occupy(int32_t n_ctas, int32_t threads, int32_t smem_bytes, int32_t microseconds, void* stream);
+
+/* Unit-test hook for the block-wide exclusive prefix sum inside the selection kernels (select_impl.inl, block_excl_scan),
+ * which is compiled once per CTA size: `threads` in {256, 512, 1024} picks the instantiation.  Every CTA scans its own
+ * `threads` values twice, v and v + 1 (mod 2^32).  in: device uint32 [n_blocks][threads];  out: device uint32
+ * [2][n_blocks][threads] (exclusive prefixes);  total: device uint32 [2][n_blocks] (block sums).  Not counted as a launch. */
+int dustin_debug_block_scan(int32_t threads, int32_t n_blocks, const uint32_t* in, uint32_t* out, uint32_t* total,
+                            void* stream);
 
 #ifdef __cplusplus
 }

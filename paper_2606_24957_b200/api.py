@@ -103,6 +103,8 @@ def lib():
                                                 vp, vp, vp, sz, vp]
         L.dustin_probe_gather.restype = ctypes.c_int
         L.dustin_probe_gather.argtypes = [sp, kp, vp, vp, i32, i32, vp, sz, vp]
+        L.dustin_debug_block_scan.restype = ctypes.c_int
+        L.dustin_debug_block_scan.argtypes = [i32, i32, vp, vp, vp, vp]
         L.dustin_arr.restype = ctypes.c_int
         L.dustin_arr.argtypes = [i32, i32, i32, vp, vp, vp, vp, i32, vp, vp]
         L.dustin_append_kv.restype = ctypes.c_int
@@ -125,7 +127,7 @@ EXPORTS = ("dustin_version", "dustin_status_string", "dustin_last_cuda_error",
 # ... and include/dustin_debug.h (measurement / tuning / testing aids)
 DEBUG_EXPORTS = ("dustin_tune_attn_split_tokens", "dustin_tune_attn_impl", "dustin_tune_set", "dustin_tune_get",
                  "dustin_debug_trace_buffer", "dustin_launch_count", "dustin_profile_enable", "dustin_profile_collect",
-                 "dustin_kernel_name", "dustin_probe_gather", "dustin_debug_occupy")
+                 "dustin_kernel_name", "dustin_probe_gather", "dustin_debug_occupy", "dustin_debug_block_scan")
 
 # enum dustin_knob (dustin_debug.h)
 (KNOB_PDL, KNOB_FUSED_ROWS, KNOB_ATTN_TRACE, KNOB_SELECT_SPLIT, KNOB_DRAFT_HOIST, KNOB_SCORE_CHUNK, KNOB_SELECT_TRACE,
@@ -244,6 +246,19 @@ def debug_occupy(n_ctas: int, threads: int, smem_bytes: int, microseconds: int, 
     """dustin_debug_occupy: CTAs that hold SM resources for a while (occupancy experiments)."""
     st = ctypes.c_void_p((stream or torch.cuda.current_stream()).cuda_stream)
     _check("dustin_debug_occupy", lib().dustin_debug_occupy(n_ctas, threads, smem_bytes, microseconds, st))
+
+
+def debug_block_scan(threads: int, values: torch.Tensor):
+    """dustin_debug_block_scan: values int32 [n_blocks, threads] (bit patterns of uint32) -> (prefixes int32
+    [2, n_blocks, threads], totals int32 [2, n_blocks]) of v and v + 1, by the `threads`-wide selection-kernel scan."""
+    n_blocks = values.shape[0]
+    if values.shape[1] != threads:
+        raise ValueError("values must be [n_blocks, threads]")
+    out = torch.empty((2, n_blocks, threads), dtype=torch.int32, device=values.device)
+    total = torch.empty((2, n_blocks), dtype=torch.int32, device=values.device)
+    _check("dustin_debug_block_scan", lib().dustin_debug_block_scan(threads, n_blocks, _dense(values, torch.int32),
+                                                                    _ptr(out), _ptr(total), _stream()))
+    return out, total
 
 
 def launch_count() -> int:

@@ -588,6 +588,14 @@ int dustin_debug_occupy(int32_t n_ctas, int32_t threads, int32_t smem_bytes, int
     return e == cudaSuccess ? DUSTIN_OK : fail_cuda(e);
 }
 
+int dustin_debug_block_scan(int32_t threads, int32_t n_blocks, const uint32_t* in, uint32_t* out, uint32_t* total,
+                            void* stream) {
+    if ((threads != 256 && threads != 512 && threads != 1024) || n_blocks <= 0 || !in || !out || !total)
+        return DUSTIN_ERR_INVALID_ARG;
+    const cudaError_t e = launch_scan_test(threads, n_blocks, in, out, total, static_cast<cudaStream_t>(stream));
+    return e == cudaSuccess ? DUSTIN_OK : fail_cuda(e);
+}
+
 int dustin_arr(int32_t batch, int32_t n_lists, int32_t max_ctx, const int32_t* seq_lens, const float* a,
                const int32_t* idx, const int32_t* cnt, int32_t k_max, float* arr_out, void* stream) {
     if (batch <= 0 || n_lists <= 0 || max_ctx < 0 || k_max <= 0 || !a || !idx || !cnt || !arr_out)

@@ -7,8 +7,9 @@
 // selected cache rows.  The token lists of all units are laid end to end and cut
 // into gridDim.x equal ranges, one persistent CTA per SM; a CTA therefore works on a few SEGMENTS (pieces of
 // units).  A unit that lies inside one CTA is written straight to `out`; otherwise each piece leaves a normalised
-// partial (o, lse) in the workspace and the LAST piece to finish (a per-unit arrival counter) merges them in
-// segment order, so the result does not depend on which CTA happens to be last.
+// partial (o, lse) and a completion flag in the workspace, and the CTA that holds the unit's FIRST piece merges them in
+// segment order once their flags are up (it pulls from CTAs with lower block indices only, see `rid` below), so the
+// result does not depend on the order in which the pieces finish; the merging CTA clears the flags it consumed.
 //
 // Roles inside a CTA (384 threads; setmaxnreg moves registers from the other warpgroups to the softmax one: 240 / 96 / 96;
 // with two softmax warpgroups, 512 threads: 200 / 200 / 56 / 56 -- measured: resolvers or producers below 56 registers
@@ -28,6 +29,14 @@
 #include "../../include/dustin_debug.h"
 
 #include <climits>
+
+// DUSTIN_KNOB_ATTN_TRACE bits 1 / 2 (skip the P.V / S MMAs: timing experiments whose results are wrong) exist only in a
+// library built with -DDUSTIN_DEBUG_BUILD; the shipped build has no run-time branch in the MMA issue loop.
+#ifdef DUSTIN_DEBUG_BUILD
+#define DUSTIN_DBG_SKIP(dbg, bit) (((dbg) & (bit)) != 0)
+#else
+#define DUSTIN_DBG_SKIP(dbg, bit) false
+#endif
 
 namespace dustin {
 
@@ -822,7 +831,7 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
                     // 8-row blocks 2 KB apart (SBO), 8-token groups 128 B apart (LBO).
                     const uint64_t ad = umma_desc(vb + (uint32_t)ks * 2048, kTile * 128, 1024, kLayoutSw128);
                     const uint64_t bd = umma_desc(pbuf + (uint32_t)ks * 256, 128, 2048, kLayoutNone);
-                    if (!(p.dbg & 1)) umma_bf16(tmem + kColO, ad, bd, idesc_pv, (first_of_seg && ks == 0) ? 0u : 1u);
+                    if (!DUSTIN_DBG_SKIP(p.dbg, 1)) umma_bf16(tmem + kColO, ad, bd, idesc_pv, (first_of_seg && ks == 0) ? 0u : 1u);
                 }
                 umma_commit(bar(kSlotEmpty + slot));
                 umma_commit(bar(kPvDone));
@@ -851,7 +860,7 @@ __global__ void __launch_bounds__(kTcThreads + 128 * (NWG - 1), 1) attn_tc_kerne
                                                   1024, kLayoutSw128);
                     const uint64_t bd = umma_desc(qbuf + (uint32_t)(ks >> 2) * (NQ * 128) + (uint32_t)(ks & 3) * 32, 16,
                                                   1024, kLayoutSw128);
-                    if (!(p.dbg & 2)) umma_bf16(tmem + kColS + (uint32_t)sb * 128, ad, bd, idesc_s, ks > 0 ? 1u : 0u);
+                    if (!DUSTIN_DBG_SKIP(p.dbg, 2)) umma_bf16(tmem + kColS + (uint32_t)sb * 128, ad, bd, idesc_s, ks > 0 ? 1u : 0u);
                 }
                 umma_commit(bar(kSlotEmpty + slot));
                 umma_commit(bar(kSFull + sb));

@@ -132,6 +132,10 @@ cudaError_t launch_append(const KvView& kv, int* seq_lens, const int* n_append, 
 cudaError_t launch_gather_probe(const KvView& kv, const int* idx, const int* cnt, int batch, int n_kv_heads, int head_dim,
                                 int n_lists, int k_max, void* sink, cudaStream_t stream);
 
+// Test hook: the block-wide exclusive scan of the selection kernels alone, per CTA-size instantiation (256 / 512 / 1024).
+cudaError_t launch_scan_test(int threads, int n_blocks, const uint32_t* in, uint32_t* out, uint32_t* total,
+                             cudaStream_t stream);
+
 cudaError_t launch_occupy(int n_ctas, int threads, int smem_bytes, int microseconds, cudaStream_t stream);
 
 // ---- launch bookkeeping (profile.cu) ----------------------------------------------------------------------------

@@ -77,6 +77,13 @@ __global__ void __launch_bounds__(kScoreThreads, 3) score_logits_kernel(const Sc
     const int chunk = blockIdx.x, b = blockIdx.y;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int g = lane >> 2, c = lane & 3;
+    // defer_wait (fused call, hoisted draft tier): everything below reads q / K and WRITES the logits scratch without a
+    // dependency wait of this kernel's own.  That is safe only because the kernel launched just before this one -- the
+    // draft-tier selection (select_impl.inl, select_kernel, kSelDraft) -- executes griddepcontrol.wait BEFORE its
+    // launch_dependents: by the time this grid may start, everything older than that kernel (in particular the previous
+    // call's attention kernel, whose stream-K scratch overlaps the logits) is complete and visible.  The wait is per
+    // waiting grid, so this ordering is transitive, not direct: keep "wait, then trigger" in that kernel
+    // (tests/test_gpu_pdl_chain.py runs unsynchronised chains of calls on one workspace against synchronised ones).
     if (!p.defer_wait) pdl_wait();
     const int N = seq_len_of(p.kv.seq_lens, b, p.max_ctx);
     const int slots = p.group_slots, n_sub = kScoreWarps / slots;

@@ -86,6 +86,15 @@ cudaError_t launch_one(const SelectParams& p, dim3 grid, int threads, size_t sme
 
 }  // namespace
 
+cudaError_t launch_scan_test(int threads, int n_blocks, const uint32_t* in, uint32_t* out, uint32_t* total,
+                             cudaStream_t stream) {
+    if (threads == 256) sel256::scan_test_kernel<<<n_blocks, 256, 0, stream>>>(in, out, total);
+    else if (threads == 512) sel512::scan_test_kernel<<<n_blocks, 512, 0, stream>>>(in, out, total);
+    else if (threads == 1024) sel1024::scan_test_kernel<<<n_blocks, 1024, 0, stream>>>(in, out, total);
+    else return cudaErrorInvalidValue;
+    return cudaGetLastError();
+}
+
 size_t select_mask_words(int max_ctx) { return (size_t)(((max_ctx + 31) / 32 + 3) & ~3); }
 
 cudaError_t launch_select(const SelectParams& p_in, cudaStream_t stream, int mode) {
@@ -98,7 +107,11 @@ cudaError_t launch_select(const SelectParams& p_in, cudaStream_t stream, int mod
     const int sms = device_sm_count();
     const bool half = mode == 2 && n_rows > sms && n_rows <= 2 * sms && p.max_ctx <= (1 << 18) &&
                       knob(DUSTIN_KNOB_SELECT_SPLIT) != 1;
-    const bool light = (mode == 1 && n_rows > 32 && p.max_ctx <= (1 << 18)) || half;
+    const bool vec = (p.max_ctx & 3) == 0 && (((uintptr_t)p.s_draft | (uintptr_t)p.s_target) & 15) == 0 &&
+                     (p.draft_batch_stride & 3) == 0 && (p.draft_list_stride & 3) == 0;
+    // The light plan (one histogram replica) belongs to the small-CTA kernels only: the 512-thread target tier exists in
+    // its vectorised form alone, so an unaligned row falls back to the 1024-thread kernel WITH the full plan.
+    const bool light = (mode == 1 && n_rows > 32 && p.max_ctx <= (1 << 18)) || (half && vec);
     select_plan(p.max_ctx, light, &p.mask_words, &p.replicas, &p.list_cap);
     const size_t smem = select_smem_bytes(p.max_ctx, light);
     p.trace = nullptr;
@@ -108,8 +121,6 @@ cudaError_t launch_select(const SelectParams& p_in, cudaStream_t stream, int mod
         if (buf && bytes >= 2 * (size_t)n_rows * 64 * sizeof(unsigned long long))
             p.trace = static_cast<unsigned long long*>(buf);
     }
-    const bool vec = (p.max_ctx & 3) == 0 && (((uintptr_t)p.s_draft | (uintptr_t)p.s_target) & 15) == 0 &&
-                     (p.draft_batch_stride & 3) == 0 && (p.draft_list_stride & 3) == 0;
     using namespace sel1024;
     const dim3 rows(p.n_lists, p.batch);
     if (mode == 1) {

@@ -61,6 +61,23 @@ __device__ __forceinline__ uint32_t block_excl_scan(uint32_t v, SelShared& sh, u
     return __shfl_sync(0xffffffffu, ti - t, warp) + inc - v;
 }
 
+// Test hook (dustin_debug_block_scan, dustin_debug.h): block_excl_scan on its own, twice in a row on different values
+// (the second use must not see the first one's warp totals).  in: [gridDim.x][kSelThreads];  out: [2][gridDim.x][kSelThreads]
+// exclusive prefixes of in and of in + 1;  total: [2][gridDim.x].
+__global__ void __launch_bounds__(kSelThreads) scan_test_kernel(const uint32_t* __restrict__ in, uint32_t* __restrict__ out,
+                                                                uint32_t* __restrict__ total) {
+    __shared__ SelShared sh;
+    const size_t i = (size_t)blockIdx.x * kSelThreads + threadIdx.x, n = (size_t)gridDim.x * kSelThreads;
+    const uint32_t v = in[i];
+    uint32_t t0, t1;
+    out[i] = block_excl_scan(v, sh, &t0);
+    out[n + i] = block_excl_scan(v + 1u, sh, &t1);
+    if (threadIdx.x == kSelThreads - 1) {
+        total[blockIdx.x] = t0;
+        total[gridDim.x + blockIdx.x] = t1;
+    }
+}
+
 // Key of descending rank `rank` (1-based) among the candidates n in [lo, hi) whose bit in `mem` is clear.
 // Returns the key; need_eq = how many candidates equal to it must still be admitted (in index order);
 // eq_total = how many candidates carry exactly that key.
@@ -640,11 +657,9 @@ __device__ __forceinline__ void select_from_list(const float* __restrict__ s, co
 //      no atomics;  (c) exact selection on the list (list_select_ranged).
 // Returns false (nothing admitted) when the list came out too short or too long; the caller then takes path (2).
 // On entry hist (replica 0) must be all zero; it is left all zero.
-// pre (optional): the row is one chunk and the caller already holds it in registers in exactly this layout
-// (materialize_row<true>): the first read of the row is skipped.
 constexpr int kVecPerChunk = 8;
 __device__ bool sampled_tier_vec(const float* __restrict__ s, int lo, int hi, int rank, const SelLayout& L,
-                                 SelShared& sh, Phase& ph, const float4* pre = nullptr) {
+                                 SelShared& sh, Phase& ph) {
     const float4* s4 = reinterpret_cast<const float4*>(s);
     const int t = threadIdx.x;
     const int v0 = lo >> 2, v_end = (hi + 3) >> 2;
@@ -678,12 +693,7 @@ __device__ bool sampled_tier_vec(const float* __restrict__ s, int lo, int hi, in
     }
     int n_slots;
     if (one) {
-        if (pre != nullptr) {
-#pragma unroll
-            for (int u = 0; u < kVecPerChunk; ++u) x[u] = pre[u];
-        } else {
-            load_chunk(0);
-        }
+        load_chunk(0);
         const int u_s = t & 7, e_s = (t >> 3) & 3;
         float4 xv = x[0];
 #pragma unroll
@@ -791,15 +801,14 @@ __device__ __noinline__ void fallback_tier(const float* __restrict__ s, int lo, 
 
 template <bool VEC>
 __device__ __forceinline__ void select_tier(const float* __restrict__ s, int lo, int hi, int rank, const SelLayout& L,
-                                            int n_words, SelShared& sh, Phase& ph, bool& hist_clean,
-                                            const float4* pre = nullptr) {
+                                            int n_words, SelShared& sh, Phase& ph, bool& hist_clean) {
     if (VEC) {
         if (!hist_clean) {
             clear_hist(L.hist, 1);
             __syncthreads();
         }
         hist_clean = true;
-        if (sampled_tier_vec(s, lo, hi, rank, L, sh, ph, pre)) return;
+        if (sampled_tier_vec(s, lo, hi, rank, L, sh, ph)) return;
         hist_clean = false;   // the paths below leave their counts behind
         __syncthreads();
     }
@@ -1069,6 +1078,11 @@ __global__ void __launch_bounds__(kSelThreads, kSelThreads <= 256 ? 3 : (kSelThr
         p.trace ? p.trace + ((size_t)blockIdx.y * gridDim.x + blockIdx.x + (MODE == kSelDraft ? (size_t)p.n_lists * p.batch : 0)) * 64
                 : nullptr;
     sel_ts(tr, 0);
+    // PDL chain invariant ("PDL chain invariant"): WAIT FIRST, THEN TRIGGER -- never the other way round.
+    // The scoring kernel released here (ScoreParams::defer_wait) writes the logits scratch before any dependency wait of
+    // its own, and that scratch shares the front of the workspace with the stream-K partials of the PREVIOUS call's
+    // attention kernel, which released this kernel at its very start.  This wait (previous attention kernel complete and
+    // visible) is therefore the only thing that orders the scoring kernel behind it.
     pdl_wait();
     if (MODE == kSelDraft) pdl_trigger();   // the scoring kernel may start now: it needs nothing from this one
     sel_ts(tr, 1);

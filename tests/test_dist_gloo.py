@@ -77,3 +77,22 @@ def test_reference_arm_runs_only_on_rank0(monkeypatch, capsys):
     d.rank, d.world, d.on = 1, 2, True
     bench.run_reference(A, d)                                     # non-zero rank: no work, no output
     assert capsys.readouterr().out == ""
+
+
+def test_gpus_flag_without_launcher_spawns_the_ranks():
+    """`python bench.py --gpus 2` with no WORLD_SIZE in the environment must start two ranks itself (never print
+    n_gpus = 2 from one process): checked on the reference arm, which needs no GPU -- rank 0 prints the one line and
+    reports the world it ran in, rank 1 exits quietly."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--impl", "reference", "--gpus", "2", "--batch",
+                        "1", "--ctx", "256", "--layers", "1", "--steps", "1", "--warmup", "0"],
+                       capture_output=True, text=True, env=env, cwd=root, timeout=600)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [json.loads(l) for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    assert lines[0]["impl"] == "reference" and lines[0]["n_gpus"] == 2
+    assert lines[0]["run"]["world"] == 2 and "self-spawned" in lines[0]["run"]["launcher"]

@@ -99,3 +99,25 @@ def test_scale_invariance():
     a = run_gpu(sd, st, 512, 4, 16, 1, 2)
     b = run_gpu(sd * 4.0, st * 0.125, 512, 4, 16, 1, 2)  # power-of-two rescale is exact in fp32
     assert torch.equal(a[0], b[0])
+
+
+@pytest.mark.parametrize("threads", [256, 512, 1024])
+def test_block_excl_scan_of_every_cta_size(threads):
+    """The block-wide exclusive prefix sum of the selection kernels, alone, in each of its three instantiations (the 256-
+    and 512-thread ones carry a work-around for a lane-31 store that nvcc 12.9 mis-addressed): against torch.cumsum in
+    int64, on random counts, all-ones, a single non-zero and values that wrap 2^32; two scans in a row per CTA."""
+    g = torch.Generator(device="cpu").manual_seed(1234 + threads)
+    rows = [torch.randint(0, 5000, (threads,), generator=g), torch.ones(threads, dtype=torch.int64),
+            torch.zeros(threads, dtype=torch.int64), torch.randint(0, 2, (threads,), generator=g),
+            torch.randint(0, 1 << 31, (threads,), generator=g)]
+    rows[2][threads - 1] = 7
+    for k in range(11):
+        rows.append(torch.randint(0, 40000, (threads,), generator=g))
+    v = torch.stack(rows)                                          # int64 [n_blocks, threads], values < 2^31
+    out, total = api.debug_block_scan(threads, v.to(torch.int32).cuda())
+    torch.cuda.synchronize()
+    out, total = out.cpu().to(torch.int64) & 0xFFFFFFFF, total.cpu().to(torch.int64) & 0xFFFFFFFF
+    for j, vv in enumerate((v, v + 1)):
+        inc = torch.cumsum(vv, dim=1)
+        assert torch.equal(out[j], (inc - vv) & 0xFFFFFFFF), f"threads={threads} scan {j}: prefixes differ"
+        assert torch.equal(total[j], inc[:, -1] & 0xFFFFFFFF), f"threads={threads} scan {j}: totals differ"
