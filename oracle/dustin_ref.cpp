@@ -22,6 +22,13 @@
 //   dustin_ref_arr                :72-75 Eq. 1 (Attention Recovery Rate), Eq. 2-4 by composition.
 //   dustin_ref_append_kv          :153 (accepted tokens appended, rejected discarded).
 //   dustin_ref_draft_aggregate    :157-161 Eq. 5, first line (S_Draft = sum over draft heads, layers, lookahead tokens).
+//   dustin_ref_quest_page_minmax  :401 "aggregates token-level Key statistics (e.g., minimum and maximum values) into
+//                                 page-level metadata"; :297 "Quest-16 denotes Quest with page size 16".
+//   dustin_ref_quest_score_pages  :51 "scores KV pages using inexpensive min/max key statistics (avoiding exact QK^T)",
+//                                 :401 "estimate the relevance of a block of tokens using a single computation".
+//                                 The paper names the estimator without its formula: DESIGN.md reading A20 takes the
+//                                 channel-wise upper bound of the published method, reading A21 its use as a page-level
+//                                 score in the format of O1.
 //
 // Pins (tests/test_oracle_pins.py): brute force on tiny inputs, closed forms (uniform softmax, one
 // planted key, constant V, zero K), library cross-checks (torch fp64 softmax / SDPA, full sort),
@@ -408,6 +415,107 @@ int dustin_ref_draft_aggregate(int batch, int n_q_heads, int n_kv_heads, int hea
         }
         float* dst = s_draft + (int64_t)b * max_ctx;
         for (int n = 0; n < max_ctx; ++n) dst[n] = n < N ? (float)sum[n] : 0.0f;
+    }
+    return 0;
+}
+
+// ---------------------------------------------------------------------------------------------
+// O8 -- page-level key metadata of the Quest-style estimator (page size 16).
+// Logical page p of sequence b holds the tokens [p*P, (p+1)*P) that exist (n < N_b), whatever the physical layout of
+// the cache.  Per (b, p, KV head g, channel c):  kmin = min_n K[b,n,g,c],  kmax = max_n K[b,n,g,c].
+// A page without any token (p*P >= N_b) gets kmin = kmax = 0.   Outputs: fp64 [batch, n_pages, n_kv_heads, head_dim]
+// with n_pages = ceil(max_ctx / P)  (the values are bf16 numbers, so any float type holds them exactly).
+// ---------------------------------------------------------------------------------------------
+int dustin_ref_quest_page_minmax(int batch, int n_kv_heads, int head_dim, int max_ctx, const uint16_t* k_cache,
+                                 int64_t stride_seq, int64_t stride_token, int64_t stride_head,
+                                 const int32_t* page_table, int page_size, int max_pages, const int32_t* seq_lens,
+                                 int quest_page, double* kmin_out, double* kmax_out) {
+    if (quest_page <= 0) return -1;
+    KvView kv{k_cache, nullptr, stride_seq, stride_token, stride_head, page_table, page_size, max_pages};
+    const int n_pages = (max_ctx + quest_page - 1) / quest_page;
+    for (int b = 0; b < batch; ++b) {
+        const int N = seq_len(seq_lens, b, max_ctx);
+        for (int p = 0; p < n_pages; ++p)
+            for (int g = 0; g < n_kv_heads; ++g)
+                for (int c = 0; c < head_dim; ++c) {
+                    double lo = 0.0, hi = 0.0;
+                    bool any = false;
+                    for (int n = p * quest_page; n < (p + 1) * quest_page && n < N; ++n) {
+                        const double x = bf16_to_double(k_cache[row_offset(kv, b, n, g) + c]);
+                        if (!any || x < lo) lo = x;
+                        if (!any || x > hi) hi = x;
+                        any = true;
+                    }
+                    const int64_t o = (((int64_t)b * n_pages + p) * n_kv_heads + g) * head_dim + c;
+                    kmin_out[o] = lo;
+                    kmax_out[o] = hi;
+                }
+    }
+    return 0;
+}
+
+// ---------------------------------------------------------------------------------------------
+// O9 -- page scores from the metadata alone (readings A20, A21).
+// For every subset head h (KV group g = h div r) and every page p that holds a token (p*P < N_b):
+//   U_h[p] = scale * sum_c max(q[b,h,c] * kmin[b,p,g,c], q[b,h,c] * kmax[b,p,g,c])
+// -- per channel the larger of the two products bounds q_c * k_c for every key of the page, so U_h[p] is an upper
+// bound of every exact logit scale * q.k_n inside the page, computed without touching K (A20).
+//   P_h[p] = softmax_p(U_h) over the pages that hold a token;  page_scores[b,l,p] = sum of P_h over the subset heads
+// feeding list l, with the list rule of O1 (n_lists = 1: all subset heads; n_lists = Hkv: the heads of KV group l, a
+// group without a subset head receives the sum over all subset heads) (A21).  Pages without a token score 0.
+//   kmin, kmax: fp64 [batch, n_pages, n_kv_heads, head_dim] (O8);  q as in O1.
+//   page_scores: fp32 [batch, n_lists, n_pages];  ub_out (optional): fp64 [batch, n_q_heads, n_pages], U_h[p] for the
+//   subset heads (0 elsewhere).
+// ---------------------------------------------------------------------------------------------
+int dustin_ref_quest_score_pages(int batch, int n_q_heads, int n_kv_heads, int head_dim, int max_ctx, float sm_scale,
+                                 const int32_t* seq_lens, int quest_page, const double* kmin, const double* kmax,
+                                 const uint16_t* q, int64_t q_stride_batch, int64_t q_stride_head, uint64_t head_mask,
+                                 int n_lists, float* page_scores, double* ub_out) {
+    if (quest_page <= 0 || n_q_heads % n_kv_heads != 0 || (n_lists != 1 && n_lists != n_kv_heads)) return -1;
+    const int r = n_q_heads / n_kv_heads;
+    const double scale = scale_of(sm_scale, head_dim);
+    const int n_pages = (max_ctx + quest_page - 1) / quest_page;
+    for (int b = 0; b < batch; ++b) {
+        const int N = seq_len(seq_lens, b, max_ctx);
+        const int n_live = (N + quest_page - 1) / quest_page;   // pages that hold a token
+        std::vector<double> group_sum((size_t)n_kv_heads * n_pages, 0.0), global_sum(n_pages, 0.0), U(n_pages);
+        std::vector<int> heads_in_group(n_kv_heads, 0);
+        for (int h = 0; h < n_q_heads; ++h) {
+            if (ub_out)
+                for (int p = 0; p < n_pages; ++p) ub_out[((int64_t)b * n_q_heads + h) * n_pages + p] = 0.0;
+            if (!((head_mask >> h) & 1ull)) continue;
+            const int g = h / r;
+            heads_in_group[g] += 1;
+            const uint16_t* qh = q + (int64_t)b * q_stride_batch + (int64_t)h * q_stride_head;
+            double M = -INFINITY;
+            for (int p = 0; p < n_live; ++p) {
+                const int64_t o = (((int64_t)b * n_pages + p) * n_kv_heads + g) * head_dim;
+                double acc = 0.0;
+                for (int c = 0; c < head_dim; ++c) {
+                    const double qc = bf16_to_double(qh[c]);
+                    acc += std::max(qc * kmin[o + c], qc * kmax[o + c]);
+                }
+                U[p] = acc * scale;
+                if (U[p] > M) M = U[p];
+                if (ub_out) ub_out[((int64_t)b * n_q_heads + h) * n_pages + p] = U[p];
+            }
+            double Z = 0.0;
+            for (int p = 0; p < n_live; ++p) Z += std::exp(U[p] - M);
+            for (int p = 0; p < n_live; ++p) {
+                const double pr = std::exp(U[p] - M) / Z;
+                group_sum[(size_t)g * n_pages + p] += pr;
+                global_sum[p] += pr;
+            }
+        }
+        for (int l = 0; l < n_lists; ++l) {
+            float* dst = page_scores + ((int64_t)b * n_lists + l) * n_pages;
+            const bool use_global = (n_lists == 1) || heads_in_group[l] == 0;
+            for (int p = 0; p < n_pages; ++p) {
+                double sc = 0.0;
+                if (p < n_live) sc = use_global ? global_sum[p] : group_sum[(size_t)l * n_pages + p];
+                dst[p] = (float)sc;
+            }
+        }
     }
     return 0;
 }

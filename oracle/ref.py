@@ -214,3 +214,44 @@ def draft_aggregate(layer_k: list, layer_q: list, head_mask: int, n_kv_heads: in
     if rc != 0:
         raise ValueError(f"dustin_ref_draft_aggregate: status {rc}")
     return out
+
+
+def quest_page_minmax(kv: KV, n_kv_heads: int, max_ctx: int, quest_page: int = 16):
+    """O8: per-page, per-channel min / max of the keys.  Returns (kmin, kmax), fp64
+    [B, ceil(max_ctx / quest_page), Hkv, d]; B and d are taken from the (contiguous or paged) cache tensor."""
+    k = _bits(kv.k)
+    d = k.shape[-1]
+    pt, sl = _i32(kv.page_table), _i32(kv.seq_lens)
+    B = pt.shape[0] if pt is not None else k.shape[0]
+    n_pages = (max_ctx + quest_page - 1) // quest_page
+    kmin = torch.zeros(B, n_pages, n_kv_heads, d, dtype=torch.float64)
+    kmax = torch.zeros_like(kmin)
+    rc = lib().dustin_ref_quest_page_minmax(
+        ctypes.c_int(B), ctypes.c_int(n_kv_heads), ctypes.c_int(d), ctypes.c_int(max_ctx), _p(k),
+        ctypes.c_int64(kv.stride_seq), ctypes.c_int64(kv.stride_token), ctypes.c_int64(kv.stride_head), _p(pt),
+        ctypes.c_int(kv.page_size), ctypes.c_int(0 if pt is None else pt.shape[1]), _p(sl), ctypes.c_int(quest_page),
+        _p(kmin), _p(kmax))
+    if rc != 0:
+        raise ValueError(f"dustin_ref_quest_page_minmax: status {rc}")
+    return kmin, kmax
+
+
+def quest_score_pages(kmin: torch.Tensor, kmax: torch.Tensor, q: torch.Tensor, head_mask: int, n_lists: int,
+                      max_ctx: int, quest_page: int = 16, seq_lens=None, sm_scale: float = 0.0, want_ub: bool = False):
+    """O9 (readings A20 / A21).  q: [B, Hq, d] bf16.  Returns fp32 [B, n_lists, n_pages] page
+    scores (and, with want_ub, the fp64 [B, Hq, n_pages] upper-bound logits of the subset heads)."""
+    B, Hq, d = q.shape
+    assert q.dtype == torch.bfloat16 and q.device.type == "cpu" and q.stride(2) == 1
+    n_pages, Hkv = kmin.shape[1], kmin.shape[2]
+    assert kmin.dtype == torch.float64 and kmin.is_contiguous() and kmax.is_contiguous() and kmax.shape == kmin.shape
+    assert n_pages == (max_ctx + quest_page - 1) // quest_page
+    out = torch.zeros(B, n_lists, n_pages, dtype=torch.float32)
+    ub = torch.zeros(B, Hq, n_pages, dtype=torch.float64) if want_ub else None
+    rc = lib().dustin_ref_quest_score_pages(
+        ctypes.c_int(B), ctypes.c_int(Hq), ctypes.c_int(Hkv), ctypes.c_int(d), ctypes.c_int(max_ctx),
+        ctypes.c_float(sm_scale), _p(_i32(seq_lens)), ctypes.c_int(quest_page), _p(kmin), _p(kmax),
+        ctypes.c_void_p(q.data_ptr()), ctypes.c_int64(q.stride(0)), ctypes.c_int64(q.stride(1)),
+        ctypes.c_uint64(head_mask), ctypes.c_int(n_lists), _p(out), _p(ub))
+    if rc != 0:
+        raise ValueError(f"dustin_ref_quest_score_pages: status {rc}")
+    return (out, ub) if want_ub else out
