@@ -184,6 +184,28 @@ class Workload:
             self.api.score_heads(self.shape, self.kv[s], self.q[l][:, 0], (1 << c.n_q_heads) - 1, c.n_lists,
                                  self.scratch_scores, self.ws_all)
 
+    def quest_setup(self):
+        """Page metadata of every distinct cache (built once, like after prefill) for the Quest-16 estimator leg."""
+        if not hasattr(self, "quest_meta"):
+            self.quest_meta = [self.api.quest_alloc_meta(self.shape, self.device) for _ in self.sets]
+            n_pages = self.quest_meta[0].shape[1]
+            self.quest_scores = torch.empty((self.cfg.batch, self.cfg.n_lists, n_pages), device=self.device)
+            self.step_quest_build()
+
+    def step_quest_build(self):
+        """dustin_quest_build_pages for every distinct cache: one pass over K per cache."""
+        for s in range(self.n_sets):
+            self.api.quest_build_pages(self.shape, self.kv[s], self.quest_meta[s])
+
+    def step_score_quest16(self):
+        """The Quest-16 estimator of PAPER.md:297-299 (Fig. 8) in every layer: page scores for the SAME subset heads from
+        the page min / max metadata alone (no read of K)."""
+        c = self.cfg
+        for l in range(self.L):
+            s = l % self.n_sets
+            self.api.quest_score_pages(self.shape, self.quest_meta[s], self.q[l][:, 0], c.head_mask, c.n_lists,
+                                       self.quest_scores, self.ws, self.sets[s].seq_lens)
+
     def step_attn_only(self):
         """a4 alone in every layer, each with the index lists its own fused pass left in idx[l] / cnt[l] (kernel-only
         timing of the gathered attention: the region holds nothing but L launches of that kernel)."""
@@ -633,6 +655,9 @@ def sweep_point(api, cfg: synth.Config, n_sets: int, dist: Dist, device, peak: f
     if naive:
         w.step_score_all_heads()
         legs.append(("score_all_heads", w.step_score_all_heads))
+        w.quest_setup()
+        w.step_score_quest16()
+        legs.append(("score_quest16", w.step_score_quest16))
     for name, fn in legs:
         t[name] = 1e3 * time_steps(graphed(fn), 3, 3, dist, device) / cfg.n_layers
     # the streaming kernel of a1 alone (event pairs inside the library): "score" above is the whole staged a1 stage --
@@ -645,6 +670,16 @@ def sweep_point(api, cfg: synth.Config, n_sets: int, dist: Dist, device, peak: f
     if naive:
         out["score_all_heads_us"] = round(t["score_all_heads"], 2)
         out["score_all_heads_over_dense"] = round(t["score_all_heads"] / t["dense"], 3)
+        # Fig. 8's third estimator: Quest with 16-token pages on the same subset heads (metadata bytes = 1/8 of the K bytes
+        # of the scored groups), and the one-off cost of building that metadata (one pass over K per cache)
+        out["score_quest16_us"] = round(t["score_quest16"], 2)
+        out["score_quest16_over_dense"] = round(t["score_quest16"] / t["dense"], 3)
+        out["score_subset_over_dense"] = round(t["score"] / t["dense"], 3)
+        meta_bytes = by["a1_k"] / 8.0
+        out["score_quest16_gbs"] = round(meta_bytes / t["score_quest16"] / 1e3, 1)
+        tb = 1e3 * time_steps(graphed(w.step_quest_build), 3, 3, dist, device) / w.n_sets
+        out["quest16_build_us_per_cache"] = round(tb, 2)
+        out["quest16_build_gbs"] = round((cfg.batch * cfg.ctx * cfg.n_kv_heads * cfg.head_dim * 2 * 1.125) / tb / 1e3, 1)
     out.update({
         "fused_us": round(t["fused"], 2), "score_us": round(t["score"], 2), "sparse_attn_us": round(t["attn"], 2),
         "dense_us": round(t["dense"], 2), "speedup_vs_dense": round(t["dense"] / t["fused"], 2),

@@ -8,7 +8,7 @@
  *   a5 the same call with idx == NULL is the full-cache verification baseline
  *   a6 dustin_verify_layer_fused a1..a4 enqueued on one stream, no host sync
  * and the steps either side of it: dustin_arr (Eq. 1-4), dustin_append_kv,
- * dustin_draft_aggregate (Eq. 5, first line).  Measurement / tuning / testing aids live in dustin_debug.h.
+ * dustin_draft_aggregate (Eq. 5, first line), the Quest-16 page estimator of Fig. 8 (dustin_quest_*).  Measurement / tuning / testing aids live in dustin_debug.h.
  *
  * Conventions (all entry points):
  *  - Every pointer marked "device" is a CUDA device pointer owned by the caller; the library never allocates,
@@ -206,6 +206,37 @@ size_t dustin_draft_workspace_bytes(const dustin_shape_t* shape, uint64_t head_m
 int dustin_draft_aggregate(const dustin_shape_t* shape, const dustin_kv_t* kv_layers, const void* const* q_layers,
                            int32_t n_layers, uint64_t head_mask, float* s_draft, void* ws, size_t ws_bytes,
                            void* stream);
+
+/* ---- alternative estimator: Quest with 16-token pages -----------------------------------
+ * The estimator the paper measures its head-subset scoring against ("scores KV pages using inexpensive
+ * min/max key statistics (avoiding exact QK^T)"; :297-299, Fig. 8 "Quest-16 denotes Quest with page size 16"; :401
+ * "aggregates token-level Key statistics (e.g., minimum and maximum values) into page-level metadata ... reducing the
+ * sequence length dimension for estimation from N to N/page size").  The paper names it without a formula; DESIGN.md
+ * readings A20 / A21 fix one.  Logical page p of sequence b = the tokens [16p, 16p+16) below N_b, whatever the physical
+ * layout of the cache.
+ *
+ * dustin_quest_build_pages: per (b, p, KV head g, channel c)  kmin = min_n K[b,n,g,c], kmax = max_n K[b,n,g,c] over the
+ *   page's tokens (a page without a token: both 0).  page_meta: device bf16 [B, ceil(max_ctx/16), Hkv, 2, d] (kmin row,
+ *   then kmax row; dustin_quest_meta_bytes bytes, 16-byte aligned), written.  first_token: device int32 [B] or NULL;
+ *   when given, only the pages from first_token[b] / 16 on are rebuilt (after dustin_append_kv: pass the lengths from
+ *   BEFORE the append, kv->seq_lens being the new ones); NULL rebuilds every page.  One pass over K (only kv->k is read).
+ * dustin_quest_score_pages: for every subset head h (KV group g) and page p with a token
+ *     U_h[p] = sm_scale * sum_c max(q[b,h,c] * kmin[b,p,g,c], q[b,h,c] * kmax[b,p,g,c])
+ *   -- an upper bound of every exact logit sm_scale * q . K[b,n,g,:] of the page, from the metadata alone (A20) --
+ *   then P_h = softmax over the pages that hold a token, and page_scores[b,l,p] = sum of P_h over the subset heads that
+ *   feed list l, with the list rule of dustin_score_heads (A21); pages without a token score 0.  The result has the
+ *   format of a1's scores with pages for tokens: dustin_topk_select with max_ctx = ceil(max_ctx/16) ranks pages.
+ *   seq_lens: device int32 [B] or NULL (all max_ctx);  q, strides, head_mask, n_lists as in dustin_score_heads;
+ *   page_scores: device fp32 [B, n_lists, ceil(max_ctx/16)], written;  ub_out: device fp32 [B, |subset|, ceil(max_ctx/16)]
+ *   (subset heads in ascending order; U_h[p], 0 for pages without a token) or NULL;
+ *   ws: dustin_workspace_bytes(shape, head_mask, 1) bytes are enough. */
+#define DUSTIN_QUEST_PAGE 16
+size_t dustin_quest_meta_bytes(const dustin_shape_t* shape);
+int dustin_quest_build_pages(const dustin_shape_t* shape, const dustin_kv_t* kv, const int32_t* first_token,
+                             void* page_meta, void* stream);
+int dustin_quest_score_pages(const dustin_shape_t* shape, const int32_t* seq_lens, const void* page_meta, const void* q,
+                             int64_t q_stride_batch, int64_t q_stride_head, uint64_t head_mask, int32_t n_lists,
+                             float* page_scores, float* ub_out, void* ws, size_t ws_bytes, void* stream);
 
 /* ---- a1 without a workspace argument --------------------------------------------------------------------------------
  * dustin_score_heads_static computes exactly what dustin_score_heads computes (same arguments, same kernels, same

@@ -58,7 +58,7 @@ void dustin_debug_trace_buffer(void* device_ptr, size_t bytes);
  * (and drops earlier records); dustin_profile_enable(0) stops.  dustin_profile_collect is the one call that
  * synchronises: it waits for the recorded events and writes, per kernel id in [0, DUSTIN_N_KERNELS), the summed
  * device time in ms and the number of launches (host arrays), then clears the records. */
-#define DUSTIN_N_KERNELS 10
+#define DUSTIN_N_KERNELS 13
 uint64_t    dustin_launch_count(void);
 void        dustin_profile_enable(int32_t on);
 int         dustin_profile_collect(double* ms_out, int64_t* launches_out);

@@ -109,6 +109,12 @@ def lib():
         L.dustin_arr.argtypes = [i32, i32, i32, vp, vp, vp, vp, i32, vp, vp]
         L.dustin_append_kv.restype = ctypes.c_int
         L.dustin_append_kv.argtypes = [sp, kp, vp, vp, vp, vp, vp, i32, vp]
+        L.dustin_quest_meta_bytes.restype = sz
+        L.dustin_quest_meta_bytes.argtypes = [sp]
+        L.dustin_quest_build_pages.restype = ctypes.c_int
+        L.dustin_quest_build_pages.argtypes = [sp, kp, vp, vp, vp]
+        L.dustin_quest_score_pages.restype = ctypes.c_int
+        L.dustin_quest_score_pages.argtypes = [sp, vp, vp, vp, i64, i64, u64, i32, vp, vp, vp, sz, vp]
         L.dustin_draft_workspace_bytes.restype = sz
         L.dustin_draft_workspace_bytes.argtypes = [sp, u64]
         L.dustin_draft_aggregate.restype = ctypes.c_int
@@ -117,13 +123,14 @@ def lib():
     return _lib
 
 
-N_KERNELS = 10
+N_KERNELS = 13
 
 # include/dustin.h (the product surface) ...
 EXPORTS = ("dustin_version", "dustin_status_string", "dustin_last_cuda_error",
            "dustin_workspace_bytes", "dustin_score_heads", "dustin_fuse_scores", "dustin_topk_select",
            "dustin_sparse_verify_attn", "dustin_verify_layer_fused", "dustin_arr", "dustin_append_kv",
-           "dustin_draft_workspace_bytes", "dustin_draft_aggregate", "dustin_score_heads_static")
+           "dustin_draft_workspace_bytes", "dustin_draft_aggregate", "dustin_score_heads_static",
+           "dustin_quest_meta_bytes", "dustin_quest_build_pages", "dustin_quest_score_pages")
 # ... and include/dustin_debug.h (measurement / tuning / testing aids)
 DEBUG_EXPORTS = ("dustin_tune_attn_split_tokens", "dustin_tune_attn_impl", "dustin_tune_set", "dustin_tune_get",
                  "dustin_debug_trace_buffer", "dustin_launch_count", "dustin_profile_enable", "dustin_profile_collect",
@@ -425,3 +432,38 @@ def alloc_draft_workspace(shape: Shape, head_mask: int, device="cuda") -> torch.
     if n == 0:
         raise ValueError("dustin_draft_workspace_bytes: invalid shape or empty head mask")
     return torch.zeros(n, dtype=torch.uint8, device=device)
+
+
+QUEST_PAGE = 16     # DUSTIN_QUEST_PAGE
+
+
+def quest_alloc_meta(shape: Shape, device="cuda") -> torch.Tensor:
+    """bf16 [B, ceil(max_ctx/16), Hkv, 2, d] page metadata buffer (dustin_quest_meta_bytes)."""
+    n_pages = (shape.max_ctx + QUEST_PAGE - 1) // QUEST_PAGE
+    meta = torch.empty((shape.batch, n_pages, shape.n_kv_heads, 2, shape.head_dim), dtype=torch.bfloat16, device=device)
+    assert meta.numel() * 2 == int(lib().dustin_quest_meta_bytes(ctypes.byref(shape)))
+    return meta
+
+
+def quest_build_pages(shape: Shape, kv: KV, page_meta: torch.Tensor, first_token: Optional[torch.Tensor] = None) -> None:
+    """per-page, per-channel key min / max; first_token (int32 [B]) limits the rebuild to later pages."""
+    kvc = kv.c()
+    rc = lib().dustin_quest_build_pages(ctypes.byref(shape), ctypes.byref(kvc),
+                                        None if first_token is None else _dense(first_token, torch.int32),
+                                        _dense(page_meta, torch.bfloat16), _stream())
+    _check("dustin_quest_build_pages", rc)
+
+
+def quest_score_pages(shape: Shape, page_meta: torch.Tensor, q: torch.Tensor, head_mask: int, n_lists: int,
+                      page_scores: torch.Tensor, ws: torch.Tensor, seq_lens: Optional[torch.Tensor] = None,
+                      ub_out: Optional[torch.Tensor] = None) -> None:
+    """PAPER.md:51 / :297: page scores from the metadata alone.  q: bf16 [B, Hq, d] view; page_scores fp32
+    [B, n_lists, n_pages]; ub_out fp32 [B, |subset|, n_pages] or None."""
+    if q.dim() != 3 or q.stride(2) != 1:
+        raise ValueError("q must be a [B, Hq, d] view with a contiguous last dimension")
+    rc = lib().dustin_quest_score_pages(
+        ctypes.byref(shape), None if seq_lens is None else _dense(seq_lens, torch.int32),
+        _dense(page_meta, torch.bfloat16), _ptr(q, torch.bfloat16), q.stride(0), q.stride(1),
+        ctypes.c_uint64(head_mask), n_lists, _dense(page_scores, torch.float32),
+        None if ub_out is None else _dense(ub_out, torch.float32), _ptr(ws), ws.numel(), _stream())
+    _check("dustin_quest_score_pages", rc)

@@ -17,7 +17,7 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libdustin.so")
 OBJ_DIR = os.path.join(HERE, "build")
-SOURCES = ["api.cu", "score.cu", "select.cu", "select_cluster.cu", "attn.cu", "attn_tc.cu", "extras.cu", "profile.cu"]
+SOURCES = ["api.cu", "score.cu", "select.cu", "select_cluster.cu", "attn.cu", "attn_tc.cu", "extras.cu", "quest.cu", "profile.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC"]
 

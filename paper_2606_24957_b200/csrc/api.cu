@@ -658,6 +658,75 @@ int dustin_draft_aggregate(const dustin_shape_t* shape, const dustin_kv_t* kv_la
     return DUSTIN_OK;
 }
 
+// ---- Quest-16 estimator -------------------------------------------------------------------------------------------------
+size_t dustin_quest_meta_bytes(const dustin_shape_t* shape) {
+    if (check_shape(shape) != DUSTIN_OK) return 0;
+    const size_t n_pages = ((size_t)shape->max_ctx + DUSTIN_QUEST_PAGE - 1) / DUSTIN_QUEST_PAGE;
+    return (size_t)shape->batch * n_pages * shape->n_kv_heads * 2 * shape->head_dim * sizeof(__nv_bfloat16);
+}
+
+int dustin_quest_build_pages(const dustin_shape_t* shape, const dustin_kv_t* kv, const int32_t* first_token,
+                             void* page_meta, void* stream) {
+    int rc = check_shape(shape);
+    if (rc) return rc;
+    KvView view;
+    rc = check_kv(shape, kv, false, &view);
+    if (rc) return rc;
+    if (!page_meta || ((uintptr_t)page_meta & 15)) return DUSTIN_ERR_INVALID_ARG;
+    const int n_pages = (shape->max_ctx + DUSTIN_QUEST_PAGE - 1) / DUSTIN_QUEST_PAGE;
+    const cudaError_t e = launch_quest_build(view, first_token, static_cast<__nv_bfloat16*>(page_meta), shape->batch,
+                                             shape->n_kv_heads, shape->head_dim, shape->max_ctx, n_pages,
+                                             static_cast<cudaStream_t>(stream));
+    return e == cudaSuccess ? DUSTIN_OK : fail_cuda(e);
+}
+
+int dustin_quest_score_pages(const dustin_shape_t* shape, const int32_t* seq_lens, const void* page_meta, const void* q,
+                             int64_t q_stride_batch, int64_t q_stride_head, uint64_t head_mask, int32_t n_lists,
+                             float* page_scores, float* ub_out, void* ws, size_t ws_bytes, void* stream) {
+    int rc = check_shape(shape);
+    if (rc) return rc;
+    if (!page_meta || ((uintptr_t)page_meta & 15) || !page_scores) return DUSTIN_ERR_INVALID_ARG;
+    if (!q || ((uintptr_t)q & 15) || ((q_stride_batch | q_stride_head) & 7) || q_stride_batch < 0 || q_stride_head < 0)
+        return DUSTIN_ERR_INVALID_ARG;
+    ScoreParams sp;
+    std::memset(&sp, 0, sizeof sp);
+    rc = build_subset(shape, head_mask, n_lists, &sp);   // same subset / list tables as stage a1
+    if (rc) return rc;
+    QuestParams p;
+    std::memset(&p, 0, sizeof p);
+    p.meta = static_cast<const __nv_bfloat16*>(page_meta);
+    p.q = static_cast<const __nv_bfloat16*>(q);
+    p.q_stride_batch = q_stride_batch;
+    p.seq_lens = seq_lens;
+    p.batch = shape->batch;
+    p.n_kv_heads = shape->n_kv_heads;
+    p.head_dim = shape->head_dim;
+    p.max_ctx = shape->max_ctx;
+    p.n_pages = (shape->max_ctx + DUSTIN_QUEST_PAGE - 1) / DUSTIN_QUEST_PAGE;
+    p.n_lists = n_lists;
+    p.scale_log2 = scale_log2_of(shape);
+    p.scale = p.scale_log2 / kLog2e;
+    p.nsel = sp.nsel;
+    p.n_groups = sp.n_groups;
+    int max_nh = 1;
+    for (int gi = 0; gi < sp.n_groups; ++gi) max_nh = sp.group_cnt[gi] > max_nh ? sp.group_cnt[gi] : max_nh;
+    quest_plan(p.batch, p.n_groups, max_nh, p.n_pages, &p.group_slots, &p.chunk_pages, &p.n_chunks);
+    for (int i = 0; i < sp.nsel; ++i) p.sel_qoff[i] = (int)(sp.sel_head[i] * q_stride_head);
+    std::memcpy(p.group_id, sp.group_id, sizeof p.group_id);
+    std::memcpy(p.group_first, sp.group_first, sizeof p.group_first);
+    std::memcpy(p.group_cnt, sp.group_cnt, sizeof p.group_cnt);
+    std::memcpy(p.list_first, sp.list_first, sizeof p.list_first);
+    std::memcpy(p.list_cnt, sp.list_cnt, sizeof p.list_cnt);
+    p.u_stride = ((long long)p.n_pages + 3) & ~3ll;
+    const size_t u_bytes = align256((size_t)p.batch * p.nsel * p.u_stride * sizeof(float));
+    if (!ws || ((uintptr_t)ws & 255) || ws_bytes < kWsHeader + u_bytes) return DUSTIN_ERR_WORKSPACE;
+    char* base = static_cast<char*>(ws) + kWsHeader;   // the persistent header belongs to the attention stage
+    p.u = reinterpret_cast<float*>(base);
+    p.ub_out = ub_out;
+    const cudaError_t e = launch_quest_score(p, page_scores, static_cast<cudaStream_t>(stream));
+    return e == cudaSuccess ? DUSTIN_OK : fail_cuda(e);
+}
+
 size_t dustin_draft_workspace_bytes(const dustin_shape_t* shape, uint64_t head_mask) {
     if (check_shape(shape) != DUSTIN_OK || head_mask == 0) return 0;
     int nsel = popcount64(head_mask) * shape->n_new;

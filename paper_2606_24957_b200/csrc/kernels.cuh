@@ -127,6 +127,28 @@ cudaError_t launch_append(const KvView& kv, int* seq_lens, const int* n_append, 
                           const __nv_bfloat16* v_new, int batch, int T, int n_kv_heads, int head_dim, int max_ctx,
                           float* hist, int n_lists, cudaStream_t stream);
 
+// ---- Quest-16 estimator (quest.cu) ----------------------------------------------------------
+struct QuestParams {
+    const __nv_bfloat16* meta;      // [B, n_pages, Hkv, 2, D]: kmin then kmax of every 16-token page
+    const __nv_bfloat16* q;
+    long long q_stride_batch;
+    const int* seq_lens;
+    int batch, n_kv_heads, head_dim, max_ctx, n_pages, n_lists;
+    float scale, scale_log2;
+    int nsel, n_groups, n_chunks;   // subset size; scored KV groups; scoring CTAs per sequence
+    int group_slots, chunk_pages;   // scored KV groups served side by side by the 8 warps of a CTA; pages per CTA (quest_plan)
+    int sel_qoff[64];
+    unsigned char group_id[64], group_first[64], group_cnt[64], list_first[64], list_cnt[64];   // as in ScoreParams
+    long long u_stride;             // n_pages rounded up to a multiple of 4
+    float* u;                       // ws: [B, nsel, u_stride] upper-bound logits, log2 domain
+    float* ub_out;                  // optional output [B, nsel, n_pages]: the upper-bound logits themselves, or nullptr
+};
+void quest_plan(int batch, int n_groups, int max_heads_per_group, int n_pages, int* group_slots, int* chunk_pages,
+                int* n_chunks);
+cudaError_t launch_quest_build(const KvView& kv, const int* first_token, __nv_bfloat16* meta, int batch, int n_kv_heads,
+                               int head_dim, int max_ctx, int n_pages, cudaStream_t stream);
+cudaError_t launch_quest_score(const QuestParams& p, float* page_scores, cudaStream_t stream);
+
 // Measurement aid: reads the K / V rows that a4 would gather for these lists and does nothing else (sink: >= batch *
 // n_kv_heads words of scratch).
 cudaError_t launch_gather_probe(const KvView& kv, const int* idx, const int* cnt, int batch, int n_kv_heads, int head_dim,
@@ -141,7 +163,7 @@ cudaError_t launch_occupy(int n_ctas, int threads, int smem_bytes, int microseco
 // ---- launch bookkeeping (profile.cu) ----------------------------------------------------------------------------
 enum KernelId {
     kKernScoreLogits = 0, kKernScoreStats, kKernScoreNormalize, kKernFuse, kKernSelect, kKernAttn, kKernSelectDraft,
-    kKernArr, kKernAppend, kKernSelectCluster,
+    kKernArr, kKernAppend, kKernSelectCluster, kKernQuestBuild, kKernQuestScore, kKernQuestNormalize,
     kKernCount
 };
 // Put one on the stack around a kernel launch: counts it and, when profiling is on, brackets it with CUDA events.

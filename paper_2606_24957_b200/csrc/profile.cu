@@ -36,7 +36,8 @@ cudaEvent_t take_event() {
 }
 const char* const kNames[kKernCount] = {"score_logits_kernel", "score_stats_kernel", "score_normalize_kernel",
                                         "fuse_kernel", "select_kernel", "attn_kernel", "select_draft_kernel",
-                                        "arr_kernel", "append_kernel", "select_cluster_kernel"};
+                                        "arr_kernel", "append_kernel", "select_cluster_kernel", "quest_build_kernel",
+                                        "quest_score_kernel", "quest_normalize_kernel"};
 static_assert(kKernCount == DUSTIN_N_KERNELS, "dustin_debug.h and kernels.cuh disagree on the kernel count");
 }  // namespace
 
