@@ -23,6 +23,13 @@ def full_cases():
         "qwen72b_4k_b16_gamma2_k256": synth.config_qwen72b(ctx=4096, gamma=2, budget=256),
         "qwen72b_128k_b4_gamma8_k8192": synth.config_qwen72b(batch=4, ctx=131072, gamma=8, budget=8192),
         "qwen72b_64k_b8_gamma8_k2048": synth.config_qwen72b(batch=8, ctx=65536, gamma=8),
+        # the benched gamma-4 points of the sweep whose few long units take the even-pieces attention plan, the middle
+        # contexts, and the paper's own budget (k = 512, S = 4, W = 16)
+        "qwen72b_64k_b8_gamma4_k2048": synth.config_qwen72b(batch=8, ctx=65536),
+        "qwen72b_128k_b4_gamma4_k2048": synth.config_qwen72b(batch=4, ctx=131072),
+        "qwen72b_8k_b16_gamma4_k2048": synth.config_qwen72b(ctx=8192),
+        "qwen72b_16k_b16_gamma4_k1024": synth.config_qwen72b(ctx=16384, budget=1024),
+        "qwen72b_32k_b16_gamma4_k512_paper": synth.shrink(synth.config_qwen72b(budget=512), n_sink=4, n_recent=16),
         # configs[4]
         "paged_ragged_b32": synth.config_paged(),
     }

@@ -196,3 +196,69 @@ def test_probe_gather_runs_on_the_lists_of_a_fused_layer(paged):
     torch.cuda.synchronize()
     assert torch.equal(dev.k.view(torch.int16), k0.view(torch.int16)) and torch.equal(got.idx, idx0)
     assert int(ws[:4096].max()) == 0                     # the persistent header of the workspace stays zero
+
+
+def test_graph_replayed_decode_steps_equal_eager_steps():
+    """The decode step -- two target layers (paged caches, ragged lengths, per-sequence budgets) through the one-shot
+    call, then the appends -- captured ONCE as a CUDA graph and replayed for three steps must leave bit for bit the state
+    that the same calls leave when issued one by one: caches, lengths, accumulated scores, outputs, index lists.  Lengths,
+    accept counts and every per-step input live in fixed device buffers, so one graph serves every step (bench.py --loop).
+    The eager path is the one test_multi_step_decode_loop_matches_oracle holds against the oracle."""
+    cfg = synth.shrink(synth.config_paged(), batch=3, ctx=2048, ragged_min=600, n_sink=4, n_recent=16, n_layers=2)
+    T, n_steps = cfg.n_new, 3
+    sh = H.shape_of(cfg)
+
+    def run(use_graph: bool):
+        layers = [synth.make_layer(cfg, l, "cuda") for l in (0, 1)]
+        lens = layers[0].seq_lens.clamp(max=cfg.ctx - n_steps * T).contiguous()      # room for every append
+        for x in layers:
+            x.seq_lens = lens                                                        # one set of lengths for all layers
+            for b in range(cfg.batch):
+                x.hist[b, :, int(lens[b]):] = 0
+        ws = api.alloc_workspace(sh, cfg.head_mask, layers[0].k_max)
+        outs = [torch.zeros_like(x.q) for x in layers]
+        idxs = [torch.full((cfg.batch, cfg.n_lists, x.k_max), -1, dtype=torch.int32, device="cuda") for x in layers]
+        cnts = [torch.zeros((cfg.batch, cfg.n_lists), dtype=torch.int32, device="cuda") for x in layers]
+        n_app = torch.zeros(cfg.batch, dtype=torch.int32, device="cuda")
+        scratch = torch.zeros_like(lens)
+
+        def step():
+            for l, x in enumerate(layers):
+                api.verify_layer_fused(sh, H.gpu_kv(x), x.q, x.k_new, x.v_new, cfg.head_mask, x.s_draft, x.hist, 1.0,
+                                       H.select_of(x), outs[l], idxs[l], cnts[l], ws)
+            scratch.copy_(lens)
+            api.append_kv(sh, H.gpu_kv(layers[0]), scratch, layers[0].k_new, layers[0].v_new, n_app, layers[0].hist)
+            api.append_kv(sh, H.gpu_kv(layers[1]), lens, layers[1].k_new, layers[1].v_new, n_app, layers[1].hist)
+
+        replay = None
+        if use_graph:
+            torch.cuda.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g):
+                step()
+            replay = g.replay
+        trail = []
+        gen = torch.Generator().manual_seed(4242)
+        for s in range(n_steps):
+            for l, x in enumerate(layers):                                           # this step's inputs, in place
+                x.q.copy_(_rand_bf16(*x.q.shape, seed=1000 + 10 * s + l))
+                x.k_new.copy_(_rand_bf16(*x.k_new.shape, seed=2000 + 10 * s + l))
+                x.v_new.copy_(_rand_bf16(*x.v_new.shape, seed=3000 + 10 * s + l))
+                x.s_draft.copy_(torch.rand(x.s_draft.shape, generator=gen))
+            n_app.copy_(torch.randint(0, T + 1, (cfg.batch,), generator=gen, dtype=torch.int32))
+            (replay or step)()
+            torch.cuda.synchronize()
+            trail.append([t.clone() for t in (*outs, *idxs, *cnts, lens)])
+        state = [t for x in layers for t in (x.k, x.v, x.hist)] + [lens, ws[:4096]]
+        return trail, state
+
+    eager_trail, eager_state = run(False)        # also loads every kernel before the capture below
+    graph_trail, graph_state = run(True)
+    bits = lambda t: t.view(torch.int16) if t.dtype == torch.bfloat16 else t
+    for s, (a, b) in enumerate(zip(eager_trail, graph_trail)):
+        for i, (x, y) in enumerate(zip(a, b)):
+            assert torch.equal(bits(x), bits(y)), f"step {s}: tensor {i} differs between eager and graph replay"
+    for i, (x, y) in enumerate(zip(eager_state, graph_state)):
+        assert torch.equal(bits(x), bits(y)), f"final state tensor {i} differs"
+    assert int(eager_state[-2].sum()) > int(synth.make_layer(cfg, 0, "cpu").seq_lens.clamp(max=cfg.ctx - n_steps * T).sum())
+    assert not graph_state[-1].any()             # the workspace header is zero again
