@@ -170,6 +170,17 @@ int dustin_verify_layer_fused(const dustin_shape_t* shape, const dustin_kv_t* kv
                               float* lse_out, int32_t* idx_out, int32_t* cnt_out, void* ws, size_t ws_bytes,
                               void* stream);
 
+/* Cost hint for short contexts.  The one-shot call pays for a1 and a3 before it saves anything in a4, so below some
+ * context length the dense call (dustin_sparse_verify_attn with idx == NULL) is faster: at k = 2048, B = 16 on the
+ * Qwen2.5-72B-shaped layer the two cost the same near 10-12 k tokens, with the paper's 6.25 % budgets near 4 k
+ * (profiles/r03_sweep.json, `crossover`).  The library never switches paths on its own (the caller owns the index lists
+ * and the history); this helper returns 1 when dense is predicted to be at least as fast, 0 when the sparse layer is,
+ * or a negative dustin_status, and optionally writes the two predicted times in microseconds.  The prediction is a
+ * linear byte model fitted to B200 measurements of full-length sequences (shape->max_ctx tokens each) -- a hint, good
+ * to roughly 10 % around the crossover on that machine, not a guarantee.  Host arithmetic only; no GPU is touched. */
+int dustin_prefer_dense(const dustin_shape_t* shape, uint64_t head_mask, int32_t k, double* fused_us_out,
+                        double* dense_us_out);
+
 /* ---- steps either side of the layer path ---------------------------------------------------- */
 
 /* Attention Recovery Rate, Eq. 1: the share of the attention mass of row (b,l) that the index list

@@ -109,6 +109,8 @@ def lib():
         L.dustin_arr.argtypes = [i32, i32, i32, vp, vp, vp, vp, i32, vp, vp]
         L.dustin_append_kv.restype = ctypes.c_int
         L.dustin_append_kv.argtypes = [sp, kp, vp, vp, vp, vp, vp, i32, vp]
+        L.dustin_prefer_dense.restype = ctypes.c_int
+        L.dustin_prefer_dense.argtypes = [sp, u64, i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
         L.dustin_quest_meta_bytes.restype = sz
         L.dustin_quest_meta_bytes.argtypes = [sp]
         L.dustin_quest_build_pages.restype = ctypes.c_int
@@ -130,7 +132,7 @@ EXPORTS = ("dustin_version", "dustin_status_string", "dustin_last_cuda_error",
            "dustin_workspace_bytes", "dustin_score_heads", "dustin_fuse_scores", "dustin_topk_select",
            "dustin_sparse_verify_attn", "dustin_verify_layer_fused", "dustin_arr", "dustin_append_kv",
            "dustin_draft_workspace_bytes", "dustin_draft_aggregate", "dustin_score_heads_static",
-           "dustin_quest_meta_bytes", "dustin_quest_build_pages", "dustin_quest_score_pages")
+           "dustin_quest_meta_bytes", "dustin_quest_build_pages", "dustin_quest_score_pages", "dustin_prefer_dense")
 # ... and include/dustin_debug.h (measurement / tuning / testing aids)
 DEBUG_EXPORTS = ("dustin_tune_attn_split_tokens", "dustin_tune_attn_impl", "dustin_tune_set", "dustin_tune_get",
                  "dustin_debug_trace_buffer", "dustin_launch_count", "dustin_profile_enable", "dustin_profile_collect",
@@ -467,3 +469,13 @@ def quest_score_pages(shape: Shape, page_meta: torch.Tensor, q: torch.Tensor, he
         ctypes.c_uint64(head_mask), n_lists, _dense(page_scores, torch.float32),
         None if ub_out is None else _dense(ub_out, torch.float32), _ptr(ws), ws.numel(), _stream())
     _check("dustin_quest_score_pages", rc)
+
+
+def prefer_dense(shape: Shape, head_mask: int, k: int):
+    """dustin_prefer_dense: (dense is predicted at least as fast, predicted fused us, predicted dense us) -- a hint from
+    a byte model fitted on a B200 (dustin.h); host arithmetic only."""
+    f, d = ctypes.c_double(), ctypes.c_double()
+    rc = lib().dustin_prefer_dense(ctypes.byref(shape), ctypes.c_uint64(head_mask), int(k), ctypes.byref(f), ctypes.byref(d))
+    if rc < 0:
+        raise DustinError("dustin_prefer_dense", rc)
+    return bool(rc), f.value, d.value

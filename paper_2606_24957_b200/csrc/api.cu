@@ -658,6 +658,32 @@ int dustin_draft_aggregate(const dustin_shape_t* shape, const dustin_kv_t* kv_la
     return DUSTIN_OK;
 }
 
+// ---- cost hint: one-shot sparse layer or dense attention? ---------------------------------------------------------------
+// Linear models fitted to the B200 measurements of profiles/r03_sweep.json (Qwen2.5-72B-shaped layer, gamma 4; within
+// ~8 % of every point of the fixed-2048 and paper-512 series): each stage is a fixed cost plus its algorithmic bytes over
+// the bandwidth that stage reaches.
+int dustin_prefer_dense(const dustin_shape_t* shape, uint64_t head_mask, int32_t k, double* fused_us_out,
+                        double* dense_us_out) {
+    if (check_shape(shape) != DUSTIN_OK || head_mask == 0 || k <= 0) return DUSTIN_ERR_INVALID_ARG;
+    const int r = shape->n_q_heads / shape->n_kv_heads;
+    int groups = 0;
+    for (int g = 0; g < shape->n_kv_heads; ++g) {
+        const uint64_t gm = (r >= 64 ? ~0ull : ((1ull << r) - 1ull)) << (g * r);
+        if (head_mask & gm) ++groups;
+    }
+    const double row = (double)shape->head_dim * 2.0;                                     // bytes of one K (or V) row
+    const double BN = (double)shape->batch * shape->max_ctx;
+    const double keep = k < shape->max_ctx ? (double)k : (double)shape->max_ctx;
+    const double a1_us = 12.0 + groups * BN * row / 6.65e6;                               // K stream of the scored groups
+    const double a3_us = 27.0;                                                            // selection left on the critical path
+    const double a4_us = 9.0 + 2.0 * shape->n_kv_heads * shape->batch * keep * row / 6.1e6;   // gather of the kept K and V rows
+    const double a5_us = 12.0 + 2.0 * shape->n_kv_heads * BN * row / 6.6e6;               // every K and V row
+    const double fused = a1_us + a3_us + a4_us;
+    if (fused_us_out) *fused_us_out = fused;
+    if (dense_us_out) *dense_us_out = a5_us;
+    return a5_us <= fused ? 1 : 0;
+}
+
 // ---- Quest-16 estimator -------------------------------------------------------------------------------------------------
 size_t dustin_quest_meta_bytes(const dustin_shape_t* shape) {
     if (check_shape(shape) != DUSTIN_OK) return 0;

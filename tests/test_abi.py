@@ -168,3 +168,22 @@ def test_binding_refuses_cpu_tensors():
     import torch
     with pytest.raises(TypeError):
         api.fuse_scores(torch.zeros(1, 1, 8), torch.zeros(1, 1, 8), 1.0)
+
+
+def test_prefer_dense_hint_brackets_the_measured_crossover(lib):
+    """dustin_prefer_dense is host arithmetic fitted to the B200 sweep (profiles/r03_sweep.json): at k = 2048, B = 16 the
+    fused layer loses to dense at 4k and 8k and wins from 16k on (measured crossing: 10.5 k tokens); the predicted times
+    stay within 10 % of the measured ones at the sweep points; a budget that keeps everything always prefers dense."""
+    mask = sum(1 << (8 * g) for g in range(8))
+    measured = {4096: (95.06, 56.79), 8192: (111.82, 96.56), 16384: (146.01, 182.78), 32768: (222.26, 337.4)}
+    prev = None
+    for ctx, (fused_us, dense_us) in measured.items():
+        dense, f, d = api.prefer_dense(api.Shape(16, 64, 8, 128, 5, ctx, 0.0), mask, 2048)
+        assert dense == (ctx <= 8192)
+        assert abs(f - fused_us) <= 0.10 * fused_us and abs(d - dense_us) <= 0.10 * dense_us
+        assert prev is None or (f > prev[0] and d > prev[1])
+        prev = (f, d)
+    assert api.prefer_dense(api.Shape(16, 64, 8, 128, 5, 32768, 0.0), mask, 32768)[0]
+    assert not api.prefer_dense(api.Shape(16, 64, 8, 128, 5, 32768, 0.0), mask, 512)[0]
+    assert lib.dustin_prefer_dense(None, mask, 2048, None, None) == api.ERR_INVALID_ARG
+    assert lib.dustin_prefer_dense(ctypes.byref(shape()), 0, 2048, None, None) == api.ERR_INVALID_ARG
