@@ -22,6 +22,15 @@ namespace {
 
 constexpr int kQuestWarps = 8;
 
+__device__ __forceinline__ uint32_t bf162_min(uint32_t a, uint32_t b) {
+    const __nv_bfloat162 r = __hmin2(*reinterpret_cast<const __nv_bfloat162*>(&a), *reinterpret_cast<const __nv_bfloat162*>(&b));
+    return *reinterpret_cast<const uint32_t*>(&r);
+}
+__device__ __forceinline__ uint32_t bf162_max(uint32_t a, uint32_t b) {
+    const __nv_bfloat162 r = __hmax2(*reinterpret_cast<const __nv_bfloat162*>(&a), *reinterpret_cast<const __nv_bfloat162*>(&b));
+    return *reinterpret_cast<const uint32_t*>(&r);
+}
+
 template <int E>
 struct LaneVec;                    // E bf16 values of one lane: D = 128 -> 8 bytes, D = 64 -> 4 bytes
 template <>
@@ -34,12 +43,9 @@ struct LaneVec<4> {
         f[2] = __uint_as_float(v.y << 16);
         f[3] = __uint_as_float(v.y & 0xffff0000u);
     }
-    __device__ __forceinline__ static void store(__nv_bfloat16* p, const float (&f)[4]) {
-        // the values are bf16 numbers already: truncation is exact
-        uint2 o;
-        o.x = (__float_as_uint(f[0]) >> 16) | (__float_as_uint(f[1]) & 0xffff0000u);
-        o.y = (__float_as_uint(f[2]) >> 16) | (__float_as_uint(f[3]) & 0xffff0000u);
-        *reinterpret_cast<uint2*>(p) = o;
+    __device__ __forceinline__ uint32_t word(int e) const { return e == 0 ? v.x : v.y; }   // two bf16 each
+    __device__ __forceinline__ static void store_words(__nv_bfloat16* p, const uint32_t (&w)[2]) {
+        *reinterpret_cast<uint2*>(p) = make_uint2(w[0], w[1]);
     }
 };
 template <>
@@ -50,8 +56,9 @@ struct LaneVec<2> {
         f[0] = __uint_as_float(v << 16);
         f[1] = __uint_as_float(v & 0xffff0000u);
     }
-    __device__ __forceinline__ static void store(__nv_bfloat16* p, const float (&f)[2]) {
-        *reinterpret_cast<uint32_t*>(p) = (__float_as_uint(f[0]) >> 16) | (__float_as_uint(f[1]) & 0xffff0000u);
+    __device__ __forceinline__ uint32_t word(int) const { return v; }
+    __device__ __forceinline__ static void store_words(__nv_bfloat16* p, const uint32_t (&w)[1]) {
+        *reinterpret_cast<uint32_t*>(p) = w[0];
     }
 };
 
@@ -76,26 +83,23 @@ __global__ void __launch_bounds__(kQuestWarps * 32) quest_build_kernel(const KvV
 #pragma unroll
         for (int i = 0; i < P; ++i)
             if (i < cnt) rows[i].load(kv.k + kv_row_offset(kv, b, n0 + i, g) + lane * E);
-        float lo[E], hi[E];
+        // packed bf16x2 min / max (no unpacking: the float version executed 47 warp instructions per row load and was
+        // issue-bound, ncu: 199 M instructions, issue active 73 %); a page without a token keeps the zeros
+        uint32_t lo[E / 2], hi[E / 2];
 #pragma unroll
-        for (int e = 0; e < E; ++e) {
-            lo[e] = cnt > 0 ? INFINITY : 0.f;
-            hi[e] = cnt > 0 ? -INFINITY : 0.f;
-        }
+        for (int e = 0; e < E / 2; ++e) lo[e] = hi[e] = cnt > 0 ? rows[0].word(e) : 0u;
 #pragma unroll
-        for (int i = 0; i < P; ++i)
+        for (int i = 1; i < P; ++i)
             if (i < cnt) {
-                float f[E];
-                rows[i].unpack(f);
 #pragma unroll
-                for (int e = 0; e < E; ++e) {
-                    lo[e] = fminf(lo[e], f[e]);
-                    hi[e] = fmaxf(hi[e], f[e]);
+                for (int e = 0; e < E / 2; ++e) {
+                    lo[e] = bf162_min(lo[e], rows[i].word(e));
+                    hi[e] = bf162_max(hi[e], rows[i].word(e));
                 }
             }
         __nv_bfloat16* dst = meta + ((((long long)b * n_pages + p) * n_kv_heads + g) * 2) * D + lane * E;
-        LaneVec<E>::store(dst, lo);
-        LaneVec<E>::store(dst + D, hi);
+        LaneVec<E>::store_words(dst, lo);
+        LaneVec<E>::store_words(dst + D, hi);
     }
 }
 
