@@ -111,7 +111,8 @@ __global__ void __launch_bounds__(kQuestWarps * 32) quest_build_kernel(const KvV
 // softmax statistics now come from the normalise kernel, which re-reads the small L2-resident rows of bounds.
 constexpr int kQuestUnroll = 4;
 template <int D, int NH>
-__global__ void __launch_bounds__(kQuestWarps * 32) quest_score_kernel(const QuestParams p) {
+// Resident CTAs per SM that quest_plan counts on: three with one or two heads per KV group (<= 85 registers), else two.
+__global__ void __launch_bounds__(kQuestWarps * 32, NH > 2 ? 2 : 3) quest_score_kernel(const QuestParams p) {
     constexpr int E = D / 32, U = kQuestUnroll;
     const int chunk = blockIdx.x, b = blockIdx.y, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int N = seq_len_of(p.seq_lens, b, p.max_ctx);
@@ -121,15 +122,23 @@ __global__ void __launch_bounds__(kQuestWarps * 32) quest_score_kernel(const Que
     const long long pstride = (long long)p.n_kv_heads * 2 * D;   // elements between consecutive pages of one KV head
     for (int gi = warp % slots; gi < p.n_groups; gi += slots) {
         const int grp = p.group_id[gi], first = p.group_first[gi], nh = p.group_cnt[gi];
-        float qv[NH][E];
+        // max(q * kmin, q * kmax) = max(q, 0) * kmax + min(q, 0) * kmin: two FMAs per channel, one of them adding an exact
+        // zero (bf16 x bf16 is exact in fp32), instead of two products, a max and an add
+        float qp[NH][E], qn[NH][E];
 #pragma unroll
         for (int j = 0; j < NH; ++j) {
 #pragma unroll
-            for (int e = 0; e < E; ++e) qv[j][e] = 0.f;
+            for (int e = 0; e < E; ++e) qp[j][e] = qn[j][e] = 0.f;
             if (j < nh) {
                 LaneVec<E> t;
+                float f[E];
                 t.load(p.q + (long long)b * p.q_stride_batch + p.sel_qoff[first + j] + lane * E);
-                t.unpack(qv[j]);
+                t.unpack(f);
+#pragma unroll
+                for (int e = 0; e < E; ++e) {
+                    qp[j][e] = fmaxf(f[e], 0.f);
+                    qn[j][e] = fminf(f[e], 0.f);
+                }
             }
         }
         const int step = n_sub * U;
@@ -138,32 +147,28 @@ __global__ void __launch_bounds__(kQuestWarps * 32) quest_score_kernel(const Que
         const long long sstep = step * pstride;
         float* urow = p.u + ((long long)b * p.nsel + first) * p.u_stride;
         float* brow = p.ub_out ? p.ub_out + ((long long)b * p.nsel + first) * p.n_pages : nullptr;
-        LaneVec<E> cmn[U], cmx[U], nmn[U], nmx[U];
-#pragma unroll
-        for (int u = 0; u < U; ++u)
-            if (pg + u < p_hi) {
-                cmn[u].load(src + u * pstride);
-                cmx[u].load(src + u * pstride + D);
-            }
-        for (; pg < p_hi; pg += step, src += sstep) {
+        // request the U pages from page pg0 on (src0 = address of page pg0)
+        auto request = [&](LaneVec<E>(&mn)[U], LaneVec<E>(&mx)[U], const __nv_bfloat16* src0, int pg0) {
 #pragma unroll
             for (int u = 0; u < U; ++u)
-                if (pg + step + u < p_hi) {
-                    nmn[u].load(src + sstep + u * pstride);
-                    nmx[u].load(src + sstep + u * pstride + D);
+                if (pg0 + u < p_hi) {
+                    mn[u].load(src0 + u * pstride);
+                    mx[u].load(src0 + u * pstride + D);
                 }
+        };
+        // bounds of the U pages from pg0 on, for every head of the group; lane u stores page pg0 + u
+        auto consume = [&](const LaneVec<E>(&mn)[U], const LaneVec<E>(&mx)[U], int pg0) {
             float a[NH][U];
 #pragma unroll
             for (int u = 0; u < U; ++u) {
                 float fmn[E], fmx[E];
-                cmn[u].unpack(fmn);
-                cmx[u].unpack(fmx);
+                mn[u].unpack(fmn);
+                mx[u].unpack(fmx);
 #pragma unroll
                 for (int j = 0; j < NH; ++j) {
-                    // per channel the larger product bounds q_c * k_c over the page; bf16 x bf16 is exact in fp32
                     float t = 0.f;
 #pragma unroll
-                    for (int e = 0; e < E; ++e) t += fmaxf(qv[j][e] * fmn[e], qv[j][e] * fmx[e]);
+                    for (int e = 0; e < E; ++e) t = __fmaf_rn(qn[j][e], fmn[e], __fmaf_rn(qp[j][e], fmx[e], t));
                     a[j][u] = t;
                 }
             }
@@ -173,22 +178,30 @@ __global__ void __launch_bounds__(kQuestWarps * 32) quest_score_kernel(const Que
                 for (int j = 0; j < NH; ++j)
 #pragma unroll
                     for (int u = 0; u < U; ++u) a[j][u] += __shfl_xor_sync(0xffffffffu, a[j][u], off);
-            // lane u stores page pg + u of every head (pages past p_hi hold stale registers: not stored)
 #pragma unroll
             for (int j = 0; j < NH; ++j) {
                 float v = a[j][0];
 #pragma unroll
                 for (int u = 1; u < U; ++u) v = lane == u ? a[j][u] : v;
-                if (lane < U && pg + lane < p_hi && j < nh) {
-                    urow[(long long)j * p.u_stride + pg + lane] = v * p.scale_log2;
-                    if (brow) brow[(long long)j * p.n_pages + pg + lane] = v * p.scale;
+                if (lane < U && pg0 + lane < p_hi && j < nh) {   // pages past p_hi hold stale registers: not stored
+                    urow[(long long)j * p.u_stride + pg0 + lane] = v * p.scale_log2;
+                    if (brow) brow[(long long)j * p.n_pages + pg0 + lane] = v * p.scale;
                 }
             }
-#pragma unroll
-            for (int u = 0; u < U; ++u) {
-                cmn[u] = nmn[u];
-                cmx[u] = nmx[u];
-            }
+        };
+        // two register buffers in turn: the next round is in flight while the current one is consumed, without copies
+        LaneVec<E> amn[U], amx[U], bmn[U], bmx[U];
+        request(amn, amx, src, pg);
+        while (pg < p_hi) {
+            request(bmn, bmx, src + sstep, pg + step);
+            consume(amn, amx, pg);
+            pg += step;
+            src += sstep;
+            if (pg >= p_hi) break;
+            request(amn, amx, src + sstep, pg + step);
+            consume(bmn, bmx, pg);
+            pg += step;
+            src += sstep;
         }
     }
     // ub_out of the pages without a token: 0
@@ -269,9 +282,9 @@ void quest_plan(int batch, int n_groups, int max_heads_per_group, int n_pages, i
     int slots = 1;
     while (slots < n_groups && slots < kQuestWarps) slots <<= 1;
     const int unit = kQuestUnroll * (kQuestWarps / slots);   // pages that the warps of one group take per round
-    // CTAs per sequence for ONE wave: three CTAs fit an SM (80 registers), two with more than four heads per group (128);
+    // CTAs per sequence for ONE wave: three CTAs fit an SM, two with more than two heads per group (the kernel's launch bounds);
     // rounded DOWN -- a grid just over the resident limit runs a second wave (measured: 93 -> 158 us)
-    const int target = (max_heads_per_group > 4 ? 2 : 3) * device_sm_count() / batch;
+    const int target = (max_heads_per_group > 2 ? 2 : 3) * device_sm_count() / batch;
     int chunk = (n_pages + target - 1) / (target > 0 ? target : 1);
     chunk = (chunk + unit - 1) / unit * unit;
     if (chunk < 2 * unit) chunk = 2 * unit;
