@@ -799,6 +799,37 @@ def run_loop(api, args, dist: Dist, device):
     return res
 
 
+def run_quest(api, args, dist: Dist, device):
+    """Quest-16 estimator alone at the headline shape (Fig. 8): the metadata build of one K cache and the
+    page scoring of the subset heads, each replayed as a CUDA graph over 4 distinct caches, beside the subset a1 on the same
+    caches.  This is also the command the ncu capture of the Quest kernels runs (profiles/r03_ncu.md)."""
+    cfg = synth.config_qwen72b(batch=args.batch, ctx=args.ctx, n_layers=4, gamma=args.gamma)
+    w = Workload(cfg, 4, device)
+    w.quest_setup()
+    w.step_score_quest16()
+    w.step_score_only()
+    by = w.bytes_per_layer()
+    t_score = 1e3 * time_steps(graphed(w.step_score_quest16), args.steps, args.warmup, dist, device) / cfg.n_layers
+    t_build = 1e3 * time_steps(graphed(w.step_quest_build), args.steps, args.warmup, dist, device) / w.n_sets
+    t_a1 = 1e3 * time_steps(graphed(w.step_score_only), args.steps, args.warmup, dist, device) / cfg.n_layers
+    kern = profile_steps(api, lambda: (w.step_quest_build(), w.step_score_quest16()), 2)
+    peak, _ = measured_peak()
+    k_bytes = cfg.batch * cfg.ctx * cfg.n_kv_heads * cfg.head_dim * 2
+    res = {"quest16": {
+        "workload": f"Qwen2.5-72B-shaped layer, B={cfg.batch}, N={cfg.ctx}, {len(cfg.heads)} subset heads, page 16",
+        "score_pages_us": round(t_score, 2), "score_pages_gbs": round(by["a1_k"] / 8 / t_score / 1e3, 1),
+        "score_pages_frac_of_peak": round(by["a1_k"] / 8 / t_score / 1e3 / peak, 3),
+        "build_us_per_cache": round(t_build, 2), "build_gbs": round(1.125 * k_bytes / t_build / 1e3, 1),
+        "build_frac_of_peak": round(1.125 * k_bytes / t_build / 1e3 / peak, 3),
+        "subset_a1_us": round(t_a1, 2),
+        "kernels_us_per_launch": {k: round(v[0], 2) for k, v in kern.items()},
+        "what": "graph-replayed, CUDA events; bytes: metadata = 1/8 of the K bytes of the scored groups (scoring), K + "
+                "metadata (build); kernels_us_per_launch: eager event pairs inside the library"}}
+    if dist.rank == 0:
+        print(json.dumps(res), flush=True)
+    return res
+
+
 def run_arr(api, args, dist: Dist, device):
     """Quality read-out on the synthetic saliency-drift workload (shape of PAPER.md Table 3 /
     Fig. 4, no datasets): lists are selected at drift step l (history = step l-1's scores, draft = noisy step-l scores)
@@ -893,6 +924,7 @@ def main():
     ap.add_argument("--arr", action="store_true", help="ARR read-out of the selection policies on the drift workload")
     ap.add_argument("--sweep", action="store_true", help="context / gamma / budget sweep (configs[3]) + paged (configs[4])")
     ap.add_argument("--loop", action="store_true", help="multi-step decode loop: draft aggregate -> L fused layers -> append")
+    ap.add_argument("--quest", action="store_true", help="Quest-16 estimator alone: metadata build + page scoring at the headline shape")
     ap.add_argument("--loop-layers", type=int, default=8)
     ap.add_argument("--loop-steps", type=int, default=12)
     args = ap.parse_args()
@@ -918,8 +950,8 @@ def main():
         dist.barrier()
     api.lib()
 
-    if args.sweep or args.arr or args.loop:
-        (run_sweep if args.sweep else (run_arr if args.arr else run_loop))(api, args, dist, device)
+    if args.sweep or args.arr or args.loop or args.quest:
+        (run_sweep if args.sweep else (run_arr if args.arr else (run_loop if args.loop else run_quest)))(api, args, dist, device)
         dist.finish()
         return
     cfg = rank_seed(headline_config(args), dist.rank)
